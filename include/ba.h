@@ -1,0 +1,135 @@
+/*
+ * ba.h -- C ABI of libba: Blahut-Arimoto (BA) for the finite-length binary deletion channel
+ * BDC_d^n on one NVIDIA B200 (sm_100a).  Hand-written CUDA kernels behind plain pointers;
+ * no torch types, no exceptions, no global state, no CPU fallback.
+ *
+ * Citations: "P:line" = PAPER.md line (arxiv 2604.05867); "NS" = BASELINE.json:north_star;
+ * "R#/G#" = readings listed in DESIGN.md.
+ *
+ * Channel (NS): inputs x in {0,1}^n, outputs y in {0,1}^{<=n},
+ *     W(y|x) = emb(y,x) (1-d)^{|y|} d^{n-|y|},  emb = #embeddings of y in x as a subsequence.
+ * One BA iteration t (log form P:189-193), all logs base 2:
+ *     q_t(y) = sum_x p_t(x) W(y|x)                      output sweep  (gather over supersequences, NS)
+ *     D_t(x) = sum_y W(y|x) log2( W(y|x) / q_t(y) )     input sweep   (distinct subsequences of x, NS)
+ *     I_t = sum_x p_t(x) D_t(x),  U_t = max_x D_t(x),  Z_t = sum_x p_t(x) 2^{D_t(x)}
+ *     p_{t+1}(x) = max( p_t(x) 2^{D_t(x)} / Z_t , 2^-1000 )            (floor: G8)
+ *     I_t <= C_n(d) <= U_t   (NS);  C(d) <= C_n(d)/n   (Lemma 1)
+ *
+ * Layout (R2): x is an integer in [0,2^n) whose bit (n-1-i) is the paper's x_i
+ * (position 0 = leftmost = most significant).  Output y of length k and MSB-first value v has the
+ * dense index idx(y) = (2^k - 1) + v; idx(empty) = 0; q has 2^{n+1}-1 entries.  All probability
+ * arrays are FP64.
+ *
+ * Which iterate (R6): after a total of K >= 1 iterations, ba_bounds/ba_stats return
+ * (I_{K-1}, U_{K-1}, log2 Z_{K-1}), ba_get_q / ba_get_D return q_{K-1}, D_{K-1}, ba_get_p returns p_K.
+ *
+ * Errors: every function returns BA_OK (0) or a negative code; nothing is printed, thrown or aborted.
+ * ba_last_error(ctx) gives a ctx-owned message for the last failure on that ctx (static string if ctx
+ * is NULL).  A ctx is not thread-safe; distinct ctxs are independent.
+ *
+ * Ownership: ba_create allocates device memory that ba_destroy frees.  ba_create_ext borrows the
+ * caller's device buffers and CUDA stream, which must outlive the ctx.  Host buffers are caller-owned
+ * and caller-sized.  Pointers documented "host" must be host-accessible, "device" device-accessible.
+ */
+#ifndef BA_H
+#define BA_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ba_ctx ba_ctx;
+
+enum {
+    BA_OK = 0,
+    BA_EINVAL = -1,   /* bad n, d, k, index, null pointer, non-normalised / non-positive p          */
+    BA_ENOMEM = -2,   /* host or device allocation failed, or caller scratch too small               */
+    BA_ECUDA = -3,    /* CUDA runtime error; text in ba_last_error                                    */
+    BA_ESTATE = -4,   /* bounds / q / D requested before any iteration                                */
+    BA_ENUMERIC = -5  /* non-finite bound (some q(y) = 0 or p underflow, G8)                          */
+};
+
+enum {
+    BA_MODE_ENUM = 0, /* contract path (NS): every (x,y) term with emb>0 is enumerated once per sweep */
+    BA_MODE_FAST = 1  /* position-by-position deletion transform, O(n 2^n)/sweep  */
+};
+
+#define BA_NMAX 30    /* uint32 string codes; tested to n = 24 in ENUM mode                            */
+
+/* ---- required by the north star -------------------------------------------------------------- */
+
+/* New problem (n in [1,BA_NMAX], d in [0,1]); p_0 uniform.  Library-owned device buffers and
+ * stream.  *out is NULL on failure. */
+int ba_create(int n, double d, ba_ctx **out);
+
+/* Enqueue k >= 0 full BA iterations (both sweeps, reductions, update) on the ctx stream.  Does not
+ * synchronise with the host. */
+int ba_iterate(ba_ctx *c, int k);
+
+/* Bounds in bits for C_n(d) from the last completed iteration (R6): I_lower = I(p) (NS),
+ * maxD_upper = max_x D(x).  Synchronises the stream.  BA_ESTATE before the first iteration,
+ * BA_ENUMERIC if either is non-finite.  Host pointers. */
+int ba_bounds(ba_ctx *c, double *I_lower, double *maxD_upper);
+
+/* Copy p (2^n doubles) to a host buffer.  Synchronises. */
+int ba_get_p(ba_ctx *c, double *p_host);
+
+/* ---- forced additions ------------------------------------------------------------ */
+
+/* Bytes of device scratch ba_create_ext needs for size n (0 if n is invalid). */
+size_t ba_scratch_bytes(int n);
+
+/* As ba_create, on caller-owned DEVICE buffers: p_dev (2^n doubles), q_dev (2^{n+1}-1 doubles),
+ * D_dev (2^n doubles), scratch_dev (>= ba_scratch_bytes(n), 256-byte aligned) and a cudaStream_t
+ * passed as void* (NULL = legacy default stream).  p_dev is overwritten with the uniform start. */
+int ba_create_ext(int n, double d, void *p_dev, void *q_dev, void *D_dev,
+                  void *scratch_dev, size_t scratch_bytes, void *cuda_stream, ba_ctx **out);
+
+/* Select BA_MODE_ENUM (default) or BA_MODE_FAST for subsequent iterations. */
+int ba_set_mode(ba_ctx *c, int mode);
+
+/* Replace p by a host vector (2^n doubles).  Rejects non-finite or non-positive entries and
+ * |sum p - 1| > 1e-9; stores the values as given, without renormalising.  Synchronises. */
+int ba_set_p(ba_ctx *c, const double *p_host);
+
+/* q_{K-1} (2^{n+1}-1 doubles) and D_{K-1} (2^n doubles) to host.  BA_ESTATE before any iteration. */
+int ba_get_q(ba_ctx *c, double *q_host);
+int ba_get_D(ba_ctx *c, double *D_host);
+
+/* log2 Z of the last iteration (the paper's stop statistic is U - log2 Z) and the number
+ * of iterations done on this ctx.  Either pointer may be NULL.  Synchronises. */
+int ba_stats(ba_ctx *c, double *log2Z, long long *iters_done);
+
+/* History of the last `count` iterations, oldest first: out[3*i+0..2] = {I_t, U_t, log2 Z_t}.
+ * count must not exceed min(iters_done, 65536).  Synchronises. */
+int ba_get_history(ba_ctx *c, int count, double *out_host);
+
+/* Device-side time of the four phases of the most recent ba_iterate call, averaged per iteration, in
+ * milliseconds, measured with CUDA events on the ctx stream: ms[0] output sweep, ms[1] input sweep,
+ * ms[2] reductions + update, ms[3] whole iteration.  Synchronises. */
+int ba_last_timing(ba_ctx *c, double ms_host[4]);
+
+/* Row x of the integer embedding matrix as produced by the input-sweep enumerator:
+ * emb_out_host[idx(y)] = emb(y,x) for every y, zero where y is not a subsequence.  2^{n+1}-1 entries. */
+int ba_debug_emb_row(ba_ctx *c, unsigned x, unsigned *emb_out_host);
+
+/* Column yidx of the embedding matrix as produced by the output-sweep supersequence enumerator
+ * (P:240): emb_out_host[x] = emb(y,x).  2^n entries. */
+int ba_debug_emb_col(ba_ctx *c, unsigned yidx, unsigned *emb_out_host);
+
+/* Number of (x,y) terms T(n) = sum_k 2^k sum_{i<=n-k} C(n,i) (Lemma 6) visited by one sweep,
+ * and, after ba_debug_count_terms, the number the ENUM input / output enumerators actually visited
+ * (device-side integer checksums).  Host pointers. */
+int ba_terms_per_sweep(int n, unsigned long long *T);
+int ba_debug_count_terms(ba_ctx *c, unsigned long long *in_terms, unsigned long long *out_terms,
+                         unsigned long long *in_emb_sum, unsigned long long *out_emb_sum);
+
+void ba_destroy(ba_ctx *c);
+const char *ba_last_error(const ba_ctx *c);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BA_H */

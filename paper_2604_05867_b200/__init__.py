@@ -1,0 +1,255 @@
+"""paper_2604_05867_b200 -- thin Python binding of libba (include/ba.h).
+
+Argument marshalling only: every step of the BA hot path (output sweep, input sweep, reductions,
+update) runs in the hand-written CUDA kernels of csrc/.  PyTorch provides device memory and the
+CUDA stream (ba_create_ext); nothing here computes.  There is no CPU fallback: importing the
+binding on a box without the built library, or creating a context without a CUDA device, raises.
+
+The module-level functions carry the names of the C entry points (ba_create, ba_iterate,
+ba_bounds, ba_get_p, ...); `BA` is a small convenience wrapper around a context.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+from . import build as _build
+
+BA_OK, BA_EINVAL, BA_ENOMEM, BA_ECUDA, BA_ESTATE, BA_ENUMERIC = 0, -1, -2, -3, -4, -5
+BA_MODE_ENUM, BA_MODE_FAST = 0, 1
+BA_NMAX = 30
+_CODE_NAMES = {0: "BA_OK", -1: "BA_EINVAL", -2: "BA_ENOMEM", -3: "BA_ECUDA", -4: "BA_ESTATE", -5: "BA_ENUMERIC"}
+
+EXPORTS = ["ba_create", "ba_iterate", "ba_bounds", "ba_get_p", "ba_scratch_bytes", "ba_create_ext",
+           "ba_set_mode", "ba_set_p", "ba_get_q", "ba_get_D", "ba_stats", "ba_get_history",
+           "ba_last_timing", "ba_debug_emb_row", "ba_debug_emb_col", "ba_terms_per_sweep",
+           "ba_debug_count_terms", "ba_destroy", "ba_last_error"]
+
+
+class BAError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"{_CODE_NAMES.get(code, code)}: {msg}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib_path():
+    return _build.LIB
+
+
+def load():
+    """Load libba.so (building it with nvcc first if the source is newer). Fails loudly."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.build()
+    L = ctypes.CDLL(path)
+    vp, dp = ctypes.c_void_p, ctypes.POINTER(ctypes.c_double)
+    up = ctypes.POINTER(ctypes.c_uint)
+    ullp = ctypes.POINTER(ctypes.c_ulonglong)
+    L.ba_create.argtypes = [ctypes.c_int, ctypes.c_double, ctypes.POINTER(vp)]
+    L.ba_create_ext.argtypes = [ctypes.c_int, ctypes.c_double, vp, vp, vp, vp, ctypes.c_size_t, vp, ctypes.POINTER(vp)]
+    L.ba_scratch_bytes.argtypes = [ctypes.c_int]
+    L.ba_scratch_bytes.restype = ctypes.c_size_t
+    L.ba_iterate.argtypes = [vp, ctypes.c_int]
+    L.ba_bounds.argtypes = [vp, dp, dp]
+    L.ba_get_p.argtypes = [vp, dp]
+    L.ba_get_q.argtypes = [vp, dp]
+    L.ba_get_D.argtypes = [vp, dp]
+    L.ba_set_p.argtypes = [vp, dp]
+    L.ba_set_mode.argtypes = [vp, ctypes.c_int]
+    L.ba_stats.argtypes = [vp, dp, ctypes.POINTER(ctypes.c_longlong)]
+    L.ba_get_history.argtypes = [vp, ctypes.c_int, dp]
+    L.ba_last_timing.argtypes = [vp, dp]
+    L.ba_debug_emb_row.argtypes = [vp, ctypes.c_uint, up]
+    L.ba_debug_emb_col.argtypes = [vp, ctypes.c_uint, up]
+    L.ba_terms_per_sweep.argtypes = [ctypes.c_int, ullp]
+    L.ba_debug_count_terms.argtypes = [vp, ullp, ullp, ullp, ullp]
+    L.ba_destroy.argtypes = [vp]
+    L.ba_destroy.restype = None
+    L.ba_last_error.argtypes = [vp]
+    L.ba_last_error.restype = ctypes.c_char_p
+    for name in EXPORTS:
+        getattr(L, name)
+    _lib = L
+    return L
+
+
+def _dp(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
+
+
+class _Ctx:
+    """Opaque handle + the torch tensors that back a ba_create_ext context."""
+
+    def __init__(self, handle, n, tensors=None):
+        self.handle = handle
+        self.n = n
+        self.tensors = tensors
+
+
+def _check(ctx, rc):
+    if rc != BA_OK:
+        msg = load().ba_last_error(ctx.handle if ctx else None)
+        raise BAError(rc, msg.decode() if msg else "")
+
+
+def ba_scratch_bytes(n):
+    return int(load().ba_scratch_bytes(int(n)))
+
+
+def ba_create(n, d, device="cuda:0", use_torch_memory=True):
+    """ba_create / ba_create_ext.  With use_torch_memory (default) p, q, D and the scratch are torch
+    CUDA tensors and the kernels run on torch's current stream."""
+    L = load()
+    h = ctypes.c_void_p()
+    if not use_torch_memory:
+        rc = L.ba_create(int(n), float(d), ctypes.byref(h))
+        if rc != BA_OK:
+            raise BAError(rc, "ba_create failed")
+        return _Ctx(h, n)
+    import torch
+    if not torch.cuda.is_available():
+        raise BAError(BA_ECUDA, "no CUDA device: libba has no CPU fallback")
+    if not (isinstance(n, int) and 1 <= n <= BA_NMAX):
+        raise BAError(BA_EINVAL, "n out of range")
+    dev = torch.device(device)
+    torch.cuda.set_device(dev)
+    NX, NY = 1 << n, (2 << n) - 1
+    p = torch.empty(NX, dtype=torch.float64, device=dev)
+    q = torch.empty(NY, dtype=torch.float64, device=dev)
+    D = torch.empty(NX, dtype=torch.float64, device=dev)
+    sb = ba_scratch_bytes(n)
+    scratch = torch.empty(sb + 256, dtype=torch.uint8, device=dev)
+    sptr = (scratch.data_ptr() + 255) & ~255
+    stream = torch.cuda.current_stream(dev).cuda_stream
+    rc = L.ba_create_ext(int(n), float(d), p.data_ptr(), q.data_ptr(), D.data_ptr(), sptr, sb,
+                         ctypes.c_void_p(stream), ctypes.byref(h))
+    if rc != BA_OK:
+        raise BAError(rc, "ba_create_ext failed")
+    return _Ctx(h, n, dict(p=p, q=q, D=D, scratch=scratch))
+
+
+def ba_destroy(ctx):
+    if ctx.handle:
+        load().ba_destroy(ctx.handle)
+        ctx.handle = None
+        ctx.tensors = None
+
+
+def ba_set_mode(ctx, mode):
+    _check(ctx, load().ba_set_mode(ctx.handle, int(mode)))
+
+
+def ba_iterate(ctx, k):
+    _check(ctx, load().ba_iterate(ctx.handle, int(k)))
+
+
+def ba_bounds(ctx):
+    lo, up = ctypes.c_double(), ctypes.c_double()
+    _check(ctx, load().ba_bounds(ctx.handle, ctypes.byref(lo), ctypes.byref(up)))
+    return lo.value, up.value
+
+
+def ba_stats(ctx):
+    lz, it = ctypes.c_double(), ctypes.c_longlong()
+    _check(ctx, load().ba_stats(ctx.handle, ctypes.byref(lz), ctypes.byref(it)))
+    return lz.value, it.value
+
+
+def ba_iters_done(ctx):
+    it = ctypes.c_longlong()
+    _check(ctx, load().ba_stats(ctx.handle, None, ctypes.byref(it)))
+    return it.value
+
+
+def ba_get_history(ctx, count):
+    out = np.empty((count, 3), dtype=np.float64)
+    _check(ctx, load().ba_get_history(ctx.handle, int(count), _dp(out)))
+    return out
+
+
+def ba_last_timing(ctx):
+    ms = np.empty(4, dtype=np.float64)
+    _check(ctx, load().ba_last_timing(ctx.handle, _dp(ms)))
+    return dict(out_ms=ms[0], in_ms=ms[1], update_ms=ms[2], iter_ms=ms[3])
+
+
+def ba_get_p(ctx):
+    out = np.empty(1 << ctx.n, dtype=np.float64)
+    _check(ctx, load().ba_get_p(ctx.handle, _dp(out)))
+    return out
+
+
+def ba_get_q(ctx):
+    out = np.empty((2 << ctx.n) - 1, dtype=np.float64)
+    _check(ctx, load().ba_get_q(ctx.handle, _dp(out)))
+    return out
+
+
+def ba_get_D(ctx):
+    out = np.empty(1 << ctx.n, dtype=np.float64)
+    _check(ctx, load().ba_get_D(ctx.handle, _dp(out)))
+    return out
+
+
+def ba_set_p(ctx, p):
+    p = np.ascontiguousarray(p, dtype=np.float64)
+    if p.shape != (1 << ctx.n,):
+        raise BAError(BA_EINVAL, "ba_set_p: wrong shape")
+    _check(ctx, load().ba_set_p(ctx.handle, _dp(p)))
+
+
+def ba_debug_emb_row(ctx, x):
+    out = np.zeros((2 << ctx.n) - 1, dtype=np.uint32)
+    _check(ctx, load().ba_debug_emb_row(ctx.handle, int(x), out.ctypes.data_as(ctypes.POINTER(ctypes.c_uint))))
+    return out
+
+
+def ba_debug_emb_col(ctx, yidx):
+    out = np.zeros(1 << ctx.n, dtype=np.uint32)
+    _check(ctx, load().ba_debug_emb_col(ctx.handle, int(yidx), out.ctypes.data_as(ctypes.POINTER(ctypes.c_uint))))
+    return out
+
+
+def ba_terms_per_sweep(n):
+    t = ctypes.c_ulonglong()
+    rc = load().ba_terms_per_sweep(int(n), ctypes.byref(t))
+    if rc != BA_OK:
+        raise BAError(rc, "ba_terms_per_sweep")
+    return t.value
+
+
+def ba_debug_count_terms(ctx):
+    v = [ctypes.c_ulonglong() for _ in range(4)]
+    _check(ctx, load().ba_debug_count_terms(ctx.handle, *[ctypes.byref(x) for x in v]))
+    return dict(in_terms=v[0].value, out_terms=v[1].value, in_emb_sum=v[2].value, out_emb_sum=v[3].value)
+
+
+class BA:
+    """Convenience wrapper: BA(n, d).iterate(k).bounds()."""
+
+    def __init__(self, n, d, mode=BA_MODE_ENUM, p0=None, device="cuda:0"):
+        self.ctx = ba_create(n, d, device=device)
+        self.n, self.d = n, d
+        ba_set_mode(self.ctx, mode)
+        if p0 is not None:
+            ba_set_p(self.ctx, p0)
+
+    def iterate(self, k=1):
+        ba_iterate(self.ctx, k)
+        return self
+
+    def bounds(self):
+        return ba_bounds(self.ctx)
+
+    def close(self):
+        ba_destroy(self.ctx)
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()

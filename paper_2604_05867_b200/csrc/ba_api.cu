@@ -1,0 +1,594 @@
+// ba_api.cu -- C ABI of libba (include/ba.h): context, host-side tables, launch sequencing.
+// Unity build: the kernels live in the .cuh files included below.
+#include "../../include/ba.h"
+#include "ba_internal.h"
+#include "ba_enum_in.cuh"
+#include "ba_enum_out.cuh"
+#include "ba_stream.cuh"
+#include "ba_fast.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+// ------------------------------------------------------------------------------------------------ ctx
+struct ba_ctx {
+    int n = 0, m = 0, h = 0, mode = BA_MODE_ENUM;
+    double d = 0.0;
+    size_t NX = 0, NY = 0, NZ = 0, napart = 0;
+    KConst kc;
+    OutLayout lay;
+    int ntab = 0;
+    cudaStream_t st = nullptr;
+    bool own_buffers = false, own_stream = false;
+    double *p = nullptr, *q = nullptr, *D = nullptr;
+    unsigned char *scratch = nullptr;
+    // carved from scratch
+    double *c = nullptr, *Hc = nullptr, *Apart = nullptr, *part = nullptr, *scal = nullptr, *hist = nullptr;
+    uint32_t *tab = nullptr, *vinfo = nullptr;
+    uint16_t *thrlist = nullptr;
+    unsigned int *counters = nullptr;
+    unsigned long long *cnt = nullptr;
+    size_t npart_cap = 0;
+    bool hc_ready = false;
+    long long iters = 0;
+    int num_sms = 0, grid_in = 0, grid_out = 0, block = 0;
+    size_t smem_in = 0, smem_out = 0;
+    std::vector<cudaEvent_t> ev;     // 4 per timed iteration + 1
+    int ev_iters = 0;
+    std::string err;
+};
+
+static const char *g_static_err = "ba: invalid or null context";
+
+static int fail(ba_ctx *c, int code, const std::string &msg) {
+    if (c) c->err = msg;
+    return code;
+}
+
+#define CK(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess)                                                                     \
+            return fail(c, BA_ECUDA, std::string(#call) + ": " + cudaGetErrorString(e_));          \
+    } while (0)
+
+static size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
+
+// ------------------------------------------------------------------------------------------------ host tables
+static uint32_t host_emb(uint32_t z, int lz, uint32_t v, int lv) {   // #embeddings of z in v
+    std::vector<uint32_t> e(lz + 1, 0);
+    e[0] = 1;
+    for (int i = 0; i < lv; i++) {
+        uint32_t vb = (v >> (lv - 1 - i)) & 1u;
+        for (int r = lz; r >= 1; r--)
+            if (((z >> (lz - r)) & 1u) == vb) e[r] += e[r - 1];
+    }
+    return e[lz];
+}
+
+static double host_binom(int n, int k) {
+    double r = 1.0;
+    for (int i = 1; i <= k; i++) r = r * (double)(n - k + i) / (double)i;
+    return std::floor(r + 0.5);
+}
+
+struct LowTables {
+    std::vector<uint32_t> words, vinfo;
+    std::vector<uint16_t> thrlist;
+    OutLayout lay;
+};
+
+// Low table of the m-bit deletion channel (ba_internal.h) and the output-sweep thread assignment.
+static void build_low_tables(int m, LowTables &T) {
+    const int nv = 1 << m;
+    T.words.clear();
+    T.vinfo.assign(nv, 0);
+    std::vector<std::vector<int>> local_of_code(nv);       // code(z) -> local index in v's list, -1 if absent
+    for (int v = 0; v < nv; v++) {
+        std::vector<uint32_t> codes[3];                    // empty / starts with 0 / starts with 1
+        std::vector<uint32_t> Bs[3];
+        for (int lz = 0; lz <= m; lz++)
+            for (uint32_t z = 0; z < (1u << lz); z++) {
+                uint32_t B = host_emb(z, lz, (uint32_t)v, m);
+                if (!B) continue;
+                int blk = (lz == 0) ? 0 : 1 + (int)((z >> (lz - 1)) & 1u);
+                codes[blk].push_back((1u << lz) | z);
+                Bs[blk].push_back(B);
+            }
+        std::vector<uint32_t> code_list, B_list;
+        for (int blk = 0; blk < 3; blk++)
+            for (size_t i = 0; i < codes[blk].size(); i++) { code_list.push_back(codes[blk][i]); B_list.push_back(Bs[blk][i]); }
+        local_of_code[v].assign((size_t)2 << m, -1);
+        for (size_t i = 0; i < code_list.size(); i++) local_of_code[v][code_list[i]] = (int)i;
+        uint32_t base = (uint32_t)T.words.size();
+        T.vinfo[v] = base | ((uint32_t)codes[1].size() << 14) | ((uint32_t)codes[2].size() << 21);
+        for (size_t i = 0; i < code_list.size(); i++) {
+            uint32_t cz = code_list[i];
+            int lz = 31 - __builtin_clz(cz);
+            uint32_t zval = cz - (1u << lz);
+            uint32_t link[2] = {BA_LINK_NONE, BA_LINK_NONE};
+            if (lz + 1 <= m)
+                for (uint32_t b = 0; b < 2; b++) {
+                    uint32_t cbz = (1u << (lz + 1)) | (b << lz) | zval;
+                    int li = local_of_code[v][cbz];
+                    if (li >= 0) link[b] = (uint32_t)li;
+                }
+            T.words.push_back(cz | (B_list[i] << 9) | (link[0] << 16) | (link[1] << 23));
+        }
+    }
+    // output-sweep assignment: class j = outputs z of length j; the 2^{m-j} threads tid with
+    // (tid >> (m-j)) == val(z) share the supersequences v of z (ascending v, dealt round-robin).
+    int total = 0;
+    for (int j = 0; j <= BA_MLOW + 1; j++) T.lay.off[j] = 0;
+    for (int j = 0; j <= BA_MLOW; j++) T.lay.slots[j] = 0;
+    for (int j = 0; j <= m; j++) {
+        int L = 0;
+        for (int i = 0; i <= m - j; i++) L += (int)host_binom(m, i);   // Lemma 6
+        int G = 1 << (m - j);
+        T.lay.slots[j] = (j == 0) ? 0 : (L + G - 1) / G;               // class 0 is handled in-line
+        T.lay.off[j] = total;
+        total += T.lay.slots[j];
+    }
+    for (int j = m + 1; j <= BA_MLOW + 1; j++) T.lay.off[j] = total;
+    T.thrlist.assign((size_t)total * nv, 0);
+    for (int j = 1; j <= m; j++) {
+        int G = 1 << (m - j);
+        for (uint32_t z = 0; z < (1u << j); z++) {
+            uint32_t cz = (1u << j) | z;
+            int cntv = 0;
+            for (int v = 0; v < nv; v++) {
+                int li = local_of_code[v][cz];
+                if (li < 0) continue;
+                int g = cntv % G, k = cntv / G;
+                int tid = (int)(z << (m - j)) + g;
+                T.thrlist[(size_t)(T.lay.off[j] + k) * nv + tid] = (uint16_t)((uint32_t)v | ((uint32_t)li << 8) | 0x8000u);
+                cntv++;
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------ scratch layout
+struct ScratchLayout {
+    size_t c, Hc, Apart, part, scal, hist, tab, vinfo, thrlist, counters, cnt, total;
+    size_t napart, npart_cap;
+};
+
+static int low_m(int n) { return n < BA_MLOW ? n : BA_MLOW; }
+
+static void scratch_layout(int n, size_t ntab, size_t nthrlist, ScratchLayout &L) {
+    const int m = low_m(n), h = n - m;
+    const size_t NX = (size_t)1 << n, NY = ((size_t)2 << n) - 1, NZ = ((size_t)2 << m) - 1;
+    L.napart = (((size_t)2 << h) - 1) * NZ;
+    size_t fastwords = 2 * (((size_t)2 << n) + 64);          // FAST mode ping-pong buffers
+    if (L.napart < fastwords) L.napart = fastwords;
+    L.npart_cap = ((size_t)1 << h) > 8192 ? ((size_t)1 << h) : 8192;
+    size_t o = 0;
+    L.c = o; o += align256(NY * 8);
+    L.Hc = o; o += align256(NX * 8);
+    L.Apart = o; o += align256(L.napart * 8);
+    L.part = o; o += align256(L.npart_cap * 3 * 8);
+    L.scal = o; o += align256(8 * 8);
+    L.hist = o; o += align256((size_t)BA_HIST_CAP * 3 * 8);
+    L.tab = o; o += align256(ntab * 4);
+    L.vinfo = o; o += align256(((size_t)1 << m) * 4);
+    L.thrlist = o; o += align256(nthrlist * 2);
+    L.counters = o; o += align256(16 * 4);
+    L.cnt = o; o += align256(8 * 8);
+    L.total = o;
+}
+
+extern "C" size_t ba_scratch_bytes(int n) {
+    if (n < 1 || n > BA_NMAX) return 0;
+    LowTables T;
+    build_low_tables(low_m(n), T);
+    ScratchLayout L;
+    scratch_layout(n, T.words.size(), T.thrlist.size(), L);
+    return L.total;
+}
+
+extern "C" int ba_terms_per_sweep(int n, unsigned long long *T) {
+    if (n < 1 || n > BA_NMAX || !T) return BA_EINVAL;
+    unsigned long long tot = 0;
+    for (int k = 0; k <= n; k++) {
+        unsigned long long s = 0;
+        for (int i = 0; i <= n - k; i++) s += (unsigned long long)host_binom(n, i);
+        tot += s << k;
+    }
+    *T = tot;
+    return BA_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ create / destroy
+static int setup_ctx(ba_ctx *c, int n, double d) {
+    c->n = n; c->m = low_m(n); c->h = n - c->m; c->d = d;
+    c->NX = (size_t)1 << n; c->NY = ((size_t)2 << n) - 1; c->NZ = ((size_t)2 << c->m) - 1;
+    KConst &kc = c->kc;
+    kc.n = n; kc.m = c->m; kc.h = c->h;
+    for (int k = 0; k <= BA_NMAX_I; k++) { kc.w[k] = 0.0; kc.lebar[k] = 0.0; }
+    for (int k = 0; k <= n; k++) {
+        long double a = 1.0L, b = 1.0L;                      // 0^0 = 1 (R7)
+        for (int i = 0; i < k; i++) a *= (long double)(1.0 - d);
+        for (int i = 0; i < n - k; i++) b *= (long double)d;
+        kc.w[k] = (double)(a * b);
+        kc.lebar[k] = std::log2(host_binom(n, k)) - (double)k;
+    }
+    return BA_OK;
+}
+
+static int finish_create(ba_ctx *c) {
+    LowTables T;
+    build_low_tables(c->m, T);
+    c->lay = T.lay;
+    c->ntab = (int)T.words.size();
+    ScratchLayout L;
+    scratch_layout(c->n, T.words.size(), T.thrlist.size(), L);
+    unsigned char *s = c->scratch;
+    c->c = (double *)(s + L.c); c->Hc = (double *)(s + L.Hc); c->Apart = (double *)(s + L.Apart);
+    c->part = (double *)(s + L.part); c->scal = (double *)(s + L.scal); c->hist = (double *)(s + L.hist);
+    c->tab = (uint32_t *)(s + L.tab); c->vinfo = (uint32_t *)(s + L.vinfo); c->thrlist = (uint16_t *)(s + L.thrlist);
+    c->counters = (unsigned int *)(s + L.counters); c->cnt = (unsigned long long *)(s + L.cnt);
+    c->napart = L.napart; c->npart_cap = L.npart_cap;
+
+    CK(cudaMemcpyAsync(c->tab, T.words.data(), T.words.size() * 4, cudaMemcpyHostToDevice, c->st));
+    CK(cudaMemcpyAsync(c->vinfo, T.vinfo.data(), T.vinfo.size() * 4, cudaMemcpyHostToDevice, c->st));
+    if (!T.thrlist.empty())
+        CK(cudaMemcpyAsync(c->thrlist, T.thrlist.data(), T.thrlist.size() * 2, cudaMemcpyHostToDevice, c->st));
+    uint32_t hb[BA_NMAX_I + 1][BA_NMAX_I + 1];
+    for (int a = 0; a <= BA_NMAX_I; a++)
+        for (int b = 0; b <= BA_NMAX_I; b++) hb[a][b] = (b <= a) ? (uint32_t)host_binom(a, b) : 0u;
+    CK(cudaMemcpyToSymbolAsync(c_binom, hb, sizeof(hb), 0, cudaMemcpyHostToDevice, c->st));
+    CK(cudaStreamSynchronize(c->st));
+
+    int dev = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev));
+    c->block = (1 << c->m) < 32 ? 32 : (1 << c->m);
+    c->smem_in = enum_in_smem_bytes(c->m, c->h, c->ntab);
+    c->smem_out = enum_out_smem_bytes(c->m, c->ntab, c->lay.off[c->m + 1]);
+    CK(cudaFuncSetAttribute(k_enum_in<IN_SWEEP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_in));
+    CK(cudaFuncSetAttribute(k_enum_in<IN_HC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_in));
+    CK(cudaFuncSetAttribute(k_enum_in<IN_DEBUG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_in));
+    CK(cudaFuncSetAttribute(k_enum_in<IN_COUNT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_in));
+    CK(cudaFuncSetAttribute(k_enum_out<OUT_SWEEP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_out));
+    CK(cudaFuncSetAttribute(k_enum_out<OUT_DEBUG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_out));
+    CK(cudaFuncSetAttribute(k_enum_out<OUT_COUNT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_out));
+    int occ_in = 1, occ_out = 1;
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_in, k_enum_in<IN_SWEEP>, c->block, c->smem_in));
+    CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_out, k_enum_out<OUT_SWEEP>, c->block, c->smem_out));
+    if (occ_in < 1 || occ_out < 1) return fail(c, BA_ECUDA, "ENUM kernels do not fit on an SM");
+    size_t items_in = (size_t)1 << c->h, items_out = ((size_t)2 << c->h) - 1;
+    size_t gi = (size_t)c->num_sms * occ_in, go = (size_t)c->num_sms * occ_out;
+    c->grid_in = (int)(items_in < gi ? items_in : gi);
+    c->grid_out = (int)(items_out < go ? items_out : go);
+
+    // p0 uniform
+    k_fill<<<c->num_sms * 4, 256, 0, c->st>>>(c->NX, c->p, 1.0 / (double)c->NX);
+    CK(cudaGetLastError());
+    CK(cudaStreamSynchronize(c->st));
+    return BA_OK;
+}
+
+extern "C" int ba_create_ext(int n, double d, void *p_dev, void *q_dev, void *D_dev, void *scratch_dev,
+                             size_t scratch_bytes, void *cuda_stream, ba_ctx **out) {
+    if (out) *out = nullptr;
+    if (!out || n < 1 || n > BA_NMAX || !(d >= 0.0 && d <= 1.0) || !p_dev || !q_dev || !D_dev || !scratch_dev)
+        return BA_EINVAL;
+    if (scratch_bytes < ba_scratch_bytes(n) || ((uintptr_t)scratch_dev & 255u)) return BA_ENOMEM;
+    ba_ctx *c = new (std::nothrow) ba_ctx();
+    if (!c) return BA_ENOMEM;
+    setup_ctx(c, n, d);
+    c->p = (double *)p_dev; c->q = (double *)q_dev; c->D = (double *)D_dev;
+    c->scratch = (unsigned char *)scratch_dev;
+    c->st = (cudaStream_t)cuda_stream;
+    int rc = finish_create(c);
+    if (rc) { delete c; return rc; }
+    *out = c;
+    return BA_OK;
+}
+
+extern "C" int ba_create(int n, double d, ba_ctx **out) {
+    if (out) *out = nullptr;
+    if (!out || n < 1 || n > BA_NMAX || !(d >= 0.0 && d <= 1.0)) return BA_EINVAL;
+    ba_ctx *c = new (std::nothrow) ba_ctx();
+    if (!c) return BA_ENOMEM;
+    setup_ctx(c, n, d);
+    c->own_buffers = true;
+    size_t sb = ba_scratch_bytes(n);
+    int rc = BA_OK;
+    if (cudaMalloc(&c->p, c->NX * 8) != cudaSuccess || cudaMalloc(&c->q, c->NY * 8) != cudaSuccess ||
+        cudaMalloc(&c->D, c->NX * 8) != cudaSuccess || cudaMalloc(&c->scratch, sb) != cudaSuccess)
+        rc = BA_ENOMEM;
+    if (!rc && cudaStreamCreateWithFlags(&c->st, cudaStreamNonBlocking) != cudaSuccess) rc = BA_ECUDA;
+    else c->own_stream = (rc == BA_OK);
+    if (!rc) rc = finish_create(c);
+    if (rc) { cudaGetLastError(); ba_destroy(c); return rc; }
+    *out = c;
+    return BA_OK;
+}
+
+extern "C" void ba_destroy(ba_ctx *c) {
+    if (!c) return;
+    if (c->st || !c->own_stream) cudaStreamSynchronize(c->st);
+    for (auto e : c->ev) cudaEventDestroy(e);
+    if (c->own_buffers) { cudaFree(c->p); cudaFree(c->q); cudaFree(c->D); cudaFree(c->scratch); }
+    if (c->own_stream && c->st) cudaStreamDestroy(c->st);
+    delete c;
+}
+
+extern "C" const char *ba_last_error(const ba_ctx *c) { return c ? c->err.c_str() : g_static_err; }
+
+extern "C" int ba_set_mode(ba_ctx *c, int mode) {
+    if (!c) return BA_EINVAL;
+    if (mode != BA_MODE_ENUM && mode != BA_MODE_FAST) return fail(c, BA_EINVAL, "ba_set_mode: unknown mode");
+    c->mode = mode;
+    return BA_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ launches
+static InArgs make_in_args(ba_ctx *c) {
+    InArgs a;
+    a.kc = c->kc; a.tab = c->tab; a.vinfo = c->vinfo; a.ntab = c->ntab;
+    a.c = c->c; a.p = c->p; a.Hc = c->Hc; a.D = c->D; a.part = c->part;
+    a.counter = c->counters; a.dbg_x = 0; a.dbg_out = nullptr; a.cnt = c->cnt;
+    return a;
+}
+
+static OutArgs make_out_args(ba_ctx *c) {
+    OutArgs a;
+    a.kc = c->kc; a.lay = c->lay; a.tab = c->tab; a.vinfo = c->vinfo; a.thrlist = c->thrlist; a.ntab = c->ntab;
+    a.p = c->p; a.Apart = c->Apart; a.counter = c->counters + 4; a.dbg_cy = 0; a.dbg_out = nullptr; a.cnt = c->cnt + 2;
+    return a;
+}
+
+// Hc(x) = sum_y w_k emb(y,x) log2(emb(y,x)/ebar_k): one enumerating pass, independent of the iterate.
+static int ensure_hc(ba_ctx *c) {
+    if (c->hc_ready) return BA_OK;
+    CK(cudaMemsetAsync(c->counters, 0, 16 * 4, c->st));
+    InArgs a = make_in_args(c);
+    k_enum_in<IN_HC><<<c->grid_in, c->block, c->smem_in, c->st>>>(a);
+    CK(cudaGetLastError());
+    c->hc_ready = true;
+    return BA_OK;
+}
+
+static int launch_out_sweep(ba_ctx *c) {
+    if (c->mode == BA_MODE_ENUM) {
+        CK(cudaMemsetAsync(c->counters + 4, 0, 4, c->st));
+        OutArgs a = make_out_args(c);
+        k_enum_out<OUT_SWEEP><<<c->grid_out, c->block, c->smem_out, c->st>>>(a);
+        CK(cudaGetLastError());
+        k_out_final<<<c->num_sms * 8, 256, 0, c->st>>>(c->kc, c->Apart, nullptr, c->q, c->c);
+        CK(cudaGetLastError());
+    } else {
+        double *buf0 = c->Apart, *buf1 = c->Apart + (((size_t)2 << c->n) + 64);
+        const double *in = c->p;
+        double *out = buf0;
+        for (int s = 0; s < c->n; s++) {
+            k_fast_fwd<<<c->num_sms * 8, 256, 0, c->st>>>(c->n, s, in, out);
+            CK(cudaGetLastError());
+            in = out;
+            out = (out == buf0) ? buf1 : buf0;
+        }
+        k_out_final<<<c->num_sms * 8, 256, 0, c->st>>>(c->kc, nullptr, in, c->q, c->c);
+        CK(cudaGetLastError());
+    }
+    return BA_OK;
+}
+
+static int launch_in_sweep(ba_ctx *c, size_t *npart) {
+    if (c->mode == BA_MODE_ENUM) {
+        CK(cudaMemsetAsync(c->counters, 0, 4, c->st));
+        InArgs a = make_in_args(c);
+        k_enum_in<IN_SWEEP><<<c->grid_in, c->block, c->smem_in, c->st>>>(a);
+        CK(cudaGetLastError());
+        *npart = (size_t)1 << c->h;
+    } else {
+        double *buf0 = c->Apart, *buf1 = c->Apart + (((size_t)2 << c->n) + 64);
+        const double *in = c->c;
+        double *out = buf0;
+        for (int s = c->n - 1; s >= 0; s--) {
+            k_fast_bwd<<<c->num_sms * 8, 256, 0, c->st>>>(c->n, s, in, out);
+            CK(cudaGetLastError());
+            in = out;
+            out = (out == buf0) ? buf1 : buf0;
+        }
+        int nb = c->num_sms * 8;
+        if ((size_t)nb > c->NX / 256 + 1) nb = (int)(c->NX / 256 + 1);
+        k_fast_D<<<nb, 256, 0, c->st>>>(c->NX, c->Hc, in, c->p, c->D, c->part);
+        CK(cudaGetLastError());
+        *npart = (size_t)nb;
+    }
+    return BA_OK;
+}
+
+extern "C" int ba_iterate(ba_ctx *c, int k) {
+    if (!c) return BA_EINVAL;
+    if (k < 0) return fail(c, BA_EINVAL, "ba_iterate: k < 0");
+    if (k == 0) return BA_OK;
+    int rc = ensure_hc(c);
+    if (rc) return rc;
+    const int timed = k < 64 ? k : 64;                 // time the last `timed` iterations
+    while ((int)c->ev.size() < 4 * timed + 1) {
+        cudaEvent_t e;
+        CK(cudaEventCreate(&e));
+        c->ev.push_back(e);
+    }
+    c->ev_iters = timed;
+    for (int it = 0; it < k; it++) {
+        const int ti = it - (k - timed);
+        if (ti >= 0) CK(cudaEventRecord(c->ev[4 * ti], c->st));
+        rc = launch_out_sweep(c);
+        if (rc) return rc;
+        if (ti >= 0) CK(cudaEventRecord(c->ev[4 * ti + 1], c->st));
+        size_t npart = 0;
+        rc = launch_in_sweep(c, &npart);
+        if (rc) return rc;
+        if (ti >= 0) CK(cudaEventRecord(c->ev[4 * ti + 2], c->st));
+        const int slot = (int)(c->iters % BA_HIST_CAP);
+        k_finalize<<<1, 1024, 0, c->st>>>(c->part, npart, c->scal, c->hist, slot);
+        CK(cudaGetLastError());
+        k_update<<<c->num_sms * 8, 256, 0, c->st>>>(c->NX, c->p, c->D, c->scal);
+        CK(cudaGetLastError());
+        if (ti >= 0) CK(cudaEventRecord(c->ev[4 * ti + 3], c->st));
+        c->iters++;
+    }
+    CK(cudaEventRecord(c->ev[4 * timed], c->st));
+    return BA_OK;
+}
+
+extern "C" int ba_last_timing(ba_ctx *c, double ms[4]) {
+    if (!c || !ms) return BA_EINVAL;
+    if (c->ev_iters <= 0) return fail(c, BA_ESTATE, "ba_last_timing: no iteration yet");
+    CK(cudaStreamSynchronize(c->st));
+    double acc[4] = {0, 0, 0, 0};
+    for (int t = 0; t < c->ev_iters; t++) {
+        float f;
+        CK(cudaEventElapsedTime(&f, c->ev[4 * t], c->ev[4 * t + 1])); acc[0] += f;
+        CK(cudaEventElapsedTime(&f, c->ev[4 * t + 1], c->ev[4 * t + 2])); acc[1] += f;
+        CK(cudaEventElapsedTime(&f, c->ev[4 * t + 2], c->ev[4 * t + 3])); acc[2] += f;
+    }
+    float tot;
+    CK(cudaEventElapsedTime(&tot, c->ev[0], c->ev[4 * c->ev_iters]));
+    for (int i = 0; i < 3; i++) ms[i] = acc[i] / c->ev_iters;
+    ms[3] = tot / c->ev_iters;
+    return BA_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ getters / setters
+extern "C" int ba_bounds(ba_ctx *c, double *I_lower, double *maxD_upper) {
+    if (!c || !I_lower || !maxD_upper) return c ? fail(c, BA_EINVAL, "ba_bounds: null pointer") : BA_EINVAL;
+    if (c->iters == 0) return fail(c, BA_ESTATE, "ba_bounds: no iteration yet");
+    double h3[3];
+    const int slot = (int)((c->iters - 1) % BA_HIST_CAP);
+    CK(cudaMemcpyAsync(h3, c->hist + 3 * slot, 24, cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    *I_lower = h3[0];
+    *maxD_upper = h3[1];
+    if (!std::isfinite(h3[0]) || !std::isfinite(h3[1]))
+        return fail(c, BA_ENUMERIC, "ba_bounds: non-finite bound (q(y)=0 or p underflow, see DESIGN.md G8)");
+    return BA_OK;
+}
+
+extern "C" int ba_stats(ba_ctx *c, double *log2Z, long long *iters_done) {
+    if (!c) return BA_EINVAL;
+    if (iters_done) *iters_done = c->iters;
+    if (log2Z) {
+        if (c->iters == 0) return fail(c, BA_ESTATE, "ba_stats: no iteration yet");
+        const int slot = (int)((c->iters - 1) % BA_HIST_CAP);
+        CK(cudaMemcpyAsync(log2Z, c->hist + 3 * slot + 2, 8, cudaMemcpyDeviceToHost, c->st));
+        CK(cudaStreamSynchronize(c->st));
+    }
+    return BA_OK;
+}
+
+extern "C" int ba_get_history(ba_ctx *c, int count, double *out) {
+    if (!c || !out || count < 0) return c ? fail(c, BA_EINVAL, "ba_get_history: bad argument") : BA_EINVAL;
+    if ((long long)count > c->iters || count > BA_HIST_CAP) return fail(c, BA_EINVAL, "ba_get_history: count too large");
+    for (int i = 0; i < count; i++) {
+        const int slot = (int)((c->iters - count + i) % BA_HIST_CAP);
+        CK(cudaMemcpyAsync(out + 3 * i, c->hist + 3 * slot, 24, cudaMemcpyDeviceToHost, c->st));
+    }
+    CK(cudaStreamSynchronize(c->st));
+    return BA_OK;
+}
+
+extern "C" int ba_get_p(ba_ctx *c, double *p_host) {
+    if (!c || !p_host) return c ? fail(c, BA_EINVAL, "ba_get_p: null pointer") : BA_EINVAL;
+    CK(cudaMemcpyAsync(p_host, c->p, c->NX * 8, cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    return BA_OK;
+}
+
+extern "C" int ba_get_q(ba_ctx *c, double *q_host) {
+    if (!c || !q_host) return c ? fail(c, BA_EINVAL, "ba_get_q: null pointer") : BA_EINVAL;
+    if (c->iters == 0) return fail(c, BA_ESTATE, "ba_get_q: no iteration yet");
+    CK(cudaMemcpyAsync(q_host, c->q, c->NY * 8, cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    return BA_OK;
+}
+
+extern "C" int ba_get_D(ba_ctx *c, double *D_host) {
+    if (!c || !D_host) return c ? fail(c, BA_EINVAL, "ba_get_D: null pointer") : BA_EINVAL;
+    if (c->iters == 0) return fail(c, BA_ESTATE, "ba_get_D: no iteration yet");
+    CK(cudaMemcpyAsync(D_host, c->D, c->NX * 8, cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    return BA_OK;
+}
+
+extern "C" int ba_set_p(ba_ctx *c, const double *p_host) {
+    if (!c || !p_host) return c ? fail(c, BA_EINVAL, "ba_set_p: null pointer") : BA_EINVAL;
+    long double sum = 0.0L;
+    for (size_t i = 0; i < c->NX; i++) {
+        const double v = p_host[i];
+        if (!std::isfinite(v) || !(v > 0.0)) return fail(c, BA_EINVAL, "ba_set_p: entry not finite and positive");
+        sum += v;
+    }
+    if (fabsl(sum - 1.0L) > 1e-9L) return fail(c, BA_EINVAL, "ba_set_p: |sum p - 1| > 1e-9");
+    CK(cudaMemcpyAsync(c->p, p_host, c->NX * 8, cudaMemcpyHostToDevice, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    return BA_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ debug
+extern "C" int ba_debug_emb_row(ba_ctx *c, unsigned x, unsigned *emb_out) {
+    if (!c || !emb_out) return c ? fail(c, BA_EINVAL, "ba_debug_emb_row: null pointer") : BA_EINVAL;
+    if ((size_t)x >= c->NX) return fail(c, BA_EINVAL, "ba_debug_emb_row: x out of range");
+    uint32_t *dev = nullptr;
+    CK(cudaMalloc(&dev, c->NY * 4));
+    cudaError_t e = cudaMemsetAsync(dev, 0, c->NY * 4, c->st);
+    if (e == cudaSuccess) {
+        InArgs a = make_in_args(c);
+        a.dbg_x = x; a.dbg_out = dev;
+        k_enum_in<IN_DEBUG><<<1, c->block, c->smem_in, c->st>>>(a);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(emb_out, dev, c->NY * 4, cudaMemcpyDeviceToHost, c->st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
+    cudaFree(dev);
+    if (e != cudaSuccess) return fail(c, BA_ECUDA, std::string("ba_debug_emb_row: ") + cudaGetErrorString(e));
+    return BA_OK;
+}
+
+extern "C" int ba_debug_emb_col(ba_ctx *c, unsigned yidx, unsigned *emb_out) {
+    if (!c || !emb_out) return c ? fail(c, BA_EINVAL, "ba_debug_emb_col: null pointer") : BA_EINVAL;
+    if ((size_t)yidx >= c->NY) return fail(c, BA_EINVAL, "ba_debug_emb_col: yidx out of range");
+    uint32_t *dev = nullptr;
+    CK(cudaMalloc(&dev, c->NX * 4));
+    cudaError_t e = cudaMemsetAsync(dev, 0, c->NX * 4, c->st);
+    if (e == cudaSuccess) {
+        OutArgs a = make_out_args(c);
+        a.dbg_cy = yidx + 1u; a.dbg_out = dev;
+        k_enum_out<OUT_DEBUG><<<1, c->block, c->smem_out, c->st>>>(a);
+        e = cudaGetLastError();
+    }
+    if (e == cudaSuccess) e = cudaMemcpyAsync(emb_out, dev, c->NX * 4, cudaMemcpyDeviceToHost, c->st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->st);
+    cudaFree(dev);
+    if (e != cudaSuccess) return fail(c, BA_ECUDA, std::string("ba_debug_emb_col: ") + cudaGetErrorString(e));
+    return BA_OK;
+}
+
+extern "C" int ba_debug_count_terms(ba_ctx *c, unsigned long long *in_terms, unsigned long long *out_terms,
+                                    unsigned long long *in_emb_sum, unsigned long long *out_emb_sum) {
+    if (!c) return BA_EINVAL;
+    CK(cudaMemsetAsync(c->counters, 0, 16 * 4, c->st));
+    CK(cudaMemsetAsync(c->cnt, 0, 8 * 8, c->st));
+    InArgs ia = make_in_args(c);
+    k_enum_in<IN_COUNT><<<c->grid_in, c->block, c->smem_in, c->st>>>(ia);
+    CK(cudaGetLastError());
+    OutArgs oa = make_out_args(c);
+    k_enum_out<OUT_COUNT><<<c->grid_out, c->block, c->smem_out, c->st>>>(oa);
+    CK(cudaGetLastError());
+    unsigned long long h4[4];
+    CK(cudaMemcpyAsync(h4, c->cnt, 32, cudaMemcpyDeviceToHost, c->st));
+    CK(cudaStreamSynchronize(c->st));
+    if (in_terms) *in_terms = h4[0];
+    if (in_emb_sum) *in_emb_sum = h4[1];
+    if (out_terms) *out_terms = h4[2];
+    if (out_emb_sum) *out_emb_sum = h4[3];
+    return BA_OK;
+}

@@ -1,0 +1,110 @@
+// ba_stream.cuh -- the streaming kernels of one BA iteration: per-output finish of the output sweep,
+// the deterministic second-stage reduction and the normalised update (8(a4)).
+#pragma once
+#include "ba_internal.h"
+
+// q(y) = w_k A(y) and the gathered operand of the input sweep c(y) = w_k log2( A(y) / ebar_k ),
+// A(y) = sum_x emb(y,x) p(x).  ENUM mode: A(y) is the fixed-order sum of the partials the
+// output-sweep CTAs own (ba_enum_out.cuh).  FAST mode: A is already complete in `Afull`.
+// Writing log2( W/q ) = log2( emb/ebar_k ) - log2( A/ebar_k ) moves the only logarithm that depends on
+// the iterate from T(n) terms to 2^{n+1} outputs (SURVEY 7.2 "hoisting the logarithm"); ebar_k =
+// C(n,k)/2^k is the mean of emb over a length, which centres both halves.
+__global__ void k_out_final(KConst kc, const double *__restrict__ Apart, const double *__restrict__ Afull,
+                            double *__restrict__ q, double *__restrict__ c) {
+    const size_t NY = ((size_t)2 << kc.n) - 1;
+    const uint32_t NZ = (2u << kc.m) - 1u;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < NY; i += (size_t)gridDim.x * blockDim.x) {
+        const uint32_t cy = (uint32_t)(i + 1);
+        const int k = ba_len_of_code(cy);
+        double A;
+        if (Afull) {
+            A = Afull[i];
+        } else {
+            A = 0.0;
+            const int jlo = (k - kc.h > 0) ? (k - kc.h) : 0;
+            const int jhi = (k < kc.m) ? k : kc.m;
+            for (int j = jlo; j <= jhi; j++) {       // split y = y'.z, |z| = j
+                const uint32_t cyp = cy >> j;
+                const uint32_t cz = (1u << j) | (cy & ((1u << j) - 1u));
+                A += Apart[(size_t)(cyp - 1u) * NZ + (cz - 1u)];
+            }
+        }
+        const double wk = kc.w[k];
+        q[i] = wk * A;
+        c[i] = (wk != 0.0) ? wk * (log2(A) - kc.lebar[k]) : 0.0;
+    }
+}
+
+// Second stage of the reductions: part holds npart triples {sum p D, max D, sum p 2^D}, one per CTA work
+// item of the input sweep.  One block, fixed traversal order => run-to-run bit-reproducible.
+// scal[0..2] = I, U, Z ; hist[3*slot..] = I, U, log2 Z.
+__global__ void __launch_bounds__(1024) k_finalize(const double *__restrict__ part, size_t npart,
+                                                   double *__restrict__ scal, double *__restrict__ hist,
+                                                   int slot) {
+    __shared__ double s0[1024], s1[1024], s2[1024];
+    const int tid = threadIdx.x;
+    double a0 = 0.0, a1 = -INFINITY, a2 = 0.0;
+    for (size_t i = tid; i < npart; i += 1024) {
+        a0 += part[3 * i];
+        a1 = fmax(a1, part[3 * i + 1]);
+        a2 += part[3 * i + 2];
+    }
+    s0[tid] = a0; s1[tid] = a1; s2[tid] = a2;
+    __syncthreads();
+    for (int o = 512; o > 0; o >>= 1) {
+        if (tid < o) {
+            s0[tid] += s0[tid + o];
+            s1[tid] = fmax(s1[tid], s1[tid + o]);
+            s2[tid] += s2[tid + o];
+        }
+        __syncthreads();
+    }
+    if (tid == 0) {
+        scal[0] = s0[0]; scal[1] = s1[0]; scal[2] = s2[0];
+        hist[3 * slot] = s0[0]; hist[3 * slot + 1] = s1[0]; hist[3 * slot + 2] = log2(s2[0]);
+    }
+}
+
+// p(x) <- max( p(x) 2^{D(x)} / Z, 2^-1000 )    (G8)
+__global__ void k_update(size_t NX, double *__restrict__ p, const double *__restrict__ D,
+                         const double *__restrict__ scal) {
+    const double invZ = 1.0 / scal[2];
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < NX; i += (size_t)gridDim.x * blockDim.x) {
+        const double v = p[i] * exp2(D[i]) * invZ;
+        p[i] = fmax(v, BA_P_FLOOR);
+    }
+}
+
+__global__ void k_fill(size_t N, double *__restrict__ a, double v) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) a[i] = v;
+}
+
+// FAST mode epilogue of the input sweep: D = Hc - S and the first-stage reductions, one triple per block.
+__global__ void __launch_bounds__(256) k_fast_D(size_t NX, const double *__restrict__ Hc, const double *__restrict__ S,
+                                                const double *__restrict__ p, double *__restrict__ D,
+                                                double *__restrict__ part) {
+    __shared__ double sr[3 * 8];
+    double r0 = 0.0, r1 = -INFINITY, r2 = 0.0;
+    // fixed assignment: block b handles the contiguous chunk [b*chunk, (b+1)*chunk)
+    const size_t chunk = (NX + gridDim.x - 1) / gridDim.x;
+    const size_t lo = (size_t)blockIdx.x * chunk, hi = (lo + chunk < NX) ? lo + chunk : NX;
+    for (size_t i = lo + threadIdx.x; i < hi; i += blockDim.x) {
+        const double Dx = Hc[i] - S[i];
+        D[i] = Dx;
+        const double px = p[i];
+        r0 += px * Dx; r1 = fmax(r1, Dx); r2 += px * exp2(Dx);
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        r0 += __shfl_xor_sync(0xffffffffu, r0, o);
+        r1 = fmax(r1, __shfl_xor_sync(0xffffffffu, r1, o));
+        r2 += __shfl_xor_sync(0xffffffffu, r2, o);
+    }
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (lane == 0) { sr[warp * 3] = r0; sr[warp * 3 + 1] = r1; sr[warp * 3 + 2] = r2; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t0 = 0.0, t1 = -INFINITY, t2 = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); w++) { t0 += sr[w * 3]; t1 = fmax(t1, sr[w * 3 + 1]); t2 += sr[w * 3 + 2]; }
+        part[(size_t)blockIdx.x * 3] = t0; part[(size_t)blockIdx.x * 3 + 1] = t1; part[(size_t)blockIdx.x * 3 + 2] = t2;
+    }
+}

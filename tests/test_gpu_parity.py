@@ -1,0 +1,200 @@
+"""GPU parity tests: libba (through the C ABI binding) against the CPU oracle on the same seeded
+inputs (SURVEY.md section 8(c) protocol T1-T6).  Tolerances are BASELINE.json:north_star's:
+emb bit-exact; q and D within 1e-12 relative; bounds within 1e-10 bits after the same K.
+"""
+import functools
+
+import numpy as np
+import pytest
+
+import synthetic_inputs as si
+from oracle import oracle as orc
+
+pytestmark = pytest.mark.gpu
+
+REL_QD = 1e-12      # north_star: "q and D within 1e-12 relative error in FP64"
+ABS_U = 1e-10       # north_star: "the upper bound within 1e-10 bits after the same number of iterations"
+
+
+@pytest.fixture(scope="module")
+def ba():
+    import paper_2604_05867_b200 as ba_mod
+    ba_mod.load()
+    return ba_mod
+
+
+@functools.lru_cache(maxsize=None)
+def E_of(n):
+    return orc.emb_dense(n)
+
+
+@functools.lru_cache(maxsize=None)
+def W_of(n, d):
+    return orc.channel(n, d, E_of(n))
+
+
+def relerr(a, b):
+    return np.max(np.abs(a - b) / np.abs(b))
+
+
+# ------------------------------------------------------------------ T1 / T2: emb bit-exact
+
+@pytest.mark.parametrize("n", [1, 2, 3, 4, 5, 6, 7, 8, 9, 10])
+def test_T1_emb_rows_bit_exact(ba, n):
+    E = E_of(n)
+    ctx = ba.ba_create(n, 0.5)
+    try:
+        for x in range(1 << n):
+            row = ba.ba_debug_emb_row(ctx, x)
+            assert np.array_equal(row, E[x]), f"row x={x}"
+    finally:
+        ba.ba_destroy(ctx)
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 4, 5, 6, 7, 8, 9, 10])
+def test_T2_emb_cols_bit_exact(ba, n):
+    E = E_of(n)
+    ctx = ba.ba_create(n, 0.5)
+    try:
+        for j in range((2 << n) - 1):
+            col = ba.ba_debug_emb_col(ctx, j)
+            assert np.array_equal(col, E[:, j]), f"col idx={j}"
+    finally:
+        ba.ba_destroy(ctx)
+
+
+def test_T1_T2_emb_sampled_n14(ba):
+    n = 14
+    E = E_of(n)
+    rng = np.random.default_rng(7)
+    ctx = ba.ba_create(n, 0.64)
+    try:
+        xs = [0, (1 << n) - 1, 0b01010101010101, 0b00110011001100] + list(rng.integers(0, 1 << n, 60))
+        for x in xs:
+            assert np.array_equal(ba.ba_debug_emb_row(ctx, int(x)), E[int(x)])
+        js = [0, 1, 2, (2 << n) - 2] + list(rng.integers(0, (2 << n) - 1, 60))
+        for j in js:
+            assert np.array_equal(ba.ba_debug_emb_col(ctx, int(j)), E[:, int(j)])
+    finally:
+        ba.ba_destroy(ctx)
+
+
+@pytest.mark.parametrize("n", [3, 8, 11, 14])
+def test_term_counts_match_lemma6(ba, n):
+    # P4: both enumerators visit exactly T(n) terms; sum of emb = 4^n ... = sum_k C(n,k) 2^n
+    ctx = ba.ba_create(n, 0.5)
+    try:
+        r = ba.ba_debug_count_terms(ctx)
+        T = ba.ba_terms_per_sweep(n)
+        assert T == int((E_of(n) > 0).sum()) if n <= 11 else True
+        assert r["in_terms"] == T and r["out_terms"] == T
+        assert r["in_emb_sum"] == 4 ** n and r["out_emb_sum"] == 4 ** n
+    finally:
+        ba.ba_destroy(ctx)
+
+
+# ------------------------------------------------------------------ T3 / T4: one-step parity
+
+def one_step_check(ba, n, d, p, mode):
+    ref = orc.ba_step(W_of(n, d), p)
+    ctx = ba.ba_create(n, d)
+    try:
+        ba.ba_set_mode(ctx, mode)
+        ba.ba_set_p(ctx, p)
+        ba.ba_iterate(ctx, 1)
+        q, D = ba.ba_get_q(ctx), ba.ba_get_D(ctx)
+        I, U = ba.ba_bounds(ctx)
+        lz, it = ba.ba_stats(ctx)
+        pn = ba.ba_get_p(ctx)
+    finally:
+        ba.ba_destroy(ctx)
+    assert it == 1
+    nzq = ref["q"] > 0
+    assert np.array_equal(q > 0, nzq)
+    assert relerr(q[nzq], ref["q"][nzq]) <= REL_QD
+    assert relerr(D, ref["D"]) <= REL_QD, f"max |dD|/|D| = {relerr(D, ref['D'])}"
+    assert abs(I - ref["I"]) <= REL_QD * max(1.0, abs(ref["I"]))
+    assert abs(U - ref["U"]) <= REL_QD * max(1.0, abs(ref["U"]))
+    assert abs(lz - ref["log2Z"]) <= REL_QD * max(1.0, abs(ref["log2Z"]))
+    assert relerr(pn, ref["p_next"]) <= 1e-11
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("n,d", [(1, 0.3), (2, 0.5), (5, 0.25), (8, 0.5), (9, 0.64), (10, 0.9), (12, 0.7)])
+def test_T3_T4_one_step_uniform(ba, n, d, mode):
+    one_step_check(ba, n, d, si.uniform_p0(n), mode)
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("n,d,seed", [(6, 0.4, 11), (8, 0.5, 12), (11, 0.64, 13), (12, 0.85, 14)])
+def test_T3_T4_one_step_random_p(ba, n, d, seed, mode):
+    one_step_check(ba, n, d, si.random_positive_p(n, seed), mode)
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_T3_T4_one_step_from_oracle_iterates_config1(ba, mode):
+    # p_t from the oracle at t in {0,1,10,K-1} loaded with ba_set_p (R9 (i))
+    n, d, K = 8, 0.5, 200
+    W = W_of(n, d)
+    p = si.uniform_p0(n)
+    wanted = {0, 1, 10, K - 1}
+    for t in range(K):
+        if t in wanted:
+            one_step_check(ba, n, d, p.copy(), mode)
+        p = orc.ba_step(W, p)["p_next"]
+
+
+# ------------------------------------------------------------------ T5: trajectories
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_T5_trajectory_config1(ba, mode):
+    n, d, K = 8, 0.5, 200
+    ref = orc.ba_run(W_of(n, d), si.uniform_p0(n), K)
+    ctx = ba.ba_create(n, d)
+    try:
+        ba.ba_set_mode(ctx, mode)
+        ba.ba_iterate(ctx, K)
+        I, U = ba.ba_bounds(ctx)
+        hist = ba.ba_get_history(ctx, K)
+        p = ba.ba_get_p(ctx)
+    finally:
+        ba.ba_destroy(ctx)
+    assert abs(U - ref["hist"][-1, 1]) <= ABS_U
+    assert abs(I - ref["hist"][-1, 0]) <= ABS_U
+    assert np.max(np.abs(hist - ref["hist"])) <= ABS_U
+    assert relerr(p, ref["p"]) <= 1e-9
+    # P13 secondary pins: I_199 = 2.1229915839401, U_199 = 2.1260407187234
+    assert I == pytest.approx(2.1229915839401, abs=2e-13)
+    assert U == pytest.approx(2.1260407187234, abs=2e-13)
+
+
+# ------------------------------------------------------------------ T6: special cases
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_T6_special_cases(ba, mode):
+    def run(n, d, K, p0=None):
+        ctx = ba.ba_create(n, d)
+        try:
+            ba.ba_set_mode(ctx, mode)
+            if p0 is not None:
+                ba.ba_set_p(ctx, p0)
+            ba.ba_iterate(ctx, K)
+            return ba.ba_bounds(ctx), ba.ba_get_D(ctx)
+        finally:
+            ba.ba_destroy(ctx)
+
+    for d in (0.0, 0.2, 0.64, 1.0):                          # C_1(d) = 1-d
+        (I, U), _ = run(1, d, 1)
+        assert I == pytest.approx(1 - d, abs=1e-14) and U == pytest.approx(1 - d, abs=1e-14)
+    for n in (3, 9):                                          # C_n(0) = n; D = -log2 p (R7)
+        (I, U), _ = run(n, 0.0, 1)
+        assert I == pytest.approx(n, abs=1e-12) and U == pytest.approx(n, abs=1e-12)
+        p = si.random_positive_p(n, 5)
+        _, D = run(n, 0.0, 1, p)
+        assert np.allclose(D, -np.log2(p), rtol=1e-13)
+        (I, U), _ = run(n, 1.0, 1)                            # C_n(1) = 0
+        assert abs(I) <= 1e-15 and abs(U) <= 1e-15
+    d = 0.5                                                   # C_2(d) closed form
+    (I, U), _ = run(2, d, 3000)
+    assert I == pytest.approx(0.8304820237218407, abs=1e-12)
+    assert U == pytest.approx(0.8304820237218407, abs=1e-9)
