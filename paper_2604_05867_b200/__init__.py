@@ -177,8 +177,12 @@ def ba_last_timing(ctx):
     return dict(out_ms=ms[0], in_ms=ms[1], update_ms=ms[2], iter_ms=ms[3])
 
 
-def ba_get_p(ctx):
-    out = np.empty(1 << ctx.n, dtype=np.float64)
+def ba_get_p(ctx, out=None):
+    """p (2^n doubles) into a new array, or into `out` (e.g. the numpy view of a pinned buffer)."""
+    if out is None:
+        out = np.empty(1 << ctx.n, dtype=np.float64)
+    elif out.dtype != np.float64 or out.shape != (1 << ctx.n,) or not out.flags.c_contiguous:
+        raise BAError(BA_EINVAL, "ba_get_p: out must be a contiguous float64 array of 2^n entries")
     _check(ctx, load().ba_get_p(ctx.handle, _dp(out)))
     return out
 
