@@ -2,6 +2,7 @@
 // Unity build: the kernels live in the .cuh files included below.
 #include "../../include/ba.h"
 #include "ba_internal.h"
+#include "ba_tables.h"
 #include "ba_enum_in.cuh"
 #include "ba_enum_out.cuh"
 #include "ba_stream.cuh"
@@ -19,16 +20,16 @@ struct ba_ctx {
     double d = 0.0;
     size_t NX = 0, NY = 0, NZ = 0, napart = 0;
     KConst kc;
-    OutLayout lay;
-    int ntab = 0;
+    int nT64 = 0, nTz = 0, n_in_csr = 0, n_out_csr = 0;
     cudaStream_t st = nullptr;
     bool own_buffers = false, own_stream = false;
     double *p = nullptr, *q = nullptr, *D = nullptr;
     unsigned char *scratch = nullptr;
     // carved from scratch
     double *c = nullptr, *Hc = nullptr, *Apart = nullptr, *part = nullptr, *scal = nullptr, *hist = nullptr;
-    uint32_t *tab = nullptr, *vinfo = nullptr;
-    uint16_t *thrlist = nullptr;
+    uint2 *T64 = nullptr, *Tz = nullptr, *in_desc = nullptr, *out_desc = nullptr;
+    uint32_t *Wv = nullptr, *vbase = nullptr;
+    uint16_t *in_csr_off = nullptr, *in_csr_idx = nullptr, *out_csr_off = nullptr, *out_csr_idx = nullptr;
     unsigned int *counters = nullptr;
     unsigned long long *cnt = nullptr;
     size_t npart_cap = 0;
@@ -57,109 +58,23 @@ static int fail(ba_ctx *c, int code, const std::string &msg) {
 
 static size_t align256(size_t b) { return (b + 255) & ~(size_t)255; }
 
-// ------------------------------------------------------------------------------------------------ host tables
-static uint32_t host_emb(uint32_t z, int lz, uint32_t v, int lv) {   // #embeddings of z in v
-    std::vector<uint32_t> e(lz + 1, 0);
-    e[0] = 1;
-    for (int i = 0; i < lv; i++) {
-        uint32_t vb = (v >> (lv - 1 - i)) & 1u;
-        for (int r = lz; r >= 1; r--)
-            if (((z >> (lz - r)) & 1u) == vb) e[r] += e[r - 1];
-    }
-    return e[lz];
-}
-
+// ------------------------------------------------------------------------------------------------ host helpers
 static double host_binom(int n, int k) {
     double r = 1.0;
     for (int i = 1; i <= k; i++) r = r * (double)(n - k + i) / (double)i;
     return std::floor(r + 0.5);
 }
 
-struct LowTables {
-    std::vector<uint32_t> words, vinfo;
-    std::vector<uint16_t> thrlist;
-    OutLayout lay;
-};
-
-// Low table of the m-bit deletion channel (ba_internal.h) and the output-sweep thread assignment.
-static void build_low_tables(int m, LowTables &T) {
-    const int nv = 1 << m;
-    T.words.clear();
-    T.vinfo.assign(nv, 0);
-    std::vector<std::vector<int>> local_of_code(nv);       // code(z) -> local index in v's list, -1 if absent
-    for (int v = 0; v < nv; v++) {
-        std::vector<uint32_t> codes[3];                    // empty / starts with 0 / starts with 1
-        std::vector<uint32_t> Bs[3];
-        for (int lz = 0; lz <= m; lz++)
-            for (uint32_t z = 0; z < (1u << lz); z++) {
-                uint32_t B = host_emb(z, lz, (uint32_t)v, m);
-                if (!B) continue;
-                int blk = (lz == 0) ? 0 : 1 + (int)((z >> (lz - 1)) & 1u);
-                codes[blk].push_back((1u << lz) | z);
-                Bs[blk].push_back(B);
-            }
-        std::vector<uint32_t> code_list, B_list;
-        for (int blk = 0; blk < 3; blk++)
-            for (size_t i = 0; i < codes[blk].size(); i++) { code_list.push_back(codes[blk][i]); B_list.push_back(Bs[blk][i]); }
-        local_of_code[v].assign((size_t)2 << m, -1);
-        for (size_t i = 0; i < code_list.size(); i++) local_of_code[v][code_list[i]] = (int)i;
-        uint32_t base = (uint32_t)T.words.size();
-        T.vinfo[v] = base | ((uint32_t)codes[1].size() << 14) | ((uint32_t)codes[2].size() << 21);
-        for (size_t i = 0; i < code_list.size(); i++) {
-            uint32_t cz = code_list[i];
-            int lz = 31 - __builtin_clz(cz);
-            uint32_t zval = cz - (1u << lz);
-            uint32_t link[2] = {BA_LINK_NONE, BA_LINK_NONE};
-            if (lz + 1 <= m)
-                for (uint32_t b = 0; b < 2; b++) {
-                    uint32_t cbz = (1u << (lz + 1)) | (b << lz) | zval;
-                    int li = local_of_code[v][cbz];
-                    if (li >= 0) link[b] = (uint32_t)li;
-                }
-            T.words.push_back(cz | (B_list[i] << 9) | (link[0] << 16) | (link[1] << 23));
-        }
-    }
-    // output-sweep assignment: class j = outputs z of length j; the 2^{m-j} threads tid with
-    // (tid >> (m-j)) == val(z) share the supersequences v of z (ascending v, dealt round-robin).
-    int total = 0;
-    for (int j = 0; j <= BA_MLOW + 1; j++) T.lay.off[j] = 0;
-    for (int j = 0; j <= BA_MLOW; j++) T.lay.slots[j] = 0;
-    for (int j = 0; j <= m; j++) {
-        int L = 0;
-        for (int i = 0; i <= m - j; i++) L += (int)host_binom(m, i);   // Lemma 6
-        int G = 1 << (m - j);
-        T.lay.slots[j] = (j == 0) ? 0 : (L + G - 1) / G;               // class 0 is handled in-line
-        T.lay.off[j] = total;
-        total += T.lay.slots[j];
-    }
-    for (int j = m + 1; j <= BA_MLOW + 1; j++) T.lay.off[j] = total;
-    T.thrlist.assign((size_t)total * nv, 0);
-    for (int j = 1; j <= m; j++) {
-        int G = 1 << (m - j);
-        for (uint32_t z = 0; z < (1u << j); z++) {
-            uint32_t cz = (1u << j) | z;
-            int cntv = 0;
-            for (int v = 0; v < nv; v++) {
-                int li = local_of_code[v][cz];
-                if (li < 0) continue;
-                int g = cntv % G, k = cntv / G;
-                int tid = (int)(z << (m - j)) + g;
-                T.thrlist[(size_t)(T.lay.off[j] + k) * nv + tid] = (uint16_t)((uint32_t)v | ((uint32_t)li << 8) | 0x8000u);
-                cntv++;
-            }
-        }
-    }
-}
-
 // ------------------------------------------------------------------------------------------------ scratch layout
 struct ScratchLayout {
-    size_t c, Hc, Apart, part, scal, hist, tab, vinfo, thrlist, counters, cnt, total;
+    size_t c, Hc, Apart, part, scal, hist, T64, Tz, Wv, vbase, in_desc, out_desc, in_csr_off, in_csr_idx, out_csr_off,
+        out_csr_idx, counters, cnt, total;
     size_t napart, npart_cap;
 };
 
 static int low_m(int n) { return n < BA_MLOW ? n : BA_MLOW; }
 
-static void scratch_layout(int n, size_t ntab, size_t nthrlist, ScratchLayout &L) {
+static void scratch_layout(int n, const TileTables &T, ScratchLayout &L) {
     const int m = low_m(n), h = n - m;
     const size_t NX = (size_t)1 << n, NY = ((size_t)2 << n) - 1, NZ = ((size_t)2 << m) - 1;
     L.napart = (((size_t)2 << h) - 1) * NZ;
@@ -167,15 +82,22 @@ static void scratch_layout(int n, size_t ntab, size_t nthrlist, ScratchLayout &L
     if (L.napart < fastwords) L.napart = fastwords;
     L.npart_cap = ((size_t)1 << h) > 8192 ? ((size_t)1 << h) : 8192;
     size_t o = 0;
-    L.c = o; o += align256(NY * 8);
+    L.c = o; o += align256((NY + 1) * 8);                    // c[code], entry 0 unused
     L.Hc = o; o += align256(NX * 8);
     L.Apart = o; o += align256(L.napart * 8);
     L.part = o; o += align256(L.npart_cap * 3 * 8);
     L.scal = o; o += align256(8 * 8);
     L.hist = o; o += align256((size_t)BA_HIST_CAP * 3 * 8);
-    L.tab = o; o += align256(ntab * 4);
-    L.vinfo = o; o += align256(((size_t)1 << m) * 4);
-    L.thrlist = o; o += align256(nthrlist * 2);
+    L.T64 = o; o += align256(T.T64.size() * 8);
+    L.Tz = o; o += align256(T.Tz.size() * 8);
+    L.Wv = o; o += align256(T.Wv.size() * 4);
+    L.vbase = o; o += align256(T.vbase.size() * 4);
+    L.in_desc = o; o += align256(T.in_desc.size() * 8);
+    L.out_desc = o; o += align256(T.out_desc.size() * 8);
+    L.in_csr_off = o; o += align256(T.in_csr_off.size() * 2);
+    L.in_csr_idx = o; o += align256(T.in_csr_idx.size() * 2 + 2);
+    L.out_csr_off = o; o += align256(T.out_csr_off.size() * 2);
+    L.out_csr_idx = o; o += align256(T.out_csr_idx.size() * 2 + 2);
     L.counters = o; o += align256(16 * 4);
     L.cnt = o; o += align256(8 * 8);
     L.total = o;
@@ -183,10 +105,11 @@ static void scratch_layout(int n, size_t ntab, size_t nthrlist, ScratchLayout &L
 
 extern "C" size_t ba_scratch_bytes(int n) {
     if (n < 1 || n > BA_NMAX) return 0;
-    LowTables T;
-    build_low_tables(low_m(n), T);
+    TileTables T;
+    build_tile_tables(low_m(n), T);
+    if (!T.ok) return 0;
     ScratchLayout L;
-    scratch_layout(n, T.words.size(), T.thrlist.size(), L);
+    scratch_layout(n, T, L);
     return L.total;
 }
 
@@ -219,36 +142,47 @@ static int setup_ctx(ba_ctx *c, int n, double d) {
     return BA_OK;
 }
 
+template <typename V>
+static cudaError_t upload(void *dst, const std::vector<V> &src, cudaStream_t st) {
+    if (src.empty()) return cudaSuccess;
+    return cudaMemcpyAsync(dst, src.data(), src.size() * sizeof(V), cudaMemcpyHostToDevice, st);
+}
+
 static int finish_create(ba_ctx *c) {
-    LowTables T;
-    build_low_tables(c->m, T);
-    c->lay = T.lay;
-    c->ntab = (int)T.words.size();
+    TileTables T;
+    build_tile_tables(c->m, T);
+    if (!T.ok) return fail(c, BA_EINVAL, "internal: tile tables do not fit their packed formats");
     ScratchLayout L;
-    scratch_layout(c->n, T.words.size(), T.thrlist.size(), L);
+    scratch_layout(c->n, T, L);
     unsigned char *s = c->scratch;
     c->c = (double *)(s + L.c); c->Hc = (double *)(s + L.Hc); c->Apart = (double *)(s + L.Apart);
     c->part = (double *)(s + L.part); c->scal = (double *)(s + L.scal); c->hist = (double *)(s + L.hist);
-    c->tab = (uint32_t *)(s + L.tab); c->vinfo = (uint32_t *)(s + L.vinfo); c->thrlist = (uint16_t *)(s + L.thrlist);
+    c->T64 = (uint2 *)(s + L.T64); c->Tz = (uint2 *)(s + L.Tz); c->Wv = (uint32_t *)(s + L.Wv);
+    c->vbase = (uint32_t *)(s + L.vbase); c->in_desc = (uint2 *)(s + L.in_desc); c->out_desc = (uint2 *)(s + L.out_desc);
+    c->in_csr_off = (uint16_t *)(s + L.in_csr_off); c->in_csr_idx = (uint16_t *)(s + L.in_csr_idx);
+    c->out_csr_off = (uint16_t *)(s + L.out_csr_off); c->out_csr_idx = (uint16_t *)(s + L.out_csr_idx);
     c->counters = (unsigned int *)(s + L.counters); c->cnt = (unsigned long long *)(s + L.cnt);
     c->napart = L.napart; c->npart_cap = L.npart_cap;
+    c->nT64 = (int)T.T64.size(); c->nTz = (int)T.Tz.size();
+    c->n_in_csr = (int)T.in_csr_idx.size(); c->n_out_csr = (int)T.out_csr_idx.size();
 
-    CK(cudaMemcpyAsync(c->tab, T.words.data(), T.words.size() * 4, cudaMemcpyHostToDevice, c->st));
-    CK(cudaMemcpyAsync(c->vinfo, T.vinfo.data(), T.vinfo.size() * 4, cudaMemcpyHostToDevice, c->st));
-    if (!T.thrlist.empty())
-        CK(cudaMemcpyAsync(c->thrlist, T.thrlist.data(), T.thrlist.size() * 2, cudaMemcpyHostToDevice, c->st));
+    CK(upload(c->T64, T.T64, c->st)); CK(upload(c->Tz, T.Tz, c->st)); CK(upload(c->Wv, T.Wv, c->st));
+    CK(upload(c->vbase, T.vbase, c->st)); CK(upload(c->in_desc, T.in_desc, c->st)); CK(upload(c->out_desc, T.out_desc, c->st));
+    CK(upload(c->in_csr_off, T.in_csr_off, c->st)); CK(upload(c->in_csr_idx, T.in_csr_idx, c->st));
+    CK(upload(c->out_csr_off, T.out_csr_off, c->st)); CK(upload(c->out_csr_idx, T.out_csr_idx, c->st));
+    CK(cudaMemsetAsync(c->c, 0, 8, c->st));                  // c[0] is never written by k_out_final
     uint32_t hb[BA_NMAX_I + 1][BA_NMAX_I + 1];
     for (int a = 0; a <= BA_NMAX_I; a++)
         for (int b = 0; b <= BA_NMAX_I; b++) hb[a][b] = (b <= a) ? (uint32_t)host_binom(a, b) : 0u;
     CK(cudaMemcpyToSymbolAsync(c_binom, hb, sizeof(hb), 0, cudaMemcpyHostToDevice, c->st));
-    CK(cudaStreamSynchronize(c->st));
+    CK(cudaStreamSynchronize(c->st));                        // T and hb go out of scope
 
     int dev = 0;
     CK(cudaGetDevice(&dev));
     CK(cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev));
-    c->block = (1 << c->m) < 32 ? 32 : (1 << c->m);
-    c->smem_in = enum_in_smem_bytes(c->m, c->h, c->ntab);
-    c->smem_out = enum_out_smem_bytes(c->m, c->ntab, c->lay.off[c->m + 1]);
+    c->block = BA_NT;
+    c->smem_in = enum_in_smem(c->m, c->nT64, c->n_in_csr).total;
+    c->smem_out = enum_out_smem(c->m, c->nTz, c->nT64, c->n_out_csr).total;
     CK(cudaFuncSetAttribute(k_enum_in<IN_SWEEP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_in));
     CK(cudaFuncSetAttribute(k_enum_in<IN_HC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_in));
     CK(cudaFuncSetAttribute(k_enum_in<IN_DEBUG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_in));
@@ -331,7 +265,8 @@ extern "C" int ba_set_mode(ba_ctx *c, int mode) {
 // ------------------------------------------------------------------------------------------------ launches
 static InArgs make_in_args(ba_ctx *c) {
     InArgs a;
-    a.kc = c->kc; a.tab = c->tab; a.vinfo = c->vinfo; a.ntab = c->ntab;
+    a.kc = c->kc; a.T64 = c->T64; a.vbase = c->vbase; a.desc = c->in_desc;
+    a.csr_off = c->in_csr_off; a.csr_idx = c->in_csr_idx; a.nT64 = c->nT64; a.ncsr = c->n_in_csr;
     a.c = c->c; a.p = c->p; a.Hc = c->Hc; a.D = c->D; a.part = c->part;
     a.counter = c->counters; a.dbg_x = 0; a.dbg_out = nullptr; a.cnt = c->cnt;
     return a;
@@ -339,8 +274,10 @@ static InArgs make_in_args(ba_ctx *c) {
 
 static OutArgs make_out_args(ba_ctx *c) {
     OutArgs a;
-    a.kc = c->kc; a.lay = c->lay; a.tab = c->tab; a.vinfo = c->vinfo; a.thrlist = c->thrlist; a.ntab = c->ntab;
-    a.p = c->p; a.Apart = c->Apart; a.counter = c->counters + 4; a.dbg_cy = 0; a.dbg_out = nullptr; a.cnt = c->cnt + 2;
+    a.kc = c->kc; a.Tz = c->Tz; a.Wv = c->Wv; a.vbase = c->vbase; a.desc = c->out_desc;
+    a.csr_off = c->out_csr_off; a.csr_idx = c->out_csr_idx; a.nTz = c->nTz; a.nWv = c->nT64; a.ncsr = c->n_out_csr;
+    a.p = c->p; a.Apart = c->Apart; a.counter = c->counters + 4; a.dbg_item = 0; a.dbg_cz = 0; a.dbg_out = nullptr;
+    a.cnt = c->cnt + 2;
     return a;
 }
 
@@ -388,7 +325,7 @@ static int launch_in_sweep(ba_ctx *c, size_t *npart) {
         *npart = (size_t)1 << c->h;
     } else {
         double *buf0 = c->Apart, *buf1 = c->Apart + (((size_t)2 << c->n) + 64);
-        const double *in = c->c;
+        const double *in = c->c + 1;                          // c is stored by code: idx(y) = code(y) - 1
         double *out = buf0;
         for (int s = c->n - 1; s >= 0; s--) {
             k_fast_bwd<<<c->num_sms * 8, 256, 0, c->st>>>(c->n, s, in, out);
@@ -559,9 +496,14 @@ extern "C" int ba_debug_emb_col(ba_ctx *c, unsigned yidx, unsigned *emb_out) {
     uint32_t *dev = nullptr;
     CK(cudaMalloc(&dev, c->NX * 4));
     cudaError_t e = cudaMemsetAsync(dev, 0, c->NX * 4, c->st);
-    if (e == cudaSuccess) {
+    const uint32_t cyt = yidx + 1u;                          // code of the target y
+    const int ky = 31 - __builtin_clz(cyt);
+    for (int j = 0; j <= c->m && j <= ky && e == cudaSuccess; j++) {   // the splits y = y'.z, |z| = j
+        if (ky - j > c->h) continue;
         OutArgs a = make_out_args(c);
-        a.dbg_cy = yidx + 1u; a.dbg_out = dev;
+        a.dbg_item = cyt >> j;
+        a.dbg_cz = (1u << j) | (cyt & ((1u << j) - 1u));
+        a.dbg_out = dev;
         k_enum_out<OUT_DEBUG><<<1, c->block, c->smem_out, c->st>>>(a);
         e = cudaGetLastError();
     }

@@ -9,6 +9,8 @@
 // Writing log2( W/q ) = log2( emb/ebar_k ) - log2( A/ebar_k ) moves the only logarithm that depends on
 // the iterate from T(n) terms to 2^{n+1} outputs (SURVEY 7.2 "hoisting the logarithm"); ebar_k =
 // C(n,k)/2^k is the mean of emb over a length, which centres both halves.
+// c is stored by CODE (c[code(y)] = c[idx(y)+1], entry 0 unused) so that the 2^j outputs y'.z, |z| = j,
+// of a prefix y' start at the even index code(y') << j: 16-byte aligned pieces for cp.async.
 __global__ void k_out_final(KConst kc, const double *__restrict__ Apart, const double *__restrict__ Afull,
                             double *__restrict__ q, double *__restrict__ c) {
     const size_t NY = ((size_t)2 << kc.n) - 1;
@@ -31,7 +33,7 @@ __global__ void k_out_final(KConst kc, const double *__restrict__ Apart, const d
         }
         const double wk = kc.w[k];
         q[i] = wk * A;
-        c[i] = (wk != 0.0) ? wk * (log2(A) - kc.lebar[k]) : 0.0;
+        c[i + 1] = (wk != 0.0) ? wk * (log2(A) - kc.lebar[k]) : 0.0;
     }
 }
 
