@@ -24,8 +24,6 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-D_REPLICAS = (0.70, 0.64, 0.75, 0.80, 0.85, 0.90, 0.95, 0.60)   # rank r runs d = D_REPLICAS[r % 8]
-
 
 def terms_per_sweep(n):
     """T(n) = sum_k 2^k sum_{i<=n-k} C(n,i)   (Lemma 6)."""
@@ -170,6 +168,7 @@ def run_ours(args, rank, world, local_rank):
     import torch
     import torch.distributed as dist
     import paper_2604_05867_b200 as ba
+    from paper_2604_05867_b200 import replicas
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- libba has no CPU fallback")
@@ -178,7 +177,7 @@ def run_ours(args, rank, world, local_rank):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device(dev))
     n = args.n
-    d = args.d if world == 1 else D_REPLICAS[rank % len(D_REPLICAS)]
+    d = replicas.replica_d(rank, world, args.d)
     mode = ba.BA_MODE_ENUM if args.mode == "enum" else ba.BA_MODE_FAST
     T = terms_per_sweep(n)
     NX = 1 << n
@@ -207,10 +206,7 @@ def run_ours(args, rank, world, local_rank):
     clocks = sampler.stop() if rank == 0 else None
     tm = ba.ba_last_timing(ctx)
     I, U = ba.ba_bounds(ctx)
-    if world > 1:
-        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = replicas.max_over_ranks(ms_total, world, dev)
 
     # ---- end-to-end arm: the C ABI with HOST buffers; H2D of p and D2H of p + bounds every step -----
     p_host = torch.empty(NX, dtype=torch.float64).pin_memory()
@@ -226,10 +222,7 @@ def run_ours(args, rank, world, local_rank):
         ba.ba_get_p(ctx, out=p_np)        # D2H  8*2^n bytes
     barrier()
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = replicas.max_over_ranks(e2e_s, world, dev)
     ba.ba_destroy(ctx)
 
     if rank != 0:

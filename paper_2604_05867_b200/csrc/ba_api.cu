@@ -20,15 +20,17 @@ struct ba_ctx {
     double d = 0.0;
     size_t NX = 0, NY = 0, NZ = 0, napart = 0;
     KConst kc;
-    int nT64 = 0, nTz = 0, n_in_csr = 0, n_out_csr = 0;
+    int nWv = 0, nri = 0, nro = 0, n_in_csr = 0, n_out_csr = 0;
     cudaStream_t st = nullptr;
     bool own_buffers = false, own_stream = false;
     double *p = nullptr, *q = nullptr, *D = nullptr;
     unsigned char *scratch = nullptr;
     // carved from scratch
     double *c = nullptr, *Hc = nullptr, *Apart = nullptr, *part = nullptr, *scal = nullptr, *hist = nullptr;
-    uint2 *T64 = nullptr, *Tz = nullptr, *in_desc = nullptr, *out_desc = nullptr;
+    uint2 *FI = nullptr, *FO = nullptr;
+    uint4 *RI = nullptr, *RO = nullptr;
     uint32_t *Wv = nullptr, *vbase = nullptr;
+    uint16_t *in_owner = nullptr, *out_owner = nullptr, *ri_cnt = nullptr, *ro_cnt = nullptr, *ri_csr = nullptr, *ro_csr = nullptr;
     uint16_t *in_csr_off = nullptr, *in_csr_idx = nullptr, *out_csr_off = nullptr, *out_csr_idx = nullptr;
     unsigned int *counters = nullptr;
     unsigned long long *cnt = nullptr;
@@ -67,8 +69,8 @@ static double host_binom(int n, int k) {
 
 // ------------------------------------------------------------------------------------------------ scratch layout
 struct ScratchLayout {
-    size_t c, Hc, Apart, part, scal, hist, T64, Tz, Wv, vbase, in_desc, out_desc, in_csr_off, in_csr_idx, out_csr_off,
-        out_csr_idx, counters, cnt, total;
+    size_t c, Hc, Apart, part, scal, hist, FI, FO, RI, RO, Wv, vbase, in_owner, out_owner, ri_cnt, ro_cnt, ri_csr, ro_csr,
+        in_csr_off, in_csr_idx, out_csr_off, out_csr_idx, counters, cnt, total;
     size_t napart, npart_cap;
 };
 
@@ -88,12 +90,18 @@ static void scratch_layout(int n, const TileTables &T, ScratchLayout &L) {
     L.part = o; o += align256(L.npart_cap * 3 * 8);
     L.scal = o; o += align256(8 * 8);
     L.hist = o; o += align256((size_t)BA_HIST_CAP * 3 * 8);
-    L.T64 = o; o += align256(T.T64.size() * 8);
-    L.Tz = o; o += align256(T.Tz.size() * 8);
+    L.FI = o; o += align256(T.FI.size() * 8);
+    L.FO = o; o += align256(T.FO.size() * 8);
+    L.RI = o; o += align256(T.RI.size() * 16);
+    L.RO = o; o += align256(T.RO.size() * 16);
     L.Wv = o; o += align256(T.Wv.size() * 4);
     L.vbase = o; o += align256(T.vbase.size() * 4);
-    L.in_desc = o; o += align256(T.in_desc.size() * 8);
-    L.out_desc = o; o += align256(T.out_desc.size() * 8);
+    L.in_owner = o; o += align256(T.in_owner.size() * 2);
+    L.out_owner = o; o += align256(T.out_owner.size() * 2);
+    L.ri_cnt = o; o += align256(T.ri_cnt.size() * 2);
+    L.ro_cnt = o; o += align256(T.ro_cnt.size() * 2);
+    L.ri_csr = o; o += align256(T.ri_csr.size() * 2);
+    L.ro_csr = o; o += align256(T.ro_csr.size() * 2);
     L.in_csr_off = o; o += align256(T.in_csr_off.size() * 2);
     L.in_csr_idx = o; o += align256(T.in_csr_idx.size() * 2 + 2);
     L.out_csr_off = o; o += align256(T.out_csr_off.size() * 2);
@@ -157,17 +165,23 @@ static int finish_create(ba_ctx *c) {
     unsigned char *s = c->scratch;
     c->c = (double *)(s + L.c); c->Hc = (double *)(s + L.Hc); c->Apart = (double *)(s + L.Apart);
     c->part = (double *)(s + L.part); c->scal = (double *)(s + L.scal); c->hist = (double *)(s + L.hist);
-    c->T64 = (uint2 *)(s + L.T64); c->Tz = (uint2 *)(s + L.Tz); c->Wv = (uint32_t *)(s + L.Wv);
-    c->vbase = (uint32_t *)(s + L.vbase); c->in_desc = (uint2 *)(s + L.in_desc); c->out_desc = (uint2 *)(s + L.out_desc);
+    c->FI = (uint2 *)(s + L.FI); c->FO = (uint2 *)(s + L.FO); c->RI = (uint4 *)(s + L.RI); c->RO = (uint4 *)(s + L.RO);
+    c->Wv = (uint32_t *)(s + L.Wv); c->vbase = (uint32_t *)(s + L.vbase);
+    c->in_owner = (uint16_t *)(s + L.in_owner); c->out_owner = (uint16_t *)(s + L.out_owner);
+    c->ri_cnt = (uint16_t *)(s + L.ri_cnt); c->ro_cnt = (uint16_t *)(s + L.ro_cnt);
+    c->ri_csr = (uint16_t *)(s + L.ri_csr); c->ro_csr = (uint16_t *)(s + L.ro_csr);
     c->in_csr_off = (uint16_t *)(s + L.in_csr_off); c->in_csr_idx = (uint16_t *)(s + L.in_csr_idx);
     c->out_csr_off = (uint16_t *)(s + L.out_csr_off); c->out_csr_idx = (uint16_t *)(s + L.out_csr_idx);
     c->counters = (unsigned int *)(s + L.counters); c->cnt = (unsigned long long *)(s + L.cnt);
     c->napart = L.napart; c->npart_cap = L.npart_cap;
-    c->nT64 = (int)T.T64.size(); c->nTz = (int)T.Tz.size();
+    c->nWv = (int)T.Wv.size(); c->nri = T.nri; c->nro = T.nro;
     c->n_in_csr = (int)T.in_csr_idx.size(); c->n_out_csr = (int)T.out_csr_idx.size();
 
-    CK(upload(c->T64, T.T64, c->st)); CK(upload(c->Tz, T.Tz, c->st)); CK(upload(c->Wv, T.Wv, c->st));
-    CK(upload(c->vbase, T.vbase, c->st)); CK(upload(c->in_desc, T.in_desc, c->st)); CK(upload(c->out_desc, T.out_desc, c->st));
+    CK(upload(c->FI, T.FI, c->st)); CK(upload(c->FO, T.FO, c->st)); CK(upload(c->RI, T.RI, c->st)); CK(upload(c->RO, T.RO, c->st));
+    CK(upload(c->Wv, T.Wv, c->st)); CK(upload(c->vbase, T.vbase, c->st));
+    CK(upload(c->in_owner, T.in_owner, c->st)); CK(upload(c->out_owner, T.out_owner, c->st));
+    CK(upload(c->ri_cnt, T.ri_cnt, c->st)); CK(upload(c->ro_cnt, T.ro_cnt, c->st));
+    CK(upload(c->ri_csr, T.ri_csr, c->st)); CK(upload(c->ro_csr, T.ro_csr, c->st));
     CK(upload(c->in_csr_off, T.in_csr_off, c->st)); CK(upload(c->in_csr_idx, T.in_csr_idx, c->st));
     CK(upload(c->out_csr_off, T.out_csr_off, c->st)); CK(upload(c->out_csr_idx, T.out_csr_idx, c->st));
     CK(cudaMemsetAsync(c->c, 0, 8, c->st));                  // c[0] is never written by k_out_final
@@ -181,8 +195,8 @@ static int finish_create(ba_ctx *c) {
     CK(cudaGetDevice(&dev));
     CK(cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev));
     c->block = BA_NT;
-    c->smem_in = enum_in_smem(c->m, c->nT64, c->n_in_csr).total;
-    c->smem_out = enum_out_smem(c->m, c->nTz, c->nT64, c->n_out_csr).total;
+    c->smem_in = enum_in_smem(c->m, c->nWv, c->n_in_csr, c->nri).total;
+    c->smem_out = enum_out_smem(c->m, c->nWv, c->n_out_csr, c->nro).total;
     CK(cudaFuncSetAttribute(k_enum_in<IN_SWEEP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_in));
     CK(cudaFuncSetAttribute(k_enum_in<IN_HC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_in));
     CK(cudaFuncSetAttribute(k_enum_in<IN_DEBUG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_in));
@@ -265,8 +279,9 @@ extern "C" int ba_set_mode(ba_ctx *c, int mode) {
 // ------------------------------------------------------------------------------------------------ launches
 static InArgs make_in_args(ba_ctx *c) {
     InArgs a;
-    a.kc = c->kc; a.T64 = c->T64; a.vbase = c->vbase; a.desc = c->in_desc;
-    a.csr_off = c->in_csr_off; a.csr_idx = c->in_csr_idx; a.nT64 = c->nT64; a.ncsr = c->n_in_csr;
+    a.kc = c->kc; a.Wv = c->Wv; a.vbase = c->vbase; a.nWv = c->nWv;
+    a.FI = c->FI; a.RI = c->RI; a.ri_cnt = c->ri_cnt; a.ri_csr = c->ri_csr; a.nri = c->nri; a.owner = c->in_owner;
+    a.csr_off = c->in_csr_off; a.csr_idx = c->in_csr_idx; a.ncsr = c->n_in_csr;
     a.c = c->c; a.p = c->p; a.Hc = c->Hc; a.D = c->D; a.part = c->part;
     a.counter = c->counters; a.dbg_x = 0; a.dbg_out = nullptr; a.cnt = c->cnt;
     return a;
@@ -274,8 +289,9 @@ static InArgs make_in_args(ba_ctx *c) {
 
 static OutArgs make_out_args(ba_ctx *c) {
     OutArgs a;
-    a.kc = c->kc; a.Tz = c->Tz; a.Wv = c->Wv; a.vbase = c->vbase; a.desc = c->out_desc;
-    a.csr_off = c->out_csr_off; a.csr_idx = c->out_csr_idx; a.nTz = c->nTz; a.nWv = c->nT64; a.ncsr = c->n_out_csr;
+    a.kc = c->kc; a.Wv = c->Wv; a.vbase = c->vbase; a.nWv = c->nWv;
+    a.FO = c->FO; a.RO = c->RO; a.ro_cnt = c->ro_cnt; a.ro_csr = c->ro_csr; a.nro = c->nro; a.owner = c->out_owner;
+    a.csr_off = c->out_csr_off; a.csr_idx = c->out_csr_idx; a.ncsr = c->n_out_csr;
     a.p = c->p; a.Apart = c->Apart; a.counter = c->counters + 4; a.dbg_item = 0; a.dbg_cz = 0; a.dbg_out = nullptr;
     a.cnt = c->cnt + 2;
     return a;

@@ -2,19 +2,23 @@
 // with their integer embedding counts emb(y,x) exactly once each.
 //
 // Work item = a high part u (h bits) with its 2^m inputs x = u.v; one persistent CTA per SM takes
-// items from an atomic counter.  Per item:
+// items from an atomic counter.  Per item, in super-batches of BA_NT nodes:
 //   phase A  every thread UNRANKS one node: the r-th distinct subsequence y' of u in trie pre-order
 //            (the paper's stringUnrank idea, Alg. 4, with the subtree sizes Sub[pos] in the
 //            role of the Count table P:260-274 and NextPos P:256-258 done with clz on bit masks), and
 //            carries the integer embedding-count DP  E[i] = emb(y', u[0:i])  in registers along the
 //            descent; the node record {alpha_0..8, code(y'), mask} goes to shared memory.
-//   phase B  all threads walk the node list.  The (x,y) terms of a node are its pairs (v, z)
-//            (ba_internal.h); they are dealt to the threads by a STATIC schedule: chunks of BA_C
-//            consecutive entries of one v's list, the same chunks at every node, so each thread keeps
-//            one FP64 accumulator per chunk in registers for the whole item and nothing is reduced or
-//            synchronised per node.  emb(y'.z, u.v) is the integer chain sum_s alpha_s B(sigma_s.z, v)
-//             walked through byte-packed prepend links; the operand c(y'.z) comes from the
-//            node's row of c, staged with cp.async (9 contiguous segments of c, 16-byte pieces).
+//   sort     the nodes that have non-empty-z pairs (mask != 0) are ranked, stably, by (class, mask).
+//   eps      the pair (v, empty) of every node: thread (v, node), whole chain walked (ba_chain_single).
+//   phase B  batches of <= BA_RB_IN nodes of one (class, mask).  The operand rows c(y'.z), z in
+//            {0,1}^{<=m}, of the batch are staged with 16-byte cp.async (9 contiguous segments of c per
+//            node), double buffered.  Every thread owns BA_NC chunks of BA_C pairs (v,z) per list; the
+//            chunk's B_0..B_3 and row offsets are constants of the batch (ba_internal.h "CLASSES"), so
+//            the loop over the nodes of the batch costs, per (x,y) term,
+//                 4 IMAD (emb) + 1 LDS.64 (operand) + 1 DADD (exact u32->f64) + 1 DFMA
+//            with one FP64 accumulator per chunk kept in a register for the whole item.  Deep pairs
+//            ride along, one per thread, their partial sums handed to thread v through shared memory
+//            in a fixed order.
 //   epilogue thread v adds the accumulators of v's chunks in a fixed order: D(x) = Hc(x) - sum_y emb c(y).
 // MODE:
 //   IN_SWEEP  D(x) and the fused reductions of 8(a3) (sum p D, max D, sum p 2^D per item)
@@ -26,14 +30,23 @@
 
 enum { IN_SWEEP = 0, IN_HC = 1, IN_DEBUG = 2, IN_COUNT = 3 };
 
+#define BA_IN_NKEY (BA_NCLS * 3)
+#define BA_IN_MAXB (BA_IN_NKEY + BA_NT / BA_RB_IN)
+
 struct InArgs {
     KConst kc;
-    const uint2 *T64;         // v-major low table
+    const uint32_t *Wv;       // v-major prepend links
     const uint32_t *vbase;    // [2^m]
-    const uint2 *desc;        // [2][BA_NC][BA_NT]
+    int nWv;
+    const uint2 *FI;          // fast pairs [cls][b][c][q][tid]
+    const uint4 *RI;          // riders [cls][b][nri]
+    const uint16_t *ri_cnt;   // [cls][b]
+    const uint16_t *ri_csr;   // [cls][b][2^m + 1]
+    int nri;
+    const uint16_t *owner;    // [b][c][tid] -> v
     const uint16_t *csr_off;  // [2^m + 1]
     const uint16_t *csr_idx;
-    int nT64, ncsr;
+    int ncsr;
     const double *c;          // IN_SWEEP: c[code(y)], 2^{n+1} entries (entry 0 unused)
     const double *p;          // IN_SWEEP: p(x)
     double *Hc;               // IN_HC: out; IN_SWEEP: in
@@ -45,23 +58,30 @@ struct InArgs {
     unsigned long long *cnt;  // IN_COUNT: [0] terms, [1] emb sum
 };
 
-struct InSmem { size_t T64, rec, ceps, stage, csr_off, csr_idx, sub, red, kcw, item, total; };
+struct InSmem { size_t Wv, rec, ceps, rows, bal, bnode, order, wcnt, bstart, batch, rsum, csr_off, csr_idx, sub, red, kcw, item, total; };
 
-__host__ __device__ static inline InSmem enum_in_smem(int m, int nT64, int ncsr) {
+__host__ __device__ static inline InSmem enum_in_smem(int m, int nWv, int ncsr, int nri) {
     InSmem s;
     size_t o = 0;
-    s.T64 = o; o += ((size_t)nT64 * 8 + 15) & ~(size_t)15;
-    s.rec = o; o += (size_t)BA_NT * sizeof(NodeRec);
-    s.ceps = o; o += (size_t)BA_NT * 8;
-    s.stage = o;
-    size_t st = (size_t)BA_NSTAGE * ((size_t)2 << m) * 8, ac = (size_t)2 * BA_NC * BA_NT * 8 + (size_t)BA_NT * 8;
-    o += st > ac ? st : ac;                                // accumulator staging of the epilogue aliases the rows
-    s.csr_off = o; o += (((size_t)(1 << m) + 1) * 2 + 15) & ~(size_t)15;
-    s.csr_idx = o; o += ((size_t)ncsr * 2 + 15) & ~(size_t)15;
-    s.sub = o; o += 32 * 4;
-    s.red = o; o += 64 * 8;
-    s.kcw = o; o += 2 * (BA_NMAX_I + 1) * 8;
-    s.item = o; o += 16;
+    auto take = [&](size_t bytes) { size_t at = o; o += (bytes + 15) & ~(size_t)15; return at; };
+    s.Wv = take((size_t)nWv * 4);
+    s.rec = take((size_t)BA_NT * sizeof(NodeRec));
+    s.ceps = take((size_t)BA_NT * 8);
+    size_t rows = (size_t)2 * BA_RB_IN * ((size_t)2 << m) * 8, ac = ((size_t)2 * BA_NC + 2) * BA_NT * 8;
+    s.rows = take(rows > ac ? rows : ac);                  // the epilogue's accumulator staging aliases the rows
+    s.bal = take((size_t)2 * BA_RB_IN * 16);
+    s.bnode = take((size_t)2 * BA_RB_IN * 2);
+    s.order = take((size_t)BA_NT * 2);
+    s.wcnt = take((size_t)(BA_NT / 32) * BA_IN_NKEY * 2);
+    s.bstart = take((size_t)(BA_IN_NKEY + 1) * 2);
+    s.batch = take((size_t)BA_IN_MAXB * 4);
+    s.rsum = take((size_t)2 * 2 * nri * 8);
+    s.csr_off = take(((size_t)(1 << m) + 1) * 2);
+    s.csr_idx = take((size_t)ncsr * 2);
+    s.sub = take(32 * 4);
+    s.red = take(64 * 8);
+    s.kcw = take(2 * (BA_NMAX_I + 1) * 8);
+    s.item = take(16);
     s.total = o;
     return s;
 }
@@ -71,49 +91,54 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
     extern __shared__ __align__(16) unsigned char smem[];
     const int m = a.kc.m, h = a.kc.h, nv = 1 << m;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const InSmem L = enum_in_smem(m, a.nT64, a.ncsr);
-    const uint32_t ROWB = (2u << m) * 8u;
+    const InSmem L = enum_in_smem(m, a.nWv, a.ncsr, a.nri);
+    const uint32_t ROWD = 2u << m, ROWB = ROWD * 8u;
 
-    uint2 *s_T64 = (uint2 *)(smem + L.T64);
+    uint32_t *s_Wv = (uint32_t *)(smem + L.Wv);
     NodeRec *s_rec = (NodeRec *)(smem + L.rec);
     double *s_ceps = (double *)(smem + L.ceps);
-    double *s_stage = (double *)(smem + L.stage);
-    double *s_acc = s_stage;                                // epilogue only
+    double *s_rows = (double *)(smem + L.rows);
+    double *s_acc = s_rows;                                 // epilogue only
+    uint4 *s_bal = (uint4 *)(smem + L.bal);
+    uint16_t *s_bnode = (uint16_t *)(smem + L.bnode);
+    uint16_t *s_order = (uint16_t *)(smem + L.order);
+    uint16_t *s_wcnt = (uint16_t *)(smem + L.wcnt);
+    uint16_t *s_bstart = (uint16_t *)(smem + L.bstart);
+    uint32_t *s_batch = (uint32_t *)(smem + L.batch);
+    double *s_rsum = (double *)(smem + L.rsum);
     uint16_t *s_csr_off = (uint16_t *)(smem + L.csr_off);
     uint16_t *s_csr_idx = (uint16_t *)(smem + L.csr_idx);
     uint32_t *s_sub = (uint32_t *)(smem + L.sub);
     double *s_red = (double *)(smem + L.red);
     double *s_w = (double *)(smem + L.kcw);
     double *s_lebar = s_w + (BA_NMAX_I + 1);
-    uint32_t *s_item = (uint32_t *)(smem + L.item);
+    uint32_t *s_item = (uint32_t *)(smem + L.item);        // [0] item, [1] number of batches
 
-    for (int i = tid; i < a.nT64; i += BA_NT) s_T64[i] = a.T64[i];
+    for (int i = tid; i < a.nWv; i += BA_NT) s_Wv[i] = a.Wv[i];
     for (int i = tid; i <= nv; i += BA_NT) s_csr_off[i] = a.csr_off[i];
     for (int i = tid; i < a.ncsr; i += BA_NT) s_csr_idx[i] = a.csr_idx[i];
     for (int i = tid; i <= BA_NMAX_I; i += BA_NT) { s_w[i] = a.kc.w[i]; s_lebar[i] = a.kc.lebar[i]; }
-    for (int i = tid; i < BA_NSTAGE; i += BA_NT) s_stage[(size_t)i * (ROWB / 8)] = 0.0;   // slot 0 of every row: padding pairs
+    for (int i = tid; i < 2 * BA_RB_IN; i += BA_NT) { s_rows[(size_t)i * ROWD] = 0.0; s_rows[(size_t)i * ROWD + 1] = 0.0; }
 
-    // static per-thread schedule
-    uint2 dsc[2][BA_NC];
+    // which of this warp's chunk slots hold pairs at all (static)
+    uint32_t whas = 0;
 #pragma unroll
-    for (int b = 0; b < 2; b++)
-#pragma unroll
-        for (int c = 0; c < BA_NC; c++) dsc[b][c] = a.desc[((size_t)b * BA_NC + c) * BA_NT + tid];
-    const uint32_t sT64 = ba_smem_addr(s_T64);
-    const uint32_t sStage = ba_smem_addr(s_stage);
-    const int ev = tid & (nv - 1);                          // v of this thread's empty-z pair
-    const int esub = tid >> m;                              // which node of an eps-round it serves
-    const int epn = (BA_NT >> m) < BA_GRP ? (BA_NT >> m) : BA_GRP;   // nodes per eps-round
-    const uint32_t evb = sT64 + a.vbase[ev] * 8u;           // v's list
+    for (int s = 0; s < 2 * BA_NC; s++)
+        if (__any_sync(0xffffffffu, a.owner[(size_t)s * BA_NT + tid] != 0xffffu)) whas |= 1u << s;
+    const uint32_t sWv = ba_smem_addr(s_Wv);
+    const uint32_t sRows = ba_smem_addr(s_rows);
+    const int ev = tid & (nv - 1);                          // v of this thread's empty-z pairs
+    const int esub = tid >> m, epn = BA_NT >> m;            // it serves nodes esub, esub + epn, ...
+    const uint32_t evb = sWv + a.vbase[ev] * 4u;            // v's list
     __syncthreads();
-    const uint32_t eW = s_T64[a.vbase[ev] + 1].x;           // W of (v, empty)
+    const uint32_t eW = s_Wv[a.vbase[ev] + 1];              // W of (v, empty)
 
     unsigned long long cnt_terms = 0, cnt_emb = 0;
 
     for (;;) {
-        if (tid == 0) *s_item = (MODE == IN_DEBUG) ? (a.dbg_x >> m) : atomicAdd(a.counter, 1u);
+        if (tid == 0) s_item[0] = (MODE == IN_DEBUG) ? (a.dbg_x >> m) : atomicAdd(a.counter, 1u);
         __syncthreads();
-        const uint32_t u = *s_item;
+        const uint32_t u = s_item[0];
         if (h < 32 && (u >> h) != 0) break;
         if (MODE == IN_DEBUG && blockIdx.x != 0) break;
 
@@ -134,11 +159,12 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
         for (int b = 0; b < 2; b++)
 #pragma unroll
             for (int c = 0; c < BA_NC; c++) acc[b][c] = 0.0;
-        double acc_eps = 0.0;
+        double acc_eps = 0.0, acc_rid = 0.0;
 
         for (uint32_t base = 0; base < NN; base += BA_NT) {
-            __syncthreads();                                   // previous chunk's records are no longer read
+            __syncthreads();                                   // previous super-batch fully consumed
             // ================= phase A: unrank node base+tid, DP along the descent =================
+            int key = -1;
             if (base + tid < NN) {
                 uint32_t r = base + tid;
                 uint32_t E[BA_HMAX + 1];
@@ -172,140 +198,199 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                     cy = (cy << 1) | b;
                 }
                 const uint32_t miss0 = ba_nextpos(u, h, pos, 0u) >= h, miss1 = ba_nextpos(u, h, pos, 1u) >= h;
+                const uint32_t mask = miss0 | (miss1 << 1);
                 NodeRec rc;
 #pragma unroll
                 for (int s = 0; s < 9; s++) rc.a[s] = al[s];
                 rc.id = cy;
-                rc.info = miss0 | (miss1 << 1) | ((uint32_t)(k < 8 ? k : 8) << 8) | ((uint32_t)k << 16);
+                rc.info = mask | ((uint32_t)(k < 8 ? k : 8) << 8) | ((uint32_t)k << 16);
                 rc.pad = 0u;
                 s_rec[tid] = rc;
                 if (MODE == IN_SWEEP) s_ceps[tid] = a.c[cy];
+                if (mask) key = (int)(cy & (BA_NCLS - 1)) * 3 + (int)mask - 1;
             }
             const int nn = (NN - base < (uint32_t)BA_NT) ? (int)(NN - base) : BA_NT;
-            const int ngrp = (nn + BA_GRP - 1) / BA_GRP;
+            ba_bucket_sort<BA_IN_NKEY>(key, s_order, s_wcnt, s_bstart);
+            if (tid == 0) {                                    // batches: <= BA_RB_IN consecutive nodes of one key
+                int nb = 0;
+                for (int kq = 0; kq < BA_IN_NKEY; kq++)
+                    for (int off = s_bstart[kq]; off < s_bstart[kq + 1]; off += BA_RB_IN) {
+                        const int len = (s_bstart[kq + 1] - off < BA_RB_IN) ? (s_bstart[kq + 1] - off) : BA_RB_IN;
+                        s_batch[nb++] = (uint32_t)off | ((uint32_t)len << 16) | ((uint32_t)kq << 24);
+                    }
+                s_item[1] = (uint32_t)nb;
+            }
             __syncthreads();
 
-            // ================= phase B: pairs of every node =================
-            auto issue_rows = [&](int g) {                     // stage the c rows of group g's masked nodes
-                if (MODE != IN_SWEEP) return;
-                if (tid >= nv) return;
-#pragma unroll
-                for (int j = 0; j < BA_GRP; j++) {
-                    const int i = g * BA_GRP + j;
-                    if (i >= nn) break;
-                    if (!(s_rec[i].info & 3u)) continue;
-                    const uint32_t cy = s_rec[i].id;
-                    const uint32_t dst = sStage + (uint32_t)((g & 1) * BA_GRP + j) * ROWB;
-                    if (tid == 0) {
-                        ba_cp_async8(dst + 8u, a.c + cy);                              // row code 1: z empty
-                    } else {
-                        const uint32_t cz = 2u * tid;                                  // row codes cz, cz+1
+            // ================= eps: the pair (v, empty) of every node =================
+            for (int i = esub; i < nn; i += epn) {
+                uint32_t al[9];
+                const uint4 r0 = *(const uint4 *)&s_rec[i].a[0], r1 = *(const uint4 *)&s_rec[i].a[4],
+                            r2 = *(const uint4 *)&s_rec[i].a[8];
+                al[0] = r0.x; al[1] = r0.y; al[2] = r0.z; al[3] = r0.w;
+                al[4] = r1.x; al[5] = r1.y; al[6] = r1.z; al[7] = r1.w; al[8] = r2.x;
+                const uint32_t cy = r2.y, info = r2.z;
+                const int Lc = (int)((info >> 8) & 0xffu), k = (int)(info >> 16);
+                const uint32_t emb = ba_chain_single<4>(eW, 1u, evb, al, cy, Lc);
+                if (MODE == IN_SWEEP) {
+                    acc_eps = fma(ba_u2d(emb), s_ceps[i], acc_eps);
+                } else if (MODE == IN_HC) {
+                    const double wk = s_w[k];
+                    if (wk != 0.0 && emb > 1u) acc_eps = fma(wk * (double)emb, log2((double)emb) - s_lebar[k], acc_eps);
+                    else if (wk != 0.0) acc_eps = fma(wk, -s_lebar[k], acc_eps);
+                } else if (MODE == IN_DEBUG) {
+                    if (((u << m) | (uint32_t)ev) == a.dbg_x) a.dbg_out[cy - 1u] = emb;
+                } else {
+                    cnt_terms += 1ull; cnt_emb += emb;
+                }
+            }
+
+            // ================= phase B: batches of one (class, mask) =================
+            const int nbatch = (int)s_item[1];
+            auto stage = [&](int j) {                          // rows, alpha_0..3 and node ids of batch j
+                const uint32_t bi = s_batch[j];
+                const int start = (int)(bi & 0xffffu), len = (int)((bi >> 16) & 0xffu), buf = j & 1;
+                if (MODE == IN_SWEEP) {
+                    for (int pidx = tid; pidx < (len << m); pidx += BA_NT) {
+                        const int i = pidx >> m, pc = pidx & (nv - 1);
+                        if (pc == 0) continue;                 // codes 0, 1: padding target / the eps pair
+                        const uint32_t cy = s_rec[s_order[start + i]].id;
+                        const uint32_t cz = 2u * (uint32_t)pc;
                         const int jz = ba_len_of_code(cz);
-                        ba_cp_async16(dst + cz * 8u, a.c + (((size_t)cy << jz) + (cz - (1u << jz))));
+                        ba_cp_async16(sRows + ((uint32_t)(buf * BA_RB_IN + i) * ROWD + cz) * 8u,
+                                      a.c + (((size_t)cy << jz) + (cz - (1u << jz))));
                     }
+                }
+                if (tid < len) {
+                    const int node = s_order[start + tid];
+                    s_bal[buf * BA_RB_IN + tid] = *(const uint4 *)&s_rec[node].a[0];
+                    s_bnode[buf * BA_RB_IN + tid] = (uint16_t)node;
                 }
             };
-            issue_rows(0);
-            for (int g = 0; g < ngrp; g++) {
-                ba_cp_async_wait_all();
-                __syncthreads();                               // rows of group g visible; group g-1 fully consumed
-                if (g + 1 < ngrp) issue_rows(g + 1);
-
-                // ---- the empty-z pair of every node: thread (v, node) ----------------------------------
-                for (int e0 = 0; e0 < BA_GRP; e0 += epn) {
-                    const int i = g * BA_GRP + e0 + esub;
-                    if (esub < epn && e0 + esub < BA_GRP && i < nn) {
-                        uint32_t al[9];
-                        const uint4 r0 = *(const uint4 *)&s_rec[i].a[0], r1 = *(const uint4 *)&s_rec[i].a[4],
-                                    r2 = *(const uint4 *)&s_rec[i].a[8];
-                        al[0] = r0.x; al[1] = r0.y; al[2] = r0.z; al[3] = r0.w;
-                        al[4] = r1.x; al[5] = r1.y; al[6] = r1.z; al[7] = r1.w; al[8] = r2.x;
-                        const uint32_t cy = r2.y, info = r2.z;
-                        const int Lc = (int)((info >> 8) & 0xffu), k = (int)(info >> 16);
-                        const uint32_t emb = ba_chain_single<8>(eW, 1u, evb, al, cy, Lc);
-                        if (MODE == IN_SWEEP) {
-                            acc_eps = fma(ba_u2d(emb), s_ceps[i], acc_eps);
-                        } else if (MODE == IN_HC) {
-                            const double wk = s_w[k];
-                            if (wk != 0.0 && emb > 1u) acc_eps = fma(wk * (double)emb, log2((double)emb) - s_lebar[k], acc_eps);
-                            else if (wk != 0.0) acc_eps = fma(wk, -s_lebar[k], acc_eps);
-                        } else if (MODE == IN_DEBUG) {
-                            if (((u << m) | (uint32_t)ev) == a.dbg_x) a.dbg_out[cy - 1u] = emb;
-                        } else {
-                            cnt_terms += 1ull; cnt_emb += emb;
-                        }
-                    }
+            auto flush = [&](int j) {                          // thread v collects the rider sums of batch j
+                if (MODE != IN_SWEEP && MODE != IN_HC) return;
+                if (tid >= nv) return;
+                const uint32_t bi = s_batch[j];
+                const int kq = (int)(bi >> 24), cls = kq / 3, mask = kq % 3 + 1, buf = j & 1;
+#pragma unroll
+                for (int b = 0; b < 2; b++) {
+                    if (!((mask >> b) & 1)) continue;
+                    const uint16_t *cs = a.ri_csr + ((size_t)cls * 2 + b) * (nv + 1) + tid;
+                    const int e0 = cs[0], e1 = cs[1];
+                    for (int e = e0; e < e1; e++) acc_rid += s_rsum[((size_t)buf * 2 + b) * a.nri + e];
                 }
-                // ---- pairs with a non-empty z: static chunk schedule -------------------------------------
-                for (int j = 0; j < BA_GRP; j++) {
-                    const int i = g * BA_GRP + j;
-                    if (i >= nn) break;
-                    const uint32_t info = s_rec[i].info;
-                    const uint32_t mask = info & 3u;
-                    if (!mask) continue;
-                    uint32_t al[9];
-                    const uint4 r0 = *(const uint4 *)&s_rec[i].a[0], r1 = *(const uint4 *)&s_rec[i].a[4],
-                                r2 = *(const uint4 *)&s_rec[i].a[8];
-                    al[0] = r0.x; al[1] = r0.y; al[2] = r0.z; al[3] = r0.w;
-                    al[4] = r1.x; al[5] = r1.y; al[6] = r1.z; al[7] = r1.w; al[8] = r2.x;
-                    const uint32_t cy = r2.y;
-                    const int Lc = (int)((info >> 8) & 0xffu), k = (int)(info >> 16);
-                    const uint32_t sel1 = (cy & 1u) ? 0x4432u : 0x4410u;
-                    const uint32_t row = sStage + (uint32_t)((g & 1) * BA_GRP + j) * ROWB;
+            };
+            if (nbatch > 0) stage(0);
+            for (int j = 0; j < nbatch; j++) {
+                ba_cp_async_wait_all();
+                __syncthreads();                               // batch j staged; batch j-1 fully consumed
+                if (j + 1 < nbatch) stage(j + 1);
+                if (j > 0) flush(j - 1);
+                const uint32_t bi = s_batch[j];
+                const int len = (int)((bi >> 16) & 0xffu), kq = (int)(bi >> 24), buf = j & 1;
+                const int cls = kq / 3, mask = kq % 3 + 1;
+                const uint32_t rowbase = sRows + (uint32_t)(buf * BA_RB_IN) * ROWB;
+                const uint4 *bal = s_bal + buf * BA_RB_IN;
+                const uint16_t *bnode = s_bnode + buf * BA_RB_IN;
 #pragma unroll
-                    for (int b = 0; b < 2; b++) {
-                        if (!((mask >> b) & 1u)) continue;
+                for (int b = 0; b < 2; b++) {
+                    if (!((mask >> b) & 1)) continue;
+                    // ---- fast pairs -----------------------------------------------------------------------
+                    const uint2 *F = a.FI + (((size_t)cls * 2 + b) * BA_NC) * BA_C * BA_NT + tid;
 #pragma unroll
-                        for (int c = 0; c < BA_NC; c++) {
-                            const uint2 d = dsc[b][c];
-                            if (!__any_sync(0xffffffffu, d.x >> 31)) continue;
-                            const uint32_t pa = sT64 + (d.x & 0xfffffu);
-                            uint32_t emb[BA_C], lk[BA_C], P[BA_C], vb[BA_C];
-                            uint32_t anyl = 0u;
+                    for (int c = 0; c < BA_NC; c++) {
+                        if (!((whas >> (b * BA_NC + c)) & 1u)) continue;
+                        uint32_t B0[BA_C], B1[BA_C], B2[BA_C], B3[BA_C], ad[BA_C];
 #pragma unroll
-                            for (int q = 0; q < BA_C; q++) {
-                                const uint2 wp = ba_lds_v2(pa + 8u * q);
-                                P[q] = wp.y;
-                                const uint32_t hw = __byte_perm(wp.x, 0u, sel1);
-                                lk[q] = hw & 0xffu;
-                                emb[q] = al[0] * (wp.y & 0xffu) + al[1] * (hw >> 8);   // al[s] = 0 beyond k
-                                anyl |= lk[q];
-                                vb[q] = sT64 + d.y;
-                            }
-                            BaChain<2, BA_C, 8>::run(emb, lk, vb, anyl, al, cy, Lc);
-                            if (MODE == IN_SWEEP) {
-#pragma unroll
-                                for (int q = 0; q < BA_C; q++)
-                                    acc[b][c] = fma(ba_u2d(emb[q]), ba_lds_f64(row + (P[q] >> 16)), acc[b][c]);
-                            } else if (MODE == IN_HC) {
+                        for (int q = 0; q < BA_C; q++) {
+                            const uint2 pr = __ldg(F + (size_t)(c * BA_C + q) * BA_NT);
+                            B0[q] = pr.x & 0xffu; B1[q] = (pr.x >> 8) & 0xffu; B2[q] = (pr.x >> 16) & 0xffu; B3[q] = pr.x >> 24;
+                            ad[q] = pr.y;
+                        }
+                        if (MODE == IN_SWEEP) {
+                            double s = acc[b][c];
+#pragma unroll 2
+                            for (int i = 0; i < len; i++) {
+                                const uint4 al = bal[i];
+                                const uint32_t rb = rowbase + (uint32_t)i * ROWB;
 #pragma unroll
                                 for (int q = 0; q < BA_C; q++) {
-                                    const int kk = k + (int)((P[q] >> 8) & 0xfu);
-                                    const double wk = s_w[kk];
-                                    if (wk != 0.0 && emb[q] > 0u) {
-                                        const double le = (emb[q] > 1u) ? log2((double)emb[q]) : 0.0;
-                                        acc[b][c] = fma(wk * (double)emb[q], le - s_lebar[kk], acc[b][c]);
+                                    const uint32_t emb = al.x * B0[q] + al.y * B1[q] + al.z * B2[q] + al.w * B3[q];
+                                    s = fma(ba_u2d(emb), ba_lds_f64(rb + ad[q]), s);
+                                }
+                            }
+                            acc[b][c] = s;
+                        } else {
+                            const uint32_t ov = a.owner[((size_t)b * BA_NC + c) * BA_NT + tid];
+                            for (int i = 0; i < len; i++) {
+                                const uint4 al = bal[i];
+                                const NodeRec &rc = s_rec[bnode[i]];
+                                const int k = (int)(rc.info >> 16);
+#pragma unroll
+                                for (int q = 0; q < BA_C; q++) {
+                                    if (!B0[q]) continue;
+                                    const uint32_t emb = al.x * B0[q] + al.y * B1[q] + al.z * B2[q] + al.w * B3[q];
+                                    const uint32_t cz = ad[q] >> 3;
+                                    const int jz = ba_len_of_code(cz);
+                                    if (MODE == IN_HC) {
+                                        const double wk = s_w[k + jz];
+                                        if (wk != 0.0) {
+                                            const double le = (emb > 1u) ? log2((double)emb) : 0.0;
+                                            acc[b][c] = fma(wk * (double)emb, le - s_lebar[k + jz], acc[b][c]);
+                                        }
+                                    } else if (MODE == IN_DEBUG) {
+                                        if (((u << m) | ov) == a.dbg_x)
+                                            a.dbg_out[((size_t)rc.id << jz) + (cz - (1u << jz)) - 1u] = emb;
+                                    } else {
+                                        cnt_terms += 1ull; cnt_emb += emb;
                                     }
                                 }
-                            } else if (MODE == IN_DEBUG) {
-                                const uint32_t v = (d.x >> 20) & 0xffu;
-                                if ((d.x >> 31) && ((u << m) | v) == a.dbg_x) {
-#pragma unroll
-                                    for (int q = 0; q < BA_C; q++) {
-                                        if (!(P[q] & 0xffu)) continue;
-                                        const uint32_t cz = P[q] >> 19;
-                                        const int jz = (int)((P[q] >> 8) & 0xfu);
-                                        a.dbg_out[((size_t)cy << jz) + (cz - (1u << jz)) - 1u] = emb[q];
-                                    }
-                                }
-                            } else {
-#pragma unroll
-                                for (int q = 0; q < BA_C; q++)
-                                    if (P[q] & 0xffu) { cnt_terms += 1ull; cnt_emb += emb[q]; }
                             }
                         }
                     }
+                    // ---- riders: deep pairs of this class, one per thread ------------------------------------
+                    const int nr = a.ri_cnt[cls * 2 + b];
+                    if (warp * 32 < nr) {
+                        double s = 0.0;
+                        if (tid < nr) {
+                            const uint4 rd = __ldg(a.RI + ((size_t)cls * 2 + b) * a.nri + tid);
+                            const uint32_t B0 = rd.x & 0xffu, B1 = (rd.x >> 8) & 0xffu, B2 = (rd.x >> 16) & 0xffu, B3 = rd.x >> 24;
+                            const uint32_t B4 = rd.y & 0xffu, lk4 = (rd.y >> 8) & 0xffu, ov = rd.y >> 16;
+                            const uint32_t cz = rd.z >> 3;
+                            const int jz = ba_len_of_code(cz);
+                            const uint32_t vb = sWv + rd.w;
+                            for (int i = 0; i < len; i++) {
+                                const NodeRec &rc = s_rec[bnode[i]];
+                                uint32_t al[9];
+                                const uint4 r0 = *(const uint4 *)&rc.a[0], r1 = *(const uint4 *)&rc.a[4], r2 = *(const uint4 *)&rc.a[8];
+                                al[0] = r0.x; al[1] = r0.y; al[2] = r0.z; al[3] = r0.w;
+                                al[4] = r1.x; al[5] = r1.y; al[6] = r1.z; al[7] = r1.w; al[8] = r2.x;
+                                const uint32_t cy = r2.y, info = r2.z;
+                                const int Lc = (int)((info >> 8) & 0xffu), k = (int)(info >> 16);
+                                const uint32_t emb = al[0] * B0 + al[1] * B1 + al[2] * B2 + al[3] * B3 + al[4] * B4 +
+                                                     ba_chain_from(BA_KB + 1, lk4, vb, al, cy, Lc);
+                                if (MODE == IN_SWEEP) {
+                                    s = fma(ba_u2d(emb), ba_lds_f64(rowbase + (uint32_t)i * ROWB + rd.z), s);
+                                } else if (MODE == IN_HC) {
+                                    const double wk = s_w[k + jz];
+                                    if (wk != 0.0) {
+                                        const double le = (emb > 1u) ? log2((double)emb) : 0.0;
+                                        s = fma(wk * (double)emb, le - s_lebar[k + jz], s);
+                                    }
+                                } else if (MODE == IN_DEBUG) {
+                                    if (((u << m) | ov) == a.dbg_x) a.dbg_out[((size_t)cy << jz) + (cz - (1u << jz)) - 1u] = emb;
+                                } else {
+                                    cnt_terms += 1ull; cnt_emb += emb;
+                                }
+                            }
+                        }
+                        if ((MODE == IN_SWEEP || MODE == IN_HC) && tid < nr) s_rsum[((size_t)buf * 2 + b) * a.nri + tid] = s;
+                    }
                 }
+            }
+            if (nbatch > 0) {
+                __syncthreads();                               // rider sums of the last batch are visible
+                flush(nbatch - 1);
             }
         }
 
@@ -320,7 +405,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
             __syncthreads();
             double r0 = 0.0, r1 = -INFINITY, r2 = 0.0;
             if (tid < nv) {
-                double S = 0.0;
+                double S = acc_rid;
                 for (int t = ev; t < BA_NT; t += nv) S += s_acc[(size_t)2 * BA_NC * BA_NT + t];
                 for (int q = s_csr_off[tid]; q < s_csr_off[tid + 1]; q++) S += s_acc[s_csr_idx[q]];
                 const size_t x = ((size_t)u << m) | (size_t)tid;
@@ -354,7 +439,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 }
             }
             __syncthreads();
-            for (int i = tid; i < BA_NSTAGE; i += BA_NT) s_stage[(size_t)i * (ROWB / 8)] = 0.0;   // restore slot 0 of the rows
+            for (int i = tid; i < 2 * BA_RB_IN; i += BA_NT) { s_rows[(size_t)i * ROWD] = 0.0; s_rows[(size_t)i * ROWD + 1] = 0.0; }
         }
         if (MODE == IN_DEBUG) break;
         __syncthreads();

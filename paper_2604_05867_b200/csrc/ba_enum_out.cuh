@@ -3,17 +3,21 @@
 // single owner, nothing is accumulated with atomics.
 //
 // Work item = a high output prefix y' (length t <= h, code cy); one persistent CTA per SM takes items
-// from an atomic counter (short y' = many supersequences first).  Per item:
+// from an atomic counter (short y' = many supersequences first).  The class of an item is fixed, so the
+// B_s of every pair are constants of the whole item.  Per item, in super-batches of BA_NT nodes:
 //   phase A  every thread UNRANKS one node: the r-th length-h supersequence u of y' (the paper's
 //            subsetUnrank / RecSuperSeq, Alg. 5-6, with the G3 correction for the unmatched
 //            tail; there are sum_{i<=h-t} C(h,i) of them by Lemma 6) and runs the textbook
 //            integer DP  f[s] = emb(y'[0:t-s], u)  in registers; record {alpha_0..8, u, mask}.
-//   phase B  all threads walk the node list.  For node u the 2^m inputs p(u.*) -- the run of inputs
-//            whose low m bits are free (SURVEY 7.2 "coalescing the gather") -- are one contiguous
-//            2^m-double row, staged with 16-byte cp.async.  The pairs (v, z) of the node (ba_internal.h)
-//            are dealt to the threads by a STATIC z-major schedule: chunks of BA_C supersequences v of
-//            one z, so each thread keeps one FP64 accumulator per chunk in registers for the whole
-//            item.  emb(y'.z, u.v) = sum_s alpha_s B(sigma_s.z, v).
+//   sort     nodes are ranked, stably, by mask (which lists of non-empty z they carry).
+//   phase B  batches of <= BA_RB_OUT nodes of one mask.  For node u the 2^m inputs p(u.*) -- the run
+//            of inputs whose low m bits are free (SURVEY 7.2 "coalescing the gather") -- are one
+//            contiguous 2^m-double row, staged with 16-byte cp.async, double buffered.  Pairs (v,z) are
+//            dealt z-major: every thread owns BA_NC chunks of BA_C supersequences v of one z per list,
+//            with one FP64 accumulator per chunk kept in a register for the whole item, and runs
+//                 4 IMAD (emb) + 1 LDS.64 (p) + 1 DADD (exact u32->f64) + 1 DFMA        per (x,y) term.
+//            The pair (v, empty) of every node and the deep pairs (riders) use all nine B_s, which are
+//            walked once per item.
 //   epilogue the chunks of each z are added in a fixed order and written once:
 //            Apart[y'][z] = sum_{u, v} emb(y'.z, u.v) p(u.v) over the nodes where y' is the longest
 //            prefix of y'.z embeddable in u.
@@ -24,17 +28,24 @@
 
 enum { OUT_SWEEP = 0, OUT_DEBUG = 1, OUT_COUNT = 2 };
 
+#define BA_OUT_MAXB (4 + BA_NT / BA_RB_OUT)
+
 __constant__ uint32_t c_binom[BA_NMAX_I + 1][BA_NMAX_I + 1];
 
 struct OutArgs {
     KConst kc;
-    const uint2 *Tz;           // z-major pairs
-    const uint32_t *Wv;        // v-major W words
+    const uint32_t *Wv;        // v-major prepend links
     const uint32_t *vbase;     // [2^m]
-    const uint2 *desc;         // [2][BA_NC][BA_NT]
+    int nWv;
+    const uint2 *FO;           // fast pairs [cls][b][c][q][tid]
+    const uint4 *RO;           // riders [cls][b][nro]
+    const uint16_t *ro_cnt;    // [cls][b]
+    const uint16_t *ro_csr;    // [cls][b][2^{m+1} + 1] by code(z)
+    int nro;
+    const uint16_t *owner;     // [b][c][tid] -> code(z)
     const uint16_t *csr_off;   // [2^{m+1}] by code(z)-1
     const uint16_t *csr_idx;
-    int nTz, nWv, ncsr;
+    int ncsr;
     const double *p;           // NX
     double *Apart;             // (2^{h+1}-1) * (2^{m+1}-1)
     unsigned int *counter;
@@ -44,22 +55,26 @@ struct OutArgs {
     unsigned long long *cnt;   // OUT_COUNT
 };
 
-struct OutSmem { size_t Tz, Wv, rec, stage, csr_off, csr_idx, red, item, total; };
+struct OutSmem { size_t Wv, rec, rows, bal, bnode, order, wcnt, bstart, batch, csr_off, csr_idx, red, item, total; };
 
-__host__ __device__ static inline OutSmem enum_out_smem(int m, int nTz, int nWv, int ncsr) {
+__host__ __device__ static inline OutSmem enum_out_smem(int m, int nWv, int ncsr, int nro) {
     OutSmem s;
     size_t o = 0;
-    s.Tz = o; o += ((size_t)nTz * 8 + 15) & ~(size_t)15;
-    s.Wv = o; o += ((size_t)nWv * 4 + 15) & ~(size_t)15;
-    s.rec = o;                                             // records + rows; the epilogue's accumulator staging aliases both
-    size_t rr = (size_t)BA_NT * sizeof(NodeRec) + (size_t)BA_NSTAGE * ((size_t)1 << m) * 8;
-    size_t ac = (size_t)2 * BA_NC * BA_NT * 8;
-    o += rr > ac ? rr : ac;
-    s.stage = s.rec + (size_t)BA_NT * sizeof(NodeRec);
-    s.csr_off = o; o += (((size_t)2 << m) * 2 + 15) & ~(size_t)15;
-    s.csr_idx = o; o += ((size_t)ncsr * 2 + 15) & ~(size_t)15;
-    s.red = o; o += 32 * 8;
-    s.item = o; o += 16;
+    auto take = [&](size_t bytes) { size_t at = o; o += (bytes + 15) & ~(size_t)15; return at; };
+    s.Wv = take((size_t)nWv * 4);
+    s.rec = take((size_t)BA_NT * sizeof(NodeRec));
+    size_t rows = (size_t)2 * BA_RB_OUT * ((size_t)1 << m) * 8, ac = ((size_t)2 * BA_NC * BA_NT + 2 * (size_t)nro) * 8;
+    s.rows = take(rows > ac ? rows : ac);                  // the epilogue's accumulator staging aliases the rows
+    s.bal = take((size_t)2 * BA_RB_OUT * 16);
+    s.bnode = take((size_t)2 * BA_RB_OUT * 2);
+    s.order = take((size_t)BA_NT * 2);
+    s.wcnt = take((size_t)(BA_NT / 32) * 4 * 2);
+    s.bstart = take(5 * 2);
+    s.batch = take((size_t)BA_OUT_MAXB * 4);
+    s.csr_off = take(((size_t)2 << m) * 2);
+    s.csr_idx = take((size_t)ncsr * 2);
+    s.red = take(32 * 8);
+    s.item = take(16);
     s.total = o;
     return s;
 }
@@ -69,35 +84,37 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
     extern __shared__ __align__(16) unsigned char smem[];
     const int m = a.kc.m, h = a.kc.h, nv = 1 << m;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const OutSmem L = enum_out_smem(m, a.nTz, a.nWv, a.ncsr);
+    const OutSmem L = enum_out_smem(m, a.nWv, a.ncsr, a.nro);
     const uint32_t ROWB = (uint32_t)nv * 8u;
     const uint32_t NZ = (2u << m) - 1u;
 
-    uint2 *s_Tz = (uint2 *)(smem + L.Tz);
     uint32_t *s_Wv = (uint32_t *)(smem + L.Wv);
     NodeRec *s_rec = (NodeRec *)(smem + L.rec);
-    double *s_acc = (double *)(smem + L.rec);               // epilogue only
+    double *s_rows = (double *)(smem + L.rows);
+    double *s_acc = s_rows;                                 // epilogue only
+    uint4 *s_bal = (uint4 *)(smem + L.bal);
+    uint16_t *s_bnode = (uint16_t *)(smem + L.bnode);
+    uint16_t *s_order = (uint16_t *)(smem + L.order);
+    uint16_t *s_wcnt = (uint16_t *)(smem + L.wcnt);
+    uint16_t *s_bstart = (uint16_t *)(smem + L.bstart);
+    uint32_t *s_batch = (uint32_t *)(smem + L.batch);
     uint16_t *s_csr_off = (uint16_t *)(smem + L.csr_off);
     uint16_t *s_csr_idx = (uint16_t *)(smem + L.csr_idx);
     double *s_red = (double *)(smem + L.red);
-    uint32_t *s_item = (uint32_t *)(smem + L.item);
+    uint32_t *s_item = (uint32_t *)(smem + L.item);        // [0] item, [1] number of batches
 
-    for (int i = tid; i < a.nTz; i += BA_NT) s_Tz[i] = a.Tz[i];
     for (int i = tid; i < a.nWv; i += BA_NT) s_Wv[i] = a.Wv[i];
     for (int i = tid; i < (2 << m); i += BA_NT) s_csr_off[i] = a.csr_off[i];
     for (int i = tid; i < a.ncsr; i += BA_NT) s_csr_idx[i] = a.csr_idx[i];
 
-    uint2 dsc[2][BA_NC];
+    uint32_t whas = 0;
 #pragma unroll
-    for (int b = 0; b < 2; b++)
-#pragma unroll
-        for (int c = 0; c < BA_NC; c++) dsc[b][c] = a.desc[((size_t)b * BA_NC + c) * BA_NT + tid];
-    const uint32_t sTz = ba_smem_addr(s_Tz);
+    for (int s = 0; s < 2 * BA_NC; s++)
+        if (__any_sync(0xffffffffu, a.owner[(size_t)s * BA_NT + tid] != 0xffffu)) whas |= 1u << s;
     const uint32_t sWv = ba_smem_addr(s_Wv);
-    const uint32_t sStage = ba_smem_addr(smem + L.stage);
-    const int ev = tid & (nv - 1);
-    const int esub = tid >> m;
-    const int epn = (BA_NT >> m) < BA_GRP ? (BA_NT >> m) : BA_GRP;
+    const uint32_t sRows = ba_smem_addr(s_rows);
+    const int ev = tid & (nv - 1);                          // v of this thread's empty-z pairs
+    const int esub = tid >> m, epn = BA_NT >> m;
     const uint32_t evb = sWv + a.vbase[ev] * 4u;
     __syncthreads();
     const uint32_t eW = s_Wv[a.vbase[ev] + 1];              // W of (v, empty)
@@ -106,26 +123,68 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
     const uint32_t n_items = (h >= 31) ? 0xffffffffu : ((2u << h) - 1u);   // codes 1 .. 2^{h+1}-1
 
     for (;;) {
-        if (tid == 0) *s_item = (MODE == OUT_DEBUG) ? a.dbg_item : atomicAdd(a.counter, 1u) + 1u;
+        if (tid == 0) s_item[0] = (MODE == OUT_DEBUG) ? a.dbg_item : atomicAdd(a.counter, 1u) + 1u;
         __syncthreads();
-        const uint32_t cy = *s_item;
+        const uint32_t cy = s_item[0];
         if (cy > n_items) break;
         if (MODE == OUT_DEBUG && blockIdx.x != 0) break;
         const int t = ba_len_of_code(cy);
         const uint32_t yv = cy - (1u << t);
+        const int cls = (int)(cy & (BA_NCLS - 1));
+        const int Lc = t < 8 ? t : 8;
         uint32_t R = 0;                                        // number of supersequences (Lemma 6)
         for (int w = 0; w <= h - t; w++) R += c_binom[h][w];
+
+        // ---- per item: all nine B_s of the eps pair (v = ev) and of this thread's riders --------------------
+        uint32_t Ee[9];                                        // B(sigma_s, ev)
+        {
+            Ee[0] = 1u;
+            uint32_t hw = (cy & 1u) ? (eW >> 16) : (eW & 0xffffu);
+            uint32_t lk = (Lc >= 1) ? (hw & 0xffu) : 0u;
+            Ee[1] = (Lc >= 1) ? (hw >> 8) : 0u;
+#pragma unroll
+            for (int s = 2; s <= 8; s++) {
+                Ee[s] = 0u;
+                if (Lc >= s && lk != 0u) {
+                    hw = ba_lds_u16(evb + ((cy >> (s - 1)) & 1u) * 2u + lk * 4u);
+                    Ee[s] = hw >> 8; lk = hw & 0xffu;
+                }
+            }
+        }
+        uint32_t rB[2][3], roff[2];                            // riders: B_0..B_8 packed 4+4+1 bytes, row offset
+#pragma unroll
+        for (int b = 0; b < 2; b++) {
+            rB[b][0] = rB[b][1] = rB[b][2] = 0u; roff[b] = 0u;
+            const int nr = a.ro_cnt[cls * 2 + b];
+            if (tid < nr) {
+                const uint4 rd = __ldg(a.RO + ((size_t)cls * 2 + b) * a.nro + tid);
+                rB[b][0] = rd.x;
+                roff[b] = rd.z;
+                uint32_t hi = rd.y & 0xffu, lk = (rd.y >> 8) & 0xffu, b8 = 0u;
+                const uint32_t vb = sWv + rd.w;
+#pragma unroll
+                for (int s = BA_KB + 1; s <= 8; s++) {
+                    if (Lc >= s && lk != 0u) {
+                        const uint32_t hw = ba_lds_u16(vb + ((cy >> (s - 1)) & 1u) * 2u + lk * 4u);
+                        if (s < 8) hi |= (hw >> 8) << (8 * (s - 4)); else b8 = hw >> 8;
+                        lk = hw & 0xffu;
+                    }
+                }
+                rB[b][1] = hi; rB[b][2] = b8;
+            }
+        }
 
         double acc[2][BA_NC];
 #pragma unroll
         for (int b = 0; b < 2; b++)
 #pragma unroll
             for (int c = 0; c < BA_NC; c++) acc[b][c] = 0.0;
-        double acc_eps = 0.0;
+        double acc_eps = 0.0, acc_rid[2] = {0.0, 0.0};
 
         for (uint32_t base = 0; base < R; base += BA_NT) {
             __syncthreads();
             // ================= phase A: unrank supersequence base+tid of y', DP =================
+            int key = -1;
             if (base + tid < R) {
                 uint32_t w = 0, rem = base + tid;
                 while (rem >= c_binom[h][w]) { rem -= c_binom[h][w]; w++; }
@@ -171,118 +230,151 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                 for (int s = 0; s < 9; s++) rc.a[s] = f[s];
                 const uint32_t miss0 = ba_nextpos(u, h, ell, 0u) >= h, miss1 = ba_nextpos(u, h, ell, 1u) >= h;
                 rc.id = u;
-                rc.info = miss0 | (miss1 << 1) | ((uint32_t)(t < 8 ? t : 8) << 8) | ((uint32_t)t << 16);
+                rc.info = miss0 | (miss1 << 1) | ((uint32_t)Lc << 8) | ((uint32_t)t << 16);
                 rc.pad = 0u;
                 s_rec[tid] = rc;
+                key = (int)(miss0 | (miss1 << 1));
             }
-            const int nn = (R - base < (uint32_t)BA_NT) ? (int)(R - base) : BA_NT;
-            const int ngrp = (nn + BA_GRP - 1) / BA_GRP;
+            ba_bucket_sort<4>(key, s_order, s_wcnt, s_bstart);
+            if (tid == 0) {                                    // batches: <= BA_RB_OUT consecutive nodes of one mask
+                int nb = 0;
+                for (int kq = 0; kq < 4; kq++)
+                    for (int off = s_bstart[kq]; off < s_bstart[kq + 1]; off += BA_RB_OUT) {
+                        const int len = (s_bstart[kq + 1] - off < BA_RB_OUT) ? (s_bstart[kq + 1] - off) : BA_RB_OUT;
+                        s_batch[nb++] = (uint32_t)off | ((uint32_t)len << 16) | ((uint32_t)kq << 24);
+                    }
+                s_item[1] = (uint32_t)nb;
+            }
             __syncthreads();
 
             // ================= phase B =================
-            auto issue_rows = [&](int g) {                     // stage the p rows of group g
-                if (MODE != OUT_SWEEP) return;
-                const int j = tid / (nv / 2 > 0 ? nv / 2 : 1);  // row of the group this thread copies a piece of
-                const int piece = tid - j * (nv / 2);
-                const int i = g * BA_GRP + j;
-                if (j < BA_GRP && i < nn) {
-                    const uint32_t dst = sStage + (uint32_t)((g & 1) * BA_GRP + j) * ROWB + (uint32_t)piece * 16u;
-                    ba_cp_async16(dst, a.p + (((size_t)s_rec[i].id << m) + 2u * (size_t)piece));
-                }
-            };
-            issue_rows(0);
-            for (int g = 0; g < ngrp; g++) {
-                ba_cp_async_wait_all();
-                __syncthreads();
-                if (g + 1 < ngrp) issue_rows(g + 1);
-
-                // ---- the empty-z pair of every node: thread (v, node) ----------------------------------
-                for (int e0 = 0; e0 < BA_GRP; e0 += epn) {
-                    const int i = g * BA_GRP + e0 + esub;
-                    if (esub < epn && e0 + esub < BA_GRP && i < nn) {
-                        uint32_t al[9];
-                        const uint4 r0 = *(const uint4 *)&s_rec[i].a[0], r1 = *(const uint4 *)&s_rec[i].a[4],
-                                    r2 = *(const uint4 *)&s_rec[i].a[8];
-                        al[0] = r0.x; al[1] = r0.y; al[2] = r0.z; al[3] = r0.w;
-                        al[4] = r1.x; al[5] = r1.y; al[6] = r1.z; al[7] = r1.w; al[8] = r2.x;
-                        const uint32_t u = r2.y, info = r2.z;
-                        const int Lc = (int)((info >> 8) & 0xffu);
-                        const uint32_t emb = ba_chain_single<4>(eW, 1u, evb, al, cy, Lc);
-                        if (MODE == OUT_SWEEP) {
-                            const uint32_t row = sStage + (uint32_t)((g & 1) * BA_GRP + e0 + esub) * ROWB;
-                            acc_eps = fma(ba_u2d(emb), ba_lds_f64(row + (uint32_t)ev * 8u), acc_eps);
-                        } else if (MODE == OUT_DEBUG) {
-                            if (a.dbg_cz == 1u) a.dbg_out[((size_t)u << m) | (size_t)ev] = emb;
-                        } else {
-                            cnt_terms += 1ull; cnt_emb += emb;
+            const int nbatch = (int)s_item[1];
+            auto stage = [&](int j) {                          // p rows, alpha_0..3 and node ids of batch j
+                const uint32_t bi = s_batch[j];
+                const int start = (int)(bi & 0xffffu), len = (int)((bi >> 16) & 0xffu), buf = j & 1;
+                if (MODE == OUT_SWEEP) {
+                    if (m >= 1) {
+                        const int ppr = nv >> 1;                   // 16-byte pieces per row
+                        for (int pidx = tid; pidx < len * ppr; pidx += BA_NT) {
+                            const int i = pidx / ppr, pc = pidx - i * ppr;
+                            const uint32_t u = s_rec[s_order[start + i]].id;
+                            ba_cp_async16(sRows + (uint32_t)(buf * BA_RB_OUT + i) * ROWB + (uint32_t)pc * 16u,
+                                          a.p + (((size_t)u << m) + 2u * (size_t)pc));
                         }
                     }
                 }
-                // ---- pairs with a non-empty z: static z-major chunk schedule -------------------------------
-                for (int j = 0; j < BA_GRP; j++) {
-                    const int i = g * BA_GRP + j;
-                    if (i >= nn) break;
-                    const uint32_t info = s_rec[i].info;
-                    const uint32_t mask = info & 3u;
-                    if (!mask) continue;
-                    uint32_t al[9];
-                    const uint4 r0 = *(const uint4 *)&s_rec[i].a[0], r1 = *(const uint4 *)&s_rec[i].a[4],
-                                r2 = *(const uint4 *)&s_rec[i].a[8];
-                    al[0] = r0.x; al[1] = r0.y; al[2] = r0.z; al[3] = r0.w;
-                    al[4] = r1.x; al[5] = r1.y; al[6] = r1.z; al[7] = r1.w; al[8] = r2.x;
-                    const uint32_t u = r2.y;
-                    const int Lc = (int)((info >> 8) & 0xffu);
-                    const uint32_t sel1 = (cy & 1u) ? 0x4432u : 0x4410u;
-                    const uint32_t row = sStage + (uint32_t)((g & 1) * BA_GRP + j) * ROWB;
+                if (tid < len) {
+                    const int node = s_order[start + tid];
+                    s_bal[buf * BA_RB_OUT + tid] = *(const uint4 *)&s_rec[node].a[0];
+                    s_bnode[buf * BA_RB_OUT + tid] = (uint16_t)node;
+                }
+            };
+            if (nbatch > 0) stage(0);
+            for (int j = 0; j < nbatch; j++) {
+                ba_cp_async_wait_all();
+                __syncthreads();                               // batch j staged; batch j-1 fully consumed
+                if (j + 1 < nbatch) stage(j + 1);
+                const uint32_t bi = s_batch[j];
+                const int len = (int)((bi >> 16) & 0xffu), mask = (int)(bi >> 24), buf = j & 1;
+                const uint32_t rowbase = sRows + (uint32_t)(buf * BA_RB_OUT) * ROWB;
+                const uint4 *bal = s_bal + buf * BA_RB_OUT;
+                const uint16_t *bnode = s_bnode + buf * BA_RB_OUT;
+
+                // ---- the pair (v, empty) of every node: thread (v, node) ----------------------------------
+                for (int i = esub; i < len; i += epn) {
+                    const NodeRec &rc = s_rec[bnode[i]];
+                    const uint4 r0 = *(const uint4 *)&rc.a[0], r1 = *(const uint4 *)&rc.a[4], r2 = *(const uint4 *)&rc.a[8];
+                    const uint32_t emb = r0.x * Ee[0] + r0.y * Ee[1] + r0.z * Ee[2] + r0.w * Ee[3] + r1.x * Ee[4] +
+                                         r1.y * Ee[5] + r1.z * Ee[6] + r1.w * Ee[7] + r2.x * Ee[8];
+                    if (MODE == OUT_SWEEP) {
+                        acc_eps = fma(ba_u2d(emb), ba_lds_f64(rowbase + (uint32_t)i * ROWB + (uint32_t)ev * 8u), acc_eps);
+                    } else if (MODE == OUT_DEBUG) {
+                        if (a.dbg_cz == 1u) a.dbg_out[((size_t)r2.y << m) | (size_t)ev] = emb;
+                    } else {
+                        cnt_terms += 1ull; cnt_emb += emb;
+                    }
+                }
 #pragma unroll
-                    for (int b = 0; b < 2; b++) {
-                        if (!((mask >> b) & 1u)) continue;
+                for (int b = 0; b < 2; b++) {
+                    if (!((mask >> b) & 1)) continue;
+                    // ---- fast pairs -----------------------------------------------------------------------
+                    const uint2 *F = a.FO + (((size_t)cls * 2 + b) * BA_NC) * BA_C * BA_NT + tid;
 #pragma unroll
-                        for (int c = 0; c < BA_NC; c++) {
-                            const uint2 d = dsc[b][c];
-                            if (!__any_sync(0xffffffffu, d.x >> 31)) continue;
-                            const uint32_t pa = sTz + (d.x & 0xfffffu);
-                            uint32_t emb[BA_C], lk[BA_C], P[BA_C], vb[BA_C];
-                            uint32_t anyl = 0u;
+                    for (int c = 0; c < BA_NC; c++) {
+                        if (!((whas >> (b * BA_NC + c)) & 1u)) continue;
+                        uint32_t B0[BA_C], B1[BA_C], B2[BA_C], B3[BA_C], ad[BA_C];
 #pragma unroll
-                            for (int q = 0; q < BA_C; q++) {
-                                const uint2 wp = ba_lds_v2(pa + 8u * q);
-                                P[q] = wp.y;
-                                const uint32_t hw = __byte_perm(wp.x, 0u, sel1);
-                                lk[q] = hw & 0xffu;
-                                emb[q] = al[0] * (wp.y & 0xffu) + al[1] * (hw >> 8);   // al[s] = 0 beyond t
-                                anyl |= lk[q];
-                                vb[q] = sWv + (wp.y >> 16);
-                            }
-                            BaChain<2, BA_C, 4>::run(emb, lk, vb, anyl, al, cy, Lc);
-                            if (MODE == OUT_SWEEP) {
+                        for (int q = 0; q < BA_C; q++) {
+                            const uint2 pr = __ldg(F + (size_t)(c * BA_C + q) * BA_NT);
+                            B0[q] = pr.x & 0xffu; B1[q] = (pr.x >> 8) & 0xffu; B2[q] = (pr.x >> 16) & 0xffu; B3[q] = pr.x >> 24;
+                            ad[q] = pr.y;
+                        }
+                        if (MODE == OUT_SWEEP) {
+                            double s = acc[b][c];
+#pragma unroll 2
+                            for (int i = 0; i < len; i++) {
+                                const uint4 al = bal[i];
+                                const uint32_t rb = rowbase + (uint32_t)i * ROWB;
 #pragma unroll
-                                for (int q = 0; q < BA_C; q++)
-                                    acc[b][c] = fma(ba_u2d(emb[q]), ba_lds_f64(row + ((P[q] >> 5) & 0x7f8u)), acc[b][c]);
-                            } else if (MODE == OUT_DEBUG) {
-                                if ((d.x >> 31) && ((d.x >> 20) & 0x1ffu) == a.dbg_cz) {
-#pragma unroll
-                                    for (int q = 0; q < BA_C; q++)
-                                        if (P[q] & 0xffu) a.dbg_out[((size_t)u << m) | (size_t)((P[q] >> 8) & 0xffu)] = emb[q];
+                                for (int q = 0; q < BA_C; q++) {
+                                    const uint32_t emb = al.x * B0[q] + al.y * B1[q] + al.z * B2[q] + al.w * B3[q];
+                                    s = fma(ba_u2d(emb), ba_lds_f64(rb + ad[q]), s);
                                 }
-                            } else {
+                            }
+                            acc[b][c] = s;
+                        } else {
+                            const uint32_t oz = a.owner[((size_t)b * BA_NC + c) * BA_NT + tid];
+                            for (int i = 0; i < len; i++) {
+                                const uint4 al = bal[i];
+                                const uint32_t u = s_rec[bnode[i]].id;
 #pragma unroll
-                                for (int q = 0; q < BA_C; q++)
-                                    if (P[q] & 0xffu) { cnt_terms += 1ull; cnt_emb += emb[q]; }
+                                for (int q = 0; q < BA_C; q++) {
+                                    if (!B0[q]) continue;
+                                    const uint32_t emb = al.x * B0[q] + al.y * B1[q] + al.z * B2[q] + al.w * B3[q];
+                                    if (MODE == OUT_DEBUG) {
+                                        if (oz == a.dbg_cz) a.dbg_out[((size_t)u << m) | (size_t)(ad[q] >> 3)] = emb;
+                                    } else {
+                                        cnt_terms += 1ull; cnt_emb += emb;
+                                    }
+                                }
                             }
                         }
+                    }
+                    // ---- riders: deep pairs of this class, one per thread, all B_s static -----------------------
+                    const int nr = a.ro_cnt[cls * 2 + b];
+                    if (warp * 32 < nr && tid < nr) {
+                        const uint32_t x0 = rB[b][0], x1 = rB[b][1], b8 = rB[b][2];
+                        const uint32_t oz = __ldg(a.RO + ((size_t)cls * 2 + b) * a.nro + tid).y >> 16;
+                        double s = acc_rid[b];
+                        for (int i = 0; i < len; i++) {
+                            const NodeRec &rc = s_rec[bnode[i]];
+                            const uint4 r0 = *(const uint4 *)&rc.a[0], r1 = *(const uint4 *)&rc.a[4], r2 = *(const uint4 *)&rc.a[8];
+                            const uint32_t emb = r0.x * (x0 & 0xffu) + r0.y * ((x0 >> 8) & 0xffu) + r0.z * ((x0 >> 16) & 0xffu) +
+                                                 r0.w * (x0 >> 24) + r1.x * (x1 & 0xffu) + r1.y * ((x1 >> 8) & 0xffu) +
+                                                 r1.z * ((x1 >> 16) & 0xffu) + r1.w * (x1 >> 24) + r2.x * b8;
+                            if (MODE == OUT_SWEEP) {
+                                s = fma(ba_u2d(emb), ba_lds_f64(rowbase + (uint32_t)i * ROWB + roff[b]), s);
+                            } else if (MODE == OUT_DEBUG) {
+                                if (oz == a.dbg_cz) a.dbg_out[((size_t)r2.y << m) | (size_t)(roff[b] >> 3)] = emb;
+                            } else {
+                                cnt_terms += 1ull; cnt_emb += emb;
+                            }
+                        }
+                        acc_rid[b] = s;
                     }
                 }
             }
         }
 
         // ---- epilogue: fixed-order reduction of the chunks of each z, one write per (y', z) -----------------
-        __syncthreads();                                       // records and rows are dead: the area becomes s_acc
+        __syncthreads();                                       // rows are dead: the area becomes s_acc
         if (MODE == OUT_SWEEP) {
 #pragma unroll
-            for (int b = 0; b < 2; b++)
+            for (int b = 0; b < 2; b++) {
 #pragma unroll
                 for (int c = 0; c < BA_NC; c++) s_acc[((size_t)b * BA_NC + c) * BA_NT + tid] = acc[b][c];
+                if (tid < a.nro) s_acc[(size_t)2 * BA_NC * BA_NT + (size_t)b * a.nro + tid] = acc_rid[b];
+            }
             double r0 = acc_eps;                               // z empty: block-wide sum, fixed tree
             for (int o = 16; o > 0; o >>= 1) r0 += __shfl_xor_sync(0xffffffffu, r0, o);
             if (lane == 0) s_red[warp] = r0;
@@ -293,9 +385,13 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                 for (int w = 0; w < BA_NT / 32; w++) s += s_red[w];
                 dst[0] = s;
             }
-            for (uint32_t zi = 1u + tid; zi < NZ; zi += BA_NT) {
+            for (uint32_t zi = 1u + tid; zi < NZ; zi += BA_NT) {   // zi = code(z) - 1
                 double s = 0.0;
                 for (int q = s_csr_off[zi]; q < s_csr_off[zi + 1]; q++) s += s_acc[s_csr_idx[q]];
+                const uint32_t cz = zi + 1u;
+                const int b = (int)((cz >> (ba_len_of_code(cz) - 1)) & 1u);
+                const uint16_t *cs = a.ro_csr + ((size_t)cls * 2 + b) * ((2u << m) + 1u) + cz;
+                for (int e = cs[0]; e < cs[1]; e++) s += s_acc[(size_t)2 * BA_NC * BA_NT + (size_t)b * a.nro + e];
                 dst[zi] = s;
             }
         }

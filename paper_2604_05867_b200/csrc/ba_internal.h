@@ -13,8 +13,17 @@
 //   mask    = which symbols b cannot follow y' in u after its leftmost embedding (NextPos)
 // The (x,y) terms of the node are the PAIRS (v, z), z a subsequence of v with z empty or z[0] in mask:
 // y = y'.z is then visited at exactly one node (y' = the longest prefix of y embeddable in u), and
-//   emb(y'.z, u.v) = sum_{s>=0} alpha_s * B(sigma_s.z, v),   B(w, v) = emb(w, v),
-// sigma_s = last s symbols of y'.  The sum is a CHAIN of "prepend" links in v's list of subsequences.
+//   emb(y'.z, u.v) = sum_{s>=0} alpha_s * B_s,   B_s = B(sigma_s.z, v) = emb(sigma_s.z, v),
+// sigma_s = last s symbols of y'.  B_s = 0 implies B_{s+1} = 0, and B_s = 0 for s > m - |z|.
+//
+// CLASSES.  The B_s of a pair depend on the node only through sigma.  Nodes are grouped by their CLASS
+// cls = code(y') & (2^BA_KB - 1) (the last BA_KB symbols) and processed in runs of one class, so the
+// B_0..B_3 of every pair are constants of the run: each thread loads the BA_C pairs of a chunk once
+// (class-specific FAST table, global memory / L2) and then loops over the nodes of the run with
+//   emb = a0*B0 + a1*B1 + a2*B2 + a3*B3        (4 IMAD, no unpacking, no links, no votes)
+// A pair whose chain reaches s = BA_KB under the class (3.4 % of the pairs) is DEEP: it is left out of
+// the class's fast table and handled as a RIDER, one rider per thread: B_0..B_4 static, the rest of the
+// chain walked through byte-packed prepend links (the v-major table Wv in shared memory).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -27,23 +36,21 @@
 #define BA_P_FLOOR 9.3326361850321888e-302   // 2^-1000 (G8)
 
 #define BA_NT 512            // threads per CTA of the ENUM kernels (one CTA per SM)
-#define BA_C 5               // pairs per chunk (odd: consecutive chunks are bank-conflict free)
+#define BA_C 5               // pairs per chunk
 #define BA_NC 3              // chunk slots per thread and list
-#define BA_GRP 4             // nodes per barrier group
-#define BA_NSTAGE 8          // staged rows (2 groups)
+#define BA_KB 4              // class bits
+#define BA_NCLS 16           // 2^BA_KB classes
+#define BA_RB_IN 16          // nodes per batch, input sweep (operand rows of 2^{m+1} doubles)
+#define BA_RB_OUT 32         // nodes per batch, output sweep (operand rows of 2^m doubles)
 
-// ---- low table, v-major ("T64"): one uint2 {W, P} per entry -------------------------------------
-// v's list: [0] null  [1] empty string  [2 ..) z starting with 0, longest first, zero-padded to a
-// multiple of BA_C   [..) z starting with 1, likewise.  For the entry of (v, z):
-//   W = l0 | cB0 << 8 | l1 << 16 | cB1 << 24   l_b = local index of b.z in v's list (0 = null: b.z is
-//                                              not a subsequence of v), cB_b = B(b.z, v)
-//   P = B(z,v) | |z| << 8 | (8 * code(z)) << 16     (8*code(z) = byte offset in a staged row)
-// The null entry and the padding are all-zero words: emb = 0, links stay on null.
-// ---- z-major table ("Tz"), output sweep: for each z its supersequences v, ascending, zero-padded
-//   W as above;  P' = B(z,v) | v << 8 | (4 * vbase[v]) << 16   (byte offset of v's list in Wv)
-// ---- chunk descriptors: uint2 per (list b, slot, thread)
-//   in : x = byte offset of the chunk's first pair in T64 | v << 20 | valid << 31 ; y = byte offset of v's list
-//   out: x = byte offset of the chunk's first pair in Tz  | code(z) << 20 | valid << 31 ; y = 0
+// ---- v-major prepend links Wv: one uint32 per entry of v's list ([0] null, [1] empty string, then the
+// non-empty subsequences of v):  W = l0 | cB0 << 8 | l1 << 16 | cB1 << 24,  l_b = local index of b.z in
+// v's list (0 = null: b.z is not a subsequence of v), cB_b = B(b.z, v).
+// ---- fast pairs: uint2 {B0 | B1<<8 | B2<<16 | B3<<24, byte offset of the operand in the staged row}
+//   [class][list b][slot c][pair q][thread]; slot (b,c,thread) always belongs to the same v (input sweep)
+//   or z (output sweep), so its FP64 accumulator lives in a register for the whole work item.  Within a
+//   half-warp the offsets of one (class,b,c,q) are dealt to distinct 8-byte bank pairs where possible.
+// ---- riders: uint4 {B0..B3, B4 | link4 << 8 | owner << 16, row byte offset, byte offset of v's list in Wv}
 
 struct KConst {                       // passed by value to kernels
     int n, m, h;
@@ -99,34 +106,8 @@ __device__ __forceinline__ double ba_u2d(uint32_t e) {
     return __hiloint2double(0x43300000, (int)e) - 4503599627370496.0;
 }
 
-// Chain steps S = 2..8 for CN pairs at once: lk[i] = local index of sigma_{S-1}.z in its v's list,
-// vb[i] = shared byte address of that list's W words (stride STRIDE bytes).  L = min(k,8) is uniform
-// over the CTA; the vote ends the walk as soon as every lane of the warp sits on null entries.
-template <int S, int CN, int STRIDE>
-struct BaChain {
-    static __device__ __forceinline__ void run(uint32_t (&emb)[CN], uint32_t (&lk)[CN], const uint32_t (&vb)[CN],
-                                               uint32_t anyl, const uint32_t (&al)[9], uint32_t sig, int L) {
-        if (L >= S && __any_sync(0xffffffffu, anyl != 0u)) {
-            const uint32_t bo = ((sig >> (S - 1)) & 1u) * 2u;
-            anyl = 0u;
-#pragma unroll
-            for (int i = 0; i < CN; i++) {
-                const uint32_t hw = ba_lds_u16(vb[i] + bo + lk[i] * (uint32_t)STRIDE);
-                emb[i] += al[S] * (hw >> 8);
-                lk[i] = hw & 0xffu;
-                anyl |= lk[i];
-            }
-            BaChain<S + 1, CN, STRIDE>::run(emb, lk, vb, anyl, al, sig, L);
-        }
-    }
-};
-template <int CN, int STRIDE>
-struct BaChain<9, CN, STRIDE> {
-    static __device__ __forceinline__ void run(uint32_t (&)[CN], uint32_t (&)[CN], const uint32_t (&)[CN], uint32_t,
-                                               const uint32_t (&)[9], uint32_t, int) {}
-};
-
-// The same walk for one pair without warp votes (lanes of a warp may belong to different nodes).
+// emb of one pair by walking the whole chain (lanes of a warp may belong to different nodes): W = the
+// pair's prepend word, B = B_0, vb = shared byte address of v's list in Wv, al = alpha_0..8, sig = code(y').
 template <int STRIDE>
 __device__ __forceinline__ uint32_t ba_chain_single(uint32_t W, uint32_t B, uint32_t vb, const uint32_t (&al)[9],
                                                     uint32_t sig, int L) {
@@ -145,4 +126,46 @@ __device__ __forceinline__ uint32_t ba_chain_single(uint32_t W, uint32_t B, uint
         }
     }
     return emb;
+}
+
+// Continue a chain from step s0: lk = local index of sigma_{s0-1}.z in v's list; returns the sum of the
+// remaining alpha_s B_s.
+__device__ __forceinline__ uint32_t ba_chain_from(int s0, uint32_t lk, uint32_t vb, const uint32_t (&al)[9],
+                                                  uint32_t sig, int L) {
+    uint32_t emb = 0u;
+#pragma unroll
+    for (int s = 1; s <= 8; s++) {
+        if (s >= s0 && L >= s && lk != 0u) {
+            const uint32_t hw = ba_lds_u16(vb + ((sig >> (s - 1)) & 1u) * 2u + lk * 4u);
+            emb += al[s] * (hw >> 8);
+            lk = hw & 0xffu;
+        }
+    }
+    return emb;
+}
+
+// Stable rank of every thread's key among the CTA (keys < NKEY; key < 0 = not ranked): order[pos] = tid with
+// pos = start[key] + (number of lower tids with the same key).  wcnt: [BA_NT/32][NKEY] scratch, start: [NKEY+1].
+template <int NKEY>
+__device__ __forceinline__ void ba_bucket_sort(int key, uint16_t *order, uint16_t *wcnt, uint16_t *start) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    for (int i = tid; i < (BA_NT / 32) * NKEY; i += BA_NT) wcnt[i] = 0;
+    __syncthreads();
+    const unsigned mm = __match_any_sync(0xffffffffu, key);
+    const int rank = __popc(mm & ((1u << lane) - 1u));
+    if (key >= 0 && rank == 0) wcnt[warp * NKEY + key] = (uint16_t)__popc(mm);
+    __syncthreads();
+    if (tid < NKEY) {                                       // exclusive scan over the warps, per key
+        int run = 0;
+        for (int w = 0; w < BA_NT / 32; w++) { const int c = wcnt[w * NKEY + tid]; wcnt[w * NKEY + tid] = (uint16_t)run; run += c; }
+        start[tid + 1] = (uint16_t)run;                     // bucket sizes, scanned below
+    }
+    __syncthreads();
+    if (tid == 0) {
+        int run = 0;
+        start[0] = 0;
+        for (int k = 0; k < NKEY; k++) { const int c = start[k + 1]; start[k + 1] = (uint16_t)(run + c); run += c; }
+    }
+    __syncthreads();
+    if (key >= 0) order[start[key] + wcnt[warp * NKEY + key] + rank] = (uint16_t)tid;
 }

@@ -8,116 +8,198 @@
 
 struct TileTables {
     int m = 0, nv = 0;
-    std::vector<uint2> T64;            // v-major pairs {W, P}; entries [0, BA_C) are the all-zero dummy chunk
+    std::vector<uint32_t> Wv;          // v-major prepend links (chain walks): entry vbase[v] + local index
     std::vector<uint32_t> vbase;       // [nv] entry index of v's list (its null entry)
-    std::vector<uint2> in_desc;        // [2][BA_NC][BA_NT]
+    // ---- input sweep: v-major ownership, slot (b, c, tid) <-> v
+    std::vector<uint2> FI;             // [BA_NCLS][2][BA_NC][BA_C][BA_NT] fast pairs
+    std::vector<uint16_t> in_owner;    // [2][BA_NC][BA_NT] v of the slot, 0xffff = unused
     std::vector<uint16_t> in_csr_off;  // [nv + 1]
-    std::vector<uint16_t> in_csr_idx;  // accumulator slots (b*BA_NC + slot)*BA_NT + thread of v's chunks
-    std::vector<uint2> Tz;             // z-major pairs {W, P'}; entries [0, BA_C) all-zero
-    std::vector<uint32_t> Wv;          // W words of T64 (chain walks of the output sweep)
-    std::vector<uint2> out_desc;       // [2][BA_NC][BA_NT]
-    std::vector<uint16_t> out_csr_off; // [2^{m+1}] indexed by code(z) - 1 (entry 0, the empty z, has no chunks)
+    std::vector<uint16_t> in_csr_idx;  // accumulator slots (b*BA_NC + c)*BA_NT + tid of v's chunks
+    std::vector<uint4> RI;             // [BA_NCLS][2][nri] riders (deep pairs), sorted by v
+    std::vector<uint16_t> ri_cnt;      // [BA_NCLS][2]
+    std::vector<uint16_t> ri_csr;      // [BA_NCLS][2][nv + 1] rider range of v
+    int nri = 0;
+    // ---- output sweep: z-major ownership, slot (b, c, tid) <-> code(z)
+    std::vector<uint2> FO;             // [BA_NCLS][2][BA_NC][BA_C][BA_NT]
+    std::vector<uint16_t> out_owner;   // [2][BA_NC][BA_NT] code(z) of the slot, 0xffff = unused
+    std::vector<uint16_t> out_csr_off; // [2^{m+1}] by code(z) - 1 (entry 0, the empty z, has no chunks)
     std::vector<uint16_t> out_csr_idx;
+    std::vector<uint4> RO;             // [BA_NCLS][2][nro] riders, sorted by code(z)
+    std::vector<uint16_t> ro_cnt;      // [BA_NCLS][2]
+    std::vector<uint16_t> ro_csr;      // [BA_NCLS][2][2^{m+1} + 1] rider range of code(z)
+    int nro = 0;
     bool ok = false;
 };
 
-static inline uint32_t tt_emb(uint32_t z, int lz, uint32_t v, int lv) {   // #embeddings of z in v (textbook DP)
-    uint32_t e[BA_MLOW + 2];
-    for (int r = 0; r <= lz; r++) e[r] = (r == 0);
-    for (int i = 0; i < lv; i++) {
-        const uint32_t vb = (v >> (lv - 1 - i)) & 1u;
-        for (int r = lz; r >= 1; r--)
-            if (((z >> (lz - r)) & 1u) == vb) e[r] += e[r - 1];
-    }
-    return e[lz];
+// code of sigma_s . z, sigma_s = low s bits of sig (the last s symbols of y')
+static inline uint32_t tt_prepend(uint32_t sig, int s, uint32_t cz) {
+    const int lz = 31 - __builtin_clz(cz);
+    return (1u << (lz + s)) | ((sig & ((1u << s) - 1u)) << lz) | (cz - (1u << lz));
 }
 
-struct TTChunk { int key, owner, first; };   // key = chain bound m - min|z|; owner = v or code(z); first = entry index
-
-static inline void tt_assign(std::vector<TTChunk> &ch, int b, uint32_t stride, bool in_side, const std::vector<uint32_t> &vbase,
-                             std::vector<uint2> &desc, std::vector<std::vector<uint16_t>> &owner_slots) {
-    std::stable_sort(ch.begin(), ch.end(), [](const TTChunk &x, const TTChunk &y) {
-        return x.key != y.key ? x.key < y.key : x.owner < y.owner;
-    });
-    for (size_t k = 0; k < ch.size(); k++) {
-        const int slot = (int)(k / BA_NT), thr = (int)(k % BA_NT);
-        const size_t di = ((size_t)b * BA_NC + slot) * BA_NT + thr;
-        uint2 d;
-        d.x = (uint32_t)ch[k].first * stride | ((uint32_t)ch[k].owner << 20) | 0x80000000u;
-        d.y = in_side ? vbase[ch[k].owner] * stride : 0u;
-        desc[di] = d;
-        owner_slots[ch[k].owner].push_back((uint16_t)di);
+// Deal the items of `pool[owner]` to the slots of each half-warp so that, at every pair position q, the 16
+// lanes read 16 different 8-byte bank pairs (residue = key & 15) whenever a matching exists.
+// slots: owner of slot k = (c, tid) with k = c*BA_NT + tid, or -1.  emit(k, q, owner, item).
+template <typename Emit>
+static void tt_place(const std::vector<int> &slot_owner, std::vector<std::vector<uint32_t>> &pool,
+                     const std::vector<uint8_t> &res_of_item_key, Emit emit) {
+    (void)res_of_item_key;
+    const int nslots = (int)slot_owner.size();
+    for (int k0 = 0; k0 < nslots; k0 += 16) {
+        for (int q = 0; q < BA_C; q++) {
+            int lanes[16], nl = 0;
+            for (int l = 0; l < 16 && k0 + l < nslots; l++) {
+                const int o = slot_owner[k0 + l];
+                if (o >= 0 && !pool[o].empty()) lanes[nl++] = k0 + l;
+            }
+            if (!nl) continue;
+            // bipartite matching lane -> residue (augmenting paths), lanes with the fewest options first
+            int match_res[16];                                  // residue -> lane index (into lanes[]) or -1
+            for (int r = 0; r < 16; r++) match_res[r] = -1;
+            uint32_t avail[16];
+            for (int i = 0; i < nl; i++) {
+                uint32_t a = 0;
+                for (uint32_t it : pool[slot_owner[lanes[i]]]) a |= 1u << (it & 15u);
+                avail[i] = a;
+            }
+            int order[16];
+            for (int i = 0; i < nl; i++) order[i] = i;
+            std::sort(order, order + nl, [&](int x, int y) { return __builtin_popcount(avail[x]) < __builtin_popcount(avail[y]); });
+            struct Aug {
+                static bool run(int i, uint32_t &seen, const uint32_t *avail, int *match_res) {
+                    for (int r = 0; r < 16; r++) {
+                        if (!((avail[i] >> r) & 1u) || ((seen >> r) & 1u)) continue;
+                        seen |= 1u << r;
+                        if (match_res[r] < 0 || run(match_res[r], seen, avail, match_res)) { match_res[r] = i; return true; }
+                    }
+                    return false;
+                }
+            };
+            for (int oi = 0; oi < nl; oi++) { uint32_t seen = 0; Aug::run(order[oi], seen, avail, match_res); }
+            int lane_res[16];
+            for (int i = 0; i < nl; i++) lane_res[i] = -1;
+            for (int r = 0; r < 16; r++) if (match_res[r] >= 0) lane_res[match_res[r]] = r;
+            int used[16] = {0};
+            for (int i = 0; i < nl; i++) {
+                std::vector<uint32_t> &P = pool[slot_owner[lanes[i]]];
+                if (P.empty()) continue;                        // a lane sharing its owner's pool took the last item
+                int pick = -1;
+                if (lane_res[i] >= 0)
+                    for (size_t j = 0; j < P.size(); j++) if ((int)(P[j] & 15u) == lane_res[i]) { pick = (int)j; break; }
+                if (pick < 0) {
+                    pick = 0;
+                    for (size_t j = 1; j < P.size(); j++) if (used[P[j] & 15u] < used[P[pick] & 15u]) pick = (int)j;
+                }
+                const uint32_t it = P[pick];
+                P.erase(P.begin() + pick);
+                used[it & 15u]++;
+                emit(lanes[i], q, slot_owner[lanes[i]], it);
+            }
+        }
     }
 }
 
 static inline void build_tile_tables(int m, TileTables &T) {
-    const int nv = 1 << m;
+    const int nv = 1 << m, NZc = 2 << m;                   // string codes 1 .. NZc-1
     T.m = m; T.nv = nv; T.ok = false;
-    // ---- v-major lists ------------------------------------------------------------------------
-    struct Ent { uint32_t code; uint32_t B; };
-    std::vector<std::vector<Ent>> lst(nv);                 // local index -> entry (code 0 = null / padding)
-    std::vector<std::vector<int>> loc(nv);                 // code(z) -> local index, 0 if absent
-    std::vector<int> start[2];
-    start[0].assign(nv, 0); start[1].assign(nv, 0);
-    std::vector<int> cnt[2];
-    cnt[0].assign(nv, 0); cnt[1].assign(nv, 0);
-    T.vbase.assign(nv, 0);
-    uint32_t total = BA_C;                                 // dummy chunk first
-    for (int v = 0; v < nv; v++) {
-        std::vector<Ent> &L = lst[v];
-        L.push_back({0u, 0u});                             // null
-        L.push_back({1u, 1u});                             // empty string, B = 1
-        for (int b = 0; b < 2; b++) {
-            start[b][v] = (int)L.size();
-            for (int lz = m; lz >= 1; lz--)                // longest first: short chains first
-                for (uint32_t z = 0; z < (1u << lz); z++) {
-                    if ((int)((z >> (lz - 1)) & 1u) != b) continue;
-                    const uint32_t B = tt_emb(z, lz, (uint32_t)v, m);
-                    if (B) { L.push_back({(1u << lz) | z, B}); cnt[b][v]++; }
+    // ---- B[code(w)][v] = emb(w, v): textbook DP over the positions of v, all prefixes of w at once ------
+    std::vector<uint8_t> B((size_t)NZc * nv, 0);
+    for (int v = 0; v < nv; v++)
+        for (int lw = 0; lw <= m; lw++)
+            for (uint32_t w = 0; w < (1u << lw); w++) {
+                uint32_t e[BA_MLOW + 2];
+                for (int r = 0; r <= lw; r++) e[r] = (r == 0);
+                for (int i = 0; i < m; i++) {
+                    const uint32_t vb = ((uint32_t)v >> (m - 1 - i)) & 1u;
+                    for (int r = lw; r >= 1; r--)
+                        if (((w >> (lw - r)) & 1u) == vb) e[r] += e[r - 1];
                 }
-            while ((L.size() - start[b][v]) % BA_C) L.push_back({0u, 0u});
-        }
-        if (L.size() > 255) return;                        // local links are 8 bit
-        loc[v].assign((size_t)2 << m, 0);
-        for (size_t i = 1; i < L.size(); i++)
-            if (L[i].code) loc[v][L[i].code] = (int)i;
+                B[(size_t)((1u << lw) | w) * nv + v] = (uint8_t)e[lw];       // <= C(8,4) = 70
+            }
+    auto Bof = [&](uint32_t cw, int v) -> uint32_t { return (cw < (uint32_t)NZc) ? B[(size_t)cw * nv + v] : 0u; };
+
+    // ---- v-major lists: [0] null  [1] empty string  [2..) the non-empty subsequences of v -----------------
+    std::vector<std::vector<int>> loc(nv);                 // code(z) -> local index, 0 if absent
+    T.vbase.assign(nv, 0);
+    uint32_t total = 0;
+    for (int v = 0; v < nv; v++) {
+        loc[v].assign(NZc, 0);
+        int li = 1;
+        loc[v][1] = li++;
+        for (uint32_t cz = 2; cz < (uint32_t)NZc; cz++)
+            if (Bof(cz, v)) loc[v][cz] = li++;
+        if (li > 256) return;                              // local links are 8 bit
         T.vbase[v] = total;
-        total += (uint32_t)L.size();
+        total += (uint32_t)li;
     }
-    if ((size_t)total * 8 >= (1u << 20) || (size_t)total * 4 >= (1u << 16)) return;
-    T.T64.assign(total, make_uint2(0u, 0u));
+    if ((size_t)total * 4 >= (1u << 20)) return;
     T.Wv.assign(total, 0u);
     for (int v = 0; v < nv; v++)
-        for (size_t i = 1; i < lst[v].size(); i++) {
-            const uint32_t cz = lst[v][i].code;
-            if (!cz) continue;
+        for (uint32_t cz = 1; cz < (uint32_t)NZc; cz++) {
+            const int li = loc[v][cz];
+            if (!li) continue;
             const int lz = 31 - __builtin_clz(cz);
-            const uint32_t zval = cz - (1u << lz);
             uint32_t W = 0;
             if (lz + 1 <= m)
                 for (uint32_t b = 0; b < 2; b++) {
-                    const uint32_t cbz = (1u << (lz + 1)) | (b << lz) | zval;
-                    const int li = loc[v][cbz];
-                    if (li) W |= ((uint32_t)li | (lst[v][li].B << 8)) << (16 * b);
+                    const uint32_t cbz = tt_prepend(b, 1, cz);
+                    const int lb = loc[v][cbz];
+                    if (lb) W |= ((uint32_t)lb | (Bof(cbz, v) << 8)) << (16 * b);
                 }
-            const uint32_t P = lst[v][i].B | ((uint32_t)lz << 8) | ((8u * cz) << 16);
-            T.T64[T.vbase[v] + i] = make_uint2(W, P);
-            T.Wv[T.vbase[v] + i] = W;
+            T.Wv[T.vbase[v] + li] = W;
         }
-    // ---- input-sweep schedule: chunks of BA_C consecutive pairs of one v -------------------------
-    T.in_desc.assign((size_t)2 * BA_NC * BA_NT, make_uint2(0u, 0u));
+
+    const size_t FSZ = (size_t)BA_NCLS * 2 * BA_NC * BA_C * BA_NT;
+    auto fidx = [](int cls, int b, int c, int q, int tid) -> size_t {
+        return ((((size_t)cls * 2 + b) * BA_NC + c) * BA_C + q) * BA_NT + tid;
+    };
+    auto first_bit = [](uint32_t cz) -> int { const int lz = 31 - __builtin_clz(cz); return (int)((cz >> (lz - 1)) & 1u); };
+    auto deep = [&](int cls, uint32_t cz, int v) -> bool {      // chain of (v,z) under class cls reaches s = BA_KB
+        const int lz = 31 - __builtin_clz(cz);
+        return lz + BA_KB <= m && Bof(tt_prepend((uint32_t)cls, BA_KB, cz), v) != 0;
+    };
+    auto bpack = [&](int cls, uint32_t cz, int v) -> uint32_t { // B_0..B_3 under class cls
+        uint32_t x = 0;
+        const int lz = 31 - __builtin_clz(cz);
+        for (int s = 0; s < 4; s++)
+            if (lz + s <= m) x |= Bof(tt_prepend((uint32_t)cls, s, cz), v) << (8 * s);
+        return x;
+    };
+    auto rider = [&](int cls, uint32_t cz, int v, uint32_t off, uint32_t owner) -> uint4 {
+        const uint32_t c4 = tt_prepend((uint32_t)cls, BA_KB, cz);
+        uint4 r;
+        r.x = bpack(cls, cz, v);
+        r.y = Bof(c4, v) | ((uint32_t)loc[v][c4] << 8) | (owner << 16);
+        r.z = off;
+        r.w = T.vbase[v] * 4u;
+        return r;
+    };
+
+    // ================= input sweep: chunks of v's list b, slots dealt round-robin over v =====================
+    T.FI.assign(FSZ, make_uint2(0u, 0u));
+    T.in_owner.assign((size_t)2 * BA_NC * BA_NT, 0xffffu);
     std::vector<std::vector<uint16_t>> vslots(nv);
+    std::vector<int> in_slot_owner[2];
     for (int b = 0; b < 2; b++) {
-        std::vector<TTChunk> ch;
-        for (int v = 0; v < nv; v++)
-            for (int i = 0; i * BA_C < cnt[b][v]; i++) {
-                const int first = start[b][v] + i * BA_C;
-                int last = std::min(cnt[b][v], (i + 1) * BA_C) - 1;
-                const uint32_t czl = lst[v][start[b][v] + last].code;
-                ch.push_back({m - (31 - __builtin_clz(czl)), v, (int)T.vbase[v] + first});
-            }
-        if (ch.size() > (size_t)BA_NC * BA_NT) return;
-        tt_assign(ch, b, 8u, true, T.vbase, T.in_desc, vslots);
+        std::vector<int> nch(nv, 0);
+        for (int v = 0; v < nv; v++) {
+            int cnt = 0;
+            for (uint32_t cz = 2; cz < (uint32_t)NZc; cz++) cnt += (Bof(cz, v) && first_bit(cz) == b);
+            nch[v] = (cnt + BA_C - 1) / BA_C;
+        }
+        std::vector<int> &so = in_slot_owner[b];
+        for (int r = 0;; r++) {
+            bool any = false;
+            for (int v = 0; v < nv; v++) if (nch[v] > r) { so.push_back(v); any = true; }
+            if (!any) break;
+        }
+        if (so.size() > (size_t)BA_NC * BA_NT) return;
+        for (size_t k = 0; k < so.size(); k++) {
+            const int c = (int)(k / BA_NT), tid = (int)(k % BA_NT);
+            const size_t ai = ((size_t)b * BA_NC + c) * BA_NT + tid;
+            T.in_owner[ai] = (uint16_t)so[k];
+            vslots[so[k]].push_back((uint16_t)ai);
+        }
     }
     T.in_csr_off.assign(nv + 1, 0);
     T.in_csr_idx.clear();
@@ -126,33 +208,55 @@ static inline void build_tile_tables(int m, TileTables &T) {
         for (uint16_t s : vslots[v]) T.in_csr_idx.push_back(s);
     }
     T.in_csr_off[nv] = (uint16_t)T.in_csr_idx.size();
-    // ---- z-major table and output-sweep schedule ------------------------------------------------
-    const int NZc = 2 << m;                                // codes 1 .. 2^{m+1}-1
-    T.Tz.assign(BA_C, make_uint2(0u, 0u));
-    T.out_desc.assign((size_t)2 * BA_NC * BA_NT, make_uint2(0u, 0u));
-    std::vector<std::vector<uint16_t>> zslots(NZc);
-    for (int b = 0; b < 2; b++) {
-        std::vector<TTChunk> ch;
-        for (int lz = m; lz >= 1; lz--)
-            for (uint32_t z = 0; z < (1u << lz); z++) {
-                if ((int)((z >> (lz - 1)) & 1u) != b) continue;
-                const uint32_t cz = (1u << lz) | z;
-                const int first = (int)T.Tz.size();
-                int nsup = 0;
-                for (int v = 0; v < nv; v++) {
-                    const int li = loc[v][cz];
-                    if (!li) continue;
-                    const uint32_t Pp = lst[v][li].B | ((uint32_t)v << 8) | ((4u * T.vbase[v]) << 16);
-                    T.Tz.push_back(make_uint2(T.Wv[T.vbase[v] + li], Pp));
-                    nsup++;
+
+    std::vector<std::vector<uint4>> rin((size_t)BA_NCLS * 2);
+    T.ri_csr.assign((size_t)BA_NCLS * 2 * (nv + 1), 0);
+    for (int cls = 0; cls < BA_NCLS; cls++)
+        for (int b = 0; b < 2; b++) {
+            std::vector<std::vector<uint32_t>> pool(nv);
+            std::vector<uint4> &R = rin[(size_t)cls * 2 + b];
+            for (int v = 0; v < nv; v++) {
+                T.ri_csr[((size_t)cls * 2 + b) * (nv + 1) + v] = (uint16_t)R.size();
+                for (uint32_t cz = 2; cz < (uint32_t)NZc; cz++) {
+                    if (!Bof(cz, v) || first_bit(cz) != b) continue;
+                    if (deep(cls, cz, v)) R.push_back(rider(cls, cz, v, 8u * cz, (uint32_t)v));
+                    else pool[v].push_back(cz);                  // item key = code(z): bank pair = code & 15
                 }
-                while ((T.Tz.size() - first) % BA_C) T.Tz.push_back(make_uint2(0u, 0u));
-                for (int i = 0; i * BA_C < nsup; i++) ch.push_back({m - lz, (int)cz, first + i * BA_C});
             }
-        if (ch.size() > (size_t)BA_NC * BA_NT) return;
-        tt_assign(ch, b, 8u, false, T.vbase, T.out_desc, zslots);
+            T.ri_csr[((size_t)cls * 2 + b) * (nv + 1) + nv] = (uint16_t)R.size();
+            tt_place(in_slot_owner[b], pool, std::vector<uint8_t>(), [&](int k, int q, int v, uint32_t cz) {
+                T.FI[fidx(cls, b, k / BA_NT, q, k % BA_NT)] = make_uint2(bpack(cls, cz, v), 8u * cz);
+            });
+            for (int v = 0; v < nv; v++) if (!pool[v].empty()) return;
+        }
+
+    // ================= output sweep: chunks of z's supersequence list, slots round-robin over z ===============
+    T.FO.assign(FSZ, make_uint2(0u, 0u));
+    T.out_owner.assign((size_t)2 * BA_NC * BA_NT, 0xffffu);
+    std::vector<std::vector<uint16_t>> zslots(NZc);
+    std::vector<int> out_slot_owner[2];
+    for (int b = 0; b < 2; b++) {
+        std::vector<int> nch(NZc, 0);
+        for (uint32_t cz = 2; cz < (uint32_t)NZc; cz++) {
+            if (first_bit(cz) != b) continue;
+            int cnt = 0;
+            for (int v = 0; v < nv; v++) cnt += (Bof(cz, v) != 0);
+            nch[cz] = (cnt + BA_C - 1) / BA_C;
+        }
+        std::vector<int> &so = out_slot_owner[b];
+        for (int r = 0;; r++) {
+            bool any = false;
+            for (uint32_t cz = 2; cz < (uint32_t)NZc; cz++) if (nch[cz] > r) { so.push_back((int)cz); any = true; }
+            if (!any) break;
+        }
+        if (so.size() > (size_t)BA_NC * BA_NT) return;
+        for (size_t k = 0; k < so.size(); k++) {
+            const int c = (int)(k / BA_NT), tid = (int)(k % BA_NT);
+            const size_t ai = ((size_t)b * BA_NC + c) * BA_NT + tid;
+            T.out_owner[ai] = (uint16_t)so[k];
+            zslots[so[k]].push_back((uint16_t)ai);
+        }
     }
-    if (T.Tz.size() * 8 >= (1u << 20)) return;
     T.out_csr_off.assign(NZc, 0);
     T.out_csr_idx.clear();
     for (int cz = 1; cz < NZc; cz++) {
@@ -160,5 +264,45 @@ static inline void build_tile_tables(int m, TileTables &T) {
         for (uint16_t s : zslots[cz]) T.out_csr_idx.push_back(s);
     }
     T.out_csr_off[NZc - 1] = (uint16_t)T.out_csr_idx.size();
+
+    std::vector<std::vector<uint4>> rout((size_t)BA_NCLS * 2);
+    T.ro_csr.assign((size_t)BA_NCLS * 2 * (NZc + 1), 0);
+    for (int cls = 0; cls < BA_NCLS; cls++)
+        for (int b = 0; b < 2; b++) {
+            std::vector<std::vector<uint32_t>> pool(NZc);
+            std::vector<uint4> &R = rout[(size_t)cls * 2 + b];
+            for (uint32_t cz = 0; cz < (uint32_t)NZc; cz++) {
+                T.ro_csr[((size_t)cls * 2 + b) * (NZc + 1) + cz] = (uint16_t)R.size();
+                if (cz < 2 || first_bit(cz) != b) continue;
+                for (int v = 0; v < nv; v++) {
+                    if (!Bof(cz, v)) continue;
+                    if (deep(cls, cz, v)) R.push_back(rider(cls, cz, v, 8u * (uint32_t)v, cz));
+                    else pool[cz].push_back((uint32_t)v);         // item key = v: bank pair = v & 15
+                }
+            }
+            T.ro_csr[((size_t)cls * 2 + b) * (NZc + 1) + NZc] = (uint16_t)R.size();
+            tt_place(out_slot_owner[b], pool, std::vector<uint8_t>(), [&](int k, int q, int cz, uint32_t v) {
+                T.FO[fidx(cls, b, k / BA_NT, q, k % BA_NT)] = make_uint2(bpack(cls, (uint32_t)cz, (int)v), 8u * v);
+            });
+            for (int cz = 0; cz < NZc; cz++) if (!pool[cz].empty()) return;
+        }
+
+    // ---- rider arrays, padded to a common capacity (multiple of 32, at most BA_NT) -------------------------
+    auto pack_riders = [&](std::vector<std::vector<uint4>> &src, std::vector<uint4> &dst, std::vector<uint16_t> &cnt, int &cap) {
+        size_t mx = 0;
+        for (auto &r : src) mx = std::max(mx, r.size());
+        cap = (int)((mx + 31) / 32 * 32);
+        if (cap == 0) cap = 32;
+        if (cap > BA_NT) return false;
+        dst.assign((size_t)BA_NCLS * 2 * cap, make_uint4(0u, 0u, 0u, 0u));
+        cnt.assign((size_t)BA_NCLS * 2, 0);
+        for (size_t i = 0; i < src.size(); i++) {
+            cnt[i] = (uint16_t)src[i].size();
+            std::copy(src[i].begin(), src[i].end(), dst.begin() + i * cap);
+        }
+        return true;
+    };
+    if (!pack_riders(rin, T.RI, T.ri_cnt, T.nri)) return;
+    if (!pack_riders(rout, T.RO, T.ro_cnt, T.nro)) return;
     T.ok = true;
 }
