@@ -11,6 +11,8 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <memory>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -76,6 +78,19 @@ struct ScratchLayout {
 
 static int low_m(int n) { return n < BA_MLOW ? n : BA_MLOW; }
 
+// The tile tables depend on m only and are immutable once built: one copy per process, built on first use.
+static std::shared_ptr<const TileTables> tile_tables(int m) {
+    static std::mutex mu;
+    static std::shared_ptr<const TileTables> cache[BA_MLOW + 1];
+    std::lock_guard<std::mutex> lk(mu);
+    if (!cache[m]) {
+        auto t = std::make_shared<TileTables>();
+        build_tile_tables(m, *t);
+        cache[m] = t;
+    }
+    return cache[m];
+}
+
 static void scratch_layout(int n, const TileTables &T, ScratchLayout &L) {
     const int m = low_m(n), h = n - m;
     const size_t NX = (size_t)1 << n, NY = ((size_t)2 << n) - 1, NZ = ((size_t)2 << m) - 1;
@@ -113,8 +128,8 @@ static void scratch_layout(int n, const TileTables &T, ScratchLayout &L) {
 
 extern "C" size_t ba_scratch_bytes(int n) {
     if (n < 1 || n > BA_NMAX) return 0;
-    TileTables T;
-    build_tile_tables(low_m(n), T);
+    const std::shared_ptr<const TileTables> Tp = tile_tables(low_m(n));
+    const TileTables &T = *Tp;
     if (!T.ok) return 0;
     ScratchLayout L;
     scratch_layout(n, T, L);
@@ -157,8 +172,8 @@ static cudaError_t upload(void *dst, const std::vector<V> &src, cudaStream_t st)
 }
 
 static int finish_create(ba_ctx *c) {
-    TileTables T;
-    build_tile_tables(c->m, T);
+    const std::shared_ptr<const TileTables> Tp = tile_tables(c->m);
+    const TileTables &T = *Tp;
     if (!T.ok) return fail(c, BA_EINVAL, "internal: tile tables do not fit their packed formats");
     ScratchLayout L;
     scratch_layout(c->n, T, L);
@@ -175,7 +190,7 @@ static int finish_create(ba_ctx *c) {
     c->counters = (unsigned int *)(s + L.counters); c->cnt = (unsigned long long *)(s + L.cnt);
     c->napart = L.napart; c->npart_cap = L.npart_cap;
     c->nWv = (int)T.Wv.size(); c->nri = T.nri; c->nro = T.nro;
-    c->n_in_csr = (int)T.in_csr_idx.size(); c->n_out_csr = (int)T.out_csr_idx.size();
+    c->n_in_csr = (int)T.in_csr_idx.size(); c->n_out_csr = T.out_ncsr;
 
     CK(upload(c->FI, T.FI, c->st)); CK(upload(c->FO, T.FO, c->st)); CK(upload(c->RI, T.RI, c->st)); CK(upload(c->RO, T.RO, c->st));
     CK(upload(c->Wv, T.Wv, c->st)); CK(upload(c->vbase, T.vbase, c->st));

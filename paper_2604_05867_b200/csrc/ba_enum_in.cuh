@@ -300,26 +300,14 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
 #pragma unroll
                     for (int c = 0; c < BA_NC; c++) {
                         if (!((whas >> (b * BA_NC + c)) & 1u)) continue;
-                        uint32_t B0[BA_C], B1[BA_C], B2[BA_C], B3[BA_C], ad[BA_C];
+                        uint32_t bp[BA_C], ad[BA_C];
 #pragma unroll
                         for (int q = 0; q < BA_C; q++) {
                             const uint2 pr = __ldg(F + (size_t)(c * BA_C + q) * BA_NT);
-                            B0[q] = pr.x & 0xffu; B1[q] = (pr.x >> 8) & 0xffu; B2[q] = (pr.x >> 16) & 0xffu; B3[q] = pr.x >> 24;
-                            ad[q] = pr.y;
+                            bp[q] = pr.x; ad[q] = pr.y;
                         }
                         if (MODE == IN_SWEEP) {
-                            double s = acc[b][c];
-#pragma unroll 2
-                            for (int i = 0; i < len; i++) {
-                                const uint4 al = bal[i];
-                                const uint32_t rb = rowbase + (uint32_t)i * ROWB;
-#pragma unroll
-                                for (int q = 0; q < BA_C; q++) {
-                                    const uint32_t emb = al.x * B0[q] + al.y * B1[q] + al.z * B2[q] + al.w * B3[q];
-                                    s = fma(ba_u2d(emb), ba_lds_f64(rb + ad[q]), s);
-                                }
-                            }
-                            acc[b][c] = s;
+                            acc[b][c] = ba_fast_chunk(acc[b][c], bal, rowbase, ROWB, len, bp, ad);
                         } else {
                             const uint32_t ov = a.owner[((size_t)b * BA_NC + c) * BA_NT + tid];
                             for (int i = 0; i < len; i++) {
@@ -328,8 +316,8 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                                 const int k = (int)(rc.info >> 16);
 #pragma unroll
                                 for (int q = 0; q < BA_C; q++) {
-                                    if (!B0[q]) continue;
-                                    const uint32_t emb = al.x * B0[q] + al.y * B1[q] + al.z * B2[q] + al.w * B3[q];
+                                    if (!(bp[q] & 0xffu)) continue;
+                                    const uint32_t emb = al.x * (bp[q] & 0xffu) + al.y * ((bp[q] >> 8) & 0xffu) + al.z * ((bp[q] >> 16) & 0xffu) + al.w * (bp[q] >> 24);
                                     const uint32_t cz = ad[q] >> 3;
                                     const int jz = ba_len_of_code(cz);
                                     if (MODE == IN_HC) {

@@ -42,9 +42,9 @@ struct OutArgs {
     const uint16_t *ro_cnt;    // [cls][b]
     const uint16_t *ro_csr;    // [cls][b][2^{m+1} + 1] by code(z)
     int nro;
-    const uint16_t *owner;     // [b][c][tid] -> code(z)
-    const uint16_t *csr_off;   // [2^{m+1}] by code(z)-1
-    const uint16_t *csr_idx;
+    const uint16_t *owner;     // [cls][b][c][tid] -> code(z)
+    const uint16_t *csr_off;   // [cls][2^{m+1}] by code(z)-1
+    const uint16_t *csr_idx;   // [cls][ncsr]
     int ncsr;
     const double *p;           // NX
     double *Apart;             // (2^{h+1}-1) * (2^{m+1}-1)
@@ -55,7 +55,7 @@ struct OutArgs {
     unsigned long long *cnt;   // OUT_COUNT
 };
 
-struct OutSmem { size_t Wv, rec, rows, bal, bnode, order, wcnt, bstart, batch, csr_off, csr_idx, red, item, total; };
+struct OutSmem { size_t Wv, rec, rows, bal, bnode, order, wcnt, bstart, batch, red, item, total; };
 
 __host__ __device__ static inline OutSmem enum_out_smem(int m, int nWv, int ncsr, int nro) {
     OutSmem s;
@@ -71,8 +71,7 @@ __host__ __device__ static inline OutSmem enum_out_smem(int m, int nWv, int ncsr
     s.wcnt = take((size_t)(BA_NT / 32) * 4 * 2);
     s.bstart = take(5 * 2);
     s.batch = take((size_t)BA_OUT_MAXB * 4);
-    s.csr_off = take(((size_t)2 << m) * 2);
-    s.csr_idx = take((size_t)ncsr * 2);
+    (void)ncsr;
     s.red = take(32 * 8);
     s.item = take(16);
     s.total = o;
@@ -98,19 +97,10 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
     uint16_t *s_wcnt = (uint16_t *)(smem + L.wcnt);
     uint16_t *s_bstart = (uint16_t *)(smem + L.bstart);
     uint32_t *s_batch = (uint32_t *)(smem + L.batch);
-    uint16_t *s_csr_off = (uint16_t *)(smem + L.csr_off);
-    uint16_t *s_csr_idx = (uint16_t *)(smem + L.csr_idx);
     double *s_red = (double *)(smem + L.red);
     uint32_t *s_item = (uint32_t *)(smem + L.item);        // [0] item, [1] number of batches
 
     for (int i = tid; i < a.nWv; i += BA_NT) s_Wv[i] = a.Wv[i];
-    for (int i = tid; i < (2 << m); i += BA_NT) s_csr_off[i] = a.csr_off[i];
-    for (int i = tid; i < a.ncsr; i += BA_NT) s_csr_idx[i] = a.csr_idx[i];
-
-    uint32_t whas = 0;
-#pragma unroll
-    for (int s = 0; s < 2 * BA_NC; s++)
-        if (__any_sync(0xffffffffu, a.owner[(size_t)s * BA_NT + tid] != 0xffffu)) whas |= 1u << s;
     const uint32_t sWv = ba_smem_addr(s_Wv);
     const uint32_t sRows = ba_smem_addr(s_rows);
     const int ev = tid & (nv - 1);                          // v of this thread's empty-z pairs
@@ -301,36 +291,23 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                     const uint2 *F = a.FO + (((size_t)cls * 2 + b) * BA_NC) * BA_C * BA_NT + tid;
 #pragma unroll
                     for (int c = 0; c < BA_NC; c++) {
-                        if (!((whas >> (b * BA_NC + c)) & 1u)) continue;
-                        uint32_t B0[BA_C], B1[BA_C], B2[BA_C], B3[BA_C], ad[BA_C];
+                        uint32_t bp[BA_C], ad[BA_C];
 #pragma unroll
                         for (int q = 0; q < BA_C; q++) {
                             const uint2 pr = __ldg(F + (size_t)(c * BA_C + q) * BA_NT);
-                            B0[q] = pr.x & 0xffu; B1[q] = (pr.x >> 8) & 0xffu; B2[q] = (pr.x >> 16) & 0xffu; B3[q] = pr.x >> 24;
-                            ad[q] = pr.y;
+                            bp[q] = pr.x; ad[q] = pr.y;
                         }
                         if (MODE == OUT_SWEEP) {
-                            double s = acc[b][c];
-#pragma unroll 2
-                            for (int i = 0; i < len; i++) {
-                                const uint4 al = bal[i];
-                                const uint32_t rb = rowbase + (uint32_t)i * ROWB;
-#pragma unroll
-                                for (int q = 0; q < BA_C; q++) {
-                                    const uint32_t emb = al.x * B0[q] + al.y * B1[q] + al.z * B2[q] + al.w * B3[q];
-                                    s = fma(ba_u2d(emb), ba_lds_f64(rb + ad[q]), s);
-                                }
-                            }
-                            acc[b][c] = s;
+                            acc[b][c] = ba_fast_chunk(acc[b][c], bal, rowbase, ROWB, len, bp, ad);
                         } else {
-                            const uint32_t oz = a.owner[((size_t)b * BA_NC + c) * BA_NT + tid];
+                            const uint32_t oz = a.owner[(((size_t)cls * 2 + b) * BA_NC + c) * BA_NT + tid];
                             for (int i = 0; i < len; i++) {
                                 const uint4 al = bal[i];
                                 const uint32_t u = s_rec[bnode[i]].id;
 #pragma unroll
                                 for (int q = 0; q < BA_C; q++) {
-                                    if (!B0[q]) continue;
-                                    const uint32_t emb = al.x * B0[q] + al.y * B1[q] + al.z * B2[q] + al.w * B3[q];
+                                    if (!(bp[q] & 0xffu)) continue;
+                                    const uint32_t emb = al.x * (bp[q] & 0xffu) + al.y * ((bp[q] >> 8) & 0xffu) + al.z * ((bp[q] >> 16) & 0xffu) + al.w * (bp[q] >> 24);
                                     if (MODE == OUT_DEBUG) {
                                         if (oz == a.dbg_cz) a.dbg_out[((size_t)u << m) | (size_t)(ad[q] >> 3)] = emb;
                                     } else {
@@ -387,7 +364,8 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
             }
             for (uint32_t zi = 1u + tid; zi < NZ; zi += BA_NT) {   // zi = code(z) - 1
                 double s = 0.0;
-                for (int q = s_csr_off[zi]; q < s_csr_off[zi + 1]; q++) s += s_acc[s_csr_idx[q]];
+                const uint16_t *co = a.csr_off + (size_t)cls * (2u << m) + zi, *ci = a.csr_idx + (size_t)cls * a.ncsr;
+                for (int q = co[0]; q < co[1]; q++) s += s_acc[ci[q]];
                 const uint32_t cz = zi + 1u;
                 const int b = (int)((cz >> (ba_len_of_code(cz) - 1)) & 1u);
                 const uint16_t *cs = a.ro_csr + ((size_t)cls * 2 + b) * ((2u << m) + 1u) + cz;

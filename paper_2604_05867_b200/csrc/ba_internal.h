@@ -106,6 +106,62 @@ __device__ __forceinline__ double ba_u2d(uint32_t e) {
     return __hiloint2double(0x43300000, (int)e) - 4503599627370496.0;
 }
 
+// Pair positions q of a chunk whose int->FP64 conversion goes to the conversion unit (I2F on the XU pipe)
+// instead of the FP64 pipe: spreads the per-term conversion over two otherwise idle/half-rate pipes.
+#ifndef BA_CVT_XU_MASK
+#define BA_CVT_XU_MASK 0x0a
+#endif
+template <int Q>
+__device__ __forceinline__ double ba_cvt(uint32_t e) {
+    if ((BA_CVT_XU_MASK >> Q) & 1) return __uint2double_rn(e);
+    return ba_u2d(e);
+}
+
+// The hot loop of both sweeps: the BA_C pairs of one chunk (bp = B_0 | B_1<<8 | B_2<<16 | B_3<<24, ad = byte
+// offset of the operand in a staged row) against the `len` nodes of a batch (bal[i] = alpha_0..3, operand
+// rows at rowbase + i*ROWB).  NS = number of B_s that can be non-zero in this warp's pairs (depth + 1).
+template <int NS>
+__device__ __forceinline__ double ba_fast_loop(double s, const uint4 *bal, uint32_t rowbase, uint32_t ROWB, int len,
+                                               const uint32_t (&bp)[BA_C], const uint32_t (&ad)[BA_C]) {
+    uint32_t B0[BA_C], B1[BA_C], B2[BA_C], B3[BA_C];
+#pragma unroll
+    for (int q = 0; q < BA_C; q++) {
+        B0[q] = bp[q] & 0xffu; B1[q] = (bp[q] >> 8) & 0xffu; B2[q] = (bp[q] >> 16) & 0xffu; B3[q] = bp[q] >> 24;
+    }
+    double s2 = 0.0;                                        // two dependent-FMA chains instead of one
+#pragma unroll 2
+    for (int i = 0; i < len; i++) {
+        const uint4 al = bal[i];
+        const uint32_t rb = rowbase + (uint32_t)i * ROWB;
+#pragma unroll
+        for (int q = 0; q < BA_C; q++) {
+            uint32_t emb = al.x * B0[q];
+            if (NS >= 2) emb += al.y * B1[q];
+            if (NS >= 3) emb += al.z * B2[q];
+            if (NS >= 4) emb += al.w * B3[q];
+            const double e = (q == 0) ? ba_cvt<0>(emb) : (q == 1) ? ba_cvt<1>(emb) : (q == 2) ? ba_cvt<2>(emb)
+                           : (q == 3) ? ba_cvt<3>(emb) : ba_cvt<4>(emb);
+            if (q & 1) s2 = fma(e, ba_lds_f64(rb + ad[q]), s2);
+            else s = fma(e, ba_lds_f64(rb + ad[q]), s);
+        }
+    }
+    return s + s2;
+}
+
+// Dispatch on the warp-uniform depth of the chunk (B_s = 0 implies B_{s+1} = 0).
+__device__ __forceinline__ double ba_fast_chunk(double s, const uint4 *bal, uint32_t rowbase, uint32_t ROWB, int len,
+                                                const uint32_t (&bp)[BA_C], const uint32_t (&ad)[BA_C]) {
+    uint32_t any = 0;
+#pragma unroll
+    for (int q = 0; q < BA_C; q++) any |= bp[q];
+    any = __reduce_or_sync(0xffffffffu, any);
+    if (!any) return s;                                     // no pair of this warp in the slot
+    if (any >> 24) return ba_fast_loop<4>(s, bal, rowbase, ROWB, len, bp, ad);
+    if (any >> 16) return ba_fast_loop<3>(s, bal, rowbase, ROWB, len, bp, ad);
+    if (any >> 8) return ba_fast_loop<2>(s, bal, rowbase, ROWB, len, bp, ad);
+    return ba_fast_loop<1>(s, bal, rowbase, ROWB, len, bp, ad);
+}
+
 // emb of one pair by walking the whole chain (lanes of a warp may belong to different nodes): W = the
 // pair's prepend word, B = B_0, vb = shared byte address of v's list in Wv, al = alpha_0..8, sig = code(y').
 template <int STRIDE>

@@ -19,11 +19,12 @@ struct TileTables {
     std::vector<uint16_t> ri_cnt;      // [BA_NCLS][2]
     std::vector<uint16_t> ri_csr;      // [BA_NCLS][2][nv + 1] rider range of v
     int nri = 0;
-    // ---- output sweep: z-major ownership, slot (b, c, tid) <-> code(z)
+    // ---- output sweep: z-major ownership per class, slot (cls, b, c, tid) <-> code(z)
     std::vector<uint2> FO;             // [BA_NCLS][2][BA_NC][BA_C][BA_NT]
-    std::vector<uint16_t> out_owner;   // [2][BA_NC][BA_NT] code(z) of the slot, 0xffff = unused
-    std::vector<uint16_t> out_csr_off; // [2^{m+1}] by code(z) - 1 (entry 0, the empty z, has no chunks)
-    std::vector<uint16_t> out_csr_idx;
+    std::vector<uint16_t> out_owner;   // [BA_NCLS][2][BA_NC][BA_NT] code(z) of the slot, 0xffff = unused
+    std::vector<uint16_t> out_csr_off; // [BA_NCLS][2^{m+1}] by code(z) - 1 (entry 0, the empty z, has no chunks)
+    std::vector<uint16_t> out_csr_idx; // [BA_NCLS][out_ncsr]
+    int out_ncsr = 0;
     std::vector<uint4> RO;             // [BA_NCLS][2][nro] riders, sorted by code(z)
     std::vector<uint16_t> ro_cnt;      // [BA_NCLS][2]
     std::vector<uint16_t> ro_csr;      // [BA_NCLS][2][2^{m+1} + 1] rider range of code(z)
@@ -37,13 +38,15 @@ static inline uint32_t tt_prepend(uint32_t sig, int s, uint32_t cz) {
     return (1u << (lz + s)) | ((sig & ((1u << s) - 1u)) << lz) | (cz - (1u << lz));
 }
 
-// Deal the items of `pool[owner]` to the slots of each half-warp so that, at every pair position q, the 16
-// lanes read 16 different 8-byte bank pairs (residue = key & 15) whenever a matching exists.
-// slots: owner of slot k = (c, tid) with k = c*BA_NT + tid, or -1.  emit(k, q, owner, item).
+// Deal the items of `pool[owner]` to the slots (slot k = (c, tid), k = c*BA_NT + tid, owner slot_owner[k]) and
+// their BA_C pair positions q.  An item is key | depth << 28; key & 15 is the 8-byte bank pair of its operand.
+// The pools arrive sorted by chain depth, deepest first, and only items of the head's depth are candidates, so
+// an owner's deep pairs land in its first slots.  Per (half-warp, q) a bipartite matching lane -> bank pair
+// (augmenting paths, lanes with the fewest options first) picks, where it can, 16 different bank pairs.
+// emit(k, q, owner, key).
+#define BA_PLACE_WINDOW 12
 template <typename Emit>
-static void tt_place(const std::vector<int> &slot_owner, std::vector<std::vector<uint32_t>> &pool,
-                     const std::vector<uint8_t> &res_of_item_key, Emit emit) {
-    (void)res_of_item_key;
+static void tt_place(const std::vector<int> &slot_owner, std::vector<std::vector<uint32_t>> &pool, Emit emit) {
     const int nslots = (int)slot_owner.size();
     for (int k0 = 0; k0 < nslots; k0 += 16) {
         for (int q = 0; q < BA_C; q++) {
@@ -53,13 +56,14 @@ static void tt_place(const std::vector<int> &slot_owner, std::vector<std::vector
                 if (o >= 0 && !pool[o].empty()) lanes[nl++] = k0 + l;
             }
             if (!nl) continue;
-            // bipartite matching lane -> residue (augmenting paths), lanes with the fewest options first
-            int match_res[16];                                  // residue -> lane index (into lanes[]) or -1
+            int match_res[16];                                  // bank pair -> lane index (into lanes[]) or -1
             for (int r = 0; r < 16; r++) match_res[r] = -1;
             uint32_t avail[16];
             for (int i = 0; i < nl; i++) {
                 uint32_t a = 0;
-                for (uint32_t it : pool[slot_owner[lanes[i]]]) a |= 1u << (it & 15u);
+                const std::vector<uint32_t> &P = pool[slot_owner[lanes[i]]];
+                for (size_t j = 0; j < P.size() && j < (size_t)BA_PLACE_WINDOW && (P[j] >> 28) == (P[0] >> 28); j++)
+                    a |= 1u << (P[j] & 15u);
                 avail[i] = a;
             }
             int order[16];
@@ -85,15 +89,17 @@ static void tt_place(const std::vector<int> &slot_owner, std::vector<std::vector
                 if (P.empty()) continue;                        // a lane sharing its owner's pool took the last item
                 int pick = -1;
                 if (lane_res[i] >= 0)
-                    for (size_t j = 0; j < P.size(); j++) if ((int)(P[j] & 15u) == lane_res[i]) { pick = (int)j; break; }
+                    for (size_t j = 0; j < P.size() && j < (size_t)BA_PLACE_WINDOW && (P[j] >> 28) == (P[0] >> 28); j++)
+                        if ((int)(P[j] & 15u) == lane_res[i]) { pick = (int)j; break; }
                 if (pick < 0) {
                     pick = 0;
-                    for (size_t j = 1; j < P.size(); j++) if (used[P[j] & 15u] < used[P[pick] & 15u]) pick = (int)j;
+                    for (size_t j = 1; j < P.size() && j < (size_t)BA_PLACE_WINDOW && (P[j] >> 28) == (P[0] >> 28); j++)
+                        if (used[P[j] & 15u] < used[P[pick] & 15u]) pick = (int)j;
                 }
                 const uint32_t it = P[pick];
                 P.erase(P.begin() + pick);
                 used[it & 15u]++;
-                emit(lanes[i], q, slot_owner[lanes[i]], it);
+                emit(lanes[i], q, slot_owner[lanes[i]], it & 0x0fffffffu);
             }
         }
     }
@@ -158,6 +164,13 @@ static inline void build_tile_tables(int m, TileTables &T) {
         const int lz = 31 - __builtin_clz(cz);
         return lz + BA_KB <= m && Bof(tt_prepend((uint32_t)cls, BA_KB, cz), v) != 0;
     };
+    auto depth = [&](int cls, uint32_t cz, int v) -> int {     // largest s <= 3 with B_s != 0
+        const int lz = 31 - __builtin_clz(cz);
+        int d = 0;
+        for (int s = 1; s < 4; s++)
+            if (lz + s <= m && Bof(tt_prepend((uint32_t)cls, s, cz), v)) d = s;
+        return d;
+    };
     auto bpack = [&](int cls, uint32_t cz, int v) -> uint32_t { // B_0..B_3 under class cls
         uint32_t x = 0;
         const int lz = 31 - __builtin_clz(cz);
@@ -220,72 +233,80 @@ static inline void build_tile_tables(int m, TileTables &T) {
                 for (uint32_t cz = 2; cz < (uint32_t)NZc; cz++) {
                     if (!Bof(cz, v) || first_bit(cz) != b) continue;
                     if (deep(cls, cz, v)) R.push_back(rider(cls, cz, v, 8u * cz, (uint32_t)v));
-                    else pool[v].push_back(cz);                  // item key = code(z): bank pair = code & 15
+                    else pool[v].push_back(cz | ((uint32_t)depth(cls, cz, v) << 28));   // key = code(z): bank pair = code & 15
                 }
             }
             T.ri_csr[((size_t)cls * 2 + b) * (nv + 1) + nv] = (uint16_t)R.size();
-            tt_place(in_slot_owner[b], pool, std::vector<uint8_t>(), [&](int k, int q, int v, uint32_t cz) {
+            for (int v = 0; v < nv; v++)
+                std::stable_sort(pool[v].begin(), pool[v].end(), [](uint32_t x, uint32_t y) { return (x >> 28) > (y >> 28); });
+            tt_place(in_slot_owner[b], pool, [&](int k, int q, int v, uint32_t cz) {
                 T.FI[fidx(cls, b, k / BA_NT, q, k % BA_NT)] = make_uint2(bpack(cls, cz, v), 8u * cz);
             });
             for (int v = 0; v < nv; v++) if (!pool[v].empty()) return;
         }
 
-    // ================= output sweep: chunks of z's supersequence list, slots round-robin over z ===============
+    // ================= output sweep: per class, chunks of one z sorted by chain depth ========================
+    // The class of an output-sweep item is fixed, so slot ownership (and the CSR of the epilogue) may differ
+    // from class to class: the chunks of a class are sorted by depth and dealt to the slots in that order, so
+    // a warp's 32 x BA_C pairs share one depth and most warps run the 1- or 2-IMAD loop.
     T.FO.assign(FSZ, make_uint2(0u, 0u));
-    T.out_owner.assign((size_t)2 * BA_NC * BA_NT, 0xffffu);
-    std::vector<std::vector<uint16_t>> zslots(NZc);
-    std::vector<int> out_slot_owner[2];
-    for (int b = 0; b < 2; b++) {
-        std::vector<int> nch(NZc, 0);
-        for (uint32_t cz = 2; cz < (uint32_t)NZc; cz++) {
-            if (first_bit(cz) != b) continue;
-            int cnt = 0;
-            for (int v = 0; v < nv; v++) cnt += (Bof(cz, v) != 0);
-            nch[cz] = (cnt + BA_C - 1) / BA_C;
-        }
-        std::vector<int> &so = out_slot_owner[b];
-        for (int r = 0;; r++) {
-            bool any = false;
-            for (uint32_t cz = 2; cz < (uint32_t)NZc; cz++) if (nch[cz] > r) { so.push_back((int)cz); any = true; }
-            if (!any) break;
-        }
-        if (so.size() > (size_t)BA_NC * BA_NT) return;
-        for (size_t k = 0; k < so.size(); k++) {
-            const int c = (int)(k / BA_NT), tid = (int)(k % BA_NT);
-            const size_t ai = ((size_t)b * BA_NC + c) * BA_NT + tid;
-            T.out_owner[ai] = (uint16_t)so[k];
-            zslots[so[k]].push_back((uint16_t)ai);
-        }
-    }
-    T.out_csr_off.assign(NZc, 0);
-    T.out_csr_idx.clear();
-    for (int cz = 1; cz < NZc; cz++) {
-        T.out_csr_off[cz - 1] = (uint16_t)T.out_csr_idx.size();
-        for (uint16_t s : zslots[cz]) T.out_csr_idx.push_back(s);
-    }
-    T.out_csr_off[NZc - 1] = (uint16_t)T.out_csr_idx.size();
-
+    T.out_owner.assign((size_t)BA_NCLS * 2 * BA_NC * BA_NT, 0xffffu);
+    T.out_csr_off.assign((size_t)BA_NCLS * NZc, 0);
+    T.out_ncsr = 2 * BA_NC * BA_NT;
+    T.out_csr_idx.assign((size_t)BA_NCLS * T.out_ncsr, 0);
     std::vector<std::vector<uint4>> rout((size_t)BA_NCLS * 2);
     T.ro_csr.assign((size_t)BA_NCLS * 2 * (NZc + 1), 0);
-    for (int cls = 0; cls < BA_NCLS; cls++)
+    for (int cls = 0; cls < BA_NCLS; cls++) {
+        std::vector<std::vector<uint16_t>> zslots(NZc);
         for (int b = 0; b < 2; b++) {
-            std::vector<std::vector<uint32_t>> pool(NZc);
             std::vector<uint4> &R = rout[(size_t)cls * 2 + b];
+            struct Chunk { int cz, depth, ord; std::vector<uint32_t> items; };
+            std::vector<Chunk> chunks;
             for (uint32_t cz = 0; cz < (uint32_t)NZc; cz++) {
                 T.ro_csr[((size_t)cls * 2 + b) * (NZc + 1) + cz] = (uint16_t)R.size();
                 if (cz < 2 || first_bit(cz) != b) continue;
+                std::vector<uint32_t> pz;
                 for (int v = 0; v < nv; v++) {
                     if (!Bof(cz, v)) continue;
                     if (deep(cls, cz, v)) R.push_back(rider(cls, cz, v, 8u * (uint32_t)v, cz));
-                    else pool[cz].push_back((uint32_t)v);         // item key = v: bank pair = v & 15
+                    else pz.push_back((uint32_t)v | ((uint32_t)depth(cls, cz, v) << 28));   // key = v: bank pair = v & 15
+                }
+                std::stable_sort(pz.begin(), pz.end(), [](uint32_t x, uint32_t y) { return (x >> 28) > (y >> 28); });
+                for (size_t i = 0; i < pz.size(); i += BA_C) {
+                    Chunk ch;
+                    ch.cz = (int)cz; ch.depth = (int)(pz[i] >> 28); ch.ord = (int)(i / BA_C);
+                    for (size_t j = i; j < pz.size() && j < i + BA_C; j++) ch.items.push_back(pz[j] & 0x0fffffffu);
+                    chunks.push_back(ch);
                 }
             }
             T.ro_csr[((size_t)cls * 2 + b) * (NZc + 1) + NZc] = (uint16_t)R.size();
-            tt_place(out_slot_owner[b], pool, std::vector<uint8_t>(), [&](int k, int q, int cz, uint32_t v) {
+            if (chunks.size() > (size_t)BA_NC * BA_NT) return;
+            std::stable_sort(chunks.begin(), chunks.end(), [](const Chunk &x, const Chunk &y) {
+                return x.depth != y.depth ? x.depth > y.depth : x.ord < y.ord;     // neighbours own different z
+            });
+            std::vector<int> so(chunks.size());
+            std::vector<std::vector<uint32_t>> pool(NZc);        // owner = code(z): its items, deepest first
+            for (size_t k = 0; k < chunks.size(); k++) {
+                so[k] = chunks[k].cz;
+                for (uint32_t it : chunks[k].items) pool[chunks[k].cz].push_back(it | ((uint32_t)chunks[k].depth << 28));
+                const int c = (int)(k / BA_NT), tid = (int)(k % BA_NT);
+                const size_t ai = ((size_t)b * BA_NC + c) * BA_NT + tid;
+                T.out_owner[(size_t)cls * 2 * BA_NC * BA_NT + ai] = (uint16_t)chunks[k].cz;
+                zslots[chunks[k].cz].push_back((uint16_t)ai);
+            }
+            for (auto &pl : pool) std::stable_sort(pl.begin(), pl.end(), [](uint32_t x, uint32_t y) { return (x >> 28) > (y >> 28); });
+            tt_place(so, pool, [&](int k, int q, int cz, uint32_t v) {
                 T.FO[fidx(cls, b, k / BA_NT, q, k % BA_NT)] = make_uint2(bpack(cls, (uint32_t)cz, (int)v), 8u * v);
             });
-            for (int cz = 0; cz < NZc; cz++) if (!pool[cz].empty()) return;
+            for (auto &pl : pool) if (!pl.empty()) return;
         }
+        size_t n = 0;
+        for (int cz = 1; cz < NZc; cz++) {
+            T.out_csr_off[(size_t)cls * NZc + cz - 1] = (uint16_t)n;
+            for (uint16_t sl : zslots[cz]) T.out_csr_idx[(size_t)cls * T.out_ncsr + n++] = sl;
+        }
+        T.out_csr_off[(size_t)cls * NZc + NZc - 1] = (uint16_t)n;
+    }
 
     // ---- rider arrays, padded to a common capacity (multiple of 32, at most BA_NT) -------------------------
     auto pack_riders = [&](std::vector<std::vector<uint4>> &src, std::vector<uint4> &dst, std::vector<uint16_t> &cnt, int &cap) {

@@ -1,0 +1,74 @@
+"""CPU-side checks of the C ABI (include/ba.h): the library loads, exports every declared symbol, and the
+entry points that need no device behave as the header says (host part)."""
+import ctypes
+import os
+import re
+from math import comb
+
+import pytest
+
+import paper_2604_05867_b200 as ba
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def declared_symbols():
+    src = open(os.path.join(ROOT, "include", "ba.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(ba_[a-z_A-Z0-9]+)\s*\(", src)))
+
+
+def test_library_exports_every_declared_symbol():
+    L = ba.load()
+    syms = declared_symbols()
+    assert "ba_create" in syms and "ba_iterate" in syms and "ba_bounds" in syms and "ba_get_p" in syms
+    for s in syms:
+        assert hasattr(L, s), f"libba.so does not export {s}"
+    assert set(ba.EXPORTS) == set(syms)
+
+
+def test_terms_per_sweep_is_lemma6_sum():
+    # T(n) = sum_k 2^k sum_{i<=n-k} C(n,i)   (Lemma 6); values of SURVEY 8(a)
+    for n, want in [(8, 12866), (14, 9549554), (20, 6972520226), (24, 564842295746), (28, 45753316474466)]:
+        assert ba.ba_terms_per_sweep(n) == want
+        assert want == sum((1 << k) * sum(comb(n, i) for i in range(n - k + 1)) for k in range(n + 1))
+    for bad in (0, -3, ba.BA_NMAX + 1):
+        with pytest.raises(ba.BAError):
+            ba.ba_terms_per_sweep(bad)
+
+
+def test_scratch_bytes():
+    assert ba.ba_scratch_bytes(0) == 0 and ba.ba_scratch_bytes(ba.BA_NMAX + 1) == 0
+    prev = 0
+    for n in (1, 4, 8, 12, 20, 24, 28):
+        b = ba.ba_scratch_bytes(n)
+        assert b > prev and b % 256 == 0
+        prev = b
+    # c (2^{n+1} doubles) and Hc (2^n doubles) alone need 24 * 2^n bytes
+    assert ba.ba_scratch_bytes(24) >= 24 << 24
+    assert ba.ba_scratch_bytes(28) < 40e9                      # fits a 180 GB B200 many times over
+
+
+def test_create_rejects_bad_arguments_without_touching_the_device():
+    L = ba.load()
+    h = ctypes.c_void_p()
+    for n, d in [(0, 0.5), (-1, 0.5), (ba.BA_NMAX + 1, 0.5), (8, -0.1), (8, 1.5), (8, float("nan"))]:
+        assert L.ba_create(n, d, ctypes.byref(h)) == ba.BA_EINVAL
+        assert not h.value
+    assert L.ba_create(8, 0.5, None) == ba.BA_EINVAL
+    assert L.ba_create_ext(8, 0.5, None, None, None, None, 0, None, ctypes.byref(h)) == ba.BA_EINVAL
+    # null context: every entry point returns BA_EINVAL and ba_last_error gives a static string
+    assert L.ba_iterate(None, 1) == ba.BA_EINVAL
+    assert L.ba_bounds(None, None, None) == ba.BA_EINVAL
+    assert L.ba_get_p(None, None) == ba.BA_EINVAL
+    assert L.ba_set_mode(None, 0) == ba.BA_EINVAL
+    assert b"context" in L.ba_last_error(None)
+    L.ba_destroy(None)                                          # no-op
+
+
+def test_no_cpu_fallback():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("CUDA device present")
+    with pytest.raises(ba.BAError):
+        ba.ba_create(8, 0.5)
