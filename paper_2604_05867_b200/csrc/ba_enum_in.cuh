@@ -2,20 +2,21 @@
 // with their integer embedding counts emb(y,x) exactly once each.
 //
 // Work item = a high part u (h bits) with its 2^m inputs x = u.v; one persistent CTA per SM takes
-// items from an atomic counter.  Per item, in super-batches of BA_NT nodes:
-//   phase A  every thread UNRANKS one node: the r-th distinct subsequence y' of u in trie pre-order
-//            (the paper's stringUnrank idea, Alg. 4, with the subtree sizes Sub[pos] in the
-//            role of the Count table P:260-274 and NextPos P:256-258 done with clz on bit masks), and
-//            carries the integer embedding-count DP  E[i] = emb(y', u[0:i])  in registers along the
-//            descent; the node record {alpha_0..8, code(y'), mask} goes to shared memory.
-//   sort     the nodes that have non-empty-z pairs (mask != 0) are ranked, stably, by (class, mask).
-//   eps      the pair (v, empty) of every node: thread (v, node), whole chain walked (ba_chain_single).
-//   phase B  batches of <= BA_RB_IN nodes of one (class, mask).  The operand rows c(y'.z), z in
-//            {0,1}^{<=m}, of the batch are staged with 16-byte cp.async (9 contiguous segments of c per
-//            node), double buffered.  Every thread owns BA_NC chunks of BA_C pairs (v,z) per list; the
-//            chunk's B_0..B_3 and row offsets are constants of the batch (ba_internal.h "CLASSES"), so
-//            the loop over the nodes of the batch costs, per (x,y) term,
-//                 4 IMAD (emb) + 1 LDS.64 (operand) + 1 DADD (exact u32->f64) + 1 DFMA
+// items from an atomic counter.  Per item, in super-batches of BA_SBR * BA_NT nodes:
+//   phase A  (BA_SBR rounds) every thread UNRANKS one node per round: the r-th distinct subsequence y' of
+//            u in trie pre-order (the paper's stringUnrank idea, Alg. 4, with the subtree sizes
+//            Sub[pos] in the role of the Count table P:260-274 and NextPos P:256-258 done with clz on bit
+//            masks), and carries the integer embedding-count DP  E[i] = emb(y', u[0:i])  in registers
+//            along the descent; the node record {alpha_0..8, code(y'), mask} goes to shared memory.
+//   eps      the pair (v, empty) of every node of the round: thread (v, node), whole chain walked.
+//   sort     per list b (non-empty z starting with b; a node carries list b iff b cannot follow y' in u)
+//            the nodes are ranked, stably, by class; the rounds' runs are merged into one order.
+//   phase B  batches of <= BA_RB_IN nodes of one (list, class).  The operands c(y'.z), z = b.t, of a node
+//            form a HALF ROW of 2^m doubles indexed by code(t) (8 contiguous segments of c), staged with
+//            16-byte cp.async, double buffered.  Every thread owns BA_NC chunks of BA_C pairs (v,z) per
+//            list; the chunk's B_0..B_3 and row offsets are constants of the batch (ba_internal.h
+//            "CLASSES"), so the loop over the nodes of the batch costs, per (x,y) term,
+//                 1-4 IMAD (emb) + 1 LDS.64 (operand) + 1 exact u32->f64 + 1 DFMA
 //            with one FP64 accumulator per chunk kept in a register for the whole item.  Deep pairs
 //            ride along, one per thread, their partial sums handed to thread v through shared memory
 //            in a fixed order.
@@ -30,15 +31,16 @@
 
 enum { IN_SWEEP = 0, IN_HC = 1, IN_DEBUG = 2, IN_COUNT = 3 };
 
-#define BA_IN_NKEY (BA_NCLS * 3)
-#define BA_IN_MAXB (BA_IN_NKEY + BA_NT / BA_RB_IN)
+#define BA_IN_SB (BA_SBR * BA_NT)                           // nodes per super-batch
+#define BA_IN_NBKT (2 * BA_NCLS)                            // buckets: list b, class
+#define BA_IN_MAXB (BA_IN_NBKT + 2 * BA_IN_SB / BA_RB_IN)
 
 struct InArgs {
     KConst kc;
     const uint32_t *Wv;       // v-major prepend links
     const uint32_t *vbase;    // [2^m]
     int nWv;
-    const uint2 *FI;          // fast pairs [cls][b][c][q][tid]
+    const uint2 *FI;          // fast pairs [cls][b][c][q][tid]; .y = 8 * code(z[1:])
     const uint4 *RI;          // riders [cls][b][nri]
     const uint16_t *ri_cnt;   // [cls][b]
     const uint16_t *ri_csr;   // [cls][b][2^m + 1]
@@ -58,24 +60,26 @@ struct InArgs {
     unsigned long long *cnt;  // IN_COUNT: [0] terms, [1] emb sum
 };
 
-struct InSmem { size_t Wv, rec, ceps, rows, bal, bnode, order, wcnt, bstart, batch, rsum, csr_off, csr_idx, sub, red, kcw, item, total; };
+struct InSmem { size_t Wv, rec, ceps, rows, bal, bnode, ordr, seg, order, gstart, wcnt, batch, rsum, csr_off, csr_idx, sub, red, kcw, item, total; };
 
 __host__ __device__ static inline InSmem enum_in_smem(int m, int nWv, int ncsr, int nri) {
     InSmem s;
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o += (bytes + 15) & ~(size_t)15; return at; };
     s.Wv = take((size_t)nWv * 4);
-    s.rec = take((size_t)BA_NT * sizeof(NodeRec));
+    s.rec = take((size_t)BA_IN_SB * sizeof(NodeRec));
     s.ceps = take((size_t)BA_NT * 8);
-    size_t rows = (size_t)2 * BA_RB_IN * ((size_t)2 << m) * 8, ac = ((size_t)2 * BA_NC + 2) * BA_NT * 8;
+    size_t rows = (size_t)2 * BA_RB_IN * ((size_t)1 << m) * 8, ac = ((size_t)2 * BA_NC + 2) * BA_NT * 8;
     s.rows = take(rows > ac ? rows : ac);                  // the epilogue's accumulator staging aliases the rows
     s.bal = take((size_t)2 * BA_RB_IN * 16);
     s.bnode = take((size_t)2 * BA_RB_IN * 2);
-    s.order = take((size_t)BA_NT * 2);
-    s.wcnt = take((size_t)(BA_NT / 32) * BA_IN_NKEY * 2);
-    s.bstart = take((size_t)(BA_IN_NKEY + 1) * 2);
+    s.ordr = take((size_t)BA_SBR * 2 * BA_NT * 2);         // per round and list: the round's nodes by class
+    s.seg = take((size_t)BA_SBR * 2 * (BA_NCLS + 1) * 2);
+    s.order = take((size_t)2 * BA_IN_SB * 2);              // merged: bucket-major node ids of the super-batch
+    s.gstart = take((size_t)(BA_IN_NBKT + 1) * 2);
+    s.wcnt = take((size_t)(BA_NT / 32) * BA_NCLS * 2);
     s.batch = take((size_t)BA_IN_MAXB * 4);
-    s.rsum = take((size_t)2 * 2 * nri * 8);
+    s.rsum = take((size_t)2 * nri * 8);
     s.csr_off = take(((size_t)(1 << m) + 1) * 2);
     s.csr_idx = take((size_t)ncsr * 2);
     s.sub = take(32 * 4);
@@ -86,13 +90,19 @@ __host__ __device__ static inline InSmem enum_in_smem(int m, int nWv, int ncsr, 
     return s;
 }
 
+// z = b.t from the list b and code(t)
+__device__ __forceinline__ uint32_t ba_z_of_tail(uint32_t b, uint32_t tc) {
+    const int lt = ba_len_of_code(tc);
+    return (1u << (lt + 1)) | (b << lt) | (tc - (1u << lt));
+}
+
 template <int MODE>
 __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ InArgs a) {
     extern __shared__ __align__(16) unsigned char smem[];
     const int m = a.kc.m, h = a.kc.h, nv = 1 << m;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const InSmem L = enum_in_smem(m, a.nWv, a.ncsr, a.nri);
-    const uint32_t ROWD = 2u << m, ROWB = ROWD * 8u;
+    const uint32_t ROWD = 1u << m, ROWB = ROWD * 8u;        // half row: operands of the z = b.t, by code(t)
 
     uint32_t *s_Wv = (uint32_t *)(smem + L.Wv);
     NodeRec *s_rec = (NodeRec *)(smem + L.rec);
@@ -101,9 +111,11 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
     double *s_acc = s_rows;                                 // epilogue only
     uint4 *s_bal = (uint4 *)(smem + L.bal);
     uint16_t *s_bnode = (uint16_t *)(smem + L.bnode);
+    uint16_t *s_ordr = (uint16_t *)(smem + L.ordr);
+    uint16_t *s_seg = (uint16_t *)(smem + L.seg);
     uint16_t *s_order = (uint16_t *)(smem + L.order);
+    uint16_t *s_gstart = (uint16_t *)(smem + L.gstart);
     uint16_t *s_wcnt = (uint16_t *)(smem + L.wcnt);
-    uint16_t *s_bstart = (uint16_t *)(smem + L.bstart);
     uint32_t *s_batch = (uint32_t *)(smem + L.batch);
     double *s_rsum = (double *)(smem + L.rsum);
     uint16_t *s_csr_off = (uint16_t *)(smem + L.csr_off);
@@ -118,7 +130,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
     for (int i = tid; i <= nv; i += BA_NT) s_csr_off[i] = a.csr_off[i];
     for (int i = tid; i < a.ncsr; i += BA_NT) s_csr_idx[i] = a.csr_idx[i];
     for (int i = tid; i <= BA_NMAX_I; i += BA_NT) { s_w[i] = a.kc.w[i]; s_lebar[i] = a.kc.lebar[i]; }
-    for (int i = tid; i < 2 * BA_RB_IN; i += BA_NT) { s_rows[(size_t)i * ROWD] = 0.0; s_rows[(size_t)i * ROWD + 1] = 0.0; }
+    for (int i = tid; i < 2 * BA_RB_IN; i += BA_NT) s_rows[(size_t)i * ROWD] = 0.0;   // position 0: padding pairs
 
     // which of this warp's chunk slots hold pairs at all (static)
     uint32_t whas = 0;
@@ -161,104 +173,136 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
             for (int c = 0; c < BA_NC; c++) acc[b][c] = 0.0;
         double acc_eps = 0.0, acc_rid = 0.0;
 
-        for (uint32_t base = 0; base < NN; base += BA_NT) {
+        for (uint32_t base = 0; base < NN; base += BA_IN_SB) {
             __syncthreads();                                   // previous super-batch fully consumed
-            // ================= phase A: unrank node base+tid, DP along the descent =================
-            int key = -1;
-            if (base + tid < NN) {
-                uint32_t r = base + tid;
-                uint32_t E[BA_HMAX + 1];
+            const int nsb = (NN - base < (uint32_t)BA_IN_SB) ? (int)(NN - base) : BA_IN_SB;
+            const int nrounds = (nsb + BA_NT - 1) / BA_NT;
+            for (int rd = 0; rd < nrounds; rd++) {
+                // ================= phase A: unrank node base + rd*BA_NT + tid, DP along the descent =================
+                int key0 = -1, key1 = -1;
+                const int nn = (nsb - rd * BA_NT < BA_NT) ? (nsb - rd * BA_NT) : BA_NT;
+                if (tid < nn) {
+                    uint32_t r = base + (uint32_t)(rd * BA_NT + tid);
+                    uint32_t E[BA_HMAX + 1];
 #pragma unroll
-                for (int i = 0; i <= BA_HMAX; i++) E[i] = 1u;            // emb(empty, u[0:i]) = 1
-                uint32_t al[9];
-                al[0] = 1u;
+                    for (int i = 0; i <= BA_HMAX; i++) E[i] = 1u;            // emb(empty, u[0:i]) = 1
+                    uint32_t al[9];
+                    al[0] = 1u;
 #pragma unroll
-                for (int s = 1; s < 9; s++) al[s] = 0u;
-                int pos = 0, k = 0;
-                uint32_t cy = 1u;
-                while (r > 0) {
-                    r--;
-                    const int n0 = ba_nextpos(u, h, pos, 0u);
-                    const uint32_t s0 = (n0 < h) ? s_sub[n0 + 1] : 0u;
-                    uint32_t b;
-                    int p;
-                    if (r < s0) { b = 0u; p = n0; } else { r -= s0; b = 1u; p = ba_nextpos(u, h, pos, 1u); }
-                    const uint32_t mm = (b ? ur : ~ur) & ((h >= 32) ? 0xffffffffu : ((1u << h) - 1u));
-                    uint32_t run = 0u;
+                    for (int s = 1; s < 9; s++) al[s] = 0u;
+                    int pos = 0, k = 0;
+                    uint32_t cy = 1u;
+                    while (r > 0) {
+                        r--;
+                        const int n0 = ba_nextpos(u, h, pos, 0u);
+                        const uint32_t s0 = (n0 < h) ? s_sub[n0 + 1] : 0u;
+                        uint32_t b;
+                        int p;
+                        if (r < s0) { b = 0u; p = n0; } else { r -= s0; b = 1u; p = ba_nextpos(u, h, pos, 1u); }
+                        const uint32_t mm = (b ? ur : ~ur) & ((h >= 32) ? 0xffffffffu : ((1u << h) - 1u));
+                        uint32_t run = 0u;
 #pragma unroll
-                    for (int i = 0; i <= BA_HMAX; i++) {       // N[i] = sum_{j<i, u_j=b} E[j]
-                        const uint32_t old = E[i];
-                        E[i] = run;
-                        if ((mm >> i) & 1u) run += old;
+                        for (int i = 0; i <= BA_HMAX; i++) {       // N[i] = sum_{j<i, u_j=b} E[j]
+                            const uint32_t old = E[i];
+                            E[i] = run;
+                            if ((mm >> i) & 1u) run += old;
+                        }
+#pragma unroll
+                        for (int s = 8; s >= 1; s--) al[s] = al[s - 1];
+                        al[0] = run;                               // emb(y'.b, u)
+                        pos = p + 1; k++;
+                        cy = (cy << 1) | b;
                     }
+                    const uint32_t miss0 = ba_nextpos(u, h, pos, 0u) >= h, miss1 = ba_nextpos(u, h, pos, 1u) >= h;
+                    NodeRec rc;
 #pragma unroll
-                    for (int s = 8; s >= 1; s--) al[s] = al[s - 1];
-                    al[0] = run;                               // emb(y'.b, u)
-                    pos = p + 1; k++;
-                    cy = (cy << 1) | b;
+                    for (int s = 0; s < 9; s++) rc.a[s] = al[s];
+                    rc.id = cy;
+                    rc.info = miss0 | (miss1 << 1) | ((uint32_t)(k < 8 ? k : 8) << 8) | ((uint32_t)k << 16);
+                    rc.pad = 0u;
+                    s_rec[rd * BA_NT + tid] = rc;
+                    if (MODE == IN_SWEEP) s_ceps[tid] = a.c[cy];
+                    if (miss0) key0 = (int)(cy & (BA_NCLS - 1));
+                    if (miss1) key1 = (int)(cy & (BA_NCLS - 1));
                 }
-                const uint32_t miss0 = ba_nextpos(u, h, pos, 0u) >= h, miss1 = ba_nextpos(u, h, pos, 1u) >= h;
-                const uint32_t mask = miss0 | (miss1 << 1);
-                NodeRec rc;
-#pragma unroll
-                for (int s = 0; s < 9; s++) rc.a[s] = al[s];
-                rc.id = cy;
-                rc.info = mask | ((uint32_t)(k < 8 ? k : 8) << 8) | ((uint32_t)k << 16);
-                rc.pad = 0u;
-                s_rec[tid] = rc;
-                if (MODE == IN_SWEEP) s_ceps[tid] = a.c[cy];
-                if (mask) key = (int)(cy & (BA_NCLS - 1)) * 3 + (int)mask - 1;
-            }
-            const int nn = (NN - base < (uint32_t)BA_NT) ? (int)(NN - base) : BA_NT;
-            ba_bucket_sort<BA_IN_NKEY>(key, s_order, s_wcnt, s_bstart);
-            if (tid == 0) {                                    // batches: <= BA_RB_IN consecutive nodes of one key
-                int nb = 0;
-                for (int kq = 0; kq < BA_IN_NKEY; kq++)
-                    for (int off = s_bstart[kq]; off < s_bstart[kq + 1]; off += BA_RB_IN) {
-                        const int len = (s_bstart[kq + 1] - off < BA_RB_IN) ? (s_bstart[kq + 1] - off) : BA_RB_IN;
-                        s_batch[nb++] = (uint32_t)off | ((uint32_t)len << 16) | ((uint32_t)kq << 24);
+                // ================= sort: per list, the round's nodes by class (stable) =================
+                ba_bucket_sort<BA_NCLS>(key0, s_ordr + (size_t)(rd * 2 + 0) * BA_NT, s_wcnt, s_seg + (rd * 2 + 0) * (BA_NCLS + 1));
+                ba_bucket_sort<BA_NCLS>(key1, s_ordr + (size_t)(rd * 2 + 1) * BA_NT, s_wcnt, s_seg + (rd * 2 + 1) * (BA_NCLS + 1));
+
+                // ================= eps: the pair (v, empty) of every node of the round =================
+                for (int i = esub; i < nn; i += epn) {
+                    const NodeRec &rc = s_rec[rd * BA_NT + i];
+                    uint32_t al[9];
+                    const uint4 r0 = *(const uint4 *)&rc.a[0], r1 = *(const uint4 *)&rc.a[4], r2 = *(const uint4 *)&rc.a[8];
+                    al[0] = r0.x; al[1] = r0.y; al[2] = r0.z; al[3] = r0.w;
+                    al[4] = r1.x; al[5] = r1.y; al[6] = r1.z; al[7] = r1.w; al[8] = r2.x;
+                    const uint32_t cy = r2.y, info = r2.z;
+                    const int Lc = (int)((info >> 8) & 0xffu), k = (int)(info >> 16);
+                    const uint32_t emb = ba_chain_single<4>(eW, 1u, evb, al, cy, Lc);
+                    if (MODE == IN_SWEEP) {
+                        acc_eps = fma(ba_u2d(emb), s_ceps[i], acc_eps);
+                    } else if (MODE == IN_HC) {
+                        const double wk = s_w[k];
+                        if (wk != 0.0 && emb > 1u) acc_eps = fma(wk * (double)emb, log2((double)emb) - s_lebar[k], acc_eps);
+                        else if (wk != 0.0) acc_eps = fma(wk, -s_lebar[k], acc_eps);
+                    } else if (MODE == IN_DEBUG) {
+                        if (((u << m) | (uint32_t)ev) == a.dbg_x) a.dbg_out[cy - 1u] = emb;
+                    } else {
+                        cnt_terms += 1ull; cnt_emb += emb;
                     }
-                s_item[1] = (uint32_t)nb;
+                }
+                __syncthreads();                               // s_ceps is rewritten by the next round
+            }
+            // ================= merge the rounds: bucket (b, cls) = its runs in round order =================
+            if (tid < 32) {
+                int cnt = 0;
+                const int bq = tid >> 4, cq = tid & (BA_NCLS - 1);          // BA_IN_NBKT = 32 buckets, one per lane
+                for (int rd = 0; rd < nrounds; rd++) {
+                    const uint16_t *sg = s_seg + (rd * 2 + bq) * (BA_NCLS + 1) + cq;
+                    cnt += sg[1] - sg[0];
+                }
+                int incl = cnt;
+                for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += t; }
+                int pos = incl - cnt;
+                s_gstart[tid] = (uint16_t)pos;
+                if (tid == 31) s_gstart[32] = (uint16_t)incl;
+                for (int rd = 0; rd < nrounds; rd++) {
+                    const uint16_t *sg = s_seg + (rd * 2 + bq) * (BA_NCLS + 1) + cq;
+                    const uint16_t *od = s_ordr + (size_t)(rd * 2 + bq) * BA_NT;
+                    for (int i = sg[0]; i < sg[1]; i++) s_order[pos++] = (uint16_t)(rd * BA_NT + od[i]);
+                }
+                __syncwarp();
+                if (tid == 0) {                                // batches: <= BA_RB_IN consecutive nodes of one bucket
+                    int nb = 0;
+                    for (int kq = 0; kq < BA_IN_NBKT; kq++)
+                        for (int off = s_gstart[kq]; off < s_gstart[kq + 1]; off += BA_RB_IN) {
+                            const int len = (s_gstart[kq + 1] - off < BA_RB_IN) ? (s_gstart[kq + 1] - off) : BA_RB_IN;
+                            s_batch[nb++] = (uint32_t)off | ((uint32_t)len << 16) | ((uint32_t)kq << 24);
+                        }
+                    s_item[1] = (uint32_t)nb;
+                }
             }
             __syncthreads();
 
-            // ================= eps: the pair (v, empty) of every node =================
-            for (int i = esub; i < nn; i += epn) {
-                uint32_t al[9];
-                const uint4 r0 = *(const uint4 *)&s_rec[i].a[0], r1 = *(const uint4 *)&s_rec[i].a[4],
-                            r2 = *(const uint4 *)&s_rec[i].a[8];
-                al[0] = r0.x; al[1] = r0.y; al[2] = r0.z; al[3] = r0.w;
-                al[4] = r1.x; al[5] = r1.y; al[6] = r1.z; al[7] = r1.w; al[8] = r2.x;
-                const uint32_t cy = r2.y, info = r2.z;
-                const int Lc = (int)((info >> 8) & 0xffu), k = (int)(info >> 16);
-                const uint32_t emb = ba_chain_single<4>(eW, 1u, evb, al, cy, Lc);
-                if (MODE == IN_SWEEP) {
-                    acc_eps = fma(ba_u2d(emb), s_ceps[i], acc_eps);
-                } else if (MODE == IN_HC) {
-                    const double wk = s_w[k];
-                    if (wk != 0.0 && emb > 1u) acc_eps = fma(wk * (double)emb, log2((double)emb) - s_lebar[k], acc_eps);
-                    else if (wk != 0.0) acc_eps = fma(wk, -s_lebar[k], acc_eps);
-                } else if (MODE == IN_DEBUG) {
-                    if (((u << m) | (uint32_t)ev) == a.dbg_x) a.dbg_out[cy - 1u] = emb;
-                } else {
-                    cnt_terms += 1ull; cnt_emb += emb;
-                }
-            }
-
-            // ================= phase B: batches of one (class, mask) =================
+            // ================= phase B: batches of one (list, class) =================
             const int nbatch = (int)s_item[1];
-            auto stage = [&](int j) {                          // rows, alpha_0..3 and node ids of batch j
+            auto stage = [&](int j) {                          // half rows, alpha_0..3 and node ids of batch j
                 const uint32_t bi = s_batch[j];
                 const int start = (int)(bi & 0xffffu), len = (int)((bi >> 16) & 0xffu), buf = j & 1;
+                const uint32_t b = (bi >> 24) / BA_NCLS;
                 if (MODE == IN_SWEEP) {
-                    for (int pidx = tid; pidx < (len << m); pidx += BA_NT) {
-                        const int i = pidx >> m, pc = pidx & (nv - 1);
-                        if (pc == 0) continue;                 // codes 0, 1: padding target / the eps pair
+                    const int ppr = nv >> 1;                   // 16-byte pieces per half row (positions 2pc, 2pc+1)
+                    for (int pidx = tid; pidx < len * ppr; pidx += BA_NT) {
+                        const int i = pidx / ppr, pc = pidx - i * ppr;
                         const uint32_t cy = s_rec[s_order[start + i]].id;
-                        const uint32_t cz = 2u * (uint32_t)pc;
-                        const int jz = ba_len_of_code(cz);
-                        ba_cp_async16(sRows + ((uint32_t)(buf * BA_RB_IN + i) * ROWD + cz) * 8u,
-                                      a.c + (((size_t)cy << jz) + (cz - (1u << jz))));
+                        const uint32_t dst = sRows + ((uint32_t)(buf * BA_RB_IN + i) * ROWD) * 8u;
+                        if (pc == 0) {                         // position 1: t empty, z = "b"
+                            ba_cp_async8(dst + 8u, a.c + (((size_t)cy << 1) + b));
+                        } else {
+                            const uint32_t tc = 2u * (uint32_t)pc;
+                            const int lt = ba_len_of_code(tc);
+                            ba_cp_async16(dst + tc * 8u, a.c + (((size_t)cy << (lt + 1)) + ((size_t)b << lt) + (tc - (1u << lt))));
+                        }
                     }
                 }
                 if (tid < len) {
@@ -270,15 +314,10 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
             auto flush = [&](int j) {                          // thread v collects the rider sums of batch j
                 if (MODE != IN_SWEEP && MODE != IN_HC) return;
                 if (tid >= nv) return;
-                const uint32_t bi = s_batch[j];
-                const int kq = (int)(bi >> 24), cls = kq / 3, mask = kq % 3 + 1, buf = j & 1;
-#pragma unroll
-                for (int b = 0; b < 2; b++) {
-                    if (!((mask >> b) & 1)) continue;
-                    const uint16_t *cs = a.ri_csr + ((size_t)cls * 2 + b) * (nv + 1) + tid;
-                    const int e0 = cs[0], e1 = cs[1];
-                    for (int e = e0; e < e1; e++) acc_rid += s_rsum[((size_t)buf * 2 + b) * a.nri + e];
-                }
+                const int kq = (int)(s_batch[j] >> 24), buf = j & 1;
+                const uint16_t *cs = a.ri_csr + (size_t)((kq % BA_NCLS) * 2 + kq / BA_NCLS) * (nv + 1) + tid;
+                const int e0 = cs[0], e1 = cs[1];
+                for (int e = e0; e < e1; e++) acc_rid += s_rsum[(size_t)buf * a.nri + e];
             };
             if (nbatch > 0) stage(0);
             for (int j = 0; j < nbatch; j++) {
@@ -288,13 +327,13 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 if (j > 0) flush(j - 1);
                 const uint32_t bi = s_batch[j];
                 const int len = (int)((bi >> 16) & 0xffu), kq = (int)(bi >> 24), buf = j & 1;
-                const int cls = kq / 3, mask = kq % 3 + 1;
+                const int cls = kq % BA_NCLS, bsel = kq / BA_NCLS;
                 const uint32_t rowbase = sRows + (uint32_t)(buf * BA_RB_IN) * ROWB;
                 const uint4 *bal = s_bal + buf * BA_RB_IN;
                 const uint16_t *bnode = s_bnode + buf * BA_RB_IN;
 #pragma unroll
                 for (int b = 0; b < 2; b++) {
-                    if (!((mask >> b) & 1)) continue;
+                    if (b != bsel) continue;
                     // ---- fast pairs -----------------------------------------------------------------------
                     const uint2 *F = a.FI + (((size_t)cls * 2 + b) * BA_NC) * BA_C * BA_NT + tid;
 #pragma unroll
@@ -317,8 +356,9 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
 #pragma unroll
                                 for (int q = 0; q < BA_C; q++) {
                                     if (!(bp[q] & 0xffu)) continue;
-                                    const uint32_t emb = al.x * (bp[q] & 0xffu) + al.y * ((bp[q] >> 8) & 0xffu) + al.z * ((bp[q] >> 16) & 0xffu) + al.w * (bp[q] >> 24);
-                                    const uint32_t cz = ad[q] >> 3;
+                                    const uint32_t emb = al.x * (bp[q] & 0xffu) + al.y * ((bp[q] >> 8) & 0xffu) +
+                                                         al.z * ((bp[q] >> 16) & 0xffu) + al.w * (bp[q] >> 24);
+                                    const uint32_t cz = ba_z_of_tail((uint32_t)b, ad[q] >> 3);
                                     const int jz = ba_len_of_code(cz);
                                     if (MODE == IN_HC) {
                                         const double wk = s_w[k + jz];
@@ -344,7 +384,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                             const uint4 rd = __ldg(a.RI + ((size_t)cls * 2 + b) * a.nri + tid);
                             const uint32_t B0 = rd.x & 0xffu, B1 = (rd.x >> 8) & 0xffu, B2 = (rd.x >> 16) & 0xffu, B3 = rd.x >> 24;
                             const uint32_t B4 = rd.y & 0xffu, lk4 = (rd.y >> 8) & 0xffu, ov = rd.y >> 16;
-                            const uint32_t cz = rd.z >> 3;
+                            const uint32_t cz = ba_z_of_tail((uint32_t)b, rd.z >> 3);
                             const int jz = ba_len_of_code(cz);
                             const uint32_t vb = sWv + rd.w;
                             for (int i = 0; i < len; i++) {
@@ -372,7 +412,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                                 }
                             }
                         }
-                        if ((MODE == IN_SWEEP || MODE == IN_HC) && tid < nr) s_rsum[((size_t)buf * 2 + b) * a.nri + tid] = s;
+                        if ((MODE == IN_SWEEP || MODE == IN_HC) && tid < nr) s_rsum[(size_t)buf * a.nri + tid] = s;
                     }
                 }
             }
@@ -427,7 +467,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 }
             }
             __syncthreads();
-            for (int i = tid; i < 2 * BA_RB_IN; i += BA_NT) { s_rows[(size_t)i * ROWD] = 0.0; s_rows[(size_t)i * ROWD + 1] = 0.0; }
+            for (int i = tid; i < 2 * BA_RB_IN; i += BA_NT) s_rows[(size_t)i * ROWD] = 0.0;   // restore position 0 of the rows
         }
         if (MODE == IN_DEBUG) break;
         __syncthreads();

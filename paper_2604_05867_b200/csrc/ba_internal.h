@@ -40,7 +40,8 @@
 #define BA_NC 3              // chunk slots per thread and list
 #define BA_KB 4              // class bits
 #define BA_NCLS 16           // 2^BA_KB classes
-#define BA_RB_IN 16          // nodes per batch, input sweep (operand rows of 2^{m+1} doubles)
+#define BA_RB_IN 16          // nodes per batch, input sweep (operand half-rows of 2^m doubles)
+#define BA_SBR 3             // input sweep: phase-A rounds (of BA_NT nodes) per super-batch
 #define BA_RB_OUT 32         // nodes per batch, output sweep (operand rows of 2^m doubles)
 
 // ---- v-major prepend links Wv: one uint32 per entry of v's list ([0] null, [1] empty string, then the
@@ -224,4 +225,5 @@ __device__ __forceinline__ void ba_bucket_sort(int key, uint16_t *order, uint16_
     }
     __syncthreads();
     if (key >= 0) order[start[key] + wcnt[warp * NKEY + key] + rank] = (uint16_t)tid;
+    __syncthreads();                                        // order[] complete; wcnt may be reused
 }

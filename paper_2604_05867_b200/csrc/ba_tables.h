@@ -164,6 +164,10 @@ static inline void build_tile_tables(int m, TileTables &T) {
         const int lz = 31 - __builtin_clz(cz);
         return lz + BA_KB <= m && Bof(tt_prepend((uint32_t)cls, BA_KB, cz), v) != 0;
     };
+    auto tail_of = [](uint32_t cz) -> uint32_t {               // code(t) for z = b.t
+        const int lz = 31 - __builtin_clz(cz);
+        return (1u << (lz - 1)) | (cz & ((1u << (lz - 1)) - 1u));
+    };
     auto depth = [&](int cls, uint32_t cz, int v) -> int {     // largest s <= 3 with B_s != 0
         const int lz = 31 - __builtin_clz(cz);
         int d = 0;
@@ -232,15 +236,18 @@ static inline void build_tile_tables(int m, TileTables &T) {
                 T.ri_csr[((size_t)cls * 2 + b) * (nv + 1) + v] = (uint16_t)R.size();
                 for (uint32_t cz = 2; cz < (uint32_t)NZc; cz++) {
                     if (!Bof(cz, v) || first_bit(cz) != b) continue;
-                    if (deep(cls, cz, v)) R.push_back(rider(cls, cz, v, 8u * cz, (uint32_t)v));
-                    else pool[v].push_back(cz | ((uint32_t)depth(cls, cz, v) << 28));   // key = code(z): bank pair = code & 15
+                    // the operand of z = b.t sits at position code(t) of the node's half row
+                    if (deep(cls, cz, v)) R.push_back(rider(cls, cz, v, 8u * tail_of(cz), (uint32_t)v));
+                    else pool[v].push_back(tail_of(cz) | ((uint32_t)depth(cls, cz, v) << 28));   // key = code(t): bank pair = key & 15
                 }
             }
             T.ri_csr[((size_t)cls * 2 + b) * (nv + 1) + nv] = (uint16_t)R.size();
             for (int v = 0; v < nv; v++)
                 std::stable_sort(pool[v].begin(), pool[v].end(), [](uint32_t x, uint32_t y) { return (x >> 28) > (y >> 28); });
-            tt_place(in_slot_owner[b], pool, [&](int k, int q, int v, uint32_t cz) {
-                T.FI[fidx(cls, b, k / BA_NT, q, k % BA_NT)] = make_uint2(bpack(cls, cz, v), 8u * cz);
+            tt_place(in_slot_owner[b], pool, [&](int k, int q, int v, uint32_t tc) {
+                const int lt = 31 - __builtin_clz(tc);
+                const uint32_t cz = (1u << (lt + 1)) | ((uint32_t)b << lt) | (tc - (1u << lt));
+                T.FI[fidx(cls, b, k / BA_NT, q, k % BA_NT)] = make_uint2(bpack(cls, cz, v), 8u * tc);
             });
             for (int v = 0; v < nv; v++) if (!pool[v].empty()) return;
         }
