@@ -31,6 +31,8 @@ struct ba_ctx {
     double *c = nullptr, *Hc = nullptr, *Apart = nullptr, *part = nullptr, *scal = nullptr, *hist = nullptr;
     uint2 *FI = nullptr, *FO = nullptr;
     uint4 *RI = nullptr, *RO = nullptr;
+    uint2 *EPS8 = nullptr;
+    uint32_t *RI8 = nullptr;
     uint32_t *Wv = nullptr, *vbase = nullptr;
     uint16_t *in_owner = nullptr, *out_owner = nullptr, *ri_cnt = nullptr, *ro_cnt = nullptr, *ri_csr = nullptr, *ro_csr = nullptr;
     uint16_t *in_csr_off = nullptr, *in_csr_idx = nullptr, *out_csr_off = nullptr, *out_csr_idx = nullptr;
@@ -71,7 +73,7 @@ static double host_binom(int n, int k) {
 
 // ------------------------------------------------------------------------------------------------ scratch layout
 struct ScratchLayout {
-    size_t c, Hc, Apart, part, scal, hist, FI, FO, RI, RO, Wv, vbase, in_owner, out_owner, ri_cnt, ro_cnt, ri_csr, ro_csr,
+    size_t c, Hc, Apart, part, scal, hist, FI, FO, RI, RO, EPS8, RI8, Wv, vbase, in_owner, out_owner, ri_cnt, ro_cnt, ri_csr, ro_csr,
         in_csr_off, in_csr_idx, out_csr_off, out_csr_idx, counters, cnt, total;
     size_t napart, npart_cap;
 };
@@ -109,6 +111,8 @@ static void scratch_layout(int n, const TileTables &T, ScratchLayout &L) {
     L.FO = o; o += align256(T.FO.size() * 8);
     L.RI = o; o += align256(T.RI.size() * 16);
     L.RO = o; o += align256(T.RO.size() * 16);
+    L.EPS8 = o; o += align256(T.EPS8.size() * 8);
+    L.RI8 = o; o += align256(T.RI8.size() * 4);
     L.Wv = o; o += align256(T.Wv.size() * 4);
     L.vbase = o; o += align256(T.vbase.size() * 4);
     L.in_owner = o; o += align256(T.in_owner.size() * 2);
@@ -181,6 +185,7 @@ static int finish_create(ba_ctx *c) {
     c->c = (double *)(s + L.c); c->Hc = (double *)(s + L.Hc); c->Apart = (double *)(s + L.Apart);
     c->part = (double *)(s + L.part); c->scal = (double *)(s + L.scal); c->hist = (double *)(s + L.hist);
     c->FI = (uint2 *)(s + L.FI); c->FO = (uint2 *)(s + L.FO); c->RI = (uint4 *)(s + L.RI); c->RO = (uint4 *)(s + L.RO);
+    c->EPS8 = (uint2 *)(s + L.EPS8); c->RI8 = (uint32_t *)(s + L.RI8);
     c->Wv = (uint32_t *)(s + L.Wv); c->vbase = (uint32_t *)(s + L.vbase);
     c->in_owner = (uint16_t *)(s + L.in_owner); c->out_owner = (uint16_t *)(s + L.out_owner);
     c->ri_cnt = (uint16_t *)(s + L.ri_cnt); c->ro_cnt = (uint16_t *)(s + L.ro_cnt);
@@ -193,6 +198,7 @@ static int finish_create(ba_ctx *c) {
     c->n_in_csr = (int)T.in_csr_idx.size(); c->n_out_csr = T.out_ncsr;
 
     CK(upload(c->FI, T.FI, c->st)); CK(upload(c->FO, T.FO, c->st)); CK(upload(c->RI, T.RI, c->st)); CK(upload(c->RO, T.RO, c->st));
+    CK(upload(c->EPS8, T.EPS8, c->st)); CK(upload(c->RI8, T.RI8, c->st));
     CK(upload(c->Wv, T.Wv, c->st)); CK(upload(c->vbase, T.vbase, c->st));
     CK(upload(c->in_owner, T.in_owner, c->st)); CK(upload(c->out_owner, T.out_owner, c->st));
     CK(upload(c->ri_cnt, T.ri_cnt, c->st)); CK(upload(c->ro_cnt, T.ro_cnt, c->st));
@@ -210,7 +216,7 @@ static int finish_create(ba_ctx *c) {
     CK(cudaGetDevice(&dev));
     CK(cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev));
     c->block = BA_NT;
-    c->smem_in = enum_in_smem(c->m, c->nWv, c->n_in_csr, c->nri).total;
+    c->smem_in = enum_in_smem(c->m, c->n_in_csr, c->nri).total;
     c->smem_out = enum_out_smem(c->m, c->nWv, c->n_out_csr, c->nro).total;
     CK(cudaFuncSetAttribute(k_enum_in<IN_SWEEP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_in));
     CK(cudaFuncSetAttribute(k_enum_in<IN_HC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_in));
@@ -294,8 +300,8 @@ extern "C" int ba_set_mode(ba_ctx *c, int mode) {
 // ------------------------------------------------------------------------------------------------ launches
 static InArgs make_in_args(ba_ctx *c) {
     InArgs a;
-    a.kc = c->kc; a.Wv = c->Wv; a.vbase = c->vbase; a.nWv = c->nWv;
-    a.FI = c->FI; a.RI = c->RI; a.ri_cnt = c->ri_cnt; a.ri_csr = c->ri_csr; a.nri = c->nri; a.owner = c->in_owner;
+    a.kc = c->kc;
+    a.FI = c->FI; a.RI = c->RI; a.EPS8 = c->EPS8; a.RI8 = c->RI8; a.ri_cnt = c->ri_cnt; a.ri_csr = c->ri_csr; a.nri = c->nri; a.owner = c->in_owner;
     a.csr_off = c->in_csr_off; a.csr_idx = c->in_csr_idx; a.ncsr = c->n_in_csr;
     a.c = c->c; a.p = c->p; a.Hc = c->Hc; a.D = c->D; a.part = c->part;
     a.counter = c->counters; a.dbg_x = 0; a.dbg_out = nullptr; a.cnt = c->cnt;

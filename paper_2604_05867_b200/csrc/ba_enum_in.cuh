@@ -37,9 +37,8 @@ enum { IN_SWEEP = 0, IN_HC = 1, IN_DEBUG = 2, IN_COUNT = 3 };
 
 struct InArgs {
     KConst kc;
-    const uint32_t *Wv;       // v-major prepend links
-    const uint32_t *vbase;    // [2^m]
-    int nWv;
+    const uint2 *EPS8;        // [256][2^m]: B(sigma_s, v), s = 1..8, of the pair (v, empty)
+    const uint32_t *RI8;      // [cls][b][16][nri]: B_5..B_8 of a rider by the sigma bits 4..7
     const uint2 *FI;          // fast pairs [cls][b][c][q][tid]; .y = 8 * code(z[1:])
     const uint4 *RI;          // riders [cls][b][nri]
     const uint16_t *ri_cnt;   // [cls][b]
@@ -60,13 +59,12 @@ struct InArgs {
     unsigned long long *cnt;  // IN_COUNT: [0] terms, [1] emb sum
 };
 
-struct InSmem { size_t Wv, rec, ceps, rows, bal, bnode, ordr, seg, order, gstart, wcnt, batch, rsum, csr_off, csr_idx, sub, red, kcw, item, total; };
+struct InSmem { size_t rec, ceps, rows, bal, bnode, ordr, seg, order, gstart, wcnt, batch, rsum, csr_off, csr_idx, sub, red, kcw, item, total; };
 
-__host__ __device__ static inline InSmem enum_in_smem(int m, int nWv, int ncsr, int nri) {
+__host__ __device__ static inline InSmem enum_in_smem(int m, int ncsr, int nri) {
     InSmem s;
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o += (bytes + 15) & ~(size_t)15; return at; };
-    s.Wv = take((size_t)nWv * 4);
     s.rec = take((size_t)BA_IN_SB * sizeof(NodeRec));
     s.ceps = take((size_t)BA_NT * 8);
     size_t rows = (size_t)2 * BA_RB_IN * ((size_t)1 << m) * 8, ac = ((size_t)2 * BA_NC + 2) * BA_NT * 8;
@@ -101,10 +99,9 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
     extern __shared__ __align__(16) unsigned char smem[];
     const int m = a.kc.m, h = a.kc.h, nv = 1 << m;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const InSmem L = enum_in_smem(m, a.nWv, a.ncsr, a.nri);
+    const InSmem L = enum_in_smem(m, a.ncsr, a.nri);
     const uint32_t ROWD = 1u << m, ROWB = ROWD * 8u;        // half row: operands of the z = b.t, by code(t)
 
-    uint32_t *s_Wv = (uint32_t *)(smem + L.Wv);
     NodeRec *s_rec = (NodeRec *)(smem + L.rec);
     double *s_ceps = (double *)(smem + L.ceps);
     double *s_rows = (double *)(smem + L.rows);
@@ -126,7 +123,6 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
     double *s_lebar = s_w + (BA_NMAX_I + 1);
     uint32_t *s_item = (uint32_t *)(smem + L.item);        // [0] item, [1] number of batches
 
-    for (int i = tid; i < a.nWv; i += BA_NT) s_Wv[i] = a.Wv[i];
     for (int i = tid; i <= nv; i += BA_NT) s_csr_off[i] = a.csr_off[i];
     for (int i = tid; i < a.ncsr; i += BA_NT) s_csr_idx[i] = a.csr_idx[i];
     for (int i = tid; i <= BA_NMAX_I; i += BA_NT) { s_w[i] = a.kc.w[i]; s_lebar[i] = a.kc.lebar[i]; }
@@ -137,13 +133,10 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
 #pragma unroll
     for (int s = 0; s < 2 * BA_NC; s++)
         if (__any_sync(0xffffffffu, a.owner[(size_t)s * BA_NT + tid] != 0xffffu)) whas |= 1u << s;
-    const uint32_t sWv = ba_smem_addr(s_Wv);
     const uint32_t sRows = ba_smem_addr(s_rows);
     const int ev = tid & (nv - 1);                          // v of this thread's empty-z pairs
     const int esub = tid >> m, epn = BA_NT >> m;            // it serves nodes esub, esub + epn, ...
-    const uint32_t evb = sWv + a.vbase[ev] * 4u;            // v's list
     __syncthreads();
-    const uint32_t eW = s_Wv[a.vbase[ev] + 1];              // W of (v, empty)
 
     unsigned long long cnt_terms = 0, cnt_emb = 0;
 
@@ -232,13 +225,14 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 // ================= eps: the pair (v, empty) of every node of the round =================
                 for (int i = esub; i < nn; i += epn) {
                     const NodeRec &rc = s_rec[rd * BA_NT + i];
-                    uint32_t al[9];
                     const uint4 r0 = *(const uint4 *)&rc.a[0], r1 = *(const uint4 *)&rc.a[4], r2 = *(const uint4 *)&rc.a[8];
-                    al[0] = r0.x; al[1] = r0.y; al[2] = r0.z; al[3] = r0.w;
-                    al[4] = r1.x; al[5] = r1.y; al[6] = r1.z; al[7] = r1.w; al[8] = r2.x;
-                    const uint32_t cy = r2.y, info = r2.z;
-                    const int Lc = (int)((info >> 8) & 0xffu), k = (int)(info >> 16);
-                    const uint32_t emb = ba_chain_single<4>(eW, 1u, evb, al, cy, Lc);
+                    const uint32_t cy = r2.y;
+                    const int k = (int)(r2.z >> 16);
+                    const uint2 e8 = __ldg(a.EPS8 + (size_t)(cy & 255u) * nv + ev);   // alpha_s = 0 beyond k
+                    const uint32_t emb = r0.x + r0.y * __byte_perm(e8.x, 0u, 0x4440) + r0.z * __byte_perm(e8.x, 0u, 0x4441) +
+                                         r0.w * __byte_perm(e8.x, 0u, 0x4442) + r1.x * __byte_perm(e8.x, 0u, 0x4443) +
+                                         r1.y * __byte_perm(e8.y, 0u, 0x4440) + r1.z * __byte_perm(e8.y, 0u, 0x4441) +
+                                         r1.w * __byte_perm(e8.y, 0u, 0x4442) + r2.x * __byte_perm(e8.y, 0u, 0x4443);
                     if (MODE == IN_SWEEP) {
                         acc_eps = fma(ba_u2d(emb), s_ceps[i], acc_eps);
                     } else if (MODE == IN_HC) {
@@ -291,9 +285,9 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 const int start = (int)(bi & 0xffffu), len = (int)((bi >> 16) & 0xffu), buf = j & 1;
                 const uint32_t b = (bi >> 24) / BA_NCLS;
                 if (MODE == IN_SWEEP) {
-                    const int ppr = nv >> 1;                   // 16-byte pieces per half row (positions 2pc, 2pc+1)
-                    for (int pidx = tid; pidx < len * ppr; pidx += BA_NT) {
-                        const int i = pidx / ppr, pc = pidx - i * ppr;
+                    // 16-byte pieces (positions 2pc, 2pc+1): 2^{m-1} per half row
+                    for (int pidx = tid; pidx < (len << (m - 1)); pidx += BA_NT) {
+                        const int i = pidx >> (m - 1), pc = pidx & ((nv >> 1) - 1);
                         const uint32_t cy = s_rec[s_order[start + i]].id;
                         const uint32_t dst = sRows + ((uint32_t)(buf * BA_RB_IN + i) * ROWD) * 8u;
                         if (pc == 0) {                         // position 1: t empty, z = "b"
@@ -383,20 +377,19 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                         if (tid < nr) {
                             const uint4 rd = __ldg(a.RI + ((size_t)cls * 2 + b) * a.nri + tid);
                             const uint32_t B0 = rd.x & 0xffu, B1 = (rd.x >> 8) & 0xffu, B2 = (rd.x >> 16) & 0xffu, B3 = rd.x >> 24;
-                            const uint32_t B4 = rd.y & 0xffu, lk4 = (rd.y >> 8) & 0xffu, ov = rd.y >> 16;
+                            const uint32_t B4 = rd.y & 0xffu, ov = rd.y >> 16;
                             const uint32_t cz = ba_z_of_tail((uint32_t)b, rd.z >> 3);
                             const int jz = ba_len_of_code(cz);
-                            const uint32_t vb = sWv + rd.w;
+                            const uint32_t *r8 = a.RI8 + ((size_t)cls * 2 + b) * 16 * a.nri + tid;
                             for (int i = 0; i < len; i++) {
                                 const NodeRec &rc = s_rec[bnode[i]];
-                                uint32_t al[9];
                                 const uint4 r0 = *(const uint4 *)&rc.a[0], r1 = *(const uint4 *)&rc.a[4], r2 = *(const uint4 *)&rc.a[8];
-                                al[0] = r0.x; al[1] = r0.y; al[2] = r0.z; al[3] = r0.w;
-                                al[4] = r1.x; al[5] = r1.y; al[6] = r1.z; al[7] = r1.w; al[8] = r2.x;
-                                const uint32_t cy = r2.y, info = r2.z;
-                                const int Lc = (int)((info >> 8) & 0xffu), k = (int)(info >> 16);
-                                const uint32_t emb = al[0] * B0 + al[1] * B1 + al[2] * B2 + al[3] * B3 + al[4] * B4 +
-                                                     ba_chain_from(BA_KB + 1, lk4, vb, al, cy, Lc);
+                                const uint32_t cy = r2.y;
+                                const int k = (int)(r2.z >> 16);
+                                const uint32_t x8 = __ldg(r8 + (size_t)((cy >> 4) & 15u) * a.nri);   // alpha_s = 0 beyond k
+                                const uint32_t emb = r0.x * B0 + r0.y * B1 + r0.z * B2 + r0.w * B3 + r1.x * B4 +
+                                                     r1.y * __byte_perm(x8, 0u, 0x4440) + r1.z * __byte_perm(x8, 0u, 0x4441) +
+                                                     r1.w * __byte_perm(x8, 0u, 0x4442) + r2.x * __byte_perm(x8, 0u, 0x4443);
                                 if (MODE == IN_SWEEP) {
                                     s = fma(ba_u2d(emb), ba_lds_f64(rowbase + (uint32_t)i * ROWB + rd.z), s);
                                 } else if (MODE == IN_HC) {

@@ -4,6 +4,7 @@
 #include "ba_internal.h"
 
 #include <algorithm>
+#include <utility>
 #include <vector>
 
 struct TileTables {
@@ -19,6 +20,8 @@ struct TileTables {
     std::vector<uint16_t> ri_cnt;      // [BA_NCLS][2]
     std::vector<uint16_t> ri_csr;      // [BA_NCLS][2][nv + 1] rider range of v
     int nri = 0;
+    std::vector<uint2> EPS8;           // [256][nv]: bytes s-1 = B(sigma_s, v), s = 1..8, sigma = the row index
+    std::vector<uint32_t> RI8;         // [BA_NCLS][2][16][nri]: bytes = B_5..B_8 of the rider for sigma bits 4..7
     // ---- output sweep: z-major ownership per class, slot (cls, b, c, tid) <-> code(z)
     std::vector<uint2> FO;             // [BA_NCLS][2][BA_NC][BA_C][BA_NT]
     std::vector<uint16_t> out_owner;   // [BA_NCLS][2][BA_NC][BA_NT] code(z) of the slot, 0xffff = unused
@@ -227,6 +230,7 @@ static inline void build_tile_tables(int m, TileTables &T) {
     T.in_csr_off[nv] = (uint16_t)T.in_csr_idx.size();
 
     std::vector<std::vector<uint4>> rin((size_t)BA_NCLS * 2);
+    std::vector<std::vector<std::pair<uint32_t, int>>> rin_zv((size_t)BA_NCLS * 2);
     T.ri_csr.assign((size_t)BA_NCLS * 2 * (nv + 1), 0);
     for (int cls = 0; cls < BA_NCLS; cls++)
         for (int b = 0; b < 2; b++) {
@@ -237,7 +241,10 @@ static inline void build_tile_tables(int m, TileTables &T) {
                 for (uint32_t cz = 2; cz < (uint32_t)NZc; cz++) {
                     if (!Bof(cz, v) || first_bit(cz) != b) continue;
                     // the operand of z = b.t sits at position code(t) of the node's half row
-                    if (deep(cls, cz, v)) R.push_back(rider(cls, cz, v, 8u * tail_of(cz), (uint32_t)v));
+                    if (deep(cls, cz, v)) {
+                        R.push_back(rider(cls, cz, v, 8u * tail_of(cz), (uint32_t)v));
+                        rin_zv[(size_t)cls * 2 + b].push_back(std::make_pair(cz, v));
+                    }
                     else pool[v].push_back(tail_of(cz) | ((uint32_t)depth(cls, cz, v) << 28));   // key = code(t): bank pair = key & 15
                 }
             }
@@ -332,5 +339,27 @@ static inline void build_tile_tables(int m, TileTables &T) {
     };
     if (!pack_riders(rin, T.RI, T.ri_cnt, T.nri)) return;
     if (!pack_riders(rout, T.RO, T.ro_cnt, T.nro)) return;
+    // ---- direct tables for the whole-chain pairs of the input sweep ------------------------------------------
+    T.EPS8.assign((size_t)256 * nv, make_uint2(0u, 0u));
+    for (uint32_t sig = 0; sig < 256u; sig++)
+        for (int v = 0; v < nv; v++) {
+            uint32_t w[2] = {0u, 0u};
+            for (int sft = 1; sft <= 8 && sft <= m; sft++)
+                w[(sft - 1) / 4] |= Bof((1u << sft) | (sig & ((1u << sft) - 1u)), v) << (8 * ((sft - 1) % 4));
+            T.EPS8[(size_t)sig * nv + v] = make_uint2(w[0], w[1]);
+        }
+    T.RI8.assign((size_t)BA_NCLS * 2 * 16 * T.nri, 0u);
+    for (int cls = 0; cls < BA_NCLS; cls++)
+        for (int b = 0; b < 2; b++)
+            for (uint32_t hi = 0; hi < 16u; hi++)
+                for (size_t e = 0; e < rin_zv[(size_t)cls * 2 + b].size(); e++) {
+                    const uint32_t cz = rin_zv[(size_t)cls * 2 + b][e].first;
+                    const int v = rin_zv[(size_t)cls * 2 + b][e].second;
+                    const int lz = 31 - __builtin_clz(cz);
+                    uint32_t x = 0;
+                    for (int sft = 5; sft <= 8; sft++)
+                        if (lz + sft <= m) x |= Bof(tt_prepend((hi << 4) | (uint32_t)cls, sft, cz), v) << (8 * (sft - 5));
+                    T.RI8[((((size_t)cls * 2 + b) * 16 + hi) * T.nri) + e] = x;
+                }
     T.ok = true;
 }
