@@ -372,15 +372,16 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                     }
                     // ---- riders: deep pairs of this class, one per thread ------------------------------------
                     const int nr = a.ri_cnt[cls * 2 + b];
-                    if (warp * 32 < nr) {
+                    const int re = BA_NT - 1 - tid;              // riders sit on the last warps (two chunk slots only)
+                    if (BA_NT - 32 * (warp + 1) < nr) {
                         double s = 0.0;
-                        if (tid < nr) {
-                            const uint4 rd = __ldg(a.RI + ((size_t)cls * 2 + b) * a.nri + tid);
+                        if (re < nr) {
+                            const uint4 rd = __ldg(a.RI + ((size_t)cls * 2 + b) * a.nri + re);
                             const uint32_t B0 = rd.x & 0xffu, B1 = (rd.x >> 8) & 0xffu, B2 = (rd.x >> 16) & 0xffu, B3 = rd.x >> 24;
                             const uint32_t B4 = rd.y & 0xffu, ov = rd.y >> 16;
                             const uint32_t cz = ba_z_of_tail((uint32_t)b, rd.z >> 3);
                             const int jz = ba_len_of_code(cz);
-                            const uint32_t *r8 = a.RI8 + ((size_t)cls * 2 + b) * 16 * a.nri + tid;
+                            const uint32_t *r8 = a.RI8 + ((size_t)cls * 2 + b) * 16 * a.nri + re;
                             for (int i = 0; i < len; i++) {
                                 const NodeRec &rc = s_rec[bnode[i]];
                                 const uint4 r0 = *(const uint4 *)&rc.a[0], r1 = *(const uint4 *)&rc.a[4], r2 = *(const uint4 *)&rc.a[8];
@@ -405,7 +406,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                                 }
                             }
                         }
-                        if ((MODE == IN_SWEEP || MODE == IN_HC) && tid < nr) s_rsum[(size_t)buf * a.nri + tid] = s;
+                        if ((MODE == IN_SWEEP || MODE == IN_HC) && re < nr) s_rsum[(size_t)buf * a.nri + re] = s;
                     }
                 }
             }

@@ -146,8 +146,8 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
         for (int b = 0; b < 2; b++) {
             rB[b][0] = rB[b][1] = rB[b][2] = 0u; roff[b] = 0u;
             const int nr = a.ro_cnt[cls * 2 + b];
-            if (tid < nr) {
-                const uint4 rd = __ldg(a.RO + ((size_t)cls * 2 + b) * a.nro + tid);
+            if (BA_NT - 1 - tid < nr) {                        // riders sit on the last warps (two chunk slots only)
+                const uint4 rd = __ldg(a.RO + ((size_t)cls * 2 + b) * a.nro + (BA_NT - 1 - tid));
                 rB[b][0] = rd.x;
                 roff[b] = rd.z;
                 uint32_t hi = rd.y & 0xffu, lk = (rd.y >> 8) & 0xffu, b8 = 0u;
@@ -244,9 +244,8 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                 const int start = (int)(bi & 0xffffu), len = (int)((bi >> 16) & 0xffu), buf = j & 1;
                 if (MODE == OUT_SWEEP) {
                     if (m >= 1) {
-                        const int ppr = nv >> 1;                   // 16-byte pieces per row
-                        for (int pidx = tid; pidx < len * ppr; pidx += BA_NT) {
-                            const int i = pidx / ppr, pc = pidx - i * ppr;
+                        for (int pidx = tid; pidx < (len << (m - 1)); pidx += BA_NT) {   // 16-byte pieces, 2^{m-1} per row
+                            const int i = pidx >> (m - 1), pc = pidx & ((nv >> 1) - 1);
                             const uint32_t u = s_rec[s_order[start + i]].id;
                             ba_cp_async16(sRows + (uint32_t)(buf * BA_RB_OUT + i) * ROWB + (uint32_t)pc * 16u,
                                           a.p + (((size_t)u << m) + 2u * (size_t)pc));
@@ -319,9 +318,9 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                     }
                     // ---- riders: deep pairs of this class, one per thread, all B_s static -----------------------
                     const int nr = a.ro_cnt[cls * 2 + b];
-                    if (warp * 32 < nr && tid < nr) {
+                    if (BA_NT - 1 - tid < nr) {
                         const uint32_t x0 = rB[b][0], x1 = rB[b][1], b8 = rB[b][2];
-                        const uint32_t oz = __ldg(a.RO + ((size_t)cls * 2 + b) * a.nro + tid).y >> 16;
+                        const uint32_t oz = __ldg(a.RO + ((size_t)cls * 2 + b) * a.nro + (BA_NT - 1 - tid)).y >> 16;
                         double s = acc_rid[b];
                         for (int i = 0; i < len; i++) {
                             const NodeRec &rc = s_rec[bnode[i]];
@@ -350,7 +349,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
             for (int b = 0; b < 2; b++) {
 #pragma unroll
                 for (int c = 0; c < BA_NC; c++) s_acc[((size_t)b * BA_NC + c) * BA_NT + tid] = acc[b][c];
-                if (tid < a.nro) s_acc[(size_t)2 * BA_NC * BA_NT + (size_t)b * a.nro + tid] = acc_rid[b];
+                if (BA_NT - 1 - tid < a.nro) s_acc[(size_t)2 * BA_NC * BA_NT + (size_t)b * a.nro + (BA_NT - 1 - tid)] = acc_rid[b];
             }
             double r0 = acc_eps;                               // z empty: block-wide sum, fixed tree
             for (int o = 16; o > 0; o >>= 1) r0 += __shfl_xor_sync(0xffffffffu, r0, o);

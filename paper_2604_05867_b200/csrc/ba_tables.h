@@ -41,6 +41,16 @@ static inline uint32_t tt_prepend(uint32_t sig, int s, uint32_t cz) {
     return (1u << (lz + s)) | ((sig & ((1u << s) - 1u)) << lz) | (cz - (1u << lz));
 }
 
+// Logical slot j (slots are dealt heaviest first) -> physical slot (c, tid).  Warp-slots of 32 logical slots go
+// to the warps in snake order, so that the deep chunks of slot column 0 meet the shallow end of column 1 and
+// every warp carries about the same number of IMADs between two barriers.
+static inline void tt_phys(int j, int &c, int &tid) {
+    const int ws = j / 32, nw = BA_NT / 32;
+    c = ws / nw;
+    const int w = (c & 1) ? (nw - 1 - ws % nw) : (ws % nw);
+    tid = w * 32 + j % 32;
+}
+
 // Deal the items of `pool[owner]` to the slots (slot k = (c, tid), k = c*BA_NT + tid, owner slot_owner[k]) and
 // their BA_C pair positions q.  An item is key | depth << 28; key & 15 is the 8-byte bank pair of its operand.
 // The pools arrive sorted by chain depth, deepest first, and only items of the head's depth are candidates, so
@@ -215,7 +225,8 @@ static inline void build_tile_tables(int m, TileTables &T) {
         }
         if (so.size() > (size_t)BA_NC * BA_NT) return;
         for (size_t k = 0; k < so.size(); k++) {
-            const int c = (int)(k / BA_NT), tid = (int)(k % BA_NT);
+            int c, tid;
+            tt_phys((int)k, c, tid);
             const size_t ai = ((size_t)b * BA_NC + c) * BA_NT + tid;
             T.in_owner[ai] = (uint16_t)so[k];
             vslots[so[k]].push_back((uint16_t)ai);
@@ -254,7 +265,9 @@ static inline void build_tile_tables(int m, TileTables &T) {
             tt_place(in_slot_owner[b], pool, [&](int k, int q, int v, uint32_t tc) {
                 const int lt = 31 - __builtin_clz(tc);
                 const uint32_t cz = (1u << (lt + 1)) | ((uint32_t)b << lt) | (tc - (1u << lt));
-                T.FI[fidx(cls, b, k / BA_NT, q, k % BA_NT)] = make_uint2(bpack(cls, cz, v), 8u * tc);
+                int c, tid;
+                tt_phys(k, c, tid);
+                T.FI[fidx(cls, b, c, q, tid)] = make_uint2(bpack(cls, cz, v), 8u * tc);
             });
             for (int v = 0; v < nv; v++) if (!pool[v].empty()) return;
         }
@@ -303,14 +316,17 @@ static inline void build_tile_tables(int m, TileTables &T) {
             for (size_t k = 0; k < chunks.size(); k++) {
                 so[k] = chunks[k].cz;
                 for (uint32_t it : chunks[k].items) pool[chunks[k].cz].push_back(it | ((uint32_t)chunks[k].depth << 28));
-                const int c = (int)(k / BA_NT), tid = (int)(k % BA_NT);
+                int c, tid;
+                tt_phys((int)k, c, tid);
                 const size_t ai = ((size_t)b * BA_NC + c) * BA_NT + tid;
                 T.out_owner[(size_t)cls * 2 * BA_NC * BA_NT + ai] = (uint16_t)chunks[k].cz;
                 zslots[chunks[k].cz].push_back((uint16_t)ai);
             }
             for (auto &pl : pool) std::stable_sort(pl.begin(), pl.end(), [](uint32_t x, uint32_t y) { return (x >> 28) > (y >> 28); });
             tt_place(so, pool, [&](int k, int q, int cz, uint32_t v) {
-                T.FO[fidx(cls, b, k / BA_NT, q, k % BA_NT)] = make_uint2(bpack(cls, (uint32_t)cz, (int)v), 8u * v);
+                int c, tid;
+                tt_phys(k, c, tid);
+                T.FO[fidx(cls, b, c, q, tid)] = make_uint2(bpack(cls, (uint32_t)cz, (int)v), 8u * v);
             });
             for (auto &pl : pool) if (!pl.empty()) return;
         }
