@@ -31,6 +31,16 @@ def terms_per_sweep(n):
     return sum((1 << k) * sum(comb(n, i) for i in range(n - k + 1)) for k in range(n + 1))
 
 
+def config_name(n, d):
+    if n == 24 and abs(d - 0.70) < 1e-12:
+        return "BASELINE.json configs[3], the headline throughput config"
+    if n == 28 and abs(d - 0.80) < 1e-12:
+        return "BASELINE.json configs[4]"
+    if n == 20:
+        return "one d of BASELINE.json configs[2]"
+    return "not a BASELINE.json config: parity / profiling size"
+
+
 def load_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -155,7 +165,7 @@ def run_reference(args, rank, world):
            "iterations_per_s": args.steps / dt, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
            "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
            "dtype": "f64", "data": "synthetic",
-           "config": {"workload": f"BDC_d^n BA iteration, n={args.n}, d={args.d}, uniform p0 (BASELINE.json configs[3])",
+           "config": {"workload": f"BDC_d^n BA iteration, n={args.n}, d={args.d}, uniform p0 ({config_name(args.n, args.d)})",
                       "sample": sample},
            "cpu_baseline": {"value": val, "unit": "terms/s", "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
            "e2e": {"value": val, "unit": "terms/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -206,13 +216,14 @@ def run_ours(args, rank, world, local_rank):
     clocks = sampler.stop() if rank == 0 else None
     tm = ba.ba_last_timing(ctx)
     I, U = ba.ba_bounds(ctx)
+    hist = ba.ba_get_history(ctx, min(args.steps + args.warmup, 4096))      # {I_t, U_t, log2 Z_t} of every iteration so far
     ms_total = replicas.max_over_ranks(ms_total, world, dev)
 
     # ---- end-to-end arm: the C ABI with HOST buffers; H2D of p and D2H of p + bounds every step -----
     p_host = torch.empty(NX, dtype=torch.float64).pin_memory()
     p_np = p_host.numpy()
     ba.ba_get_p(ctx, out=p_np)
-    e2e_steps = args.steps
+    e2e_steps = args.e2e_steps if args.e2e_steps > 0 else args.steps
     barrier()
     t0 = time.perf_counter()
     for _ in range(e2e_steps):
@@ -240,8 +251,14 @@ def run_ours(args, rank, world, local_rank):
         sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
         peak = alu_peak_tinst(sm_mhz)
         achieved = C_MIN * T / (dom_ms * 1e-3) / 1e12
+        smem_terms = SMS * 128.0 / 8.0 * sm_mhz * 1e6      # 128 B/clk/SM of shared-memory bandwidth, 8 B operand per term
         roofline = {"bound": "alu", "kernel": dom_name, "achieved": achieved, "peak": peak, "unit": "Tinstr/s",
                     "frac": achieved / peak, "traffic": read_traffic(dom_name),
+                    "other_kernel": {"name": "k_enum_in" if dom_name == "k_enum_out" else "k_enum_out",
+                                     "kernel_ms": min(tm["out_ms"], tm["in_ms"]),
+                                     "frac": C_MIN * T / (min(tm["out_ms"], tm["in_ms"]) * 1e-3) / 1e12 / peak},
+                    "smem_gather_roof_terms_per_s": smem_terms,
+                    "frac_of_smem_gather_roof": T / (dom_ms * 1e-3) / smem_terms,
                     "peak_source": f"148 SMs x 4 schedulers x 32 lanes x {sm_mhz:.0f} MHz (DESIGN.md), {peaks_src} max SM clock",
                     "algorithmic": f"{C_MIN} lane-instructions per term x T({n})={T} terms per launch",
                     "kernel_ms": dom_ms, "kernel_terms_per_s": T / (dom_ms * 1e-3),
@@ -268,14 +285,17 @@ def run_ours(args, rank, world, local_rank):
            "iterations_per_s": world * args.steps / (ms_total * 1e-3),
            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-           "config": {"workload": f"BDC_d^n BA iteration, n={n}, d={d}, uniform p0 (BASELINE.json configs[3])",
+           "config": {"workload": f"BDC_d^n BA iteration, n={n}, d={d}, uniform p0 ({config_name(n, d)})",
                       "mode": args.mode, "terms_per_iteration": 2 * T,
                       "term_counting": "enumerated" if args.mode == "enum" else "effective (FAST mode does not enumerate terms)",
-                      "l2_policy": "inputs_exceed_l2 (p 134 MB, q 268 MB, c 268 MB at n=24 vs 126 MB L2)" if n >= 24
+                      "l2_policy": f"inputs_exceed_l2 (p {8 * NX / 1e6:.0f} MB, q and c {16 * NX / 1e6:.0f} MB each, "
+                                   f"Apart {8 * ((2 << max(n - 8, 0)) - 1) * 511 / 1e6:.0f} MB vs 126 MB L2)" if n >= 24
                                    else "arrays fit L2 at this n (not the headline config)",
                       "parallelism": "single GPU" if world == 1 else f"{world} independent replicas (d sweep), no collective"},
            "kernels_ms": {"out_sweep": tm["out_ms"], "in_sweep": tm["in_ms"], "reduce_update": tm["update_ms"]},
-           "bounds_bits": {"I_lower": I, "maxD_upper": U, "upper_over_n": U / n},
+           "bounds_bits": {"I_lower": I, "maxD_upper": U, "upper_over_n": U / n,
+                           "running_min_upper_over_n": float(hist[:, 1].min()) / n,
+                           "upper_over_n_by_iteration": [round(float(v) / n, 9) for v in hist[:, 1]][-32:]},
            "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks,
            "e2e": {"value": 2.0 * T * world * e2e_steps / e2e_s, "unit": "terms/s", "steps": e2e_steps,
                    "ms_per_step": e2e_s / e2e_steps * 1e3,
@@ -298,6 +318,7 @@ def main():
     ap.add_argument("--oracle-n", type=int, default=14)
     ap.add_argument("--oracle-iters", type=int, default=10)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--e2e-steps", type=int, default=0, help="steps of the end-to-end arm (default: --steps)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
