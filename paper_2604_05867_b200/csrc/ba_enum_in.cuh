@@ -296,7 +296,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                         } else {
                             const uint32_t tc = 2u * (uint32_t)pc;
                             const int lt = ba_len_of_code(tc);
-                            ba_cp_async16(dst + tc * 8u, a.c + (((size_t)cy << (lt + 1)) + ((size_t)b << lt) + (tc - (1u << lt))));
+                            ba_cp_async16(dst + ba_swz(tc) * 8u, a.c + (((size_t)cy << (lt + 1)) + ((size_t)b << lt) + (tc - (1u << lt))));
                         }
                     }
                 }
@@ -316,13 +316,19 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
             };
             if (nbatch > 0) stage(0);
             for (int j = 0; j < nbatch; j++) {
+                const uint32_t bi = s_batch[j];
+                const int len = (int)((bi >> 16) & 0xffu), kq = (int)(bi >> 24), buf = j & 1;
+                const int cls = kq % BA_NCLS, bsel = kq / BA_NCLS;
+                // the pairs of a chunk do not depend on the staged rows: fetch slot 0 before waiting, and slot c+1
+                // while slot c is being computed, so that one L2 latency per batch is exposed at most
+                const uint2 *F = a.FI + (((size_t)cls * 2 + bsel) * BA_NC) * BA_C * BA_NT + tid;
+                uint32_t nbp[BA_C], nad[BA_C];
+#pragma unroll
+                for (int q = 0; q < BA_C; q++) { const uint2 pr = __ldg(F + (size_t)q * BA_NT); nbp[q] = pr.x; nad[q] = pr.y; }
                 ba_cp_async_wait_all();
                 __syncthreads();                               // batch j staged; batch j-1 fully consumed
                 if (j + 1 < nbatch) stage(j + 1);
                 if (j > 0) flush(j - 1);
-                const uint32_t bi = s_batch[j];
-                const int len = (int)((bi >> 16) & 0xffu), kq = (int)(bi >> 24), buf = j & 1;
-                const int cls = kq % BA_NCLS, bsel = kq / BA_NCLS;
                 const uint32_t rowbase = sRows + (uint32_t)(buf * BA_RB_IN) * ROWB;
                 const uint4 *bal = s_bal + buf * BA_RB_IN;
                 const uint16_t *bnode = s_bnode + buf * BA_RB_IN;
@@ -330,16 +336,19 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 for (int b = 0; b < 2; b++) {
                     if (b != bsel) continue;
                     // ---- fast pairs -----------------------------------------------------------------------
-                    const uint2 *F = a.FI + (((size_t)cls * 2 + b) * BA_NC) * BA_C * BA_NT + tid;
 #pragma unroll
                     for (int c = 0; c < BA_NC; c++) {
-                        if (!((whas >> (b * BA_NC + c)) & 1u)) continue;
                         uint32_t bp[BA_C], ad[BA_C];
 #pragma unroll
-                        for (int q = 0; q < BA_C; q++) {
-                            const uint2 pr = __ldg(F + (size_t)(c * BA_C + q) * BA_NT);
-                            bp[q] = pr.x; ad[q] = pr.y;
+                        for (int q = 0; q < BA_C; q++) { bp[q] = nbp[q]; ad[q] = nad[q]; }
+                        if (c + 1 < BA_NC) {
+#pragma unroll
+                            for (int q = 0; q < BA_C; q++) {
+                                const uint2 pr = __ldg(F + (size_t)((c + 1) * BA_C + q) * BA_NT);
+                                nbp[q] = pr.x; nad[q] = pr.y;
+                            }
                         }
+                        if (!((whas >> (b * BA_NC + c)) & 1u)) continue;
                         if (MODE == IN_SWEEP) {
                             acc[b][c] = ba_fast_chunk(acc[b][c], bal, rowbase, ROWB, len, bp, ad);
                         } else {
@@ -353,7 +362,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                                     if (!(bp[q] & 0xffu)) continue;
                                     const uint32_t emb = al.x * (bp[q] & 0xffu) + al.y * ((bp[q] >> 8) & 0xffu) +
                                                          al.z * ((bp[q] >> 16) & 0xffu) + al.w * (bp[q] >> 24);
-                                    const uint32_t cz = ba_z_of_tail((uint32_t)b, ad[q] >> 3);
+                                    const uint32_t cz = ba_z_of_tail((uint32_t)b, ba_swz(ad[q] >> 3));
                                     const int jz = ba_len_of_code(cz);
                                     if (MODE == IN_HC) {
                                         const double wk = s_w[k + jz];
@@ -380,7 +389,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                             const uint4 rd = __ldg(a.RI + ((size_t)cls * 2 + b) * a.nri + re);
                             const uint32_t B0 = rd.x & 0xffu, B1 = (rd.x >> 8) & 0xffu, B2 = (rd.x >> 16) & 0xffu, B3 = rd.x >> 24;
                             const uint32_t B4 = rd.y & 0xffu, ov = rd.y >> 16;
-                            const uint32_t cz = ba_z_of_tail((uint32_t)b, rd.z >> 3);
+                            const uint32_t cz = ba_z_of_tail((uint32_t)b, ba_swz(rd.z >> 3));
                             const int jz = ba_len_of_code(cz);
                             const uint32_t *r8 = a.RI8 + ((size_t)cls * 2 + b) * 16 * a.nri + re;
                             for (int i = 0; i < len; i++) {

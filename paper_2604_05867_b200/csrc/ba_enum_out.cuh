@@ -247,7 +247,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                         for (int pidx = tid; pidx < (len << (m - 1)); pidx += BA_NT) {   // 16-byte pieces, 2^{m-1} per row
                             const int i = pidx >> (m - 1), pc = pidx & ((nv >> 1) - 1);
                             const uint32_t u = s_rec[s_order[start + i]].id;
-                            ba_cp_async16(sRows + (uint32_t)(buf * BA_RB_OUT + i) * ROWB + (uint32_t)pc * 16u,
+                            ba_cp_async16(sRows + (uint32_t)(buf * BA_RB_OUT + i) * ROWB + ba_swz(2u * (uint32_t)pc) * 8u,
                                           a.p + (((size_t)u << m) + 2u * (size_t)pc));
                         }
                     }
@@ -260,11 +260,20 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
             };
             if (nbatch > 0) stage(0);
             for (int j = 0; j < nbatch; j++) {
+                const uint32_t bi = s_batch[j];
+                const int len = (int)((bi >> 16) & 0xffu), mask = (int)(bi >> 24), buf = j & 1;
+                // the pairs of a chunk do not depend on the staged rows: fetch the first slot before waiting, and
+                // the next slot while the current one is computed (one exposed L2 latency per batch at most)
+                const uint2 *F0 = a.FO + ((size_t)cls * 2 * BA_NC) * BA_C * BA_NT + tid;   // list 0; list 1 follows
+                uint32_t nbp[BA_C], nad[BA_C];
+                {
+                    const uint2 *Ff = F0 + ((mask & 1) ? 0 : (size_t)BA_NC * BA_C * BA_NT);
+#pragma unroll
+                    for (int q = 0; q < BA_C; q++) { const uint2 pr = __ldg(Ff + (size_t)q * BA_NT); nbp[q] = pr.x; nad[q] = pr.y; }
+                }
                 ba_cp_async_wait_all();
                 __syncthreads();                               // batch j staged; batch j-1 fully consumed
                 if (j + 1 < nbatch) stage(j + 1);
-                const uint32_t bi = s_batch[j];
-                const int len = (int)((bi >> 16) & 0xffu), mask = (int)(bi >> 24), buf = j & 1;
                 const uint32_t rowbase = sRows + (uint32_t)(buf * BA_RB_OUT) * ROWB;
                 const uint4 *bal = s_bal + buf * BA_RB_OUT;
                 const uint16_t *bnode = s_bnode + buf * BA_RB_OUT;
@@ -276,7 +285,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                     const uint32_t emb = r0.x * Ee[0] + r0.y * Ee[1] + r0.z * Ee[2] + r0.w * Ee[3] + r1.x * Ee[4] +
                                          r1.y * Ee[5] + r1.z * Ee[6] + r1.w * Ee[7] + r2.x * Ee[8];
                     if (MODE == OUT_SWEEP) {
-                        acc_eps = fma(ba_u2d(emb), ba_lds_f64(rowbase + (uint32_t)i * ROWB + (uint32_t)ev * 8u), acc_eps);
+                        acc_eps = fma(ba_u2d(emb), ba_lds_f64(rowbase + (uint32_t)i * ROWB + ba_swz((uint32_t)ev) * 8u), acc_eps);
                     } else if (MODE == OUT_DEBUG) {
                         if (a.dbg_cz == 1u) a.dbg_out[((size_t)r2.y << m) | (size_t)ev] = emb;
                     } else {
@@ -287,14 +296,15 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                 for (int b = 0; b < 2; b++) {
                     if (!((mask >> b) & 1)) continue;
                     // ---- fast pairs -----------------------------------------------------------------------
-                    const uint2 *F = a.FO + (((size_t)cls * 2 + b) * BA_NC) * BA_C * BA_NT + tid;
 #pragma unroll
                     for (int c = 0; c < BA_NC; c++) {
                         uint32_t bp[BA_C], ad[BA_C];
 #pragma unroll
-                        for (int q = 0; q < BA_C; q++) {
-                            const uint2 pr = __ldg(F + (size_t)(c * BA_C + q) * BA_NT);
-                            bp[q] = pr.x; ad[q] = pr.y;
+                        for (int q = 0; q < BA_C; q++) { bp[q] = nbp[q]; ad[q] = nad[q]; }
+                        if (c + 1 < BA_NC || (b == 0 && (mask & 2))) {      // next slot: (b, c+1), else (1, 0)
+                            const uint2 *Fn = F0 + (size_t)((c + 1 < BA_NC) ? (b * BA_NC + c + 1) : BA_NC) * BA_C * BA_NT;
+#pragma unroll
+                            for (int q = 0; q < BA_C; q++) { const uint2 pr = __ldg(Fn + (size_t)q * BA_NT); nbp[q] = pr.x; nad[q] = pr.y; }
                         }
                         if (MODE == OUT_SWEEP) {
                             acc[b][c] = ba_fast_chunk(acc[b][c], bal, rowbase, ROWB, len, bp, ad);
@@ -308,7 +318,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                                     if (!(bp[q] & 0xffu)) continue;
                                     const uint32_t emb = al.x * (bp[q] & 0xffu) + al.y * ((bp[q] >> 8) & 0xffu) + al.z * ((bp[q] >> 16) & 0xffu) + al.w * (bp[q] >> 24);
                                     if (MODE == OUT_DEBUG) {
-                                        if (oz == a.dbg_cz) a.dbg_out[((size_t)u << m) | (size_t)(ad[q] >> 3)] = emb;
+                                        if (oz == a.dbg_cz) a.dbg_out[((size_t)u << m) | (size_t)ba_swz(ad[q] >> 3)] = emb;
                                     } else {
                                         cnt_terms += 1ull; cnt_emb += emb;
                                     }
@@ -331,7 +341,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                             if (MODE == OUT_SWEEP) {
                                 s = fma(ba_u2d(emb), ba_lds_f64(rowbase + (uint32_t)i * ROWB + roff[b]), s);
                             } else if (MODE == OUT_DEBUG) {
-                                if (oz == a.dbg_cz) a.dbg_out[((size_t)r2.y << m) | (size_t)(roff[b] >> 3)] = emb;
+                                if (oz == a.dbg_cz) a.dbg_out[((size_t)r2.y << m) | (size_t)ba_swz(roff[b] >> 3)] = emb;
                             } else {
                                 cnt_terms += 1ull; cnt_emb += emb;
                             }

@@ -66,6 +66,11 @@ struct NodeRec {                      // 48 bytes, shared memory
     uint32_t pad;
 };
 
+// Position of operand number `pos` in a staged row: bits 1..3 are XORed with bits 4..6, so that operands
+// whose numbers agree in the low four bits (the strings sharing their last symbols) spread over the 8-byte bank
+// pairs.  An involution that keeps the two operands of a 16-byte piece together.
+__host__ __device__ __forceinline__ uint32_t ba_swz(uint32_t pos) { return pos ^ (((pos >> 4) & 7u) << 1); }
+
 __device__ __forceinline__ int ba_len_of_code(uint32_t code) { return 31 - __clz(code); }
 
 // First position p >= from (paper positions, 0 = leftmost) with bit b in the L-bit string s, or L.

@@ -253,21 +253,22 @@ static inline void build_tile_tables(int m, TileTables &T) {
                     if (!Bof(cz, v) || first_bit(cz) != b) continue;
                     // the operand of z = b.t sits at position code(t) of the node's half row
                     if (deep(cls, cz, v)) {
-                        R.push_back(rider(cls, cz, v, 8u * tail_of(cz), (uint32_t)v));
+                        R.push_back(rider(cls, cz, v, 8u * ba_swz(tail_of(cz)), (uint32_t)v));
                         rin_zv[(size_t)cls * 2 + b].push_back(std::make_pair(cz, v));
                     }
-                    else pool[v].push_back(tail_of(cz) | ((uint32_t)depth(cls, cz, v) << 28));   // key = code(t): bank pair = key & 15
+                    else pool[v].push_back(ba_swz(tail_of(cz)) | ((uint32_t)depth(cls, cz, v) << 28));   // key = row position: bank pair = key & 15
                 }
             }
             T.ri_csr[((size_t)cls * 2 + b) * (nv + 1) + nv] = (uint16_t)R.size();
             for (int v = 0; v < nv; v++)
                 std::stable_sort(pool[v].begin(), pool[v].end(), [](uint32_t x, uint32_t y) { return (x >> 28) > (y >> 28); });
-            tt_place(in_slot_owner[b], pool, [&](int k, int q, int v, uint32_t tc) {
+            tt_place(in_slot_owner[b], pool, [&](int k, int q, int v, uint32_t key) {
+                const uint32_t tc = ba_swz(key);
                 const int lt = 31 - __builtin_clz(tc);
                 const uint32_t cz = (1u << (lt + 1)) | ((uint32_t)b << lt) | (tc - (1u << lt));
                 int c, tid;
                 tt_phys(k, c, tid);
-                T.FI[fidx(cls, b, c, q, tid)] = make_uint2(bpack(cls, cz, v), 8u * tc);
+                T.FI[fidx(cls, b, c, q, tid)] = make_uint2(bpack(cls, cz, v), 8u * key);
             });
             for (int v = 0; v < nv; v++) if (!pool[v].empty()) return;
         }
@@ -295,8 +296,8 @@ static inline void build_tile_tables(int m, TileTables &T) {
                 std::vector<uint32_t> pz;
                 for (int v = 0; v < nv; v++) {
                     if (!Bof(cz, v)) continue;
-                    if (deep(cls, cz, v)) R.push_back(rider(cls, cz, v, 8u * (uint32_t)v, cz));
-                    else pz.push_back((uint32_t)v | ((uint32_t)depth(cls, cz, v) << 28));   // key = v: bank pair = v & 15
+                    if (deep(cls, cz, v)) R.push_back(rider(cls, cz, v, 8u * ba_swz((uint32_t)v), cz));
+                    else pz.push_back(ba_swz((uint32_t)v) | ((uint32_t)depth(cls, cz, v) << 28));   // key = row position: bank pair = key & 15
                 }
                 std::stable_sort(pz.begin(), pz.end(), [](uint32_t x, uint32_t y) { return (x >> 28) > (y >> 28); });
                 for (size_t i = 0; i < pz.size(); i += BA_C) {
@@ -323,10 +324,11 @@ static inline void build_tile_tables(int m, TileTables &T) {
                 zslots[chunks[k].cz].push_back((uint16_t)ai);
             }
             for (auto &pl : pool) std::stable_sort(pl.begin(), pl.end(), [](uint32_t x, uint32_t y) { return (x >> 28) > (y >> 28); });
-            tt_place(so, pool, [&](int k, int q, int cz, uint32_t v) {
+            tt_place(so, pool, [&](int k, int q, int cz, uint32_t key) {
+                const uint32_t v = ba_swz(key);
                 int c, tid;
                 tt_phys(k, c, tid);
-                T.FO[fidx(cls, b, c, q, tid)] = make_uint2(bpack(cls, (uint32_t)cz, (int)v), 8u * v);
+                T.FO[fidx(cls, b, c, q, tid)] = make_uint2(bpack(cls, (uint32_t)cz, (int)v), 8u * key);
             });
             for (auto &pl : pool) if (!pl.empty()) return;
         }

@@ -209,3 +209,16 @@ def test_T8_state_and_argument_errors(ba):
         assert 0 < I <= U
     finally:
         ba.ba_destroy(lib_ctx)
+
+
+# ------------------------------------------------------------------ configs[2] harness (stop rule R8, bounds R10)
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_config3_harness_small(ba, mode):
+    from paper_2604_05867_b200 import sweep
+    r = sweep.run_until_gap(8, 0.5, tol=1e-6, max_iters=6000, chunk=250, mode=mode)
+    assert r["converged"] and r["gap"] < 1e-6 and r["iterations"] <= 6000
+    # C_8(0.5) = 2.123006166059 (secondary pin): I <= C <= running min U, both within the gap
+    assert r["I_lower"] <= 2.123006166059 + 1e-9 <= r["running_min_upper"] + 2e-9
+    assert r["running_min_upper"] - r["I_lower"] < 1e-6 and r["stop_statistic_U_minus_log2Z"] <= r["gap"] + 1e-12
+    assert r["upper_over_n_over_1_minus_d"] == pytest.approx(r["running_min_upper"] / 8 / 0.5)
