@@ -56,7 +56,7 @@ enum {
     BA_MODE_FAST = 1  /* position-by-position deletion transform, O(n 2^n)/sweep  */
 };
 
-#define BA_NMAX 30    /* uint32 string codes; tested to n = 24 in ENUM mode                            */
+#define BA_NMAX 30    /* uint32 string codes; run to n = 28 in ENUM mode (profiles/r01c_bench_n28.md) */
 
 /* ---- required by the north star -------------------------------------------------------------- */
 

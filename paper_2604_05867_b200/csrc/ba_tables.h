@@ -55,12 +55,14 @@ static inline void tt_phys(int j, int &c, int &tid) {
 // their BA_C pair positions q.  An item is key | depth << 28; key & 15 is the 8-byte bank pair of its operand.
 // The pools arrive sorted by chain depth, deepest first, and only items of the head's depth are candidates, so
 // an owner's deep pairs land in its first slots.  Per (half-warp, q) a bipartite matching lane -> bank pair
-// (augmenting paths, lanes with the fewest options first) picks, where it can, 16 different bank pairs.
-// emit(k, q, owner, key).
+// (augmenting paths, lanes with the fewest options first) picks, where it can, 16 different bank pairs; a local
+// search over swaps then removes most of the remaining conflicts.  emit(k, q, owner, key).
 #define BA_PLACE_WINDOW 12
 template <typename Emit>
 static void tt_place(const std::vector<int> &slot_owner, std::vector<std::vector<uint32_t>> &pool, Emit emit) {
     const int nslots = (int)slot_owner.size();
+    const uint32_t EMPTY = 0xffffffffu;
+    std::vector<uint32_t> at((size_t)nslots * BA_C, EMPTY);     // at[k*BA_C + q] = item (key | depth << 28)
     for (int k0 = 0; k0 < nslots; k0 += 16) {
         for (int q = 0; q < BA_C; q++) {
             int lanes[16], nl = 0;
@@ -112,10 +114,53 @@ static void tt_place(const std::vector<int> &slot_owner, std::vector<std::vector
                 const uint32_t it = P[pick];
                 P.erase(P.begin() + pick);
                 used[it & 15u]++;
-                emit(lanes[i], q, slot_owner[lanes[i]], it & 0x0fffffffu);
+                at[(size_t)lanes[i] * BA_C + q] = it;
             }
         }
     }
+    // ---- local search: swap two items of one owner and one depth between their positions when that lowers
+    // (sum over groups of the worst bank-pair multiplicity, then the sum of squared multiplicities).  A group is
+    // one (half-warp, q) operand load.
+    const int ngrp = ((nslots + 15) / 16) * BA_C;
+    std::vector<uint8_t> cnt((size_t)ngrp * 16, 0);
+    auto grp = [&](int p) { return ((p / BA_C) / 16) * BA_C + p % BA_C; };
+    auto gmax = [&](int g) { int mx = 0; for (int r = 0; r < 16; r++) mx = std::max<int>(mx, cnt[(size_t)g * 16 + r]); return mx; };
+    auto gsq = [&](int g) { int sq = 0; for (int r = 0; r < 16; r++) sq += cnt[(size_t)g * 16 + r] * cnt[(size_t)g * 16 + r]; return sq; };
+    std::vector<std::vector<int>> by_owner(pool.size());
+    std::vector<uint32_t> wdepth((nslots + 31) / 32, 0);          // deepest item of every warp-slot (32 slots)
+    for (int p = 0; p < nslots * BA_C; p++)
+        if (at[p] != EMPTY) {
+            cnt[(size_t)grp(p) * 16 + (at[p] & 15u)]++;
+            by_owner[slot_owner[p / BA_C]].push_back(p);
+            wdepth[p / BA_C / 32] = std::max(wdepth[p / BA_C / 32], at[p] >> 28);
+        }
+    for (int sweep = 0; sweep < 8; sweep++) {
+        int improved = 0;
+        for (int p1 = 0; p1 < nslots * BA_C; p1++) {
+            if (at[p1] == EMPTY) continue;
+            const int g1 = grp(p1);
+            const uint32_t r1 = at[p1] & 15u;
+            if (cnt[(size_t)g1 * 16 + r1] < 2) continue;           // this lane is not part of a conflict
+            const std::vector<int> &cand = by_owner[slot_owner[p1 / BA_C]];
+            for (int p2 : cand) {
+                if (p2 == p1) continue;                            // a swap must not deepen either warp-slot
+                if ((at[p1] >> 28) > wdepth[p2 / BA_C / 32] || (at[p2] >> 28) > wdepth[p1 / BA_C / 32]) continue;
+                const int g2 = grp(p2);
+                const uint32_t r2 = at[p2] & 15u;
+                if (g2 == g1 || r2 == r1) continue;
+                const int b_mx = gmax(g1) + gmax(g2), b_sq = gsq(g1) + gsq(g2);
+                cnt[(size_t)g1 * 16 + r1]--; cnt[(size_t)g1 * 16 + r2]++;
+                cnt[(size_t)g2 * 16 + r2]--; cnt[(size_t)g2 * 16 + r1]++;
+                const int a_mx = gmax(g1) + gmax(g2), a_sq = gsq(g1) + gsq(g2);
+                if (a_mx < b_mx || (a_mx == b_mx && a_sq < b_sq)) { std::swap(at[p1], at[p2]); improved++; break; }
+                cnt[(size_t)g1 * 16 + r1]++; cnt[(size_t)g1 * 16 + r2]--;
+                cnt[(size_t)g2 * 16 + r2]++; cnt[(size_t)g2 * 16 + r1]--;
+            }
+        }
+        if (!improved) break;
+    }
+    for (int p = 0; p < nslots * BA_C; p++)
+        if (at[p] != EMPTY) emit(p / BA_C, p % BA_C, slot_owner[p / BA_C], at[p] & 0x0fffffffu);
 }
 
 static inline void build_tile_tables(int m, TileTables &T) {
