@@ -59,7 +59,7 @@ struct InArgs {
     unsigned long long *cnt;  // IN_COUNT: [0] terms, [1] emb sum
 };
 
-struct InSmem { size_t rec, ceps, rows, bal, bnode, ordr, seg, order, gstart, wcnt, batch, rsum, csr_off, csr_idx, sub, red, kcw, item, total; };
+struct InSmem { size_t rec, ceps, rows, bal, bnode, ordr, seg, order, gstart, wcnt, batch, rsum, csr_off, sub, red, kcw, item, total; };
 
 __host__ __device__ static inline InSmem enum_in_smem(int m, int ncsr, int nri) {
     InSmem s;
@@ -79,7 +79,7 @@ __host__ __device__ static inline InSmem enum_in_smem(int m, int ncsr, int nri) 
     s.batch = take((size_t)BA_IN_MAXB * 4);
     s.rsum = take((size_t)2 * nri * 8);
     s.csr_off = take(((size_t)(1 << m) + 1) * 2);
-    s.csr_idx = take((size_t)ncsr * 2);
+    (void)ncsr;                                            // the CSR indices are read from global memory (L2)
     s.sub = take(32 * 4);
     s.red = take(64 * 8);
     s.kcw = take(2 * (BA_NMAX_I + 1) * 8);
@@ -116,7 +116,6 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
     uint32_t *s_batch = (uint32_t *)(smem + L.batch);
     double *s_rsum = (double *)(smem + L.rsum);
     uint16_t *s_csr_off = (uint16_t *)(smem + L.csr_off);
-    uint16_t *s_csr_idx = (uint16_t *)(smem + L.csr_idx);
     uint32_t *s_sub = (uint32_t *)(smem + L.sub);
     double *s_red = (double *)(smem + L.red);
     double *s_w = (double *)(smem + L.kcw);
@@ -124,7 +123,6 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
     uint32_t *s_item = (uint32_t *)(smem + L.item);        // [0] item, [1] number of batches
 
     for (int i = tid; i <= nv; i += BA_NT) s_csr_off[i] = a.csr_off[i];
-    for (int i = tid; i < a.ncsr; i += BA_NT) s_csr_idx[i] = a.csr_idx[i];
     for (int i = tid; i <= BA_NMAX_I; i += BA_NT) { s_w[i] = a.kc.w[i]; s_lebar[i] = a.kc.lebar[i]; }
     for (int i = tid; i < 2 * BA_RB_IN; i += BA_NT) s_rows[(size_t)i * ROWD] = 0.0;   // position 0: padding pairs
 
@@ -439,7 +437,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
             if (tid < nv) {
                 double S = acc_rid;
                 for (int t = ev; t < BA_NT; t += nv) S += s_acc[(size_t)2 * BA_NC * BA_NT + t];
-                for (int q = s_csr_off[tid]; q < s_csr_off[tid + 1]; q++) S += s_acc[s_csr_idx[q]];
+                for (int q = s_csr_off[tid]; q < s_csr_off[tid + 1]; q++) S += s_acc[__ldg(a.csr_idx + q)];
                 const size_t x = ((size_t)u << m) | (size_t)tid;
                 if (MODE == IN_HC) {
                     a.Hc[x] = S;

@@ -40,7 +40,7 @@
 #define BA_NC 3              // chunk slots per thread and list
 #define BA_KB 4              // class bits
 #define BA_NCLS 16           // 2^BA_KB classes
-#define BA_RB_IN 16          // nodes per batch, input sweep (operand half-rows of 2^m doubles)
+#define BA_RB_IN 32          // nodes per batch, input sweep (operand half-rows of 2^m doubles)
 #define BA_SBR 3             // input sweep: phase-A rounds (of BA_NT nodes) per super-batch
 #define BA_RB_OUT 32         // nodes per batch, output sweep (operand rows of 2^m doubles)
 
