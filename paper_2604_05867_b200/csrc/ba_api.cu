@@ -32,7 +32,7 @@ struct ba_ctx {
     uint2 *FI = nullptr, *FO = nullptr;
     uint4 *RI = nullptr, *RO = nullptr;
     uint2 *EPS8 = nullptr;
-    uint32_t *RI8 = nullptr;
+    uint32_t *RI8 = nullptr, *RO8 = nullptr;
     uint32_t *Wv = nullptr, *vbase = nullptr;
     uint16_t *in_owner = nullptr, *out_owner = nullptr, *ri_cnt = nullptr, *ro_cnt = nullptr, *ri_csr = nullptr, *ro_csr = nullptr;
     uint16_t *in_csr_off = nullptr, *in_csr_idx = nullptr, *out_csr_off = nullptr, *out_csr_idx = nullptr;
@@ -73,7 +73,7 @@ static double host_binom(int n, int k) {
 
 // ------------------------------------------------------------------------------------------------ scratch layout
 struct ScratchLayout {
-    size_t c, Hc, Apart, part, scal, hist, FI, FO, RI, RO, EPS8, RI8, Wv, vbase, in_owner, out_owner, ri_cnt, ro_cnt, ri_csr, ro_csr,
+    size_t c, Hc, Apart, part, scal, hist, FI, FO, RI, RO, EPS8, RI8, RO8, Wv, vbase, in_owner, out_owner, ri_cnt, ro_cnt, ri_csr, ro_csr,
         in_csr_off, in_csr_idx, out_csr_off, out_csr_idx, counters, cnt, total;
     size_t napart, npart_cap;
 };
@@ -113,6 +113,7 @@ static void scratch_layout(int n, const TileTables &T, ScratchLayout &L) {
     L.RO = o; o += align256(T.RO.size() * 16);
     L.EPS8 = o; o += align256(T.EPS8.size() * 8);
     L.RI8 = o; o += align256(T.RI8.size() * 4);
+    L.RO8 = o; o += align256(T.RO8.size() * 4);
     L.Wv = o; o += align256(T.Wv.size() * 4);
     L.vbase = o; o += align256(T.vbase.size() * 4);
     L.in_owner = o; o += align256(T.in_owner.size() * 2);
@@ -185,7 +186,7 @@ static int finish_create(ba_ctx *c) {
     c->c = (double *)(s + L.c); c->Hc = (double *)(s + L.Hc); c->Apart = (double *)(s + L.Apart);
     c->part = (double *)(s + L.part); c->scal = (double *)(s + L.scal); c->hist = (double *)(s + L.hist);
     c->FI = (uint2 *)(s + L.FI); c->FO = (uint2 *)(s + L.FO); c->RI = (uint4 *)(s + L.RI); c->RO = (uint4 *)(s + L.RO);
-    c->EPS8 = (uint2 *)(s + L.EPS8); c->RI8 = (uint32_t *)(s + L.RI8);
+    c->EPS8 = (uint2 *)(s + L.EPS8); c->RI8 = (uint32_t *)(s + L.RI8); c->RO8 = (uint32_t *)(s + L.RO8);
     c->Wv = (uint32_t *)(s + L.Wv); c->vbase = (uint32_t *)(s + L.vbase);
     c->in_owner = (uint16_t *)(s + L.in_owner); c->out_owner = (uint16_t *)(s + L.out_owner);
     c->ri_cnt = (uint16_t *)(s + L.ri_cnt); c->ro_cnt = (uint16_t *)(s + L.ro_cnt);
@@ -198,7 +199,7 @@ static int finish_create(ba_ctx *c) {
     c->n_in_csr = (int)T.in_csr_idx.size(); c->n_out_csr = T.out_ncsr;
 
     CK(upload(c->FI, T.FI, c->st)); CK(upload(c->FO, T.FO, c->st)); CK(upload(c->RI, T.RI, c->st)); CK(upload(c->RO, T.RO, c->st));
-    CK(upload(c->EPS8, T.EPS8, c->st)); CK(upload(c->RI8, T.RI8, c->st));
+    CK(upload(c->EPS8, T.EPS8, c->st)); CK(upload(c->RI8, T.RI8, c->st)); CK(upload(c->RO8, T.RO8, c->st));
     CK(upload(c->Wv, T.Wv, c->st)); CK(upload(c->vbase, T.vbase, c->st));
     CK(upload(c->in_owner, T.in_owner, c->st)); CK(upload(c->out_owner, T.out_owner, c->st));
     CK(upload(c->ri_cnt, T.ri_cnt, c->st)); CK(upload(c->ro_cnt, T.ro_cnt, c->st));
@@ -217,7 +218,7 @@ static int finish_create(ba_ctx *c) {
     CK(cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev));
     c->block = BA_NT;
     c->smem_in = enum_in_smem(c->m, c->n_in_csr, c->nri).total;
-    c->smem_out = enum_out_smem(c->m, c->nWv, c->n_out_csr, c->nro).total;
+    c->smem_out = enum_out_smem(c->m, c->n_out_csr, c->nro).total;
     CK(cudaFuncSetAttribute(k_enum_in<IN_SWEEP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_in));
     CK(cudaFuncSetAttribute(k_enum_in<IN_HC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_in));
     CK(cudaFuncSetAttribute(k_enum_in<IN_DEBUG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_in));
@@ -310,7 +311,7 @@ static InArgs make_in_args(ba_ctx *c) {
 
 static OutArgs make_out_args(ba_ctx *c) {
     OutArgs a;
-    a.kc = c->kc; a.Wv = c->Wv; a.vbase = c->vbase; a.nWv = c->nWv;
+    a.kc = c->kc; a.EPS8 = c->EPS8; a.RO8 = c->RO8;
     a.FO = c->FO; a.RO = c->RO; a.ro_cnt = c->ro_cnt; a.ro_csr = c->ro_csr; a.nro = c->nro; a.owner = c->out_owner;
     a.csr_off = c->out_csr_off; a.csr_idx = c->out_csr_idx; a.ncsr = c->n_out_csr;
     a.p = c->p; a.Apart = c->Apart; a.counter = c->counters + 4; a.dbg_item = 0; a.dbg_cz = 0; a.dbg_out = nullptr;

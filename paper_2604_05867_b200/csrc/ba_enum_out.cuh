@@ -34,9 +34,8 @@ __constant__ uint32_t c_binom[BA_NMAX_I + 1][BA_NMAX_I + 1];
 
 struct OutArgs {
     KConst kc;
-    const uint32_t *Wv;        // v-major prepend links
-    const uint32_t *vbase;     // [2^m]
-    int nWv;
+    const uint2 *EPS8;         // [256][2^m]: B(sigma_s, v), s = 1..8, of the pair (v, empty)
+    const uint32_t *RO8;       // [cls][b][16][nro]: B_5..B_8 of a rider by the sigma bits 4..7
     const uint2 *FO;           // fast pairs [cls][b][c][q][tid]
     const uint4 *RO;           // riders [cls][b][nro]
     const uint16_t *ro_cnt;    // [cls][b]
@@ -55,13 +54,12 @@ struct OutArgs {
     unsigned long long *cnt;   // OUT_COUNT
 };
 
-struct OutSmem { size_t Wv, rec, rows, bal, bnode, order, wcnt, bstart, batch, red, item, total; };
+struct OutSmem { size_t rec, rows, bal, bnode, order, wcnt, bstart, batch, red, item, total; };
 
-__host__ __device__ static inline OutSmem enum_out_smem(int m, int nWv, int ncsr, int nro) {
+__host__ __device__ static inline OutSmem enum_out_smem(int m, int ncsr, int nro) {
     OutSmem s;
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o += (bytes + 15) & ~(size_t)15; return at; };
-    s.Wv = take((size_t)nWv * 4);
     s.rec = take((size_t)BA_NT * sizeof(NodeRec));
     size_t rows = (size_t)2 * BA_RB_OUT * ((size_t)1 << m) * 8, ac = ((size_t)2 * BA_NC * BA_NT + 2 * (size_t)nro) * 8;
     s.rows = take(rows > ac ? rows : ac);                  // the epilogue's accumulator staging aliases the rows
@@ -83,11 +81,10 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
     extern __shared__ __align__(16) unsigned char smem[];
     const int m = a.kc.m, h = a.kc.h, nv = 1 << m;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const OutSmem L = enum_out_smem(m, a.nWv, a.ncsr, a.nro);
+    const OutSmem L = enum_out_smem(m, a.ncsr, a.nro);
     const uint32_t ROWB = (uint32_t)nv * 8u;
     const uint32_t NZ = (2u << m) - 1u;
 
-    uint32_t *s_Wv = (uint32_t *)(smem + L.Wv);
     NodeRec *s_rec = (NodeRec *)(smem + L.rec);
     double *s_rows = (double *)(smem + L.rows);
     double *s_acc = s_rows;                                 // epilogue only
@@ -100,14 +97,10 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
     double *s_red = (double *)(smem + L.red);
     uint32_t *s_item = (uint32_t *)(smem + L.item);        // [0] item, [1] number of batches
 
-    for (int i = tid; i < a.nWv; i += BA_NT) s_Wv[i] = a.Wv[i];
-    const uint32_t sWv = ba_smem_addr(s_Wv);
     const uint32_t sRows = ba_smem_addr(s_rows);
     const int ev = tid & (nv - 1);                          // v of this thread's empty-z pairs
     const int esub = tid >> m, epn = BA_NT >> m;
-    const uint32_t evb = sWv + a.vbase[ev] * 4u;
     __syncthreads();
-    const uint32_t eW = s_Wv[a.vbase[ev] + 1];              // W of (v, empty)
 
     unsigned long long cnt_terms = 0, cnt_emb = 0;
     const uint32_t n_items = (h >= 31) ? 0xffffffffu : ((2u << h) - 1u);   // codes 1 .. 2^{h+1}-1
@@ -126,20 +119,12 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
         for (int w = 0; w <= h - t; w++) R += c_binom[h][w];
 
         // ---- per item: all nine B_s of the eps pair (v = ev) and of this thread's riders --------------------
-        uint32_t Ee[9];                                        // B(sigma_s, ev)
+        uint32_t Ee[9];                                        // B(sigma_s, ev); alpha_s = 0 beyond t
         {
+            const uint2 e8 = __ldg(a.EPS8 + (size_t)(cy & 255u) * nv + ev);
             Ee[0] = 1u;
-            uint32_t hw = (cy & 1u) ? (eW >> 16) : (eW & 0xffffu);
-            uint32_t lk = (Lc >= 1) ? (hw & 0xffu) : 0u;
-            Ee[1] = (Lc >= 1) ? (hw >> 8) : 0u;
-#pragma unroll
-            for (int s = 2; s <= 8; s++) {
-                Ee[s] = 0u;
-                if (Lc >= s && lk != 0u) {
-                    hw = ba_lds_u16(evb + ((cy >> (s - 1)) & 1u) * 2u + lk * 4u);
-                    Ee[s] = hw >> 8; lk = hw & 0xffu;
-                }
-            }
+            Ee[1] = e8.x & 0xffu; Ee[2] = (e8.x >> 8) & 0xffu; Ee[3] = (e8.x >> 16) & 0xffu; Ee[4] = e8.x >> 24;
+            Ee[5] = e8.y & 0xffu; Ee[6] = (e8.y >> 8) & 0xffu; Ee[7] = (e8.y >> 16) & 0xffu; Ee[8] = e8.y >> 24;
         }
         uint32_t rB[2][3], roff[2];                            // riders: B_0..B_8 packed 4+4+1 bytes, row offset
 #pragma unroll
@@ -150,16 +135,8 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                 const uint4 rd = __ldg(a.RO + ((size_t)cls * 2 + b) * a.nro + (BA_NT - 1 - tid));
                 rB[b][0] = rd.x;
                 roff[b] = rd.z;
-                uint32_t hi = rd.y & 0xffu, lk = (rd.y >> 8) & 0xffu, b8 = 0u;
-                const uint32_t vb = sWv + rd.w;
-#pragma unroll
-                for (int s = BA_KB + 1; s <= 8; s++) {
-                    if (Lc >= s && lk != 0u) {
-                        const uint32_t hw = ba_lds_u16(vb + ((cy >> (s - 1)) & 1u) * 2u + lk * 4u);
-                        if (s < 8) hi |= (hw >> 8) << (8 * (s - 4)); else b8 = hw >> 8;
-                        lk = hw & 0xffu;
-                    }
-                }
+                const uint32_t x8 = __ldg(a.RO8 + (((size_t)cls * 2 + b) * 16 + ((cy >> 4) & 15u)) * a.nro + (BA_NT - 1 - tid));
+                const uint32_t hi = (rd.y & 0xffu) | (x8 << 8), b8 = x8 >> 24;     // B_4..B_7, B_8
                 rB[b][1] = hi; rB[b][2] = b8;
             }
         }

@@ -42,7 +42,7 @@
 #define BA_NCLS 16           // 2^BA_KB classes
 #define BA_RB_IN 32          // nodes per batch, input sweep (operand half-rows of 2^m doubles)
 #define BA_SBR 3             // input sweep: phase-A rounds (of BA_NT nodes) per super-batch
-#define BA_RB_OUT 32         // nodes per batch, output sweep (operand rows of 2^m doubles)
+#define BA_RB_OUT 48         // nodes per batch, output sweep (operand rows of 2^m doubles)
 
 // ---- v-major prepend links Wv: one uint32 per entry of v's list ([0] null, [1] empty string, then the
 // non-empty subsequences of v):  W = l0 | cB0 << 8 | l1 << 16 | cB1 << 24,  l_b = local index of b.z in

@@ -32,6 +32,7 @@ struct TileTables {
     std::vector<uint16_t> ro_cnt;      // [BA_NCLS][2]
     std::vector<uint16_t> ro_csr;      // [BA_NCLS][2][2^{m+1} + 1] rider range of code(z)
     int nro = 0;
+    std::vector<uint32_t> RO8;         // [BA_NCLS][2][16][nro]: bytes = B_5..B_8 of the rider for sigma bits 4..7
     bool ok = false;
 };
 
@@ -328,6 +329,7 @@ static inline void build_tile_tables(int m, TileTables &T) {
     T.out_ncsr = 2 * BA_NC * BA_NT;
     T.out_csr_idx.assign((size_t)BA_NCLS * T.out_ncsr, 0);
     std::vector<std::vector<uint4>> rout((size_t)BA_NCLS * 2);
+    std::vector<std::vector<std::pair<uint32_t, int>>> rout_zv((size_t)BA_NCLS * 2);
     T.ro_csr.assign((size_t)BA_NCLS * 2 * (NZc + 1), 0);
     for (int cls = 0; cls < BA_NCLS; cls++) {
         std::vector<std::vector<uint16_t>> zslots(NZc);
@@ -341,7 +343,10 @@ static inline void build_tile_tables(int m, TileTables &T) {
                 std::vector<uint32_t> pz;
                 for (int v = 0; v < nv; v++) {
                     if (!Bof(cz, v)) continue;
-                    if (deep(cls, cz, v)) R.push_back(rider(cls, cz, v, 8u * ba_swz((uint32_t)v), cz));
+                    if (deep(cls, cz, v)) {
+                        R.push_back(rider(cls, cz, v, 8u * ba_swz((uint32_t)v), cz));
+                        rout_zv[(size_t)cls * 2 + b].push_back(std::make_pair(cz, v));
+                    }
                     else pz.push_back(ba_swz((uint32_t)v) | ((uint32_t)depth(cls, cz, v) << 28));   // key = row position: bank pair = key & 15
                 }
                 std::stable_sort(pz.begin(), pz.end(), [](uint32_t x, uint32_t y) { return (x >> 28) > (y >> 28); });
@@ -411,18 +416,22 @@ static inline void build_tile_tables(int m, TileTables &T) {
                 w[(sft - 1) / 4] |= Bof((1u << sft) | (sig & ((1u << sft) - 1u)), v) << (8 * ((sft - 1) % 4));
             T.EPS8[(size_t)sig * nv + v] = make_uint2(w[0], w[1]);
         }
-    T.RI8.assign((size_t)BA_NCLS * 2 * 16 * T.nri, 0u);
-    for (int cls = 0; cls < BA_NCLS; cls++)
-        for (int b = 0; b < 2; b++)
-            for (uint32_t hi = 0; hi < 16u; hi++)
-                for (size_t e = 0; e < rin_zv[(size_t)cls * 2 + b].size(); e++) {
-                    const uint32_t cz = rin_zv[(size_t)cls * 2 + b][e].first;
-                    const int v = rin_zv[(size_t)cls * 2 + b][e].second;
-                    const int lz = 31 - __builtin_clz(cz);
-                    uint32_t x = 0;
-                    for (int sft = 5; sft <= 8; sft++)
-                        if (lz + sft <= m) x |= Bof(tt_prepend((hi << 4) | (uint32_t)cls, sft, cz), v) << (8 * (sft - 5));
-                    T.RI8[((((size_t)cls * 2 + b) * 16 + hi) * T.nri) + e] = x;
-                }
+    auto tails = [&](const std::vector<std::vector<std::pair<uint32_t, int>>> &zv, int cap, std::vector<uint32_t> &dst) {
+        dst.assign((size_t)BA_NCLS * 2 * 16 * cap, 0u);
+        for (int cls = 0; cls < BA_NCLS; cls++)
+            for (int b = 0; b < 2; b++)
+                for (uint32_t hi = 0; hi < 16u; hi++)
+                    for (size_t e = 0; e < zv[(size_t)cls * 2 + b].size(); e++) {
+                        const uint32_t cz = zv[(size_t)cls * 2 + b][e].first;
+                        const int v = zv[(size_t)cls * 2 + b][e].second;
+                        const int lz = 31 - __builtin_clz(cz);
+                        uint32_t x = 0;
+                        for (int sft = 5; sft <= 8; sft++)
+                            if (lz + sft <= m) x |= Bof(tt_prepend((hi << 4) | (uint32_t)cls, sft, cz), v) << (8 * (sft - 5));
+                        dst[((((size_t)cls * 2 + b) * 16 + hi) * cap) + e] = x;
+                    }
+    };
+    tails(rin_zv, T.nri, T.RI8);
+    tails(rout_zv, T.nro, T.RO8);
     T.ok = true;
 }
