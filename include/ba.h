@@ -126,6 +126,14 @@ int ba_terms_per_sweep(int n, unsigned long long *T);
 int ba_debug_count_terms(ba_ctx *c, unsigned long long *in_terms, unsigned long long *out_terms,
                          unsigned long long *in_emb_sum, unsigned long long *out_emb_sum);
 
+/* Host-only self-check of the static pair tables the ENUM kernels use for a low tile of m bits (1 <= m <= 8;
+ * m = min(n, 8)): under each of the 16 classes every pair (v, z) -- v in {0,1}^m, z a non-empty subsequence of
+ * v -- must be served exactly once, by a fast pair or by a rider, with the embedding counts B(sigma_s.z, v)
+ * an independent DP gives.  stats[0] / stats[2] = fast pairs of the input / output tables summed over
+ * the classes, stats[1] / stats[3] = riders; so stats[0] + stats[1] = stats[2] + stats[3] = 16 (T(m) - 2^m)
+ * (Lemma 6).  Needs no device.  Returns BA_OK or BA_EINVAL.  Host pointer. */
+int ba_debug_check_tables(int m, unsigned long long stats[4]);
+
 void ba_destroy(ba_ctx *c);
 const char *ba_last_error(const ba_ctx *c);
 

@@ -23,7 +23,7 @@ _CODE_NAMES = {0: "BA_OK", -1: "BA_EINVAL", -2: "BA_ENOMEM", -3: "BA_ECUDA", -4:
 EXPORTS = ["ba_create", "ba_iterate", "ba_bounds", "ba_get_p", "ba_scratch_bytes", "ba_create_ext",
            "ba_set_mode", "ba_set_p", "ba_get_q", "ba_get_D", "ba_stats", "ba_get_history",
            "ba_last_timing", "ba_debug_emb_row", "ba_debug_emb_col", "ba_terms_per_sweep",
-           "ba_debug_count_terms", "ba_destroy", "ba_last_error"]
+           "ba_debug_count_terms", "ba_debug_check_tables", "ba_destroy", "ba_last_error"]
 
 
 class BAError(RuntimeError):
@@ -67,6 +67,7 @@ def load():
     L.ba_debug_emb_col.argtypes = [vp, ctypes.c_uint, up]
     L.ba_terms_per_sweep.argtypes = [ctypes.c_int, ullp]
     L.ba_debug_count_terms.argtypes = [vp, ullp, ullp, ullp, ullp]
+    L.ba_debug_check_tables.argtypes = [ctypes.c_int, ullp]
     L.ba_destroy.argtypes = [vp]
     L.ba_destroy.restype = None
     L.ba_last_error.argtypes = [vp]
@@ -224,6 +225,13 @@ def ba_terms_per_sweep(n):
     if rc != BA_OK:
         raise BAError(rc, "ba_terms_per_sweep")
     return t.value
+
+
+def ba_debug_check_tables(m):
+    """Host-only self-check of the pair tables for an m-bit low tile; returns (rc, [in_fast, in_riders, out_fast, out_riders])."""
+    st = (ctypes.c_ulonglong * 4)()
+    rc = load().ba_debug_check_tables(int(m), st)
+    return rc, [int(x) for x in st]
 
 
 def ba_debug_count_terms(ctx):

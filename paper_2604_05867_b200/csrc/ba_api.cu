@@ -153,6 +153,96 @@ extern "C" int ba_terms_per_sweep(int n, unsigned long long *T) {
     return BA_OK;
 }
 
+// Host-only self-check of the static tile tables of width m (include/ba.h): under every class, every pair
+// (v, z != empty) of the m-bit deletion channel must be served exactly once, by a fast pair or by a rider, with
+// the B_s an independent DP gives.
+static uint32_t chk_emb(uint32_t w, int lw, uint32_t v, int lv) {
+    if (lw > lv) return 0;
+    uint32_t e[BA_MLOW + 2];
+    for (int r = 0; r <= lw; r++) e[r] = (r == 0);
+    for (int i = 0; i < lv; i++)
+        for (int r = lw; r >= 1; r--)
+            if (((w >> (lw - r)) & 1u) == ((v >> (lv - 1 - i)) & 1u)) e[r] += e[r - 1];
+    return e[lw];
+}
+
+extern "C" int ba_debug_check_tables(int m, unsigned long long stats[4]) {
+    if (m < 1 || m > BA_MLOW || !stats) return BA_EINVAL;
+    const std::shared_ptr<const TileTables> Tp = tile_tables(m);
+    const TileTables &T = *Tp;
+    if (!T.ok) return BA_EINVAL;
+    const int nv = 1 << m, NZc = 2 << m;
+    stats[0] = stats[1] = stats[2] = stats[3] = 0;
+    auto Bs = [&](uint32_t sig, int s, uint32_t cz, int v) -> uint32_t {      // B(sigma_s.z, v)
+        const int lz = 31 - __builtin_clz(cz);
+        if (lz + s > m) return 0u;
+        return chk_emb(((sig & ((1u << s) - 1u)) << lz) | (cz - (1u << lz)), lz + s, (uint32_t)v, m);
+    };
+    for (int side = 0; side < 2; side++)                    // 0: input sweep tables, 1: output sweep tables
+        for (int cls = 0; cls < BA_NCLS; cls++)
+            for (int b = 0; b < 2; b++) {
+                std::vector<uint8_t> seen((size_t)nv * NZc, 0);
+                auto visit = [&](int v, uint32_t cz, uint32_t b0123, int nb, const uint32_t *tail8) -> bool {
+                    if (v < 0 || v >= nv || cz < 2 || cz >= (uint32_t)NZc) return false;
+                    const int lz = 31 - __builtin_clz(cz);
+                    if ((int)((cz >> (lz - 1)) & 1u) != b || seen[(size_t)v * NZc + cz]++) return false;
+                    for (int s = 0; s < 4; s++) if (((b0123 >> (8 * s)) & 0xffu) != Bs((uint32_t)cls, s, cz, v)) return false;
+                    if (nb == 4) return Bs((uint32_t)cls, 4, cz, v) == 0;                 // a fast pair must not be deep
+                    for (uint32_t hi = 0; hi < 16u; hi++)                                 // rider: B_4 .. B_8
+                        for (int s = 4; s <= 8; s++) {
+                            const uint32_t want = Bs((hi << 4) | (uint32_t)cls, s, cz, v);
+                            const uint32_t got = (s == 4) ? (uint32_t)nb - 5u : ((tail8[hi] >> (8 * (s - 5))) & 0xffu);
+                            if (want != got) return false;
+                        }
+                    return true;
+                };
+                const std::vector<uint2> &F = side ? T.FO : T.FI;
+                for (int c = 0; c < BA_NC; c++)
+                    for (int tid = 0; tid < BA_NT; tid++) {
+                        const uint32_t ow = side ? T.out_owner[(((size_t)cls * 2 + b) * BA_NC + c) * BA_NT + tid]
+                                                 : T.in_owner[((size_t)b * BA_NC + c) * BA_NT + tid];
+                        for (int q = 0; q < BA_C; q++) {
+                            const uint2 e = F[((((size_t)cls * 2 + b) * BA_NC + c) * BA_C + q) * BA_NT + tid];
+                            if (!(e.x & 0xffu)) continue;
+                            if (ow == 0xffffu) return BA_EINVAL;
+                            const uint32_t pos = ba_swz(e.y >> 3);
+                            bool okp;
+                            if (side) okp = visit((int)pos, ow, e.x, 4, nullptr);
+                            else {
+                                const int lt = 31 - __builtin_clz(pos);
+                                okp = visit((int)ow, (1u << (lt + 1)) | ((uint32_t)b << lt) | (pos - (1u << lt)), e.x, 4, nullptr);
+                            }
+                            if (!okp) return BA_EINVAL;
+                            stats[side ? 2 : 0]++;
+                        }
+                    }
+                const std::vector<uint4> &R = side ? T.RO : T.RI;
+                const std::vector<uint32_t> &R8 = side ? T.RO8 : T.RI8;
+                const int cap = side ? T.nro : T.nri, nr = side ? T.ro_cnt[cls * 2 + b] : T.ri_cnt[cls * 2 + b];
+                for (int e = 0; e < nr; e++) {
+                    const uint4 rd = R[((size_t)cls * 2 + b) * cap + e];
+                    uint32_t tail8[16];
+                    for (uint32_t hi = 0; hi < 16u; hi++) tail8[hi] = R8[(((size_t)cls * 2 + b) * 16 + hi) * cap + e];
+                    const uint32_t pos = ba_swz(rd.z >> 3), ow = rd.y >> 16;
+                    bool okp;
+                    if (side) okp = visit((int)pos, ow, rd.x, 5 + (int)(rd.y & 0xffu), tail8);
+                    else {
+                        const int lt = 31 - __builtin_clz(pos);
+                        okp = visit((int)ow, (1u << (lt + 1)) | ((uint32_t)b << lt) | (pos - (1u << lt)), rd.x, 5 + (int)(rd.y & 0xffu), tail8);
+                    }
+                    if (!okp || (rd.y & 0xffu) == 0) return BA_EINVAL;
+                    stats[side ? 3 : 1]++;
+                }
+                for (int v = 0; v < nv; v++)                 // nothing missing
+                    for (uint32_t cz = 2; cz < (uint32_t)NZc; cz++) {
+                        const int lz = 31 - __builtin_clz(cz);
+                        if ((int)((cz >> (lz - 1)) & 1u) != b) continue;
+                        if ((chk_emb(cz - (1u << lz), lz, (uint32_t)v, m) != 0) != (seen[(size_t)v * NZc + cz] != 0)) return BA_EINVAL;
+                    }
+            }
+    return BA_OK;
+}
+
 // ------------------------------------------------------------------------------------------------ create / destroy
 static int setup_ctx(ba_ctx *c, int n, double d) {
     c->n = n; c->m = low_m(n); c->h = n - c->m; c->d = d;

@@ -72,3 +72,16 @@ def test_no_cpu_fallback():
         pytest.skip("CUDA device present")
     with pytest.raises(ba.BAError):
         ba.ba_create(8, 0.5)
+
+
+@pytest.mark.parametrize("m", [1, 2, 3, 5, 8])
+def test_pair_tables_cover_every_pair_once(m):
+    # the class tables + riders of the ENUM kernels partition the pairs (v, z != empty) of the m-bit channel:
+    # 16 classes x (T(m) - 2^m) pairs (Lemma 6), with the B_s of an independent DP
+    rc, st = ba.ba_debug_check_tables(m)
+    assert rc == ba.BA_OK
+    T = sum((1 << k) * sum(comb(m, i) for i in range(m - k + 1)) for k in range(m + 1))
+    assert st[0] + st[1] == 16 * (T - (1 << m)) == st[2] + st[3]
+    if m == 8:
+        assert 0 < st[1] < 0.05 * (st[0] + st[1]) and st[1] == st[3]      # riders: the 3.4 % deep pairs
+    assert ba.ba_debug_check_tables(0)[0] == ba.BA_EINVAL and ba.ba_debug_check_tables(9)[0] == ba.BA_EINVAL
