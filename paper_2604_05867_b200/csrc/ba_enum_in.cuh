@@ -8,7 +8,8 @@
 //            Sub[pos] in the role of the Count table P:260-274 and NextPos P:256-258 done with clz on bit
 //            masks), and carries the integer embedding-count DP  E[i] = emb(y', u[0:i])  in registers
 //            along the descent; the node record {alpha_0..8, code(y'), mask} goes to shared memory.
-//   eps      the pair (v, empty) of every node of the round: thread (v, node), whole chain walked.
+//   eps      the pair (v, empty) of every node of the round: thread (v, node), all nine B(sigma_s, v) from
+//            one 8-byte read of the direct table EPS8[sigma_8][v].
 //   sort     per list b (non-empty z starting with b; a node carries list b iff b cannot follow y' in u)
 //            the nodes are ranked, stably, by class; the rounds' runs are merged into one order.
 //   phase B  batches of <= BA_RB_IN nodes of one (list, class).  The operands c(y'.z), z = b.t, of a node
@@ -66,7 +67,11 @@ __host__ __device__ static inline InSmem enum_in_smem(int m, int ncsr, int nri) 
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o += (bytes + 15) & ~(size_t)15; return at; };
     s.rec = take((size_t)BA_IN_SB * sizeof(NodeRec));
-    s.ceps = take((size_t)BA_NT * 8);
+    {                                                      // c(y') of a round (phase A / eps) and the rider sums
+        const size_t ce = (size_t)BA_NT * 8, rs = (size_t)2 * 2 * nri * 8;   // of phase B share one area
+        s.ceps = take(ce > rs ? ce : rs);
+        s.rsum = s.ceps;
+    }
     size_t rows = (size_t)2 * BA_RB_IN * ((size_t)1 << m) * 8, ac = ((size_t)2 * BA_NC + 2) * BA_NT * 8;
     s.rows = take(rows > ac ? rows : ac);                  // the epilogue's accumulator staging aliases the rows
     s.bal = take((size_t)2 * BA_RB_IN * 16);
@@ -77,7 +82,6 @@ __host__ __device__ static inline InSmem enum_in_smem(int m, int ncsr, int nri) 
     s.gstart = take((size_t)(BA_IN_NBKT + 1) * 2);
     s.wcnt = take((size_t)(BA_NT / 32) * BA_NCLS * 2);
     s.batch = take((size_t)BA_IN_MAXB * 4);
-    s.rsum = take((size_t)2 * nri * 8);
     s.csr_off = take(((size_t)(1 << m) + 1) * 2);
     (void)ncsr;                                            // the CSR indices are read from global memory (L2)
     s.sub = take(32 * 4);
@@ -310,7 +314,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 const int kq = (int)(s_batch[j] >> 24), buf = j & 1;
                 const uint16_t *cs = a.ri_csr + (size_t)((kq % BA_NCLS) * 2 + kq / BA_NCLS) * (nv + 1) + tid;
                 const int e0 = cs[0], e1 = cs[1];
-                for (int e = e0; e < e1; e++) acc_rid += s_rsum[(size_t)buf * a.nri + e];
+                for (int e = e0; e < e1; e++) acc_rid += s_rsum[((size_t)buf * 2) * a.nri + e] + s_rsum[((size_t)buf * 2 + 1) * a.nri + e];
             };
             if (nbatch > 0) stage(0);
             for (int j = 0; j < nbatch; j++) {
@@ -380,8 +384,9 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                     }
                     // ---- riders: deep pairs of this class, one per thread ------------------------------------
                     const int nr = a.ri_cnt[cls * 2 + b];
-                    const int re = BA_NT - 1 - tid;              // riders sit on the last warps (two chunk slots only)
-                    if (BA_NT - 32 * (warp + 1) < nr) {
+                    // two replicas of the rider set (threads 255 - e and 511 - e), each takes every other node
+                    const int re = (BA_NT / 2 - 1) - (tid & (BA_NT / 2 - 1)), rh = tid / (BA_NT / 2);
+                    if ((BA_NT / 2) - 32 * ((warp & (BA_NT / 64 - 1)) + 1) < nr) {
                         double s = 0.0;
                         if (re < nr) {
                             const uint4 rd = __ldg(a.RI + ((size_t)cls * 2 + b) * a.nri + re);
@@ -390,7 +395,8 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                             const uint32_t cz = ba_z_of_tail((uint32_t)b, ba_swz(rd.z >> 3));
                             const int jz = ba_len_of_code(cz);
                             const uint32_t *r8 = a.RI8 + ((size_t)cls * 2 + b) * 16 * a.nri + re;
-                            for (int i = 0; i < len; i++) {
+#pragma unroll 4                                           // four independent L2 reads of the chain tails in flight
+                            for (int i = rh; i < len; i += 2) {
                                 const NodeRec &rc = s_rec[bnode[i]];
                                 const uint4 r0 = *(const uint4 *)&rc.a[0], r1 = *(const uint4 *)&rc.a[4], r2 = *(const uint4 *)&rc.a[8];
                                 const uint32_t cy = r2.y;
@@ -414,7 +420,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                                 }
                             }
                         }
-                        if ((MODE == IN_SWEEP || MODE == IN_HC) && re < nr) s_rsum[(size_t)buf * a.nri + re] = s;
+                        if ((MODE == IN_SWEEP || MODE == IN_HC) && re < nr) s_rsum[((size_t)buf * 2 + rh) * a.nri + re] = s;
                     }
                 }
             }

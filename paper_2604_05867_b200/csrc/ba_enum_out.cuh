@@ -15,9 +15,9 @@
 //            contiguous 2^m-double row, staged with 16-byte cp.async, double buffered.  Pairs (v,z) are
 //            dealt z-major: every thread owns BA_NC chunks of BA_C supersequences v of one z per list,
 //            with one FP64 accumulator per chunk kept in a register for the whole item, and runs
-//                 4 IMAD (emb) + 1 LDS.64 (p) + 1 DADD (exact u32->f64) + 1 DFMA        per (x,y) term.
-//            The pair (v, empty) of every node and the deep pairs (riders) use all nine B_s, which are
-//            walked once per item.
+//                 1-4 IMAD (emb) + 1 LDS.64 (p) + 1 exact u32->f64 + 1 DFMA             per (x,y) term.
+//            The pair (v, empty) of every node and the deep pairs (riders) use all nine B_s, read once
+//            per item from direct tables.
 //   epilogue the chunks of each z are added in a fixed order and written once:
 //            Apart[y'][z] = sum_{u, v} emb(y'.z, u.v) p(u.v) over the nodes where y' is the longest
 //            prefix of y'.z embeddable in u.

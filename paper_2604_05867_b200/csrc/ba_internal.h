@@ -22,8 +22,8 @@
 // (class-specific FAST table, global memory / L2) and then loops over the nodes of the run with
 //   emb = a0*B0 + a1*B1 + a2*B2 + a3*B3        (4 IMAD, no unpacking, no links, no votes)
 // A pair whose chain reaches s = BA_KB under the class (3.4 % of the pairs) is DEEP: it is left out of
-// the class's fast table and handled as a RIDER, one rider per thread: B_0..B_4 static, the rest of the
-// chain walked through byte-packed prepend links (the v-major table Wv in shared memory).
+// the class's fast table and handled as a RIDER, one rider per thread: B_0..B_4 static, B_5..B_8 from a
+// direct table indexed by the sigma bits 4..7.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -44,7 +44,8 @@
 #define BA_SBR 3             // input sweep: phase-A rounds (of BA_NT nodes) per super-batch
 #define BA_RB_OUT 48         // nodes per batch, output sweep (operand rows of 2^m doubles)
 
-// ---- v-major prepend links Wv: one uint32 per entry of v's list ([0] null, [1] empty string, then the
+// ---- v-major prepend links Wv (host side only: the table builder walks them; the kernels read the direct
+// tables EPS8 / RI8 / RO8 instead): one uint32 per entry of v's list ([0] null, [1] empty string, then the
 // non-empty subsequences of v):  W = l0 | cB0 << 8 | l1 << 16 | cB1 << 24,  l_b = local index of b.z in
 // v's list (0 = null: b.z is not a subsequence of v), cB_b = B(b.z, v).
 // ---- fast pairs: uint2 {B0 | B1<<8 | B2<<16 | B3<<24, byte offset of the operand in the staged row}
@@ -166,44 +167,6 @@ __device__ __forceinline__ double ba_fast_chunk(double s, const uint4 *bal, uint
     if (any >> 16) return ba_fast_loop<3>(s, bal, rowbase, ROWB, len, bp, ad);
     if (any >> 8) return ba_fast_loop<2>(s, bal, rowbase, ROWB, len, bp, ad);
     return ba_fast_loop<1>(s, bal, rowbase, ROWB, len, bp, ad);
-}
-
-// emb of one pair by walking the whole chain (lanes of a warp may belong to different nodes): W = the
-// pair's prepend word, B = B_0, vb = shared byte address of v's list in Wv, al = alpha_0..8, sig = code(y').
-template <int STRIDE>
-__device__ __forceinline__ uint32_t ba_chain_single(uint32_t W, uint32_t B, uint32_t vb, const uint32_t (&al)[9],
-                                                    uint32_t sig, int L) {
-    uint32_t emb = al[0] * B;
-    if (L >= 1) {
-        uint32_t hw = (sig & 1u) ? (W >> 16) : (W & 0xffffu);
-        emb += al[1] * (hw >> 8);
-        uint32_t lk = hw & 0xffu;
-#pragma unroll
-        for (int s = 2; s <= 8; s++) {
-            if (L >= s && lk != 0u) {
-                hw = ba_lds_u16(vb + ((sig >> (s - 1)) & 1u) * 2u + lk * (uint32_t)STRIDE);
-                emb += al[s] * (hw >> 8);
-                lk = hw & 0xffu;
-            }
-        }
-    }
-    return emb;
-}
-
-// Continue a chain from step s0: lk = local index of sigma_{s0-1}.z in v's list; returns the sum of the
-// remaining alpha_s B_s.
-__device__ __forceinline__ uint32_t ba_chain_from(int s0, uint32_t lk, uint32_t vb, const uint32_t (&al)[9],
-                                                  uint32_t sig, int L) {
-    uint32_t emb = 0u;
-#pragma unroll
-    for (int s = 1; s <= 8; s++) {
-        if (s >= s0 && L >= s && lk != 0u) {
-            const uint32_t hw = ba_lds_u16(vb + ((sig >> (s - 1)) & 1u) * 2u + lk * 4u);
-            emb += al[s] * (hw >> 8);
-            lk = hw & 0xffu;
-        }
-    }
-    return emb;
 }
 
 // Stable rank of every thread's key among the CTA (keys < NKEY; key < 0 = not ranked): order[pos] = tid with

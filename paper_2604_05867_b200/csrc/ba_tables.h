@@ -405,7 +405,7 @@ static inline void build_tile_tables(int m, TileTables &T) {
         }
         return true;
     };
-    if (!pack_riders(rin, T.RI, T.ri_cnt, T.nri)) return;
+    if (!pack_riders(rin, T.RI, T.ri_cnt, T.nri) || T.nri > BA_NT / 2) return;   // the in sweep runs two replicas
     if (!pack_riders(rout, T.RO, T.ro_cnt, T.nro)) return;
     // ---- direct tables for the whole-chain pairs of the input sweep ------------------------------------------
     T.EPS8.assign((size_t)256 * nv, make_uint2(0u, 0u));
