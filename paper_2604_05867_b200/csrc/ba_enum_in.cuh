@@ -138,6 +138,9 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
     const uint32_t sRows = ba_smem_addr(s_rows);
     const int ev = tid & (nv - 1);                          // v of this thread's empty-z pairs
     const int esub = tid >> m, epn = BA_NT >> m;            // it serves nodes esub, esub + epn, ...
+    const int st_pc = tid & ((nv >> 1) - 1), st_i0 = tid >> (m - 1), st_step = BA_NT >> (m - 1);   // staging role
+    const int st_lt = st_pc ? ba_len_of_code(2u * (uint32_t)st_pc) : 0;
+    const uint32_t st_tv = st_pc ? (2u * (uint32_t)st_pc - (1u << st_lt)) : 0u, st_dst = ba_swz(2u * (uint32_t)st_pc) * 8u;
     __syncthreads();
 
     unsigned long long cnt_terms = 0, cnt_emb = 0;
@@ -288,18 +291,15 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 const int start = (int)(bi & 0xffffu), len = (int)((bi >> 16) & 0xffu), buf = j & 1;
                 const uint32_t b = (bi >> 24) / BA_NCLS;
                 if (MODE == IN_SWEEP) {
-                    // 16-byte pieces (positions 2pc, 2pc+1): 2^{m-1} per half row
-                    for (int pidx = tid; pidx < (len << (m - 1)); pidx += BA_NT) {
-                        const int i = pidx >> (m - 1), pc = pidx & ((nv >> 1) - 1);
+                    // 16-byte pieces (positions 2pc, 2pc+1), 2^{m-1} per half row: a thread always copies the same
+                    // piece, of every st_step-th row
+                    for (int i = st_i0; i < len; i += st_step) {
                         const uint32_t cy = s_rec[s_order[start + i]].id;
                         const uint32_t dst = sRows + ((uint32_t)(buf * BA_RB_IN + i) * ROWD) * 8u;
-                        if (pc == 0) {                         // position 1: t empty, z = "b"
+                        if (st_pc == 0)                        // position 1: t empty, z = "b"
                             ba_cp_async8(dst + 8u, a.c + (((size_t)cy << 1) + b));
-                        } else {
-                            const uint32_t tc = 2u * (uint32_t)pc;
-                            const int lt = ba_len_of_code(tc);
-                            ba_cp_async16(dst + ba_swz(tc) * 8u, a.c + (((size_t)cy << (lt + 1)) + ((size_t)b << lt) + (tc - (1u << lt))));
-                        }
+                        else
+                            ba_cp_async16(dst + st_dst, a.c + (((size_t)cy << (st_lt + 1)) + ((size_t)b << st_lt) + st_tv));
                     }
                 }
                 if (tid < len) {

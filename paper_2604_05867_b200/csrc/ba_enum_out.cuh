@@ -100,6 +100,8 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
     const uint32_t sRows = ba_smem_addr(s_rows);
     const int ev = tid & (nv - 1);                          // v of this thread's empty-z pairs
     const int esub = tid >> m, epn = BA_NT >> m;
+    const int st_pc = tid & ((nv >> 1) - 1), st_i0 = tid >> (m - 1), st_step = BA_NT >> (m - 1);   // staging role
+    const uint32_t st_src = 2u * (uint32_t)st_pc, st_dst = ba_swz(2u * (uint32_t)st_pc) * 8u;
     __syncthreads();
 
     unsigned long long cnt_terms = 0, cnt_emb = 0;
@@ -220,13 +222,10 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                 const uint32_t bi = s_batch[j];
                 const int start = (int)(bi & 0xffffu), len = (int)((bi >> 16) & 0xffu), buf = j & 1;
                 if (MODE == OUT_SWEEP) {
-                    if (m >= 1) {
-                        for (int pidx = tid; pidx < (len << (m - 1)); pidx += BA_NT) {   // 16-byte pieces, 2^{m-1} per row
-                            const int i = pidx >> (m - 1), pc = pidx & ((nv >> 1) - 1);
-                            const uint32_t u = s_rec[s_order[start + i]].id;
-                            ba_cp_async16(sRows + (uint32_t)(buf * BA_RB_OUT + i) * ROWB + ba_swz(2u * (uint32_t)pc) * 8u,
-                                          a.p + (((size_t)u << m) + 2u * (size_t)pc));
-                        }
+                    // 16-byte pieces, 2^{m-1} per row: a thread always copies the same piece, of every st_step-th row
+                    for (int i = st_i0; i < len; i += st_step) {
+                        const uint32_t u = s_rec[s_order[start + i]].id;
+                        ba_cp_async16(sRows + (uint32_t)(buf * BA_RB_OUT + i) * ROWB + st_dst, a.p + (((size_t)u << m) + st_src));
                     }
                 }
                 if (tid < len) {
