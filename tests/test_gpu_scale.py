@@ -222,3 +222,13 @@ def test_config3_harness_small(ba, mode):
     assert r["I_lower"] <= 2.123006166059 + 1e-9 <= r["running_min_upper"] + 2e-9
     assert r["running_min_upper"] - r["I_lower"] < 1e-6 and r["stop_statistic_U_minus_log2Z"] <= r["gap"] + 1e-12
     assert r["upper_over_n_over_1_minus_d"] == pytest.approx(r["running_min_upper"] / 8 / 0.5)
+
+
+@pytest.mark.slow
+def test_T7_scale_n28_config5(ba):
+    # BASELINE.json configs[4]: n=28, d=0.80 (34 GB on the device, ~8 minutes on a B200, ~20 GB of host arrays).
+    # Opt-in: BA_RUN_N28=1.  Result of the round-1 run: profiles/r01c_scale_n28.md.
+    import os
+    if os.environ.get("BA_RUN_N28") != "1":
+        pytest.skip("set BA_RUN_N28=1 to run the n=28 scale check")
+    scale_checks(ba, 28, 0.80, n_rows=3, n_cols=0, seed=28)
