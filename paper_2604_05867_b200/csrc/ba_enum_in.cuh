@@ -228,7 +228,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 ba_bucket_sort<BA_NCLS>(key1, s_ordr + (size_t)(rd * 2 + 1) * BA_NT, s_wcnt, s_seg + (rd * 2 + 1) * (BA_NCLS + 1));
 
                 // ================= eps: the pair (v, empty) of every node of the round =================
-#pragma unroll 4
+#pragma unroll 8
                 for (int i = esub; i < nn; i += epn) {
                     const NodeRec &rc = s_rec[rd * BA_NT + i];
                     const uint4 r0 = *(const uint4 *)&rc.a[0], r1 = *(const uint4 *)&rc.a[4], r2 = *(const uint4 *)&rc.a[8];
