@@ -232,3 +232,26 @@ def test_T7_scale_n28_config5(ba):
     if os.environ.get("BA_RUN_N28") != "1":
         pytest.skip("set BA_RUN_N28=1 to run the n=28 scale check")
     scale_checks(ba, 28, 0.80, n_rows=3, n_cols=0, seed=28)
+
+
+# ------------------------------------------------------------------ one-step parity at the oracle's reach, extreme d
+
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("d,seed", [(0.95, None), (0.95, 3), (0.05, 4)])
+def test_T3_T4_one_step_n14_extreme_d(ba, d, seed, mode):
+    # configs[2] sweeps d up to 0.95: the hoisted logarithm must keep 1e-12 on D where D itself is small
+    n = 14
+    p = si.uniform_p0(n) if seed is None else si.random_positive_p(n, seed)
+    ref = orc.ba_step(orc.channel(n, d), p)
+    ctx = ba.ba_create(n, d)
+    try:
+        ba.ba_set_mode(ctx, mode)
+        ba.ba_set_p(ctx, p)
+        ba.ba_iterate(ctx, 1)
+        q, D = ba.ba_get_q(ctx), ba.ba_get_D(ctx)
+        I, U = ba.ba_bounds(ctx)
+    finally:
+        ba.ba_destroy(ctx)
+    assert np.max(np.abs(q - ref["q"]) / ref["q"]) <= REL_QD
+    assert np.max(np.abs(D - ref["D"]) / np.abs(ref["D"])) <= REL_QD
+    assert abs(I - ref["I"]) <= REL_QD * max(1.0, abs(ref["I"])) and abs(U - ref["U"]) <= REL_QD * max(1.0, abs(ref["U"]))
