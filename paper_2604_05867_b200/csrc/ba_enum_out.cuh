@@ -12,7 +12,8 @@
 //   sort     nodes are ranked, stably, by mask (which lists of non-empty z they carry).
 //   phase B  batches of <= BA_RB_OUT nodes of one mask.  For node u the 2^m inputs p(u.*) -- the run
 //            of inputs whose low m bits are free (SURVEY 7.2 "coalescing the gather") -- are one
-//            contiguous 2^m-double row, staged with 16-byte cp.async, double buffered.  Pairs (v,z) are
+//            contiguous 2^m-double row, staged with 16-byte cp.async into a 3-stage ring whose FULL / EMPTY
+//            mbarriers are the only per-batch synchronisation (no CTA-wide barrier).  Pairs (v,z) are
 //            dealt z-major: every thread owns BA_NC chunks of BA_C supersequences v of one z per list,
 //            with one FP64 accumulator per chunk kept in a register for the whole item, and runs
 //                 1-4 IMAD (emb) + 1 LDS.64 (p) + 1 exact u32->f64 + 1 DFMA             per (x,y) term.
@@ -29,6 +30,7 @@
 enum { OUT_SWEEP = 0, OUT_DEBUG = 1, OUT_COUNT = 2 };
 
 #define BA_OUT_MAXB (4 + BA_NT / BA_RB_OUT)
+#define BA_OUT_NSTG 3                                       // stages of the operand-row ring
 
 __constant__ uint32_t c_binom[BA_NMAX_I + 1][BA_NMAX_I + 1];
 
@@ -54,17 +56,18 @@ struct OutArgs {
     unsigned long long *cnt;   // OUT_COUNT
 };
 
-struct OutSmem { size_t rec, rows, bal, bnode, order, wcnt, bstart, batch, red, item, total; };
+struct OutSmem { size_t rec, rows, bal, bnode, mbar, order, wcnt, bstart, batch, red, item, total; };
 
 __host__ __device__ static inline OutSmem enum_out_smem(int m, int ncsr, int nro) {
     OutSmem s;
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o += (bytes + 15) & ~(size_t)15; return at; };
     s.rec = take((size_t)BA_NT * sizeof(NodeRec));
-    size_t rows = (size_t)2 * BA_RB_OUT * ((size_t)1 << m) * 8, ac = ((size_t)2 * BA_NC * BA_NT + 2 * (size_t)nro) * 8;
+    size_t rows = (size_t)BA_OUT_NSTG * BA_RB_OUT * ((size_t)1 << m) * 8, ac = ((size_t)2 * BA_NC * BA_NT + 2 * (size_t)nro) * 8;
     s.rows = take(rows > ac ? rows : ac);                  // the epilogue's accumulator staging aliases the rows
-    s.bal = take((size_t)2 * BA_RB_OUT * 16);
-    s.bnode = take((size_t)2 * BA_RB_OUT * 2);
+    s.bal = take((size_t)BA_OUT_NSTG * BA_RB_OUT * 16);
+    s.bnode = take((size_t)BA_OUT_NSTG * BA_RB_OUT * 2);
+    s.mbar = take((size_t)2 * BA_OUT_NSTG * 8);            // FULL and EMPTY barrier of every stage
     s.order = take((size_t)BA_NT * 2);
     s.wcnt = take((size_t)(BA_NT / 32) * 4 * 2);
     s.bstart = take(5 * 2);
@@ -98,6 +101,15 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
     uint32_t *s_item = (uint32_t *)(smem + L.item);        // [0] item, [1] number of batches
 
     const uint32_t sRows = ba_smem_addr(s_rows);
+    const uint32_t sFull = ba_smem_addr(smem + L.mbar), sEmpty = sFull + BA_OUT_NSTG * 8u;
+    if (tid == 0) {
+        for (int i = 0; i < BA_OUT_NSTG; i++) {
+            ba_mbar_init(sFull + 8u * i, 2u * BA_NT);       // per thread: its copies landed + its plain stores done
+            ba_mbar_init(sEmpty + 8u * i, BA_NT);           // per thread: finished reading the stage
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    uint32_t gb = 0;                                        // batches staged so far by this CTA (uniform)
     const int ev = tid & (nv - 1);                          // v of this thread's empty-z pairs
     const int esub = tid >> m, epn = BA_NT >> m;
     const int st_pc = tid & ((nv >> 1) - 1), st_i0 = tid >> (m - 1), st_step = BA_NT >> (m - 1);   // staging role
@@ -218,9 +230,9 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
 
             // ================= phase B =================
             const int nbatch = (int)s_item[1];
-            auto stage = [&](int j) {                          // p rows, alpha_0..3 and node ids of batch j
+            auto stage = [&](int j, uint32_t g) {              // p rows, alpha_0..3 and node ids of batch j = ring batch g
                 const uint32_t bi = s_batch[j];
-                const int start = (int)(bi & 0xffffu), len = (int)((bi >> 16) & 0xffu), buf = j & 1;
+                const int start = (int)(bi & 0xffffu), len = (int)((bi >> 16) & 0xffu), buf = (int)(g % BA_OUT_NSTG);
                 if (MODE == OUT_SWEEP) {
                     // 16-byte pieces, 2^{m-1} per row: a thread always copies the same piece, of every st_step-th row
                     for (int i = st_i0; i < len; i += st_step) {
@@ -233,11 +245,14 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                     s_bal[buf * BA_RB_OUT + tid] = *(const uint4 *)&s_rec[node].a[0];
                     s_bnode[buf * BA_RB_OUT + tid] = (uint16_t)node;
                 }
+                ba_mbar_arrive_on_copies(sFull + 8u * buf);    // when this thread's rows have landed
+                ba_mbar_arrive(sFull + 8u * buf);              // releases its plain stores above
             };
-            if (nbatch > 0) stage(0);
+            for (int j = 0; j < BA_OUT_NSTG - 1 && j < nbatch; j++) stage(j, gb + j);
             for (int j = 0; j < nbatch; j++) {
                 const uint32_t bi = s_batch[j];
-                const int len = (int)((bi >> 16) & 0xffu), mask = (int)(bi >> 24), buf = j & 1;
+                const uint32_t g = gb + (uint32_t)j;
+                const int len = (int)((bi >> 16) & 0xffu), mask = (int)(bi >> 24), buf = (int)(g % BA_OUT_NSTG);
                 // the pairs of a chunk do not depend on the staged rows: fetch the first slot before waiting, and
                 // the next slot while the current one is computed (one exposed L2 latency per batch at most)
                 const uint2 *F0 = a.FO + ((size_t)cls * 2 * BA_NC) * BA_C * BA_NT + tid;   // list 0; list 1 follows
@@ -247,9 +262,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
 #pragma unroll
                     for (int q = 0; q < BA_C; q++) { const uint2 pr = __ldg(Ff + (size_t)q * BA_NT); nbp[q] = pr.x; nad[q] = pr.y; }
                 }
-                ba_cp_async_wait_all();
-                __syncthreads();                               // batch j staged; batch j-1 fully consumed
-                if (j + 1 < nbatch) stage(j + 1);
+                ba_mbar_wait(sFull + 8u * buf, (g / BA_OUT_NSTG) & 1u);          // batch j staged by every thread
                 const uint32_t rowbase = sRows + (uint32_t)(buf * BA_RB_OUT) * ROWB;
                 const uint4 *bal = s_bal + buf * BA_RB_OUT;
                 const uint16_t *bnode = s_bnode + buf * BA_RB_OUT;
@@ -325,7 +338,14 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                         acc_rid[b] = s;
                     }
                 }
+                ba_mbar_arrive(sEmpty + 8u * buf);             // this thread has finished reading the stage
+                if (j + BA_OUT_NSTG - 1 < nbatch) {            // refill the stage of ring batch g-1 with batch j+NSTG-1
+                    const uint32_t gn = g + BA_OUT_NSTG - 1;
+                    if (j >= 1) ba_mbar_wait(sEmpty + 8u * (gn % BA_OUT_NSTG), ((g - 1) / BA_OUT_NSTG) & 1u);
+                    stage(j + BA_OUT_NSTG - 1, gn);
+                }
             }
+            gb += (uint32_t)nbatch;
         }
 
         // ---- epilogue: fixed-order reduction of the chunks of each z, one write per (y', z) -----------------

@@ -42,7 +42,7 @@
 #define BA_NCLS 16           // 2^BA_KB classes
 #define BA_RB_IN 32          // nodes per batch, input sweep (operand half-rows of 2^m doubles)
 #define BA_SBR 3             // input sweep: phase-A rounds (of BA_NT nodes) per super-batch
-#define BA_RB_OUT 48         // nodes per batch, output sweep (operand rows of 2^m doubles)
+#define BA_RB_OUT 32         // nodes per batch, output sweep (operand rows of 2^m doubles)
 
 // ---- v-major prepend links Wv (host side only: the table builder walks them; the kernels read the direct
 // tables EPS8 / RI8 / RO8 instead): one uint32 per entry of v's list ([0] null, [1] empty string, then the
@@ -107,6 +107,29 @@ __device__ __forceinline__ void ba_cp_async8(uint32_t dst, const void *src) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
 }
 __device__ __forceinline__ void ba_cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+// ---- mbarrier ring (shared-memory transaction barriers): the batches' operand rows are produced by all
+// threads with cp.async and consumed by all threads; a FULL barrier per stage completes when every thread's
+// copies for that stage have landed (cp.async.mbarrier.arrive), an EMPTY barrier when every thread has finished
+// reading it.  Warps meet only through these barriers, so they may drift by a batch instead of stopping at a
+// CTA-wide barrier after every batch.
+__device__ __forceinline__ void ba_mbar_init(uint32_t addr, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(addr), "r"(count) : "memory");
+}
+__device__ __forceinline__ void ba_mbar_arrive(uint32_t addr) {
+    asm volatile("{ .reg .b64 st; mbarrier.arrive.shared::cta.b64 st, [%0]; }" ::"r"(addr) : "memory");
+}
+__device__ __forceinline__ void ba_mbar_arrive_on_copies(uint32_t addr) {      // arrives when this thread's cp.async landed
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(addr) : "memory");
+}
+__device__ __forceinline__ void ba_mbar_wait(uint32_t addr, uint32_t parity) {
+    uint32_t done = 0;
+    for (uint32_t spin = 0; !done; spin++) {
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(done) : "r"(addr), "r"(parity) : "memory");
+        if (spin > (1u << 26)) __trap();                    // a lost arrival must fail loudly, not hang the device
+    }
+}
 
 // exact uint32 -> FP64 on the FP64 pipe (a DADD) instead of the quarter-rate conversion unit
 __device__ __forceinline__ double ba_u2d(uint32_t e) {
