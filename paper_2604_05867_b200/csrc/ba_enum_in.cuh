@@ -297,9 +297,9 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                         const uint32_t cy = s_rec[s_order[start + i]].id;
                         const uint32_t dst = sRows + ((uint32_t)(buf * BA_RB_IN + i) * ROWD) * 8u;
                         if (st_pc == 0)                        // position 1: t empty, z = "b"
-                            ba_cp_async8(dst + 8u, a.c + (((size_t)cy << 1) + b));
+                            ba_cp_async8(dst + 8u, a.c + ((cy << 1) + b));             // codes fit 32 bits (n <= 30)
                         else
-                            ba_cp_async16(dst + st_dst, a.c + (((size_t)cy << (st_lt + 1)) + ((size_t)b << st_lt) + st_tv));
+                            ba_cp_async16(dst + st_dst, a.c + ((cy << (st_lt + 1)) + (b << st_lt) + st_tv));
                     }
                 }
                 if (tid < len) {

@@ -237,7 +237,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                     // 16-byte pieces, 2^{m-1} per row: a thread always copies the same piece, of every st_step-th row
                     for (int i = st_i0; i < len; i += st_step) {
                         const uint32_t u = s_rec[s_order[start + i]].id;
-                        ba_cp_async16(sRows + (uint32_t)(buf * BA_RB_OUT + i) * ROWB + st_dst, a.p + (((size_t)u << m) + st_src));
+                        ba_cp_async16(sRows + (uint32_t)(buf * BA_RB_OUT + i) * ROWB + st_dst, a.p + ((u << m) + st_src));   // x fits 32 bits (n <= 30)
                     }
                 }
                 if (tid < len) {
