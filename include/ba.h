@@ -87,6 +87,14 @@ size_t ba_scratch_bytes(int n);
 int ba_create_ext(int n, double d, void *p_dev, void *q_dev, void *D_dev,
                   void *scratch_dev, size_t scratch_bytes, void *cuda_stream, ba_ctx **out);
 
+/* Switch the context to the paper's EXACT deletion channel BDC_{n,k}:
+ * W(y|x) = emb(y,x) / C(n,k) for |y| = k and 0 for every other length, 0 <= k <= n.  The same kernels run
+ * with the weight vector w_j = [j = k] / C(n,k); the sweeps still enumerate the terms of all lengths (the other
+ * lengths carry weight 0 and q is 0 there).  ba_bounds then brackets C_{n,k}; Lemma 2
+ * combines them into a bound on C_n(d).  Only before the first iteration: BA_ESTATE otherwise; BA_EINVAL for a
+ * bad k. */
+int ba_set_exact(ba_ctx *c, int k);
+
 /* Select BA_MODE_ENUM (default) or BA_MODE_FAST for subsequent iterations. */
 int ba_set_mode(ba_ctx *c, int mode);
 

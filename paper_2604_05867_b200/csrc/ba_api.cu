@@ -381,6 +381,16 @@ extern "C" void ba_destroy(ba_ctx *c) {
 
 extern "C" const char *ba_last_error(const ba_ctx *c) { return c ? c->err.c_str() : g_static_err; }
 
+extern "C" int ba_set_exact(ba_ctx *c, int k) {
+    if (!c) return BA_EINVAL;
+    if (k < 0 || k > c->n) return fail(c, BA_EINVAL, "ba_set_exact: k outside [0, n]");
+    if (c->iters != 0) return fail(c, BA_ESTATE, "ba_set_exact: only before the first iteration");
+    for (int j = 0; j <= c->n; j++) c->kc.w[j] = 0.0;
+    c->kc.w[k] = 1.0 / host_binom(c->n, k);                 // P_{n,k}(y|x) = emb(y,x) / C(n,k)
+    c->hc_ready = false;                                    // Hc depends on the weights
+    return BA_OK;
+}
+
 extern "C" int ba_set_mode(ba_ctx *c, int mode) {
     if (!c) return BA_EINVAL;
     if (mode != BA_MODE_ENUM && mode != BA_MODE_FAST) return fail(c, BA_EINVAL, "ba_set_mode: unknown mode");

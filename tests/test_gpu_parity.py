@@ -198,3 +198,72 @@ def test_T6_special_cases(ba, mode):
     (I, U), _ = run(2, d, 3000)
     assert I == pytest.approx(0.8304820237218407, abs=1e-12)
     assert U == pytest.approx(0.8304820237218407, abs=1e-9)
+
+
+# ------------------------------------------------------------------ NEXT-3: the paper's exact channel BDC_{n,k}
+
+def exact_W(n, k):
+    # P_{n,k}(y|x) = emb(y,x)/C(n,k) on the outputs of length k, 0 elsewhere, in the dense q layout
+    from math import comb
+    W = np.zeros(E_of(n).shape, dtype=np.float64)
+    sl = slice((1 << k) - 1, (2 << k) - 1)
+    W[:, sl] = E_of(n)[:, sl].astype(np.float64) / comb(n, k)
+    return W
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("n,k", [(2, 1), (5, 3), (8, 1), (8, 4), (8, 8), (11, 6)])
+def test_exact_channel_one_step_and_trajectory(ba, n, k, mode):
+    W = exact_W(n, k)
+    p = si.random_positive_p(n, 100 + n + k)
+    ref1 = orc.ba_step(W, p)
+    refK = orc.ba_run(W, p, 40)
+    ctx = ba.ba_create(n, 0.5)
+    try:
+        ba.ba_set_mode(ctx, mode)
+        ba.ba_set_exact(ctx, k)
+        ba.ba_set_p(ctx, p)
+        ba.ba_iterate(ctx, 1)
+        q, D = ba.ba_get_q(ctx), ba.ba_get_D(ctx)
+        nz = ref1["q"] > 0
+        assert np.array_equal(q > 0, nz)
+        assert relerr(q[nz], ref1["q"][nz]) <= REL_QD
+        # D = Hc - sum emb c (hoisted logarithm) has an absolute error of a few ulp of Hc; on BDC_{n,k} an input whose
+        # only output is nearly certain has D ~ 1e-7 bits, where that is 1e-10 relative:
+        # 1e-12 relative with an absolute floor of 1e-15 bits
+        assert np.all(np.abs(D - ref1["D"]) <= REL_QD * np.abs(ref1["D"]) + 1e-15)
+        ba.ba_iterate(ctx, 39)
+        I, U = ba.ba_bounds(ctx)
+        assert abs(I - refK["hist"][-1, 0]) <= ABS_U and abs(U - refK["hist"][-1, 1]) <= ABS_U
+        with pytest.raises(ba.BAError) as ei:
+            ba.ba_set_exact(ctx, k)                          # only before the first iteration
+        assert ei.value.code == ba.BA_ESTATE
+    finally:
+        ba.ba_destroy(ctx)
+
+
+def test_exact_channel_paper_values_and_lemma2(ba):
+    from math import comb
+
+    def run(n, k, K):
+        ctx = ba.ba_create(n, 0.5)
+        try:
+            ba.ba_set_mode(ctx, 1)
+            if k is not None:
+                ba.ba_set_exact(ctx, k)
+            ba.ba_iterate(ctx, K)
+            I, U = ba.ba_bounds(ctx)
+            return I, float(ba.ba_get_history(ctx, K)[:, 1].min())
+        finally:
+            ba.ba_destroy(ctx)
+
+    assert run(2, 2, 10)[0] == pytest.approx(2.0, abs=1e-13)          # C_{2,2} = 2
+    assert run(2, 1, 4000)[0] == pytest.approx(1.0, abs=1e-9)         # C_{2,1} = 1
+    assert run(8, 8, 3)[0] == pytest.approx(8.0, abs=1e-12)           # C_{n,n} = n (Tables 1-2, last row)
+    I1, U1 = run(8, 1, 4000)
+    assert I1 == pytest.approx(1.0, abs=2e-3) and U1 >= 1.0 - 1e-12   # C_{n,1} = 1 (Tables 1-2, first row)
+    # Lemma 2 with rigorous brackets at n=8, d=0.5: I(C_n(d)) <= sum_k Bin(k) U(C_{n,k})
+    d, n = 0.5, 8
+    left = run(n, None, 300)[0]
+    right = sum(comb(n, k) * d ** (n - k) * (1 - d) ** k * run(n, k, 300)[1] for k in range(1, n + 1))
+    assert left <= right and right == pytest.approx(2.3045, abs=5e-3) and left == pytest.approx(2.1230, abs=1e-4)
