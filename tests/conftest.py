@@ -3,6 +3,10 @@ import sys
 
 import pytest
 
+# The oracle (oracle/ba_oracle.c) uses OpenMP; on a box whose cores are shared, actively spinning idle threads
+# make it many times slower.  Must be set before libgomp is loaded; it does not touch the oracle's arithmetic.
+os.environ.setdefault("OMP_WAIT_POLICY", "passive")
+
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
