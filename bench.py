@@ -199,6 +199,8 @@ def run_ours(args, rank, world, local_rank):
 
     ctx = ba.ba_create(n, d, device=dev)
     ba.ba_set_mode(ctx, mode)
+    if args.exact_k >= 0:
+        ba.ba_set_exact(ctx, args.exact_k)
 
     # ---- device-resident arm: inputs (p) already in HBM when the timed region starts ---------------
     ba.ba_iterate(ctx, args.warmup)
@@ -285,7 +287,9 @@ def run_ours(args, rank, world, local_rank):
            "iterations_per_s": world * args.steps / (ms_total * 1e-3),
            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step,
            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-           "config": {"workload": f"BDC_d^n BA iteration, n={n}, d={d}, uniform p0 ({config_name(n, d)})",
+           "config": {"workload": (f"BDC_d^n BA iteration, n={n}, d={d}, uniform p0 ({config_name(n, d)})" if args.exact_k < 0 else
+                                   f"exact channel BDC_{{n,k}} BA iteration, n={n}, k={args.exact_k}, uniform p0 (not a BASELINE.json config; "
+                                   f"the sweeps still enumerate all lengths)"),
                       "mode": args.mode, "terms_per_iteration": 2 * T,
                       "term_counting": "enumerated" if args.mode == "enum" else "effective (FAST mode does not enumerate terms)",
                       "l2_policy": f"inputs_exceed_l2 (p {8 * NX / 1e6:.0f} MB, q and c {16 * NX / 1e6:.0f} MB each, "
@@ -319,6 +323,8 @@ def main():
     ap.add_argument("--oracle-iters", type=int, default=10)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=0, help="steps of the end-to-end arm (default: --steps)")
+    ap.add_argument("--exact-k", type=int, default=-1,
+                    help="run the paper's exact channel BDC_{n,k} (ba_set_exact) instead of BDC_d^n; not a BASELINE.json config")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
