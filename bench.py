@@ -201,6 +201,8 @@ def run_ours(args, rank, world, local_rank):
     ba.ba_set_mode(ctx, mode)
     if args.exact_k >= 0:
         ba.ba_set_exact(ctx, args.exact_k)
+    if args.symmetry:
+        ba.ba_set_symmetry(ctx, 1)
 
     # ---- device-resident arm: inputs (p) already in HBM when the timed region starts ---------------
     ba.ba_iterate(ctx, args.warmup)
@@ -291,7 +293,9 @@ def run_ours(args, rank, world, local_rank):
                                    f"exact channel BDC_{{n,k}} BA iteration, n={n}, k={args.exact_k}, uniform p0 (not a BASELINE.json config; "
                                    f"the sweeps still enumerate all lengths)"),
                       "mode": args.mode, "terms_per_iteration": 2 * T,
-                      "term_counting": "enumerated" if args.mode == "enum" else "effective (FAST mode does not enumerate terms)",
+                      "term_counting": ("enumerated" if args.mode == "enum" and not args.symmetry else
+                                        "effective (complement symmetry: half the terms are enumerated, the rest mirrored)" if args.mode == "enum"
+                                        else "effective (FAST mode does not enumerate terms)"),
                       "l2_policy": f"inputs_exceed_l2 (p {8 * NX / 1e6:.0f} MB, q and c {16 * NX / 1e6:.0f} MB each, "
                                    f"Apart {8 * ((2 << max(n - 8, 0)) - 1) * 511 / 1e6:.0f} MB vs 126 MB L2)" if n >= 24
                                    else "arrays fit L2 at this n (not the headline config)",
@@ -323,6 +327,8 @@ def main():
     ap.add_argument("--oracle-iters", type=int, default=10)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--e2e-steps", type=int, default=0, help="steps of the end-to-end arm (default: --steps)")
+    ap.add_argument("--symmetry", action="store_true",
+                    help="complement symmetry (ba_set_symmetry): half the terms are enumerated; terms/s is then 'effective'")
     ap.add_argument("--exact-k", type=int, default=-1,
                     help="run the paper's exact channel BDC_{n,k} (ba_set_exact) instead of BDC_d^n; not a BASELINE.json config")
     args = ap.parse_args()

@@ -95,6 +95,14 @@ int ba_create_ext(int n, double d, void *p_dev, void *q_dev, void *D_dev,
  * bad k. */
 int ba_set_exact(ba_ctx *c, int k);
 
+/* Complement symmetry (the cpl half of Theorem 4): emb(cpl y, cpl x) = emb(y, x), so
+ * an iterate with p(x) = p(~x) for every x keeps that property, and q(~y) = q(y), D(~x) = D(x).  With on = 1 the ENUM
+ * sweeps enumerate only the inputs and the output prefixes whose first symbol is 0 and mirror the results (half the
+ * terms per iteration; identical q, D, p up to rounding order of the reductions).  Requires n >= 9 and the current p
+ * to be complement-symmetric bit for bit (the uniform start is); ba_set_p then rejects asymmetric vectors.
+ * BA_MODE_FAST ignores the setting.  BA_EINVAL otherwise. */
+int ba_set_symmetry(ba_ctx *c, int on);
+
 /* Select BA_MODE_ENUM (default) or BA_MODE_FAST for subsequent iterations. */
 int ba_set_mode(ba_ctx *c, int mode);
 

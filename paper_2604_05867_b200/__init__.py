@@ -21,7 +21,7 @@ BA_NMAX = 30
 _CODE_NAMES = {0: "BA_OK", -1: "BA_EINVAL", -2: "BA_ENOMEM", -3: "BA_ECUDA", -4: "BA_ESTATE", -5: "BA_ENUMERIC"}
 
 EXPORTS = ["ba_create", "ba_iterate", "ba_bounds", "ba_get_p", "ba_scratch_bytes", "ba_create_ext",
-           "ba_set_mode", "ba_set_exact", "ba_set_p", "ba_get_q", "ba_get_D", "ba_stats", "ba_get_history",
+           "ba_set_mode", "ba_set_exact", "ba_set_symmetry", "ba_set_p", "ba_get_q", "ba_get_D", "ba_stats", "ba_get_history",
            "ba_last_timing", "ba_debug_emb_row", "ba_debug_emb_col", "ba_terms_per_sweep",
            "ba_debug_count_terms", "ba_debug_check_tables", "ba_destroy", "ba_last_error"]
 
@@ -61,6 +61,7 @@ def load():
     L.ba_set_p.argtypes = [vp, dp]
     L.ba_set_mode.argtypes = [vp, ctypes.c_int]
     L.ba_set_exact.argtypes = [vp, ctypes.c_int]
+    L.ba_set_symmetry.argtypes = [vp, ctypes.c_int]
     L.ba_stats.argtypes = [vp, dp, ctypes.POINTER(ctypes.c_longlong)]
     L.ba_get_history.argtypes = [vp, ctypes.c_int, dp]
     L.ba_last_timing.argtypes = [vp, dp]
@@ -148,6 +149,11 @@ def ba_set_mode(ctx, mode):
 def ba_set_exact(ctx, k):
     """Switch to the paper's exact channel BDC_{n,k} (before the first iteration)."""
     _check(ctx, load().ba_set_exact(ctx.handle, int(k)))
+
+
+def ba_set_symmetry(ctx, on):
+    """Complement symmetry p(x) = p(~x): the ENUM sweeps enumerate half the inputs / output prefixes."""
+    _check(ctx, load().ba_set_symmetry(ctx.handle, int(on)))
 
 
 def ba_iterate(ctx, k):

@@ -18,7 +18,7 @@
 
 // ------------------------------------------------------------------------------------------------ ctx
 struct ba_ctx {
-    int n = 0, m = 0, h = 0, mode = BA_MODE_ENUM;
+    int n = 0, m = 0, h = 0, mode = BA_MODE_ENUM, sym = 0;
     double d = 0.0;
     size_t NX = 0, NY = 0, NZ = 0, napart = 0;
     KConst kc;
@@ -381,6 +381,26 @@ extern "C" void ba_destroy(ba_ctx *c) {
 
 extern "C" const char *ba_last_error(const ba_ctx *c) { return c ? c->err.c_str() : g_static_err; }
 
+static bool host_symmetric(const double *p, size_t NX) {
+    for (size_t x = 0; x < NX / 2; x++)
+        if (p[x] != p[NX - 1 - x]) return false;
+    return true;
+}
+
+extern "C" int ba_set_symmetry(ba_ctx *c, int on) {
+    if (!c) return BA_EINVAL;
+    if (on != 0 && on != 1) return fail(c, BA_EINVAL, "ba_set_symmetry: on must be 0 or 1");
+    if (on && c->h < 1) return fail(c, BA_EINVAL, "ba_set_symmetry: needs n >= 9 (a high part of at least one bit)");
+    if (on) {                                               // the current p must be complement-symmetric, bit for bit
+        std::vector<double> hp(c->NX);
+        CK(cudaMemcpyAsync(hp.data(), c->p, c->NX * 8, cudaMemcpyDeviceToHost, c->st));
+        CK(cudaStreamSynchronize(c->st));
+        if (!host_symmetric(hp.data(), c->NX)) return fail(c, BA_EINVAL, "ba_set_symmetry: p(x) != p(~x) for some x");
+    }
+    c->sym = on;
+    return BA_OK;
+}
+
 extern "C" int ba_set_exact(ba_ctx *c, int k) {
     if (!c) return BA_EINVAL;
     if (k < 0 || k > c->n) return fail(c, BA_EINVAL, "ba_set_exact: k outside [0, n]");
@@ -405,7 +425,7 @@ static InArgs make_in_args(ba_ctx *c) {
     a.FI = c->FI; a.RI = c->RI; a.EPS8 = c->EPS8; a.RI8 = c->RI8; a.ri_cnt = c->ri_cnt; a.ri_csr = c->ri_csr; a.nri = c->nri; a.owner = c->in_owner;
     a.csr_off = c->in_csr_off; a.csr_idx = c->in_csr_idx; a.ncsr = c->n_in_csr;
     a.c = c->c; a.p = c->p; a.Hc = c->Hc; a.D = c->D; a.part = c->part;
-    a.counter = c->counters; a.dbg_x = 0; a.dbg_out = nullptr; a.cnt = c->cnt;
+    a.counter = c->counters; a.sym = 0; a.dbg_x = 0; a.dbg_out = nullptr; a.cnt = c->cnt;
     return a;
 }
 
@@ -414,7 +434,7 @@ static OutArgs make_out_args(ba_ctx *c) {
     a.kc = c->kc; a.EPS8 = c->EPS8; a.RO8 = c->RO8;
     a.FO = c->FO; a.RO = c->RO; a.ro_cnt = c->ro_cnt; a.ro_csr = c->ro_csr; a.nro = c->nro; a.owner = c->out_owner;
     a.csr_off = c->out_csr_off; a.csr_idx = c->out_csr_idx; a.ncsr = c->n_out_csr;
-    a.p = c->p; a.Apart = c->Apart; a.counter = c->counters + 4; a.dbg_item = 0; a.dbg_cz = 0; a.dbg_out = nullptr;
+    a.p = c->p; a.Apart = c->Apart; a.counter = c->counters + 4; a.sym = 0; a.dbg_item = 0; a.dbg_cz = 0; a.dbg_out = nullptr;
     a.cnt = c->cnt + 2;
     return a;
 }
@@ -424,6 +444,7 @@ static int ensure_hc(ba_ctx *c) {
     if (c->hc_ready) return BA_OK;
     CK(cudaMemsetAsync(c->counters, 0, 16 * 4, c->st));
     InArgs a = make_in_args(c);
+    a.sym = c->sym;
     k_enum_in<IN_HC><<<c->grid_in, c->block, c->smem_in, c->st>>>(a);
     CK(cudaGetLastError());
     c->hc_ready = true;
@@ -434,9 +455,10 @@ static int launch_out_sweep(ba_ctx *c) {
     if (c->mode == BA_MODE_ENUM) {
         CK(cudaMemsetAsync(c->counters + 4, 0, 4, c->st));
         OutArgs a = make_out_args(c);
+        a.sym = c->sym;
         k_enum_out<OUT_SWEEP><<<c->grid_out, c->block, c->smem_out, c->st>>>(a);
         CK(cudaGetLastError());
-        k_out_final<<<c->num_sms * 8, 256, 0, c->st>>>(c->kc, c->Apart, nullptr, c->q, c->c);
+        k_out_final<<<c->num_sms * 8, 256, 0, c->st>>>(c->kc, c->Apart, nullptr, c->q, c->c, c->sym);
         CK(cudaGetLastError());
     } else {
         double *buf0 = c->Apart, *buf1 = c->Apart + (((size_t)2 << c->n) + 64);
@@ -448,7 +470,7 @@ static int launch_out_sweep(ba_ctx *c) {
             in = out;
             out = (out == buf0) ? buf1 : buf0;
         }
-        k_out_final<<<c->num_sms * 8, 256, 0, c->st>>>(c->kc, nullptr, in, c->q, c->c);
+        k_out_final<<<c->num_sms * 8, 256, 0, c->st>>>(c->kc, nullptr, in, c->q, c->c, 0);
         CK(cudaGetLastError());
     }
     return BA_OK;
@@ -458,9 +480,10 @@ static int launch_in_sweep(ba_ctx *c, size_t *npart) {
     if (c->mode == BA_MODE_ENUM) {
         CK(cudaMemsetAsync(c->counters, 0, 4, c->st));
         InArgs a = make_in_args(c);
+        a.sym = c->sym;
         k_enum_in<IN_SWEEP><<<c->grid_in, c->block, c->smem_in, c->st>>>(a);
         CK(cudaGetLastError());
-        *npart = (size_t)1 << c->h;
+        *npart = (size_t)1 << (c->h - c->sym);
     } else {
         double *buf0 = c->Apart, *buf1 = c->Apart + (((size_t)2 << c->n) + 64);
         const double *in = c->c + 1;                          // c is stored by code: idx(y) = code(y) - 1
@@ -603,6 +626,8 @@ extern "C" int ba_set_p(ba_ctx *c, const double *p_host) {
         sum += v;
     }
     if (fabsl(sum - 1.0L) > 1e-9L) return fail(c, BA_EINVAL, "ba_set_p: |sum p - 1| > 1e-9");
+    if (c->sym && !host_symmetric(p_host, c->NX))
+        return fail(c, BA_EINVAL, "ba_set_p: complement symmetry is on (ba_set_symmetry) and p(x) != p(~x) for some x");
     CK(cudaMemcpyAsync(c->p, p_host, c->NX * 8, cudaMemcpyHostToDevice, c->st));
     CK(cudaStreamSynchronize(c->st));
     return BA_OK;

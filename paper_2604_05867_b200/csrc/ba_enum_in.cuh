@@ -55,6 +55,7 @@ struct InArgs {
     double *D;                // IN_SWEEP: out
     double *part;             // IN_SWEEP: 3 doubles per u: sum p D, max D, sum p 2^D
     unsigned int *counter;    // work counter (zeroed before launch)
+    int sym;                  // 1: p(x) = p(~x) (Theorem 4): only the u with leading bit 0 are enumerated, D is mirrored
     uint32_t dbg_x;           // IN_DEBUG
     uint32_t *dbg_out;        // IN_DEBUG: NY zero-filled
     unsigned long long *cnt;  // IN_COUNT: [0] terms, [1] emb sum
@@ -149,7 +150,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
         if (tid == 0) s_item[0] = (MODE == IN_DEBUG) ? (a.dbg_x >> m) : atomicAdd(a.counter, 1u);
         __syncthreads();
         const uint32_t u = s_item[0];
-        if (h < 32 && (u >> h) != 0) break;
+        if (h < 32 && (u >> (h - a.sym)) != 0) break;
         if (MODE == IN_DEBUG && blockIdx.x != 0) break;
 
         // ---- Sub[pos] = number of trie nodes below a node whose leftmost embedding ends at pos -------
@@ -445,13 +446,16 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 for (int t = ev; t < BA_NT; t += nv) S += s_acc[(size_t)2 * BA_NC * BA_NT + t];
                 for (int q = s_csr_off[tid]; q < s_csr_off[tid + 1]; q++) S += s_acc[__ldg(a.csr_idx + q)];
                 const size_t x = ((size_t)u << m) | (size_t)tid;
+                const size_t xc = (((size_t)1 << a.kc.n) - 1) - x;     // complement: same row of emb up to cpl
                 if (MODE == IN_HC) {
                     a.Hc[x] = S;
+                    if (a.sym) a.Hc[xc] = S;
                 } else {
                     const double Dx = a.Hc[x] - S;
                     a.D[x] = Dx;
                     const double px = a.p[x];
                     r0 = px * Dx; r1 = Dx; r2 = px * exp2(Dx);
+                    if (a.sym) { a.D[xc] = Dx; r0 += r0; r2 += r2; }  // p(xc) = p(x) bit for bit (checked on the host)
                 }
             }
             if (MODE == IN_SWEEP) {

@@ -50,6 +50,7 @@ struct OutArgs {
     const double *p;           // NX
     double *Apart;             // (2^{h+1}-1) * (2^{m+1}-1)
     unsigned int *counter;
+    int sym;                   // 1: q(y) = q(~y): prefixes y' with leading symbol 1 are skipped (k_out_final mirrors them)
     uint32_t dbg_item;         // OUT_DEBUG: code of y'
     uint32_t dbg_cz;           // OUT_DEBUG: code of z
     uint32_t *dbg_out;         // OUT_DEBUG: NX zero-filled
@@ -127,6 +128,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
         if (MODE == OUT_DEBUG && blockIdx.x != 0) break;
         const int t = ba_len_of_code(cy);
         const uint32_t yv = cy - (1u << t);
+        if (a.sym && t >= 1 && ((cy >> (t - 1)) & 1u)) { __syncthreads(); continue; }   // served by its complement
         const int cls = (int)(cy & (BA_NCLS - 1));
         const int Lc = t < 8 ? t : 8;
         uint32_t R = 0;                                        // number of supersequences (Lemma 6)

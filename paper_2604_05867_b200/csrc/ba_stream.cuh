@@ -12,7 +12,7 @@
 // c is stored by CODE (c[code(y)] = c[idx(y)+1], entry 0 unused) so that the 2^j outputs y'.z, |z| = j,
 // of a prefix y' start at the even index code(y') << j: 16-byte aligned pieces for cp.async.
 __global__ void k_out_final(KConst kc, const double *__restrict__ Apart, const double *__restrict__ Afull,
-                            double *__restrict__ q, double *__restrict__ c) {
+                            double *__restrict__ q, double *__restrict__ c, int sym) {
     const size_t NY = ((size_t)2 << kc.n) - 1;
     const uint32_t NZ = (2u << kc.m) - 1u;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < NY; i += (size_t)gridDim.x * blockDim.x) {
@@ -23,11 +23,13 @@ __global__ void k_out_final(KConst kc, const double *__restrict__ Apart, const d
             A = Afull[i];
         } else {
             A = 0.0;
+            // complement symmetry (sym): A(y) = A(~y); the prefixes with leading symbol 1 were not enumerated
+            const uint32_t ce = (sym && k >= 1 && ((cy >> (k - 1)) & 1u)) ? ((1u << k) | (~cy & ((1u << k) - 1u))) : cy;
             const int jlo = (k - kc.h > 0) ? (k - kc.h) : 0;
             const int jhi = (k < kc.m) ? k : kc.m;
             for (int j = jlo; j <= jhi; j++) {       // split y = y'.z, |z| = j
-                const uint32_t cyp = cy >> j;
-                const uint32_t cz = (1u << j) | (cy & ((1u << j) - 1u));
+                const uint32_t cyp = ce >> j;
+                const uint32_t cz = (1u << j) | (ce & ((1u << j) - 1u));
                 A += Apart[(size_t)(cyp - 1u) * NZ + (cz - 1u)];
             }
         }

@@ -267,3 +267,48 @@ def test_exact_channel_paper_values_and_lemma2(ba):
     left = run(n, None, 300)[0]
     right = sum(comb(n, k) * d ** (n - k) * (1 - d) ** k * run(n, k, 300)[1] for k in range(1, n + 1))
     assert left <= right and right == pytest.approx(2.3045, abs=5e-3) and left == pytest.approx(2.1230, abs=1e-4)
+
+
+# ------------------------------------------------------------------ NEXT-2 (cpl half): complement symmetry
+
+@pytest.mark.parametrize("n,d,K", [(9, 0.5, 30), (11, 0.64, 25), (12, 0.8, 20)])
+def test_complement_symmetry_matches_oracle(ba, n, d, K):
+    ref = orc.ba_run(W_of(n, d), si.uniform_p0(n), K)
+    ctx = ba.ba_create(n, d)
+    try:
+        ba.ba_set_symmetry(ctx, 1)
+        ba.ba_iterate(ctx, K)
+        I, U = ba.ba_bounds(ctx)
+        q, D, p = ba.ba_get_q(ctx), ba.ba_get_D(ctx), ba.ba_get_p(ctx)
+        hist = ba.ba_get_history(ctx, K)
+        with pytest.raises(ba.BAError) as ei:               # an asymmetric p is refused while symmetry is on
+            ba.ba_set_p(ctx, si.random_positive_p(n, 1))
+        assert ei.value.code == ba.BA_EINVAL
+    finally:
+        ba.ba_destroy(ctx)
+    assert np.max(np.abs(hist - ref["hist"])) <= ABS_U and abs(I - ref["hist"][-1, 0]) <= ABS_U and abs(U - ref["hist"][-1, 1]) <= ABS_U
+    assert relerr(q, ref["q"]) <= 1e-11 and relerr(D, ref["D"]) <= 1e-11 and relerr(p, ref["p"]) <= 1e-9
+    NX = 1 << n
+    assert np.array_equal(p, p[::-1]) and np.array_equal(D, D[::-1])          # x -> ~x is index reversal of [0, 2^n)
+    for k in range(1, n + 1):                                                  # q(~y) = q(y) within every length
+        blk = q[(1 << k) - 1:(2 << k) - 1]
+        assert np.array_equal(blk, blk[::-1])
+
+
+def test_complement_symmetry_argument_errors(ba):
+    ctx = ba.ba_create(8, 0.5)
+    try:
+        with pytest.raises(ba.BAError) as ei:
+            ba.ba_set_symmetry(ctx, 1)                       # n = 8 has no high part
+        assert ei.value.code == ba.BA_EINVAL
+    finally:
+        ba.ba_destroy(ctx)
+    ctx = ba.ba_create(10, 0.5)
+    try:
+        ba.ba_set_p(ctx, si.random_positive_p(10, 2))
+        with pytest.raises(ba.BAError) as ei:
+            ba.ba_set_symmetry(ctx, 1)                       # current p is not symmetric
+        assert ei.value.code == ba.BA_EINVAL
+        ba.ba_set_symmetry(ctx, 0)
+    finally:
+        ba.ba_destroy(ctx)
