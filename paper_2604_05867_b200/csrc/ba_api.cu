@@ -22,7 +22,7 @@ struct ba_ctx {
     double d = 0.0;
     size_t NX = 0, NY = 0, NZ = 0, napart = 0;
     KConst kc;
-    int nWv = 0, nri = 0, nro = 0, n_in_csr = 0, n_out_csr = 0;
+    int nri = 0, nro = 0, n_in_csr = 0, n_out_csr = 0;
     cudaStream_t st = nullptr;
     bool own_buffers = false, own_stream = false;
     double *p = nullptr, *q = nullptr, *D = nullptr;
@@ -33,7 +33,6 @@ struct ba_ctx {
     uint4 *RI = nullptr, *RO = nullptr;
     uint2 *EPS8 = nullptr;
     uint32_t *RI8 = nullptr, *RO8 = nullptr;
-    uint32_t *Wv = nullptr, *vbase = nullptr;
     uint16_t *in_owner = nullptr, *out_owner = nullptr, *ri_cnt = nullptr, *ro_cnt = nullptr, *ri_csr = nullptr, *ro_csr = nullptr;
     uint16_t *in_csr_off = nullptr, *in_csr_idx = nullptr, *out_csr_off = nullptr, *out_csr_idx = nullptr;
     unsigned int *counters = nullptr;
@@ -73,7 +72,7 @@ static double host_binom(int n, int k) {
 
 // ------------------------------------------------------------------------------------------------ scratch layout
 struct ScratchLayout {
-    size_t c, Hc, Apart, part, scal, hist, FI, FO, RI, RO, EPS8, RI8, RO8, Wv, vbase, in_owner, out_owner, ri_cnt, ro_cnt, ri_csr, ro_csr,
+    size_t c, Hc, Apart, part, scal, hist, FI, FO, RI, RO, EPS8, RI8, RO8, in_owner, out_owner, ri_cnt, ro_cnt, ri_csr, ro_csr,
         in_csr_off, in_csr_idx, out_csr_off, out_csr_idx, counters, cnt, total;
     size_t napart, npart_cap;
 };
@@ -114,8 +113,6 @@ static void scratch_layout(int n, const TileTables &T, ScratchLayout &L) {
     L.EPS8 = o; o += align256(T.EPS8.size() * 8);
     L.RI8 = o; o += align256(T.RI8.size() * 4);
     L.RO8 = o; o += align256(T.RO8.size() * 4);
-    L.Wv = o; o += align256(T.Wv.size() * 4);
-    L.vbase = o; o += align256(T.vbase.size() * 4);
     L.in_owner = o; o += align256(T.in_owner.size() * 2);
     L.out_owner = o; o += align256(T.out_owner.size() * 2);
     L.ri_cnt = o; o += align256(T.ri_cnt.size() * 2);
@@ -277,7 +274,6 @@ static int finish_create(ba_ctx *c) {
     c->part = (double *)(s + L.part); c->scal = (double *)(s + L.scal); c->hist = (double *)(s + L.hist);
     c->FI = (uint2 *)(s + L.FI); c->FO = (uint2 *)(s + L.FO); c->RI = (uint4 *)(s + L.RI); c->RO = (uint4 *)(s + L.RO);
     c->EPS8 = (uint2 *)(s + L.EPS8); c->RI8 = (uint32_t *)(s + L.RI8); c->RO8 = (uint32_t *)(s + L.RO8);
-    c->Wv = (uint32_t *)(s + L.Wv); c->vbase = (uint32_t *)(s + L.vbase);
     c->in_owner = (uint16_t *)(s + L.in_owner); c->out_owner = (uint16_t *)(s + L.out_owner);
     c->ri_cnt = (uint16_t *)(s + L.ri_cnt); c->ro_cnt = (uint16_t *)(s + L.ro_cnt);
     c->ri_csr = (uint16_t *)(s + L.ri_csr); c->ro_csr = (uint16_t *)(s + L.ro_csr);
@@ -285,12 +281,11 @@ static int finish_create(ba_ctx *c) {
     c->out_csr_off = (uint16_t *)(s + L.out_csr_off); c->out_csr_idx = (uint16_t *)(s + L.out_csr_idx);
     c->counters = (unsigned int *)(s + L.counters); c->cnt = (unsigned long long *)(s + L.cnt);
     c->napart = L.napart; c->npart_cap = L.npart_cap;
-    c->nWv = (int)T.Wv.size(); c->nri = T.nri; c->nro = T.nro;
+    c->nri = T.nri; c->nro = T.nro;
     c->n_in_csr = (int)T.in_csr_idx.size(); c->n_out_csr = T.out_ncsr;
 
     CK(upload(c->FI, T.FI, c->st)); CK(upload(c->FO, T.FO, c->st)); CK(upload(c->RI, T.RI, c->st)); CK(upload(c->RO, T.RO, c->st));
     CK(upload(c->EPS8, T.EPS8, c->st)); CK(upload(c->RI8, T.RI8, c->st)); CK(upload(c->RO8, T.RO8, c->st));
-    CK(upload(c->Wv, T.Wv, c->st)); CK(upload(c->vbase, T.vbase, c->st));
     CK(upload(c->in_owner, T.in_owner, c->st)); CK(upload(c->out_owner, T.out_owner, c->st));
     CK(upload(c->ri_cnt, T.ri_cnt, c->st)); CK(upload(c->ro_cnt, T.ro_cnt, c->st));
     CK(upload(c->ri_csr, T.ri_csr, c->st)); CK(upload(c->ro_csr, T.ro_csr, c->st));
