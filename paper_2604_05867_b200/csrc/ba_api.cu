@@ -245,7 +245,7 @@ static int setup_ctx(ba_ctx *c, int n, double d) {
     c->n = n; c->m = low_m(n); c->h = n - c->m; c->d = d;
     c->NX = (size_t)1 << n; c->NY = ((size_t)2 << n) - 1; c->NZ = ((size_t)2 << c->m) - 1;
     KConst &kc = c->kc;
-    kc.n = n; kc.m = c->m; kc.h = c->h;
+    kc.n = n; kc.m = c->m; kc.h = c->h; kc.klen = -1;
     for (int k = 0; k <= BA_NMAX_I; k++) { kc.w[k] = 0.0; kc.lebar[k] = 0.0; }
     for (int k = 0; k <= n; k++) {
         long double a = 1.0L, b = 1.0L;                      // 0^0 = 1 (R7)
@@ -402,6 +402,7 @@ extern "C" int ba_set_exact(ba_ctx *c, int k) {
     if (c->iters != 0) return fail(c, BA_ESTATE, "ba_set_exact: only before the first iteration");
     for (int j = 0; j <= c->n; j++) c->kc.w[j] = 0.0;
     c->kc.w[k] = 1.0 / host_binom(c->n, k);                 // P_{n,k}(y|x) = emb(y,x) / C(n,k)
+    c->kc.klen = k;                                         // the sweeps skip the nodes / prefixes that cannot reach length k
     c->hc_ready = false;                                    // Hc depends on the weights
     return BA_OK;
 }

@@ -212,7 +212,9 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                         pos = p + 1; k++;
                         cy = (cy << 1) | b;
                     }
-                    const uint32_t miss0 = ba_nextpos(u, h, pos, 0u) >= h, miss1 = ba_nextpos(u, h, pos, 1u) >= h;
+                    uint32_t miss0 = ba_nextpos(u, h, pos, 0u) >= h, miss1 = ba_nextpos(u, h, pos, 1u) >= h;
+                    // exact channel BDC_{n,klen}: y = y'.z has weight only if |y'| + |z| = klen, 1 <= |z| <= m
+                    if ((MODE == IN_SWEEP || MODE == IN_HC) && a.kc.klen >= 0 && !(k < a.kc.klen && a.kc.klen <= k + m)) miss0 = miss1 = 0u;
                     NodeRec rc;
 #pragma unroll
                     for (int s = 0; s < 9; s++) rc.a[s] = al[s];
@@ -229,8 +231,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 ba_bucket_sort<BA_NCLS>(key1, s_ordr + (size_t)(rd * 2 + 1) * BA_NT, s_wcnt, s_seg + (rd * 2 + 1) * (BA_NCLS + 1));
 
                 // ================= eps: the pair (v, empty) of every node of the round =================
-#pragma unroll 8
-                for (int i = esub; i < nn; i += epn) {
+                auto eps_one = [&](int i) {
                     const NodeRec &rc = s_rec[rd * BA_NT + i];
                     const uint4 r0 = *(const uint4 *)&rc.a[0], r1 = *(const uint4 *)&rc.a[4], r2 = *(const uint4 *)&rc.a[8];
                     const uint32_t cy = r2.y;
@@ -251,6 +252,13 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                     } else {
                         cnt_terms += 1ull; cnt_emb += emb;
                     }
+                };
+                if ((MODE == IN_SWEEP || MODE == IN_HC) && a.kc.klen >= 0) {      // exact channel: only |y'| = klen has weight
+                    for (int i = esub; i < nn; i += epn)
+                        if ((int)(s_rec[rd * BA_NT + i].info >> 16) == a.kc.klen) eps_one(i);
+                } else {
+#pragma unroll 8
+                    for (int i = esub; i < nn; i += epn) eps_one(i);
                 }
                 __syncthreads();                               // s_ceps is rewritten by the next round
             }

@@ -129,6 +129,9 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
         const int t = ba_len_of_code(cy);
         const uint32_t yv = cy - (1u << t);
         if (a.sym && t >= 1 && ((cy >> (t - 1)) & 1u)) { __syncthreads(); continue; }   // served by its complement
+        // exact channel BDC_{n,klen}: this prefix reaches the outputs of length t .. t+m only
+        const int klen = (MODE == OUT_SWEEP) ? a.kc.klen : -1;
+        if (klen >= 0 && (klen < t || klen > t + m)) { __syncthreads(); continue; }
         const int cls = (int)(cy & (BA_NCLS - 1));
         const int Lc = t < 8 ? t : 8;
         uint32_t R = 0;                                        // number of supersequences (Lemma 6)
@@ -270,7 +273,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                 const uint16_t *bnode = s_bnode + buf * BA_RB_OUT;
 
                 // ---- the pair (v, empty) of every node: thread (v, node) ----------------------------------
-                for (int i = esub; i < len; i += epn) {
+                for (int i = esub; i < len && (klen < 0 || klen == t); i += epn) {
                     const NodeRec &rc = s_rec[bnode[i]];
                     const uint4 r0 = *(const uint4 *)&rc.a[0], r1 = *(const uint4 *)&rc.a[4], r2 = *(const uint4 *)&rc.a[8];
                     const uint32_t emb = r0.x * Ee[0] + r0.y * Ee[1] + r0.z * Ee[2] + r0.w * Ee[3] + r1.x * Ee[4] +
@@ -285,7 +288,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                 }
 #pragma unroll
                 for (int b = 0; b < 2; b++) {
-                    if (!((mask >> b) & 1)) continue;
+                    if (!((mask >> b) & 1) || klen == t) continue;
                     // ---- fast pairs -----------------------------------------------------------------------
 #pragma unroll
                     for (int c = 0; c < BA_NC; c++) {

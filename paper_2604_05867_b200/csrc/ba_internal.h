@@ -56,6 +56,7 @@
 
 struct KConst {                       // passed by value to kernels
     int n, m, h;
+    int klen;                         // >= 0: only outputs of this length carry weight (exact channel BDC_{n,k}); -1: all
     double w[BA_NMAX_I + 1];          // w_k = (1-d)^k d^{n-k}                  (NS; R7: 0^0 = 1)
     double lebar[BA_NMAX_I + 1];      // log2( C(n,k) / 2^k ): centring constant of the hoisted log
 };

@@ -18,6 +18,7 @@ __global__ void k_out_final(KConst kc, const double *__restrict__ Apart, const d
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < NY; i += (size_t)gridDim.x * blockDim.x) {
         const uint32_t cy = (uint32_t)(i + 1);
         const int k = ba_len_of_code(cy);
+        if (kc.w[k] == 0.0) { q[i] = 0.0; c[i + 1] = 0.0; continue; }   // R7: a length without mass (its partials may be unwritten)
         double A;
         if (Afull) {
             A = Afull[i];
