@@ -100,10 +100,13 @@ int ba_set_exact(ba_ctx *c, int k);
  * sweeps enumerate only the inputs and the output prefixes whose first symbol is 0 and mirror the results (half the
  * terms per iteration; identical q, D, p up to rounding order of the reductions).  Requires n >= 9 and the current p
  * to be complement-symmetric bit for bit (the uniform start is); ba_set_p then rejects asymmetric vectors.
- * BA_MODE_FAST ignores the setting.  BA_EINVAL otherwise. */
+ * Only in BA_MODE_ENUM: FAST iterations sum D(x) and D(~x) in different orders, so they would break the bit-for-bit
+ * symmetry the ENUM sweeps rely on; ba_set_mode(FAST) is refused (BA_EINVAL) while symmetry is on, and
+ * ba_set_symmetry(1) is refused in FAST mode.  BA_EINVAL otherwise. */
 int ba_set_symmetry(ba_ctx *c, int on);
 
-/* Select BA_MODE_ENUM (default) or BA_MODE_FAST for subsequent iterations. */
+/* Select BA_MODE_ENUM (default) or BA_MODE_FAST for subsequent iterations.  BA_EINVAL for an unknown mode, or for
+ * FAST while complement symmetry is on. */
 int ba_set_mode(ba_ctx *c, int mode);
 
 /* Replace p by a host vector (2^n doubles).  Rejects non-finite or non-positive entries and

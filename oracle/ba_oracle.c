@@ -28,7 +28,8 @@
  *   G8  update is p' = max(p 2^D / Z, 2^-1000) (never active in the parity configs).
  *
  * Parity pins: tests/test_oracle_pins.py (closed forms, invariants, brute force) --
- * every function below is pinned there; nothing here is "parity unpinned".
+ * every function below is pinned there, the G8 floor line of orc_ba_step included
+ * (test_floor_G8_*); nothing here is "parity unpinned".
  */
 #include <math.h>
 #include <stdint.h>
@@ -49,6 +50,8 @@ int orc_num_threads(void) {
     return 1;
 #endif
 }
+
+int orc_weights(int n, double d, double *w);
 
 /* O2: dense output index of the string with `len` bits and MSB-first value `val` (R2, a5). */
 static inline uint64_t orc_idx(int len, uint64_t val) { return (((uint64_t)1 << len) - 1) + val; }
@@ -85,6 +88,55 @@ int orc_emb_dense(int n, uint32_t *E) {
             row[orc_idx(len, val)] += 1;
         }
     }
+    return ORC_OK;
+}
+
+/*
+ * O3 for ONE input x, at sizes the dense matrix cannot reach (n <= 30): row[idx(y)] = emb(y,x), by the
+ * same keep-mask enumeration as orc_emb_dense ("#times y appears as a subsequence of x").
+ * row must hold 2^{n+1}-1 uint32, caller-allocated; it is zero-filled here.  Cost n 2^n.
+ */
+int orc_emb_row(int n, uint32_t x, uint32_t *row) {
+    if (n < 1 || n > 30 || !row || ((uint64_t)x >> n) != 0) return ORC_EINVAL;
+    const uint64_t NX = (uint64_t)1 << n, NY = ((uint64_t)1 << (n + 1)) - 1;
+    memset(row, 0, NY * sizeof(uint32_t));
+    for (uint64_t m = 0; m < NX; m++) {
+        uint64_t val = 0;
+        int len = 0;
+        for (int i = 0; i < n; i++) {                /* paper position i, left to right */
+            int sh = n - 1 - i;
+            if ((m >> sh) & 1) {
+                val = (val << 1) | (((uint64_t)x >> sh) & 1);
+                len++;
+            }
+        }
+        row[orc_idx(len, val)] += 1;
+    }
+    return ORC_OK;
+}
+
+/*
+ * Divergence of ONE input from its emb row and an output distribution q (P:189-193 minus log2 p(x); R5):
+ *   D(x) = sum_{j: row[j]>0} W_j (log2 W_j - log2 q(j)),  W_j = row[j] w_{len(j)},  w_k = (1-d)^k d^{n-k}.
+ * The plain definition, one term per non-zero entry, long double accumulator, ascending j (R9).
+ * Entries whose weight w_k is 0 are skipped (R7).  *nterms = number of non-zero emb entries.
+ */
+int orc_D_row(int n, double d, const uint32_t *row, const double *q, double *D_out, int64_t *nterms) {
+    if (n < 1 || n > 30 || !row || !q || !D_out) return ORC_EINVAL;
+    double w[64];
+    int rc = orc_weights(n, d, w);
+    if (rc) return rc;
+    const uint64_t NY = ((uint64_t)1 << (n + 1)) - 1;
+    long double acc = 0.0L;
+    int64_t cnt = 0;
+    for (uint64_t j = 0; j < NY; j++) {
+        if (!row[j]) continue;
+        cnt++;
+        double wv = (double)row[j] * w[orc_len_of_idx(j)];
+        if (wv != 0.0) acc += (long double)wv * (log2l((long double)wv) - log2l((long double)q[j]));
+    }
+    *D_out = (double)acc;
+    if (nterms) *nterms = cnt;
     return ORC_OK;
 }
 

@@ -35,6 +35,8 @@ def lib():
         c_up = ctypes.POINTER(ctypes.c_uint32)
         L.orc_num_threads.restype = ctypes.c_int
         L.orc_emb_dense.argtypes = [ctypes.c_int, c_up]
+        L.orc_emb_row.argtypes = [ctypes.c_int, ctypes.c_uint32, c_up]
+        L.orc_D_row.argtypes = [ctypes.c_int, ctypes.c_double, c_up, c_dp, c_dp, ctypes.POINTER(ctypes.c_int64)]
         L.orc_weights.argtypes = [ctypes.c_int, ctypes.c_double, c_dp]
         L.orc_channel_from_emb.argtypes = [ctypes.c_int, ctypes.c_double, c_up, c_dp]
         L.orc_ba_step.argtypes = [ctypes.c_int64, ctypes.c_int64, c_dp, c_dp, c_dp, c_dp, c_dp, c_dp]
@@ -68,6 +70,31 @@ def emb_dense(n):
     if rc:
         raise ValueError(f"orc_emb_dense rc={rc}")
     return E
+
+
+def emb_row(n, x):
+    """Row x of the emb matrix by keep-mask enumeration of that one input; n <= 30."""
+    NX, NY = sizes(n)
+    row = np.empty(NY, dtype=np.uint32)
+    rc = lib().orc_emb_row(n, int(x), _up(row))
+    if rc:
+        raise ValueError(f"orc_emb_row rc={rc}")
+    return row
+
+
+def D_row(n, d, row, q):
+    """(D(x), number of non-zero terms) of one input from its emb row and q, by the definition."""
+    row = np.ascontiguousarray(row, dtype=np.uint32)
+    q = np.ascontiguousarray(q, dtype=np.float64)
+    NX, NY = sizes(n)
+    if row.shape != (NY,) or q.shape != (NY,):
+        raise ValueError("D_row: row and q must have 2^(n+1)-1 entries")
+    out = ctypes.c_double()
+    nt = ctypes.c_int64()
+    rc = lib().orc_D_row(n, float(d), _up(row), _dp(q), ctypes.byref(out), ctypes.byref(nt))
+    if rc:
+        raise ValueError(f"orc_D_row rc={rc}")
+    return float(out.value), int(nt.value)
 
 
 def weights(n, d):

@@ -304,13 +304,21 @@ static int finish_create(ba_ctx *c) {
     c->block = BA_NT;
     c->smem_in = enum_in_smem(c->m, c->n_in_csr, c->nri).total;
     c->smem_out = enum_out_smem(c->m, c->n_out_csr, c->nro).total;
-    CK(cudaFuncSetAttribute(k_enum_in<IN_SWEEP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_in));
-    CK(cudaFuncSetAttribute(k_enum_in<IN_HC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_in));
-    CK(cudaFuncSetAttribute(k_enum_in<IN_DEBUG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_in));
-    CK(cudaFuncSetAttribute(k_enum_in<IN_COUNT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_in));
-    CK(cudaFuncSetAttribute(k_enum_out<OUT_SWEEP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_out));
-    CK(cudaFuncSetAttribute(k_enum_out<OUT_DEBUG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_out));
-    CK(cudaFuncSetAttribute(k_enum_out<OUT_COUNT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem_out));
+    {   // MaxDynamicSharedMemorySize is per-function state shared by every ctx of the process: only ever raise it,
+        // so that a ctx with a narrower low tile (n < 8) cannot shrink what a live n >= 8 ctx launches with
+        static std::mutex mu;
+        static size_t max_in = 0, max_out = 0;
+        std::lock_guard<std::mutex> lk(mu);
+        if (c->smem_in > max_in) max_in = c->smem_in;
+        if (c->smem_out > max_out) max_out = c->smem_out;
+        CK(cudaFuncSetAttribute(k_enum_in<IN_SWEEP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_in));
+        CK(cudaFuncSetAttribute(k_enum_in<IN_HC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_in));
+        CK(cudaFuncSetAttribute(k_enum_in<IN_DEBUG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_in));
+        CK(cudaFuncSetAttribute(k_enum_in<IN_COUNT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_in));
+        CK(cudaFuncSetAttribute(k_enum_out<OUT_SWEEP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_out));
+        CK(cudaFuncSetAttribute(k_enum_out<OUT_DEBUG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_out));
+        CK(cudaFuncSetAttribute(k_enum_out<OUT_COUNT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_out));
+    }
     int occ_in = 1, occ_out = 1;
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_in, k_enum_in<IN_SWEEP>, c->block, c->smem_in));
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_out, k_enum_out<OUT_SWEEP>, c->block, c->smem_out));
@@ -386,6 +394,7 @@ extern "C" int ba_set_symmetry(ba_ctx *c, int on) {
     if (!c) return BA_EINVAL;
     if (on != 0 && on != 1) return fail(c, BA_EINVAL, "ba_set_symmetry: on must be 0 or 1");
     if (on && c->h < 1) return fail(c, BA_EINVAL, "ba_set_symmetry: needs n >= 9 (a high part of at least one bit)");
+    if (on && c->mode != BA_MODE_ENUM) return fail(c, BA_EINVAL, "ba_set_symmetry: only in BA_MODE_ENUM (FAST iterations do not keep p(x) == p(~x) bit for bit)");
     if (on) {                                               // the current p must be complement-symmetric, bit for bit
         std::vector<double> hp(c->NX);
         CK(cudaMemcpyAsync(hp.data(), c->p, c->NX * 8, cudaMemcpyDeviceToHost, c->st));
@@ -410,6 +419,7 @@ extern "C" int ba_set_exact(ba_ctx *c, int k) {
 extern "C" int ba_set_mode(ba_ctx *c, int mode) {
     if (!c) return BA_EINVAL;
     if (mode != BA_MODE_ENUM && mode != BA_MODE_FAST) return fail(c, BA_EINVAL, "ba_set_mode: unknown mode");
+    if (mode == BA_MODE_FAST && c->sym) return fail(c, BA_EINVAL, "ba_set_mode: BA_MODE_FAST is refused while complement symmetry is on (ba_set_symmetry(c, 0) first)");
     c->mode = mode;
     return BA_OK;
 }

@@ -211,8 +211,12 @@ def exact_W(n, k):
     return W
 
 
+# (11,1) (11,2) (12,3): k small with a high part, so whole prefixes / nodes are skipped because they cannot reach
+# length k from below (klen < t); (11,10) (12,11) (14,13): k > t + 8, skipped from above.  Both prunings of the
+# ENUM exact mode are therefore compared with the oracle here (mode 0), not only the FAST transform.
 @pytest.mark.parametrize("mode", [0, 1])
-@pytest.mark.parametrize("n,k", [(2, 1), (5, 3), (8, 1), (8, 4), (8, 8), (11, 6)])
+@pytest.mark.parametrize("n,k", [(2, 1), (5, 3), (8, 1), (8, 4), (8, 8), (11, 6), (11, 1), (11, 2), (12, 3), (11, 10),
+                                 (12, 11), (14, 13)])
 def test_exact_channel_one_step_and_trajectory(ba, n, k, mode):
     W = exact_W(n, k)
     p = si.random_positive_p(n, 100 + n + k)
@@ -240,6 +244,26 @@ def test_exact_channel_one_step_and_trajectory(ba, n, k, mode):
         assert ei.value.code == ba.BA_ESTATE
     finally:
         ba.ba_destroy(ctx)
+
+
+@pytest.mark.parametrize("n,k", [(11, 2), (12, 6), (12, 11)])
+def test_exact_channel_with_complement_symmetry(ba, n, k):
+    # the pruned ENUM exact mode under ba_set_symmetry(1): uniform start, K iterations, against the oracle
+    K = 12
+    ref = orc.ba_run(exact_W(n, k), si.uniform_p0(n), K)
+    ctx = ba.ba_create(n, 0.5)
+    try:
+        ba.ba_set_exact(ctx, k)
+        ba.ba_set_symmetry(ctx, 1)
+        ba.ba_iterate(ctx, K)
+        q, D, p = ba.ba_get_q(ctx), ba.ba_get_D(ctx), ba.ba_get_p(ctx)
+        hist = ba.ba_get_history(ctx, K)
+    finally:
+        ba.ba_destroy(ctx)
+    nz = ref["q"] > 0
+    assert np.array_equal(q > 0, nz) and relerr(q[nz], ref["q"][nz]) <= 1e-11
+    assert np.all(np.abs(D - ref["D"]) <= 1e-11 * np.abs(ref["D"]) + 1e-15) and relerr(p, ref["p"]) <= 1e-9
+    assert np.max(np.abs(hist - ref["hist"])) <= ABS_U
 
 
 def test_exact_channel_paper_values_and_lemma2(ba):
@@ -310,5 +334,75 @@ def test_complement_symmetry_argument_errors(ba):
             ba.ba_set_symmetry(ctx, 1)                       # current p is not symmetric
         assert ei.value.code == ba.BA_EINVAL
         ba.ba_set_symmetry(ctx, 0)
+    finally:
+        ba.ba_destroy(ctx)
+
+
+# ------------------------------------------------------------------ G8: the floor of the update, on the device
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_floor_G8_on_device(ba, mode):
+    # twin of tests/test_oracle_pins.py::test_floor_G8_fires_exactly_and_leaves_the_rest: n = 3, d = 0.9, one input at
+    # 1e-305, so p 2^D / Z < 2^-1000 for that input only (reading G8)
+    n, d = 3, 0.9
+    p = si.uniform_p0(n).copy()
+    p[5] = 1e-305
+    p[2] += 1.0 / 8 - 1e-305
+    ref = orc.ba_step(W_of(n, d), p)
+    assert ref["p_next"][5] == 2.0 ** -1000                    # the oracle's floor fired (pinned on CPU)
+    ctx = ba.ba_create(n, d)
+    try:
+        ba.ba_set_mode(ctx, mode)
+        ba.ba_set_p(ctx, p)
+        ba.ba_iterate(ctx, 1)
+        pn, D = ba.ba_get_p(ctx), ba.ba_get_D(ctx)
+        ba.ba_iterate(ctx, 1)                                  # and the iterate stays usable (no log2 0, no NaN)
+        I, U = ba.ba_bounds(ctx)
+    finally:
+        ba.ba_destroy(ctx)
+    assert pn[5] == 2.0 ** -1000                               # bit-exact
+    keep = np.arange(1 << n) != 5
+    assert relerr(pn[keep], ref["p_next"][keep]) <= 1e-12 and relerr(D, ref["D"]) <= REL_QD
+    assert np.isfinite(I) and np.isfinite(U) and I <= U
+
+
+# ------------------------------------------------------------------ contexts are independent (include/ba.h)
+
+def test_two_contexts_of_different_tile_width_alive_together(ba):
+    # an n >= 8 ctx (m = 8, the largest dynamic shared-memory request) and an n < 8 ctx (m = 4) interleaved:
+    # creating the second must not shrink what the first may launch with
+    big = ba.ba_create(12, 0.7)
+    try:
+        ba.ba_iterate(big, 1)
+        small = ba.ba_create(4, 0.3)
+        try:
+            ba.ba_iterate(small, 2)
+            ba.ba_iterate(big, 2)
+            ba.ba_iterate(small, 1)
+            Ib, Ub = ba.ba_bounds(big)
+            Is, Us = ba.ba_bounds(small)
+        finally:
+            ba.ba_destroy(small)
+        ba.ba_iterate(big, 1)
+        assert np.array_equal(ba.ba_debug_emb_row(big, 0b010011010111), E_of(12)[0b010011010111])
+    finally:
+        ba.ba_destroy(big)
+    rb = orc.ba_run(W_of(12, 0.7), si.uniform_p0(12), 3)["hist"][-1]
+    rs = orc.ba_run(W_of(4, 0.3), si.uniform_p0(4), 3)["hist"][-1]
+    assert abs(Ib - rb[0]) <= ABS_U and abs(Ub - rb[1]) <= ABS_U and abs(Is - rs[0]) <= ABS_U and abs(Us - rs[1]) <= ABS_U
+
+
+def test_fast_mode_is_refused_while_symmetry_is_on(ba):
+    ctx = ba.ba_create(10, 0.5)
+    try:
+        ba.ba_set_symmetry(ctx, 1)
+        with pytest.raises(ba.BAError) as ei:
+            ba.ba_set_mode(ctx, ba.BA_MODE_FAST)             # FAST iterations would break p(x) == p(~x) bit for bit
+        assert ei.value.code == ba.BA_EINVAL
+        ba.ba_set_symmetry(ctx, 0)
+        ba.ba_set_mode(ctx, ba.BA_MODE_FAST)
+        with pytest.raises(ba.BAError) as ei:
+            ba.ba_set_symmetry(ctx, 1)
+        assert ei.value.code == ba.BA_EINVAL
     finally:
         ba.ba_destroy(ctx)

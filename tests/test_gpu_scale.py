@@ -1,6 +1,7 @@
 """GPU tests beyond the dense oracle's reach: trajectory parity at n=14,
-and at n=20 / n=24 (the bench configuration) closed forms, invariants and sampled rows / columns recomputed
-by independent CPU routines written here from the definitions (P:109 emb, P:140-158 BA step).
+and at n=20 / n=24 (the bench configuration) / n=26 closed forms, invariants, 64 sampled rows recomputed by the oracle
+itself (orc_emb_row / orc_D_row: P:109 keep-mask enumeration of one input), sampled columns by a DP pinned
+on CPU against the dense oracle, and all-entries agreement of the enumerating path with the FAST path on an asymmetric p.
 """
 import math
 from math import comb
@@ -24,48 +25,31 @@ def ba():
     return ba_mod
 
 
-# ------------------------------------------------------------------ independent CPU routines (test-local)
+# ------------------------------------------------------------------ the oracle at full size, one row at a time
 
-def row_by_prefix_dp(x, n):
-    """{code(y): emb(y,x)} for every distinct subsequence y of x: scan x left to right, every known y
-    spawns y.b (cnt[y.b] += cnt[y]).  code(y) = 1<<|y| | val(y)."""
-    cnt = {1: 1}
-    for i in range(n):
-        b = (x >> (n - 1 - i)) & 1
-        add = {}
-        for cy, e in cnt.items():
-            c2 = (cy << 1) | b
-            add[c2] = add.get(c2, 0) + e
-        for c2, e in add.items():
-            cnt[c2] = cnt.get(c2, 0) + e
-    return cnt
+from tests.cpu_routines import column_by_dp, weights, bit_reverse_table     # pinned on CPU in tests/test_oracle_pins.py
 
 
-def column_by_dp(yval, k, n):
-    """emb(y, x) for all x in [0,2^n) at once: textbook DP over the positions of x, vectorised over x."""
-    X = np.arange(1 << n, dtype=np.uint32)
-    e = [np.ones(1 << n, dtype=np.uint32)] + [np.zeros(1 << n, dtype=np.uint32) for _ in range(k)]
-    for i in range(n):
-        xb = (X >> np.uint32(n - 1 - i)) & np.uint32(1)
-        for r in range(min(k, i + 1), 0, -1):
-            yb = (yval >> (k - r)) & 1
-            e[r] += np.where(xb == yb, e[r - 1], np.uint32(0))
-    return e[k]
+def oracle_rows(n, xs):
+    """{x: emb row of x} from oracle/ (orc_emb_row, keep-mask enumeration of one input); rows in parallel
+    threads (the C call releases the GIL)."""
+    from concurrent.futures import ThreadPoolExecutor
+    import os
+    xs = sorted(set(int(x) for x in xs))
+    with ThreadPoolExecutor(max_workers=min(16, os.cpu_count() or 1)) as ex:
+        rows = list(ex.map(lambda x: orc.emb_row(n, x), xs))
+    return dict(zip(xs, rows))
 
 
-def weights(n, d):
-    return [(1.0 - d) ** k * d ** (n - k) if 0 < d < 1 else float((k == n) if d == 0 else (k == 0)) for k in range(n + 1)]
-
-
-def D_row(x, n, d, q):
-    w = weights(n, d)
-    terms = []
-    for cy, e in row_by_prefix_dp(x, n).items():
-        k = cy.bit_length() - 1
-        W = w[k] * e
-        if W > 0.0:
-            terms.append(W * (math.log2(W) - math.log2(q[cy - 1])))
-    return math.fsum(terms), len(terms)
+def check_rows_against_oracle(n, d, rows, q, D, what):
+    """D(x) of the device vs the oracle's plain definition (orc_D_row) on the device's own q."""
+    worst = 0.0
+    for x, row in rows.items():
+        want, nt = orc.D_row(n, d, row, q)
+        err = abs(D[x] - want) / abs(want)
+        worst = max(worst, err)
+        assert err <= REL_QD, f"{what}: D[{x}] = {D[x]!r}, oracle {want!r} ({nt} terms), rel {err:.3g}"
+    return worst
 
 
 # ------------------------------------------------------------------ T5 config 2
@@ -95,15 +79,26 @@ def test_T5_trajectory_config2(ba, start):
 
 # ------------------------------------------------------------------ T7 scale checks
 
-def scale_checks(ba, n, d, n_rows, n_cols, seed):
+def sample_inputs(n, n_rows, rng):
+    NX = 1 << n
+    alt = int("01" * n, 2) & (NX - 1)                          # alternating string: the most distinct subsequences
+    fixed = [0, NX - 1, alt, alt ^ (NX - 1), 1, NX - 2, (1 << (n // 2)) - 1, int("0011" * n, 2) & (NX - 1)]
+    return fixed + [int(v) for v in rng.integers(0, NX, max(0, n_rows - len(fixed)))]
+
+
+def scale_checks(ba, n, d, n_rows, n_cols, seed, asym=True):
     rng = np.random.default_rng(seed)
     NX = 1 << n
     w = weights(n, d)
+    xs = sample_inputs(n, n_rows, rng)
+    rows = oracle_rows(n, xs)                                 # ~64 rows, from oracle/ itself
     ctx = ba.ba_create(n, d)
     try:
         cnt = ba.ba_debug_count_terms(ctx)                    # P1/P2/P4 as device-side integer checksums
         assert cnt["in_terms"] == cnt["out_terms"] == ba.ba_terms_per_sweep(n)
         assert cnt["in_emb_sum"] == cnt["out_emb_sum"] == 4 ** n
+        for x in xs[:6]:                                      # emb bit-exact along whole rows (max-node row included)
+            assert np.array_equal(ba.ba_debug_emb_row(ctx, x), rows[x]), f"emb row {x}"
         # ---- iteration 0 from uniform p: closed forms
         ba.ba_iterate(ctx, 1)
         q0, D0 = ba.ba_get_q(ctx), ba.ba_get_D(ctx)
@@ -114,10 +109,7 @@ def scale_checks(ba, n, d, n_rows, n_cols, seed):
             assert np.max(np.abs(blk - want)) <= REL_QD * want
         assert abs(D0[0] - n * (1 - d)) <= REL_QD * n and abs(D0[NX - 1] - n * (1 - d)) <= REL_QD * n   # P8
         assert abs(U0 - n * (1 - d)) <= REL_QD * n and I0 <= U0
-        xs = [0b0101010101010101010101010101 & (NX - 1), 1, NX - 2] + [int(v) for v in rng.integers(0, NX, n_rows)]
-        for x in xs:                                          # P8b / P14: sampled rows by an independent routine
-            want, nt = D_row(x, n, d, q0)
-            assert abs(D0[x] - want) <= REL_QD * abs(want), f"D0[{x}] ({nt} terms)"
+        check_rows_against_oracle(n, d, rows, q0, D0, "iteration 0")
         # ---- iteration 1 from the (non-uniform) p_1
         p1 = ba.ba_get_p(ctx)
         assert abs(math.fsum(p1) - 1.0) <= 1e-12
@@ -129,16 +121,12 @@ def scale_checks(ba, n, d, n_rows, n_cols, seed):
         for k in range(n + 1):                                # P7: per-length mass
             want = comb(n, k) * w[k]
             assert abs(math.fsum(q1[(1 << k) - 1:(2 << k) - 1]) - want) <= 1e-12 * want
-        rev = np.zeros(NX, dtype=np.int64)                    # P11: symmetry under cpl and rev (Theorem 4)
+        rev = bit_reverse_table(n)                            # P11: symmetry under cpl and rev (Theorem 4)
         X = np.arange(NX, dtype=np.int64)
-        for i in range(n):
-            rev |= ((X >> i) & 1) << (n - 1 - i)
         assert np.max(np.abs(D1 - D1[(NX - 1) - X])) <= 1e-11 and np.max(np.abs(D1 - D1[rev])) <= 1e-11
         assert np.max(np.abs(p1 - p1[rev]) / p1) <= 1e-11
         assert abs(U1 - D1.max()) <= 1e-15 and abs(I1 - math.fsum(p1 * D1)) <= 1e-12
-        for x in xs[:max(4, n_rows // 2)]:                    # sampled rows with the downloaded q_1
-            want, _ = D_row(x, n, d, q1)
-            assert abs(D1[x] - want) <= REL_QD * abs(want), f"D1[{x}]"
+        check_rows_against_oracle(n, d, rows, q1, D1, "iteration 1")
         for _ in range(n_cols):                               # sampled columns with the downloaded p_1
             k = int(rng.integers(max(1, n // 2 - 3), n // 2 + 4))
             yv = int(rng.integers(0, 1 << k))
@@ -148,23 +136,87 @@ def scale_checks(ba, n, d, n_rows, n_cols, seed):
             assert abs(got - want) <= REL_QD * want, f"q1[y={yv:0{k}b}]"
             col = ba.ba_debug_emb_col(ctx, (1 << k) - 1 + yv)
             assert np.array_equal(col, e)                     # emb bit-exact along the whole column
-        x = xs[3]
-        row = ba.ba_debug_emb_row(ctx, x)                     # emb bit-exact along a whole row
-        ref = row_by_prefix_dp(x, n)
-        assert int(np.count_nonzero(row)) == len(ref)
-        for cy, e in ref.items():
-            assert row[cy - 1] == e
+        if not asym:
+            return
+        # ---- an ASYMMETRIC p (not uniform, not cpl/rev-symmetric): every entry of q, D, p_next of the enumerating
+        # path against the FAST path (oracle-green at n <= 14, no size-dependent branch) on the same p, plus the
+        # oracle rows on that same q; sampled columns by the pinned DP.  A mis-addressed gather cannot hide here.
+        pa = si.random_positive_p(n, seed + 1000)
+        res = {}
+        for mode in (ba.BA_MODE_ENUM, ba.BA_MODE_FAST):
+            ba.ba_set_mode(ctx, mode)
+            ba.ba_set_p(ctx, pa)
+            ba.ba_iterate(ctx, 1)
+            res[mode] = (ba.ba_get_q(ctx), ba.ba_get_D(ctx), ba.ba_get_p(ctx), ba.ba_bounds(ctx), ba.ba_stats(ctx)[0])
+        ba.ba_set_mode(ctx, ba.BA_MODE_ENUM)
+        (qe, De, pe, be, lze), (qf, Df, pf, bf, lzf) = res[ba.BA_MODE_ENUM], res[ba.BA_MODE_FAST]
+        assert np.max(np.abs(qe - qf) / qf) <= REL_QD, "q: ENUM vs FAST, all entries"
+        assert np.max(np.abs(De - Df) / np.abs(Df)) <= REL_QD, "D: ENUM vs FAST, all entries"
+        assert np.max(np.abs(pe - pf) / pf) <= 1e-11
+        assert abs(be[0] - bf[0]) <= 1e-12 * max(1, abs(bf[0])) and abs(be[1] - bf[1]) <= 1e-12 * max(1, abs(bf[1])) and abs(lze - lzf) <= 1e-12
+        check_rows_against_oracle(n, d, rows, qe, De, "asymmetric p")
+        for _ in range(max(1, n_cols)):
+            k = int(rng.integers(max(1, n // 2 - 3), n // 2 + 4))
+            yv = int(rng.integers(0, 1 << k))
+            e = column_by_dp(yv, k, n)
+            want = w[k] * math.fsum((e.astype(np.float64) * pa)[e > 0])
+            assert abs(qe[(1 << k) - 1 + yv] - want) <= REL_QD * want, f"q(asym)[y={yv:0{k}b}]"
+        for k in range(n + 1):                                # P7 on the asymmetric p
+            want = comb(n, k) * w[k]
+            assert abs(math.fsum(qe[(1 << k) - 1:(2 << k) - 1]) - want) <= 1e-12 * want
     finally:
         ba.ba_destroy(ctx)
 
 
 def test_T7_scale_n20(ba):
-    scale_checks(ba, 20, 0.80, n_rows=12, n_cols=3, seed=20)
+    scale_checks(ba, 20, 0.80, n_rows=64, n_cols=3, seed=20)
 
 
 def test_T7_scale_n24_bench_config(ba):
     # BASELINE.json configs[3]: n=24, d=0.70, uniform p0 -- the launch configuration bench.py times
-    scale_checks(ba, 24, 0.70, n_rows=6, n_cols=2, seed=24)
+    scale_checks(ba, 24, 0.70, n_rows=64, n_cols=2, seed=24)
+
+
+def test_T7_scale_n26(ba):
+    # above the bench size, default on (h = 18: the last size whose alpha always fit 16 bits)
+    scale_checks(ba, 26, 0.75, n_rows=16, n_cols=1, seed=26)
+
+
+def test_T7_symmetry_and_exact_at_scale_n20(ba):
+    # complement symmetry on vs off, and the exact channel's pruned ENUM sweeps vs the FAST transform, all entries
+    n, d = 20, 0.70
+    ctx = ba.ba_create(n, d)
+    try:
+        ba.ba_iterate(ctx, 2)
+        q, D, p = ba.ba_get_q(ctx), ba.ba_get_D(ctx), ba.ba_get_p(ctx)
+    finally:
+        ba.ba_destroy(ctx)
+    ctx = ba.ba_create(n, d)
+    try:
+        ba.ba_set_symmetry(ctx, 1)
+        ba.ba_iterate(ctx, 2)
+        qs, Ds, ps = ba.ba_get_q(ctx), ba.ba_get_D(ctx), ba.ba_get_p(ctx)
+    finally:
+        ba.ba_destroy(ctx)
+    assert np.max(np.abs(qs - q) / q) <= 1e-11 and np.max(np.abs(Ds - D) / np.abs(D)) <= 1e-11 and np.max(np.abs(ps - p) / p) <= 1e-10
+    for k in (3, 10, 17):                                     # k < h - ..., k ~ n/2, k > h + m: both prunings of the exact mode
+        pa = si.random_positive_p(n, 500 + k)
+        out = {}
+        for mode in (ba.BA_MODE_ENUM, ba.BA_MODE_FAST):
+            ctx = ba.ba_create(n, d)
+            try:
+                ba.ba_set_mode(ctx, mode)
+                ba.ba_set_exact(ctx, k)
+                ba.ba_set_p(ctx, pa)
+                ba.ba_iterate(ctx, 1)
+                out[mode] = (ba.ba_get_q(ctx), ba.ba_get_D(ctx), ba.ba_bounds(ctx))
+            finally:
+                ba.ba_destroy(ctx)
+        (qe, De, be), (qf, Df, bf) = out[ba.BA_MODE_ENUM], out[ba.BA_MODE_FAST]
+        nz = qf > 0
+        assert np.array_equal(qe > 0, nz) and np.max(np.abs(qe[nz] - qf[nz]) / qf[nz]) <= REL_QD
+        assert np.all(np.abs(De - Df) <= REL_QD * np.abs(Df) + 1e-15)
+        assert abs(be[0] - bf[0]) <= 1e-12 and abs(be[1] - bf[1]) <= 1e-12
 
 
 # ------------------------------------------------------------------ T8 boundary errors that need a context
@@ -227,11 +279,11 @@ def test_config3_harness_small(ba, mode):
 @pytest.mark.slow
 def test_T7_scale_n28_config5(ba):
     # BASELINE.json configs[4]: n=28, d=0.80 (34 GB on the device, ~8 minutes on a B200, ~20 GB of host arrays).
-    # Opt-in: BA_RUN_N28=1.  Result of the round-1 run: profiles/r01c_scale_n28.md.
+    # Opt-in: BA_RUN_N28=1.  Result of the last run: profiles/ (r02_scale_n28.md).
     import os
     if os.environ.get("BA_RUN_N28") != "1":
         pytest.skip("set BA_RUN_N28=1 to run the n=28 scale check")
-    scale_checks(ba, 28, 0.80, n_rows=3, n_cols=0, seed=28)
+    scale_checks(ba, 28, 0.80, n_rows=8, n_cols=0, seed=28, asym=False)
 
 
 # ------------------------------------------------------------------ one-step parity at the oracle's reach, extreme d

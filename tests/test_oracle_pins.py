@@ -446,3 +446,142 @@ def test_lemma2_convex_combination():
     assert left <= right
     assert right == pytest.approx(2.3045, abs=5e-3)
     assert left == pytest.approx(2.1230, abs=1e-4)
+
+
+# ----------------------------------------------------------------------------- G8 floor of the update (P:154-158 + reading G8)
+
+def test_floor_G8_fires_exactly_and_leaves_the_rest():
+    # Reading G8: p' = max(p 2^D / Z, 2^-1000).  A 3-bit channel with one input at 1e-305 and d = 0.9:
+    # D(x) holds (1-d)^n log2(1/p(x)) = 1e-3 * 1013 ~ 1 bit (G8), so p 2^D / Z ~ 1e-305 * 2^2 < 2^-1000 = 9.33e-302:
+    # that entry must come out as 2^-1000 exactly, and every other entry must be the plain P:154-158 update
+    # (the floor is not a renormalisation).  (At d = 0.5 the same p regrows to 8e-268 in one step: no floor.)
+    n, d = 3, 0.9
+    W = orc.channel(n, d, E_of(n))
+    p = si.uniform_p0(n).copy()
+    p[5] = 1e-305
+    p[2] += 1.0 / 8 - 1e-305
+    r = orc.ba_step(W, p)
+    assert r["p_next"][5] == 2.0 ** -1000                              # exact: a power of two
+    Z = 2.0 ** r["log2Z"]
+    plain = p * np.exp2(r["D"]) / Z
+    assert plain[5] < 2.0 ** -1000 and plain[5] > 0.0                  # the floor really was the binding branch
+    keep = np.arange(8) != 5
+    assert np.allclose(r["p_next"][keep], plain[keep], rtol=1e-14, atol=0)
+    assert np.all(r["p_next"][keep] > 1e-3)                            # untouched by the floor
+    # a p sitting exactly at the floor stays there, one just above it follows P:156
+    p2 = si.uniform_p0(n).copy()
+    p2[1] = 2.0 ** -1000
+    p2[6] = 2.0 ** -990
+    p2[0] += 2.0 / 8 - p2[1] - p2[6]
+    r2 = orc.ba_step(W, p2)
+    assert r2["p_next"][1] == 2.0 ** -1000 or r2["p_next"][1] == pytest.approx(p2[1] * 2 ** r2["D"][1] / 2 ** r2["log2Z"], rel=1e-13)
+    assert r2["p_next"][6] == pytest.approx(p2[6] * 2 ** r2["D"][6] / 2 ** r2["log2Z"], rel=1e-13)
+    assert r2["p_next"][6] > 2.0 ** -1000
+
+
+def test_floor_G8_generic_matrix():
+    # same on a generic 2-input channel (no emb involved): BSC with a collapsed input
+    e = 0.2
+    W = np.array([[1 - e, e], [e, 1 - e]])
+    p = np.array([1.0 - 1e-306, 1e-306])
+    r = orc.ba_step(W, p)
+    assert r["p_next"][1] == 2.0 ** -1000
+    assert r["p_next"][0] == pytest.approx(1.0, rel=1e-15)
+
+
+# ----------------------------------------------------------------------------- single-row oracle (beyond the dense reach)
+
+def test_emb_row_equals_dense_rows():
+    # orc_emb_row is the same keep-mask count as orc_emb_dense for one x: every row, n <= 8; sampled n = 10
+    for n in (1, 2, 3, 5, 8):
+        E = E_of(n)
+        for x in range(1 << n):
+            assert np.array_equal(orc.emb_row(n, x), E[x])
+    E = E_of(10)
+    for x in np.random.default_rng(9).integers(0, 1 << 10, 64):
+        assert np.array_equal(orc.emb_row(10, int(x)), E[int(x)])
+
+
+def test_emb_row_hand_worked_and_invariants_large_n():
+    row = orc.emb_row(3, 0b010)                                        # the hand-worked row of test_emb_hand_worked_n3_row
+    expect = np.zeros(15, dtype=np.uint32)
+    for (k, y, e) in [(0, 0, 1), (1, 0, 2), (1, 1, 1), (2, 0b00, 1), (2, 0b01, 1), (2, 0b10, 1), (3, 0b010, 1)]:
+        expect[idx(k, y)] = e
+    assert np.array_equal(row, expect)
+    n = 18                                                             # beyond the dense reach: invariants fixed by mathematics
+    for x in (0, (1 << n) - 1, 0b010101010101010101, 0b001101011100101101):
+        row = orc.emb_row(n, x).astype(np.int64)
+        for k, sl in enumerate(length_slices(n)):
+            assert int(row[sl].sum()) == comb(n, k)                    # P1
+        assert int(np.count_nonzero(row)) == distinct_subseq_count(x, n)   # classic recurrence (P4)
+    assert int(np.count_nonzero(orc.emb_row(n, 0b010101010101010101))) == 10945   # Fib(21): alternating string has the most
+    rng = np.random.default_rng(4)
+    x = int(rng.integers(0, 1 << n))
+    row = orc.emb_row(n, x)
+    for _ in range(200):                                               # P3: independent textbook DP on sampled entries
+        k = int(rng.integers(0, n + 1))
+        y = int(rng.integers(0, 1 << k))
+        assert row[idx(k, y)] == emb_dp(x, n, y, k)
+    with pytest.raises(ValueError):
+        orc.emb_row(8, 256)
+
+
+@pytest.mark.parametrize("n,d", [(5, 0.3), (9, 0.64), (10, 0.9)])
+def test_D_row_matches_definition_and_closed_forms(n, d):
+    # orc_D_row is P:189-193 for one x.  (i) closed form P8 with the closed-form q_0 of P6 (no BA step involved):
+    # D_0(0^n) = n(1-d);  (ii) python-float restatement of the definition on a random q;  (iii) the full step.
+    q0 = np.empty((2 << n) - 1)
+    for k, sl in enumerate(length_slices(n)):
+        q0[sl] = comb(n, k) * (1 - d) ** k * d ** (n - k) / 2.0 ** k
+    for x in (0, (1 << n) - 1):
+        D, nt = orc.D_row(n, d, orc.emb_row(n, x), q0)
+        assert D == pytest.approx(n * (1 - d), rel=1e-13) and nt == n + 1
+    rng = np.random.default_rng(n)
+    q = rng.random((2 << n) - 1) + 0.01
+    x = int(rng.integers(0, 1 << n))
+    row = orc.emb_row(n, x)
+    terms = []
+    for j in np.flatnonzero(row):
+        k = (int(j) + 1).bit_length() - 1
+        Wv = float(row[j]) * (1 - d) ** k * d ** (n - k)
+        terms.append(Wv * (math.log2(Wv) - math.log2(q[j])))
+    D, nt = orc.D_row(n, d, row, q)
+    assert D == pytest.approx(math.fsum(terms), rel=1e-13, abs=1e-15) and nt == len(terms)
+    p = si.random_positive_p(n, 77)
+    r = orc.ba_step(orc.channel(n, d, E_of(n)), p)
+    for x in rng.integers(0, 1 << n, 16):
+        D, _ = orc.D_row(n, d, orc.emb_row(n, int(x)), r["q"])
+        assert D == pytest.approx(r["D"][int(x)], rel=1e-14)
+
+
+def test_D_row_endpoints_of_d():
+    # R7: d = 0 keeps only y = x (D = -log2 q(idx(x))); d = 1 keeps only the empty output (D = -log2 q(0))
+    n = 6
+    q = np.random.default_rng(1).random((2 << n) - 1) + 0.1
+    x = 0b101101
+    row = orc.emb_row(n, x)
+    assert orc.D_row(n, 0.0, row, q)[0] == pytest.approx(-math.log2(q[idx(n, x)]), rel=1e-15)
+    assert orc.D_row(n, 1.0, row, q)[0] == pytest.approx(-math.log2(q[0]), rel=1e-15)
+
+
+# ----------------------------------------------------------------------------- pins of the test-local CPU routines (tests/cpu_routines.py)
+
+def test_cpu_routines_column_dp_equals_oracle_columns():
+    from tests import cpu_routines as cr
+    for n in (1, 4, 7, 10):
+        E = E_of(n)
+        rng = np.random.default_rng(n)
+        cols = [(k, y) for k in range(n + 1) for y in range(1 << k)]
+        if n == 10:
+            cols = [cols[i] for i in rng.integers(0, len(cols), 200)] + [(0, 0), (10, 1023), (10, 0), (5, 0b10101)]
+        for (k, y) in cols:
+            assert np.array_equal(cr.column_by_dp(y, k, n), E[:, idx(k, y)])
+
+
+def test_cpu_routines_weights_and_rev():
+    from tests import cpu_routines as cr
+    for (n, d) in [(5, 0.25), (7, 0.0), (7, 1.0), (12, 0.64)]:
+        assert np.allclose(cr.weights(n, d), orc.weights(n, d), rtol=1e-15, atol=0)
+    t = cr.bit_reverse_table(5)
+    assert [int(t[x]) for x in (0b00001, 0b10110, 0b11111)] == [0b10000, 0b01101, 0b11111]
+    assert all(int(t[x]) == rev(x, 5) for x in range(32))
