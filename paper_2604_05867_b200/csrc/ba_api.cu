@@ -22,19 +22,14 @@ struct ba_ctx {
     double d = 0.0;
     size_t NX = 0, NY = 0, NZ = 0, napart = 0;
     KConst kc;
-    int nri = 0, nro = 0, n_in_csr = 0, n_out_csr = 0;
     cudaStream_t st = nullptr;
     bool own_buffers = false, own_stream = false;
     double *p = nullptr, *q = nullptr, *D = nullptr;
     unsigned char *scratch = nullptr;
     // carved from scratch
-    double *c = nullptr, *Hc = nullptr, *Apart = nullptr, *part = nullptr, *scal = nullptr, *hist = nullptr;
-    uint2 *FI = nullptr, *FO = nullptr;
-    uint4 *RI = nullptr, *RO = nullptr;
+    double *c = nullptr, *Hc = nullptr, *Apart = nullptr, *S = nullptr, *part = nullptr, *scal = nullptr, *hist = nullptr;
+    GroupDev gin, gout;              // pair schedules of the two sweeps (device pointers into scratch)
     uint2 *EPS8 = nullptr;
-    uint32_t *RI8 = nullptr, *RO8 = nullptr;
-    uint16_t *in_owner = nullptr, *out_owner = nullptr, *ri_cnt = nullptr, *ro_cnt = nullptr, *ri_csr = nullptr, *ro_csr = nullptr;
-    uint16_t *in_csr_off = nullptr, *in_csr_idx = nullptr, *out_csr_off = nullptr, *out_csr_idx = nullptr;
     unsigned int *counters = nullptr;
     unsigned long long *cnt = nullptr;
     size_t npart_cap = 0;
@@ -71,9 +66,10 @@ static double host_binom(int n, int k) {
 }
 
 // ------------------------------------------------------------------------------------------------ scratch layout
+struct SideLayout { size_t GB, GA, GO, GW, csr_off, csr_idx, R, r_cnt, r_csr, R8; };
 struct ScratchLayout {
-    size_t c, Hc, Apart, part, scal, hist, FI, FO, RI, RO, EPS8, RI8, RO8, in_owner, out_owner, ri_cnt, ro_cnt, ri_csr, ro_csr,
-        in_csr_off, in_csr_idx, out_csr_off, out_csr_idx, counters, cnt, total;
+    size_t c, Hc, Apart, S, part, scal, hist, EPS8, counters, cnt, total;
+    SideLayout in, out;
     size_t napart, npart_cap;
 };
 
@@ -92,37 +88,39 @@ static std::shared_ptr<const TileTables> tile_tables(int m) {
     return cache[m];
 }
 
+#define BA_FINAL_BLOCKS_PER_SM 8      // grid of k_in_final = SMs x this; one reduction triple per block
+
+static void side_layout(const GroupSide &G, SideLayout &L, size_t &o) {
+    L.GB = o; o += align256(G.GB.size() * 16);
+    L.GA = o; o += align256(G.GA.size() * 4);
+    L.GO = o; o += align256(G.GO.size() * 2);
+    L.GW = o; o += align256(G.GW.size());
+    L.csr_off = o; o += align256(G.csr_off.size() * 2);
+    L.csr_idx = o; o += align256(G.csr_idx.size() * 2);
+    L.R = o; o += align256(G.R.size() * 16);
+    L.r_cnt = o; o += align256(G.r_cnt.size() * 2);
+    L.r_csr = o; o += align256(G.r_csr.size() * 2);
+    L.R8 = o; o += align256(G.R8.size() * 4);
+}
+
 static void scratch_layout(int n, const TileTables &T, ScratchLayout &L) {
     const int m = low_m(n), h = n - m;
     const size_t NX = (size_t)1 << n, NY = ((size_t)2 << n) - 1, NZ = ((size_t)2 << m) - 1;
     L.napart = (((size_t)2 << h) - 1) * NZ;
     size_t fastwords = 2 * (((size_t)2 << n) + 64);          // FAST mode ping-pong buffers
     if (L.napart < fastwords) L.napart = fastwords;
-    L.npart_cap = ((size_t)1 << h) > 8192 ? ((size_t)1 << h) : 8192;
+    L.npart_cap = 65536;                                     // >= grid of k_in_final
     size_t o = 0;
     L.c = o; o += align256((NY + 1) * 8);                    // c[code], entry 0 unused
     L.Hc = o; o += align256(NX * 8);
     L.Apart = o; o += align256(L.napart * 8);
+    L.S = o; o += align256(2 * NX * 8);                      // partial sums of the two lists (input sweep)
     L.part = o; o += align256(L.npart_cap * 3 * 8);
     L.scal = o; o += align256(8 * 8);
     L.hist = o; o += align256((size_t)BA_HIST_CAP * 3 * 8);
-    L.FI = o; o += align256(T.FI.size() * 8);
-    L.FO = o; o += align256(T.FO.size() * 8);
-    L.RI = o; o += align256(T.RI.size() * 16);
-    L.RO = o; o += align256(T.RO.size() * 16);
     L.EPS8 = o; o += align256(T.EPS8.size() * 8);
-    L.RI8 = o; o += align256(T.RI8.size() * 4);
-    L.RO8 = o; o += align256(T.RO8.size() * 4);
-    L.in_owner = o; o += align256(T.in_owner.size() * 2);
-    L.out_owner = o; o += align256(T.out_owner.size() * 2);
-    L.ri_cnt = o; o += align256(T.ri_cnt.size() * 2);
-    L.ro_cnt = o; o += align256(T.ro_cnt.size() * 2);
-    L.ri_csr = o; o += align256(T.ri_csr.size() * 2);
-    L.ro_csr = o; o += align256(T.ro_csr.size() * 2);
-    L.in_csr_off = o; o += align256(T.in_csr_off.size() * 2);
-    L.in_csr_idx = o; o += align256(T.in_csr_idx.size() * 2 + 2);
-    L.out_csr_off = o; o += align256(T.out_csr_off.size() * 2);
-    L.out_csr_idx = o; o += align256(T.out_csr_idx.size() * 2 + 2);
+    side_layout(T.in, L.in, o);
+    side_layout(T.out, L.out, o);
     L.counters = o; o += align256(16 * 4);
     L.cnt = o; o += align256(8 * 8);
     L.total = o;
@@ -151,8 +149,9 @@ extern "C" int ba_terms_per_sweep(int n, unsigned long long *T) {
 }
 
 // Host-only self-check of the static tile tables of width m (include/ba.h): under every class, every pair
-// (v, z != empty) of the m-bit deletion channel must be served exactly once, by a fast pair or by a rider, with
-// the B_s an independent DP gives.
+// (v, z != empty) of the m-bit deletion channel must be served exactly once, by a pair slot or by a rider, with
+// the B_s an independent DP gives; the slots of a group must share their operand, and a warp's loop type must cover
+// its slots.
 static uint32_t chk_emb(uint32_t w, int lw, uint32_t v, int lv) {
     if (lw > lv) return 0;
     uint32_t e[BA_MLOW + 2];
@@ -175,16 +174,25 @@ extern "C" int ba_debug_check_tables(int m, unsigned long long stats[4]) {
         if (lz + s > m) return 0u;
         return chk_emb(((sig & ((1u << s) - 1u)) << lz) | (cz - (1u << lz)), lz + s, (uint32_t)v, m);
     };
-    for (int side = 0; side < 2; side++)                    // 0: input sweep tables, 1: output sweep tables
+    for (int side = 0; side < 2; side++) {                  // 0: input sweep tables, 1: output sweep tables
+        const GroupSide &G = side ? T.out : T.in;
         for (int cls = 0; cls < BA_NCLS; cls++)
             for (int b = 0; b < 2; b++) {
                 std::vector<uint8_t> seen((size_t)nv * NZc, 0);
-                auto visit = [&](int v, uint32_t cz, uint32_t b0123, int nb, const uint32_t *tail8) -> bool {
+                // pos = operand position in the staged row (in: code(z[1:]), out: v); ow = owner (in: v, out: code(z))
+                auto visit = [&](uint32_t pos, uint32_t ow, uint32_t b0123, int nb, const uint32_t *tail8) -> bool {
+                    int v; uint32_t cz;
+                    if (side) { v = (int)pos; cz = ow; }
+                    else {
+                        if (pos == 0) return false;
+                        const int lt = 31 - __builtin_clz(pos);
+                        v = (int)ow; cz = (1u << (lt + 1)) | ((uint32_t)b << lt) | (pos - (1u << lt));
+                    }
                     if (v < 0 || v >= nv || cz < 2 || cz >= (uint32_t)NZc) return false;
                     const int lz = 31 - __builtin_clz(cz);
                     if ((int)((cz >> (lz - 1)) & 1u) != b || seen[(size_t)v * NZc + cz]++) return false;
                     for (int s = 0; s < 4; s++) if (((b0123 >> (8 * s)) & 0xffu) != Bs((uint32_t)cls, s, cz, v)) return false;
-                    if (nb == 4) return Bs((uint32_t)cls, 4, cz, v) == 0;                 // a fast pair must not be deep
+                    if (nb == 4) return Bs((uint32_t)cls, 4, cz, v) == 0;                 // a slot pair must not be deep
                     for (uint32_t hi = 0; hi < 16u; hi++)                                 // rider: B_4 .. B_8
                         for (int s = 4; s <= 8; s++) {
                             const uint32_t want = Bs((hi << 4) | (uint32_t)cls, s, cz, v);
@@ -193,41 +201,30 @@ extern "C" int ba_debug_check_tables(int m, unsigned long long stats[4]) {
                         }
                     return true;
                 };
-                const std::vector<uint2> &F = side ? T.FO : T.FI;
-                for (int c = 0; c < BA_NC; c++)
+                for (int k = 0; k < BA_KG; k++)
                     for (int tid = 0; tid < BA_NT; tid++) {
-                        const uint32_t ow = side ? T.out_owner[(((size_t)cls * 2 + b) * BA_NC + c) * BA_NT + tid]
-                                                 : T.in_owner[((size_t)b * BA_NC + c) * BA_NT + tid];
-                        for (int q = 0; q < BA_C; q++) {
-                            const uint2 e = F[((((size_t)cls * 2 + b) * BA_NC + c) * BA_C + q) * BA_NT + tid];
-                            if (!(e.x & 0xffu)) continue;
-                            if (ow == 0xffffu) return BA_EINVAL;
-                            const uint32_t pos = ba_swz(e.y >> 3);
-                            bool okp;
-                            if (side) okp = visit((int)pos, ow, e.x, 4, nullptr);
-                            else {
-                                const int lt = 31 - __builtin_clz(pos);
-                                okp = visit((int)ow, (1u << (lt + 1)) | ((uint32_t)b << lt) | (pos - (1u << lt)), e.x, 4, nullptr);
-                            }
-                            if (!okp) return BA_EINVAL;
+                        const uint4 e4 = G.GB[(((size_t)cls * 2 + b) * BA_KG + k) * BA_NT + tid];
+                        const uint32_t e[4] = {e4.x, e4.y, e4.z, e4.w};
+                        const uint32_t pos = G.GA[((size_t)b * BA_KG + k) * BA_NT + tid] >> 3;
+                        const int wm = G.GW[(size_t)b * (BA_NT / 32) + tid / 32];
+                        for (int q = 0; q < BA_GP; q++) {
+                            const uint32_t ow = G.GO[(((size_t)b * BA_KG + k) * BA_GP + q) * BA_NT + tid];
+                            if (!(e[q] & 0xffu)) { if (e[q]) return BA_EINVAL; continue; }      // unused, or deep under this class
+                            if (ow == 0xffffu || k >= (wm & 15)) return BA_EINVAL;              // the warp's loop must reach the slot
+                            if ((wm >> 4) == 2 && (e[q] >> 16)) return BA_EINVAL;               // a type-2 loop ignores B_2, B_3
+                            if (!visit(pos, ow, e[q], 4, nullptr)) return BA_EINVAL;
                             stats[side ? 2 : 0]++;
                         }
                     }
-                const std::vector<uint4> &R = side ? T.RO : T.RI;
-                const std::vector<uint32_t> &R8 = side ? T.RO8 : T.RI8;
-                const int cap = side ? T.nro : T.nri, nr = side ? T.ro_cnt[cls * 2 + b] : T.ri_cnt[cls * 2 + b];
+                const int nr = G.r_cnt[cls * 2 + b];
                 for (int e = 0; e < nr; e++) {
-                    const uint4 rd = R[((size_t)cls * 2 + b) * cap + e];
+                    const uint4 rd = G.R[((size_t)cls * 2 + b) * G.nr + e];
                     uint32_t tail8[16];
-                    for (uint32_t hi = 0; hi < 16u; hi++) tail8[hi] = R8[(((size_t)cls * 2 + b) * 16 + hi) * cap + e];
-                    const uint32_t pos = ba_swz(rd.z >> 3), ow = rd.y >> 16;
-                    bool okp;
-                    if (side) okp = visit((int)pos, ow, rd.x, 5 + (int)(rd.y & 0xffu), tail8);
-                    else {
-                        const int lt = 31 - __builtin_clz(pos);
-                        okp = visit((int)ow, (1u << (lt + 1)) | ((uint32_t)b << lt) | (pos - (1u << lt)), rd.x, 5 + (int)(rd.y & 0xffu), tail8);
-                    }
-                    if (!okp || (rd.y & 0xffu) == 0) return BA_EINVAL;
+                    for (uint32_t hi = 0; hi < 16u; hi++) tail8[hi] = G.R8[(((size_t)cls * 2 + b) * 16 + hi) * G.nr + e];
+                    if (!visit(rd.z >> 3, rd.y >> 16, rd.x, 5 + (int)(rd.y & 0xffu), tail8) || (rd.y & 0xffu) == 0) return BA_EINVAL;
+                    const uint16_t *cs = &G.r_csr[((size_t)cls * 2 + b) * (G.nown + 1)];
+                    const uint32_t ow = rd.y >> 16;
+                    if (!(cs[ow] <= e && e < cs[ow + 1])) return BA_EINVAL;                     // the epilogue finds it under its owner
                     stats[side ? 3 : 1]++;
                 }
                 for (int v = 0; v < nv; v++)                 // nothing missing
@@ -237,6 +234,21 @@ extern "C" int ba_debug_check_tables(int m, unsigned long long stats[4]) {
                         if ((chk_emb(cz - (1u << lz), lz, (uint32_t)v, m) != 0) != (seen[(size_t)v * NZc + cz] != 0)) return BA_EINVAL;
                     }
             }
+        // the epilogue's CSR lists every used slot exactly once, under its owner
+        for (int b = 0; b < 2; b++) {
+            std::vector<uint8_t> hit((size_t)BA_NSLOT * BA_NT, 0);
+            for (int o = 0; o < G.nown; o++)
+                for (int q = G.csr_off[(size_t)b * (G.nown + 1) + o]; q < G.csr_off[(size_t)b * (G.nown + 1) + o + 1]; q++) {
+                    const uint32_t sl = G.csr_idx[(size_t)b * BA_NSLOT * BA_NT + q];
+                    const int kq = (int)(sl / BA_NT), tid = (int)(sl % BA_NT);
+                    if (G.GO[(((size_t)b * BA_KG + kq / BA_GP) * BA_GP + kq % BA_GP) * BA_NT + tid] != o || hit[sl]++) return BA_EINVAL;
+                }
+            for (int k = 0; k < BA_KG; k++)
+                for (int q = 0; q < BA_GP; q++)
+                    for (int tid = 0; tid < BA_NT; tid++)
+                        if ((G.GO[(((size_t)b * BA_KG + k) * BA_GP + q) * BA_NT + tid] != 0xffffu) != (hit[(size_t)(k * BA_GP + q) * BA_NT + tid] != 0)) return BA_EINVAL;
+        }
+    }
     return BA_OK;
 }
 
@@ -263,6 +275,42 @@ static cudaError_t upload(void *dst, const std::vector<V> &src, cudaStream_t st)
     return cudaMemcpyAsync(dst, src.data(), src.size() * sizeof(V), cudaMemcpyHostToDevice, st);
 }
 
+static cudaError_t upload_side(unsigned char *s, const GroupSide &G, const SideLayout &L, GroupDev &D, cudaStream_t st) {
+    cudaError_t e;
+    if ((e = upload(s + L.GB, G.GB, st)) != cudaSuccess) return e;
+    if ((e = upload(s + L.GA, G.GA, st)) != cudaSuccess) return e;
+    if ((e = upload(s + L.GO, G.GO, st)) != cudaSuccess) return e;
+    if ((e = upload(s + L.GW, G.GW, st)) != cudaSuccess) return e;
+    if ((e = upload(s + L.csr_off, G.csr_off, st)) != cudaSuccess) return e;
+    if ((e = upload(s + L.csr_idx, G.csr_idx, st)) != cudaSuccess) return e;
+    if ((e = upload(s + L.R, G.R, st)) != cudaSuccess) return e;
+    if ((e = upload(s + L.r_cnt, G.r_cnt, st)) != cudaSuccess) return e;
+    if ((e = upload(s + L.r_csr, G.r_csr, st)) != cudaSuccess) return e;
+    if ((e = upload(s + L.R8, G.R8, st)) != cudaSuccess) return e;
+    D.GB = (const uint4 *)(s + L.GB); D.GA = (const uint32_t *)(s + L.GA); D.GO = (const uint16_t *)(s + L.GO);
+    D.GW = (const uint8_t *)(s + L.GW); D.csr_off = (const uint16_t *)(s + L.csr_off); D.csr_idx = (const uint16_t *)(s + L.csr_idx);
+    D.R = (const uint4 *)(s + L.R); D.r_cnt = (const uint16_t *)(s + L.r_cnt); D.r_csr = (const uint16_t *)(s + L.r_csr);
+    D.R8 = (const uint32_t *)(s + L.R8);
+    D.nr = G.nr; D.nown = G.nown;
+    return cudaSuccess;
+}
+
+// MaxDynamicSharedMemorySize is per-function state shared by every ctx of the process: only ever raise it, so that
+// one ctx cannot shrink what another live ctx launches with.
+static cudaError_t raise_smem_limits(size_t smem_in, size_t smem_out) {
+    static std::mutex mu;
+    static size_t max_in = 0, max_out = 0;
+    std::lock_guard<std::mutex> lk(mu);
+    if (smem_in > max_in) max_in = smem_in;
+    if (smem_out > max_out) max_out = smem_out;
+    cudaError_t e;
+#define BA_SET(k, v) if ((e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(v))) != cudaSuccess) return e
+    BA_SET(k_enum_in<IN_SWEEP>, max_in); BA_SET(k_enum_in<IN_HC>, max_in); BA_SET(k_enum_in<IN_DEBUG>, max_in); BA_SET(k_enum_in<IN_COUNT>, max_in);
+    BA_SET(k_enum_out<OUT_SWEEP>, max_out); BA_SET(k_enum_out<OUT_DEBUG>, max_out); BA_SET(k_enum_out<OUT_COUNT>, max_out);
+#undef BA_SET
+    return cudaSuccess;
+}
+
 static int finish_create(ba_ctx *c) {
     const std::shared_ptr<const TileTables> Tp = tile_tables(c->m);
     const TileTables &T = *Tp;
@@ -270,27 +318,15 @@ static int finish_create(ba_ctx *c) {
     ScratchLayout L;
     scratch_layout(c->n, T, L);
     unsigned char *s = c->scratch;
-    c->c = (double *)(s + L.c); c->Hc = (double *)(s + L.Hc); c->Apart = (double *)(s + L.Apart);
+    c->c = (double *)(s + L.c); c->Hc = (double *)(s + L.Hc); c->Apart = (double *)(s + L.Apart); c->S = (double *)(s + L.S);
     c->part = (double *)(s + L.part); c->scal = (double *)(s + L.scal); c->hist = (double *)(s + L.hist);
-    c->FI = (uint2 *)(s + L.FI); c->FO = (uint2 *)(s + L.FO); c->RI = (uint4 *)(s + L.RI); c->RO = (uint4 *)(s + L.RO);
-    c->EPS8 = (uint2 *)(s + L.EPS8); c->RI8 = (uint32_t *)(s + L.RI8); c->RO8 = (uint32_t *)(s + L.RO8);
-    c->in_owner = (uint16_t *)(s + L.in_owner); c->out_owner = (uint16_t *)(s + L.out_owner);
-    c->ri_cnt = (uint16_t *)(s + L.ri_cnt); c->ro_cnt = (uint16_t *)(s + L.ro_cnt);
-    c->ri_csr = (uint16_t *)(s + L.ri_csr); c->ro_csr = (uint16_t *)(s + L.ro_csr);
-    c->in_csr_off = (uint16_t *)(s + L.in_csr_off); c->in_csr_idx = (uint16_t *)(s + L.in_csr_idx);
-    c->out_csr_off = (uint16_t *)(s + L.out_csr_off); c->out_csr_idx = (uint16_t *)(s + L.out_csr_idx);
+    c->EPS8 = (uint2 *)(s + L.EPS8);
     c->counters = (unsigned int *)(s + L.counters); c->cnt = (unsigned long long *)(s + L.cnt);
     c->napart = L.napart; c->npart_cap = L.npart_cap;
-    c->nri = T.nri; c->nro = T.nro;
-    c->n_in_csr = (int)T.in_csr_idx.size(); c->n_out_csr = T.out_ncsr;
 
-    CK(upload(c->FI, T.FI, c->st)); CK(upload(c->FO, T.FO, c->st)); CK(upload(c->RI, T.RI, c->st)); CK(upload(c->RO, T.RO, c->st));
-    CK(upload(c->EPS8, T.EPS8, c->st)); CK(upload(c->RI8, T.RI8, c->st)); CK(upload(c->RO8, T.RO8, c->st));
-    CK(upload(c->in_owner, T.in_owner, c->st)); CK(upload(c->out_owner, T.out_owner, c->st));
-    CK(upload(c->ri_cnt, T.ri_cnt, c->st)); CK(upload(c->ro_cnt, T.ro_cnt, c->st));
-    CK(upload(c->ri_csr, T.ri_csr, c->st)); CK(upload(c->ro_csr, T.ro_csr, c->st));
-    CK(upload(c->in_csr_off, T.in_csr_off, c->st)); CK(upload(c->in_csr_idx, T.in_csr_idx, c->st));
-    CK(upload(c->out_csr_off, T.out_csr_off, c->st)); CK(upload(c->out_csr_idx, T.out_csr_idx, c->st));
+    CK(upload(c->EPS8, T.EPS8, c->st));
+    CK(upload_side(s, T.in, L.in, c->gin, c->st));
+    CK(upload_side(s, T.out, L.out, c->gout, c->st));
     CK(cudaMemsetAsync(c->c, 0, 8, c->st));                  // c[0] is never written by k_out_final
     uint32_t hb[BA_NMAX_I + 1][BA_NMAX_I + 1];
     for (int a = 0; a <= BA_NMAX_I; a++)
@@ -302,28 +338,14 @@ static int finish_create(ba_ctx *c) {
     CK(cudaGetDevice(&dev));
     CK(cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev));
     c->block = BA_NT;
-    c->smem_in = enum_in_smem(c->m, c->n_in_csr, c->nri).total;
-    c->smem_out = enum_out_smem(c->m, c->n_out_csr, c->nro).total;
-    {   // MaxDynamicSharedMemorySize is per-function state shared by every ctx of the process: only ever raise it,
-        // so that a ctx with a narrower low tile (n < 8) cannot shrink what a live n >= 8 ctx launches with
-        static std::mutex mu;
-        static size_t max_in = 0, max_out = 0;
-        std::lock_guard<std::mutex> lk(mu);
-        if (c->smem_in > max_in) max_in = c->smem_in;
-        if (c->smem_out > max_out) max_out = c->smem_out;
-        CK(cudaFuncSetAttribute(k_enum_in<IN_SWEEP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_in));
-        CK(cudaFuncSetAttribute(k_enum_in<IN_HC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_in));
-        CK(cudaFuncSetAttribute(k_enum_in<IN_DEBUG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_in));
-        CK(cudaFuncSetAttribute(k_enum_in<IN_COUNT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_in));
-        CK(cudaFuncSetAttribute(k_enum_out<OUT_SWEEP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_out));
-        CK(cudaFuncSetAttribute(k_enum_out<OUT_DEBUG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_out));
-        CK(cudaFuncSetAttribute(k_enum_out<OUT_COUNT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)max_out));
-    }
+    c->smem_in = enum_in_smem(c->gin.nr).total;
+    c->smem_out = enum_out_smem(c->gout.nr).total;
+    CK(raise_smem_limits(c->smem_in, c->smem_out));
     int occ_in = 1, occ_out = 1;
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_in, k_enum_in<IN_SWEEP>, c->block, c->smem_in));
     CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_out, k_enum_out<OUT_SWEEP>, c->block, c->smem_out));
     if (occ_in < 1 || occ_out < 1) return fail(c, BA_ECUDA, "ENUM kernels do not fit on an SM");
-    size_t items_in = (size_t)1 << c->h, items_out = ((size_t)2 << c->h) - 1;
+    size_t items_in = (size_t)2 << c->h, items_out = 2 * (((size_t)2 << c->h) - 1);      // (high part, list) pairs
     size_t gi = (size_t)c->num_sms * occ_in, go = (size_t)c->num_sms * occ_out;
     c->grid_in = (int)(items_in < gi ? items_in : gi);
     c->grid_out = (int)(items_out < go ? items_out : go);
@@ -427,19 +449,15 @@ extern "C" int ba_set_mode(ba_ctx *c, int mode) {
 // ------------------------------------------------------------------------------------------------ launches
 static InArgs make_in_args(ba_ctx *c) {
     InArgs a;
-    a.kc = c->kc;
-    a.FI = c->FI; a.RI = c->RI; a.EPS8 = c->EPS8; a.RI8 = c->RI8; a.ri_cnt = c->ri_cnt; a.ri_csr = c->ri_csr; a.nri = c->nri; a.owner = c->in_owner;
-    a.csr_off = c->in_csr_off; a.csr_idx = c->in_csr_idx; a.ncsr = c->n_in_csr;
-    a.c = c->c; a.p = c->p; a.Hc = c->Hc; a.D = c->D; a.part = c->part;
+    a.kc = c->kc; a.g = c->gin; a.EPS8 = c->EPS8;
+    a.c = c->c; a.S = c->S;
     a.counter = c->counters; a.sym = 0; a.dbg_x = 0; a.dbg_out = nullptr; a.cnt = c->cnt;
     return a;
 }
 
 static OutArgs make_out_args(ba_ctx *c) {
     OutArgs a;
-    a.kc = c->kc; a.EPS8 = c->EPS8; a.RO8 = c->RO8;
-    a.FO = c->FO; a.RO = c->RO; a.ro_cnt = c->ro_cnt; a.ro_csr = c->ro_csr; a.nro = c->nro; a.owner = c->out_owner;
-    a.csr_off = c->out_csr_off; a.csr_idx = c->out_csr_idx; a.ncsr = c->n_out_csr;
+    a.kc = c->kc; a.g = c->gout; a.EPS8 = c->EPS8;
     a.p = c->p; a.Apart = c->Apart; a.counter = c->counters + 4; a.sym = 0; a.dbg_item = 0; a.dbg_cz = 0; a.dbg_out = nullptr;
     a.cnt = c->cnt + 2;
     return a;
@@ -452,6 +470,8 @@ static int ensure_hc(ba_ctx *c) {
     InArgs a = make_in_args(c);
     a.sym = c->sym;
     k_enum_in<IN_HC><<<c->grid_in, c->block, c->smem_in, c->st>>>(a);
+    CK(cudaGetLastError());
+    k_hc_final<<<c->num_sms * 8, 256, 0, c->st>>>(c->NX, c->S, c->S + c->NX, c->Hc, c->sym);
     CK(cudaGetLastError());
     c->hc_ready = true;
     return BA_OK;
@@ -483,13 +503,16 @@ static int launch_out_sweep(ba_ctx *c) {
 }
 
 static int launch_in_sweep(ba_ctx *c, size_t *npart) {
+    int nb = c->num_sms * BA_FINAL_BLOCKS_PER_SM;
+    if ((size_t)nb > c->NX / 256 + 1) nb = (int)(c->NX / 256 + 1);
     if (c->mode == BA_MODE_ENUM) {
         CK(cudaMemsetAsync(c->counters, 0, 4, c->st));
         InArgs a = make_in_args(c);
         a.sym = c->sym;
         k_enum_in<IN_SWEEP><<<c->grid_in, c->block, c->smem_in, c->st>>>(a);
         CK(cudaGetLastError());
-        *npart = (size_t)1 << (c->h - c->sym);
+        k_in_final<<<nb, 256, 0, c->st>>>(c->NX, c->Hc, c->S, c->S + c->NX, c->p, c->D, c->part, c->sym);
+        CK(cudaGetLastError());
     } else {
         double *buf0 = c->Apart, *buf1 = c->Apart + (((size_t)2 << c->n) + 64);
         const double *in = c->c + 1;                          // c is stored by code: idx(y) = code(y) - 1
@@ -500,12 +523,10 @@ static int launch_in_sweep(ba_ctx *c, size_t *npart) {
             in = out;
             out = (out == buf0) ? buf1 : buf0;
         }
-        int nb = c->num_sms * 8;
-        if ((size_t)nb > c->NX / 256 + 1) nb = (int)(c->NX / 256 + 1);
-        k_fast_D<<<nb, 256, 0, c->st>>>(c->NX, c->Hc, in, c->p, c->D, c->part);
+        k_in_final<<<nb, 256, 0, c->st>>>(c->NX, c->Hc, in, nullptr, c->p, c->D, c->part, 0);
         CK(cudaGetLastError());
-        *npart = (size_t)nb;
     }
+    *npart = (size_t)nb;
     return BA_OK;
 }
 
@@ -592,9 +613,11 @@ extern "C" int ba_stats(ba_ctx *c, double *log2Z, long long *iters_done) {
 extern "C" int ba_get_history(ba_ctx *c, int count, double *out) {
     if (!c || !out || count < 0) return c ? fail(c, BA_EINVAL, "ba_get_history: bad argument") : BA_EINVAL;
     if ((long long)count > c->iters || count > BA_HIST_CAP) return fail(c, BA_EINVAL, "ba_get_history: count too large");
-    for (int i = 0; i < count; i++) {
-        const int slot = (int)((c->iters - count + i) % BA_HIST_CAP);
-        CK(cudaMemcpyAsync(out + 3 * i, c->hist + 3 * slot, 24, cudaMemcpyDeviceToHost, c->st));
+    if (count > 0) {                                        // the ring wraps at most once: one or two contiguous copies
+        const int first = (int)((c->iters - count) % BA_HIST_CAP);
+        const int n1 = (first + count <= BA_HIST_CAP) ? count : BA_HIST_CAP - first;
+        CK(cudaMemcpyAsync(out, c->hist + 3 * (size_t)first, (size_t)n1 * 24, cudaMemcpyDeviceToHost, c->st));
+        if (n1 < count) CK(cudaMemcpyAsync(out + 3 * (size_t)n1, c->hist, (size_t)(count - n1) * 24, cudaMemcpyDeviceToHost, c->st));
     }
     CK(cudaStreamSynchronize(c->st));
     return BA_OK;
@@ -649,7 +672,7 @@ extern "C" int ba_debug_emb_row(ba_ctx *c, unsigned x, unsigned *emb_out) {
     if (e == cudaSuccess) {
         InArgs a = make_in_args(c);
         a.dbg_x = x; a.dbg_out = dev;
-        k_enum_in<IN_DEBUG><<<1, c->block, c->smem_in, c->st>>>(a);
+        k_enum_in<IN_DEBUG><<<2, c->block, c->smem_in, c->st>>>(a);      // one CTA per list
         e = cudaGetLastError();
     }
     if (e == cudaSuccess) e = cudaMemcpyAsync(emb_out, dev, c->NY * 4, cudaMemcpyDeviceToHost, c->st);

@@ -16,14 +16,23 @@
 //   emb(y'.z, u.v) = sum_{s>=0} alpha_s * B_s,   B_s = B(sigma_s.z, v) = emb(sigma_s.z, v),
 // sigma_s = last s symbols of y'.  B_s = 0 implies B_{s+1} = 0, and B_s = 0 for s > m - |z|.
 //
+// LISTS.  The non-empty z are split by their first symbol b (list b); a node carries list b iff b is in its mask.
+// A work item of either sweep is a (high part, list) pair: it visits the nodes that carry the list.
+//
 // CLASSES.  The B_s of a pair depend on the node only through sigma.  Nodes are grouped by their CLASS
-// cls = code(y') & (2^BA_KB - 1) (the last BA_KB symbols) and processed in runs of one class, so the
-// B_0..B_3 of every pair are constants of the run: each thread loads the BA_C pairs of a chunk once
-// (class-specific FAST table, global memory / L2) and then loops over the nodes of the run with
-//   emb = a0*B0 + a1*B1 + a2*B2 + a3*B3        (4 IMAD, no unpacking, no links, no votes)
-// A pair whose chain reaches s = BA_KB under the class (3.4 % of the pairs) is DEEP: it is left out of
-// the class's fast table and handled as a RIDER, one rider per thread: B_0..B_4 static, B_5..B_8 from a
-// direct table indexed by the sigma bits 4..7.
+// cls = code(y') & (2^BA_KB - 1) (the last BA_KB symbols) and processed in batches of one class, so the
+// B_0..B_3 of every pair are constants of the batch.
+//
+// GROUPS.  Every thread owns, per list, BA_KG groups of BA_GP pair slots.  The pairs of a group share their gathered
+// operand (input sweep: one z, up to 4 different v; output sweep: one v, up to 4 different z), which is fetched from
+// the staged row ONCE per node (LDS.64) and serves the group's terms; every slot has its own FP64 accumulator, kept
+// in a register for the whole work item (static ownership: a slot always belongs to the same (v, z)).  Per term:
+//   emb = a0*B0 + a1*B1 [+ a2*B2 + a3*B3]   1-2 IDP.2A (16-bit alphas x 8-bit B's, two products per instruction)
+//   acc += (double)emb * operand            exact u32 -> f64 (DADD on the magic number 2^52) + DFMA
+// A pair whose chain reaches s = BA_KB under the class (3.4 % of the pairs) is DEEP: its slot holds B = 0 under that
+// class and it is handled as a RIDER, one rider per thread: B_0..B_4 static, B_5..B_8 from a direct table indexed by
+// the sigma bits 4..7.  When an alpha of the batch does not fit 16 bits (possible for n >= 27 only) the batch runs a
+// generic IMAD loop instead.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -36,23 +45,15 @@
 #define BA_P_FLOOR 9.3326361850321888e-302   // 2^-1000 (G8)
 
 #define BA_NT 512            // threads per CTA of the ENUM kernels (one CTA per SM)
-#define BA_C 5               // pairs per chunk
-#define BA_NC 3              // chunk slots per thread and list
+#define BA_KG 4              // groups per thread and list
+#define BA_GP 4              // pair slots per group
+#define BA_NSLOT (BA_KG * BA_GP)
 #define BA_KB 4              // class bits
 #define BA_NCLS 16           // 2^BA_KB classes
+#define BA_ROWB 2048u        // bytes between staged operand rows (2^BA_MLOW doubles)
 #define BA_RB_IN 32          // nodes per batch, input sweep (operand half-rows of 2^m doubles)
 #define BA_SBR 3             // input sweep: phase-A rounds (of BA_NT nodes) per super-batch
 #define BA_RB_OUT 32         // nodes per batch, output sweep (operand rows of 2^m doubles)
-
-// ---- v-major prepend links Wv (host side only: the table builder walks them; the kernels read the direct
-// tables EPS8 / RI8 / RO8 instead): one uint32 per entry of v's list ([0] null, [1] empty string, then the
-// non-empty subsequences of v):  W = l0 | cB0 << 8 | l1 << 16 | cB1 << 24,  l_b = local index of b.z in
-// v's list (0 = null: b.z is not a subsequence of v), cB_b = B(b.z, v).
-// ---- fast pairs: uint2 {B0 | B1<<8 | B2<<16 | B3<<24, byte offset of the operand in the staged row}
-//   [class][list b][slot c][pair q][thread]; slot (b,c,thread) always belongs to the same v (input sweep)
-//   or z (output sweep), so its FP64 accumulator lives in a register for the whole work item.  Within a
-//   half-warp the offsets of one (class,b,c,q) are dealt to distinct 8-byte bank pairs where possible.
-// ---- riders: uint4 {B0..B3, B4 | link4 << 8 | owner << 16, row byte offset, byte offset of v's list in Wv}
 
 struct KConst {                       // passed by value to kernels
     int n, m, h;
@@ -68,10 +69,38 @@ struct NodeRec {                      // 48 bytes, shared memory
     uint32_t pad;
 };
 
-// Position of operand number `pos` in a staged row: bits 1..3 are XORed with bits 4..6, so that operands
-// whose numbers agree in the low four bits (the strings sharing their last symbols) spread over the 8-byte bank
-// pairs.  An involution that keeps the two operands of a 16-byte piece together.
-__host__ __device__ __forceinline__ uint32_t ba_swz(uint32_t pos) { return pos ^ (((pos >> 4) & 7u) << 1); }
+// A node of a staged batch as the hot loops read it: alphas as 16-bit halves (IDP.2A operands), 32 bytes.
+struct BalRec {
+    uint32_t a01, a23, a45, a67, a8;  // alpha_0 | alpha_1 << 16, ...; garbage when `big`
+    uint32_t big;                     // != 0: an alpha of the node needs more than 16 bits
+    uint32_t id;                      // NodeRec::id
+    uint32_t node;                    // index of the NodeRec
+};
+
+__device__ __forceinline__ BalRec ba_make_bal(const NodeRec &rc, uint32_t node) {
+    BalRec bl;
+    bl.a01 = rc.a[0] | (rc.a[1] << 16); bl.a23 = rc.a[2] | (rc.a[3] << 16);
+    bl.a45 = rc.a[4] | (rc.a[5] << 16); bl.a67 = rc.a[6] | (rc.a[7] << 16);
+    bl.a8 = rc.a[8];
+    bl.big = (rc.a[0] | rc.a[1] | rc.a[2] | rc.a[3] | rc.a[4] | rc.a[5] | rc.a[6] | rc.a[7]) >> 16;
+    bl.id = rc.id; bl.node = node;
+    return bl;
+}
+
+// The schedule of one side, device pointers (host side: GroupSide in ba_tables.h)
+struct GroupDev {
+    const uint4 *GB;                  // [cls][b][k][tid]
+    const uint32_t *GA;               // [b][k][tid]
+    const uint16_t *GO;               // [b][k][q][tid]
+    const uint8_t *GW;                // [b][warp]
+    const uint16_t *csr_off;          // [b][nown + 1]
+    const uint16_t *csr_idx;          // [b][BA_NSLOT * BA_NT]
+    const uint4 *R;                   // riders [cls][b][nr]
+    const uint16_t *r_cnt;            // [cls][b]
+    const uint16_t *r_csr;            // [cls][b][nown + 1]
+    const uint32_t *R8;               // [cls][b][16][nr]
+    int nr, nown;
+};
 
 __device__ __forceinline__ int ba_len_of_code(uint32_t code) { return 31 - __clz(code); }
 
@@ -86,14 +115,14 @@ __device__ __forceinline__ int ba_nextpos(uint32_t s, int L, int from, uint32_t 
 
 // ---- shared-memory and async-copy primitives ---------------------------------------------------
 __device__ __forceinline__ uint32_t ba_smem_addr(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ uint32_t ba_lds_u16(uint32_t addr) {
-    uint16_t v;
-    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(addr));
-    return (uint32_t)v;
-}
 __device__ __forceinline__ uint2 ba_lds_v2(uint32_t addr) {
     uint2 v;
     asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ uint4 ba_lds_v4(uint32_t addr) {
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
     return v;
 }
 __device__ __forceinline__ double ba_lds_f64(uint32_t addr) {
@@ -123,74 +152,103 @@ __device__ __forceinline__ void ba_mbar_arrive(uint32_t addr) {
 __device__ __forceinline__ void ba_mbar_arrive_on_copies(uint32_t addr) {      // arrives when this thread's cp.async landed
     asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(addr) : "memory");
 }
+// A lost arrival must fail loudly, not hang the device: trap after ~20 s of SM clocks (far beyond any batch, also
+// under a profiler's replay or a preempted context, where a poll count would be reached much sooner than a clock).
 __device__ __forceinline__ void ba_mbar_wait(uint32_t addr, uint32_t parity) {
     uint32_t done = 0;
+    long long t0 = 0;
     for (uint32_t spin = 0; !done; spin++) {
         asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
                      : "=r"(done) : "r"(addr), "r"(parity) : "memory");
-        if (spin > (1u << 26)) __trap();                    // a lost arrival must fail loudly, not hang the device
+        if (!done && (spin & 0xfffu) == 0xfffu) {
+            const long long now = clock64();
+            if (t0 == 0) t0 = now;
+            else if (now - t0 > 40000000000ll) __trap();
+        }
     }
 }
 
-// exact uint32 -> FP64 on the FP64 pipe (a DADD) instead of the quarter-rate conversion unit
+// exact uint32 -> FP64 on the FP64 pipe (a DADD on the magic number 2^52) instead of the quarter-rate conversion unit
 __device__ __forceinline__ double ba_u2d(uint32_t e) {
     return __hiloint2double(0x43300000, (int)e) - 4503599627370496.0;
 }
 
-// Pair positions q of a chunk whose int->FP64 conversion goes to the conversion unit (I2F on the XU pipe)
-// instead of the FP64 pipe: spreads the per-term conversion over two otherwise idle/half-rate pipes.
-#ifndef BA_CVT_XU_MASK
-#define BA_CVT_XU_MASK 0x0a
-#endif
-template <int Q>
-__device__ __forceinline__ double ba_cvt(uint32_t e) {
-    if ((BA_CVT_XU_MASK >> Q) & 1) return __uint2double_rn(e);
-    return ba_u2d(e);
-}
-
-// The hot loop of both sweeps: the BA_C pairs of one chunk (bp = B_0 | B_1<<8 | B_2<<16 | B_3<<24, ad = byte
-// offset of the operand in a staged row) against the `len` nodes of a batch (bal[i] = alpha_0..3, operand
-// rows at rowbase + i*ROWB).  NS = number of B_s that can be non-zero in this warp's pairs (depth + 1).
-template <int NS>
-__device__ __forceinline__ double ba_fast_loop(double s, const uint4 *bal, uint32_t rowbase, uint32_t ROWB, int len,
-                                               const uint32_t (&bp)[BA_C], const uint32_t (&ad)[BA_C]) {
-    uint32_t B0[BA_C], B1[BA_C], B2[BA_C], B3[BA_C];
-#pragma unroll
-    for (int q = 0; q < BA_C; q++) {
-        B0[q] = bp[q] & 0xffu; B1[q] = (bp[q] >> 8) & 0xffu; B2[q] = (bp[q] >> 16) & 0xffu; B3[q] = bp[q] >> 24;
-    }
-    double s2 = 0.0;                                        // two dependent-FMA chains instead of one
+// The hot loop of both sweeps: the BA_KG x BA_GP pair slots of a thread (Bp = B_0 | B_1<<8 | B_2<<16 | B_3<<24 of the
+// slot, rb[k] = shared-memory address of group k's operand in the first staged row) against the `len` nodes of a batch
+// (bal = shared-memory address of the batch's BalRec array, rows BA_ROWB bytes apart).  TYPE 2: no slot of the warp
+// has B_2 or B_3.
+template <int TYPE, int KMAX>
+__device__ __forceinline__ void ba_group_loop(double (&acc)[BA_NSLOT], const uint32_t (&Bp)[BA_NSLOT], const uint32_t (&rb)[BA_KG],
+                                              uint32_t bal, int len) {
 #pragma unroll 2
     for (int i = 0; i < len; i++) {
-        const uint4 al = bal[i];
-        const uint32_t rb = rowbase + (uint32_t)i * ROWB;
+        uint2 a;
+        if (TYPE == 2) { asm volatile("ld.shared.u32 %0, [%1];" : "=r"(a.x) : "r"(bal + (uint32_t)i * 32u)); a.y = 0u; }
+        else a = ba_lds_v2(bal + (uint32_t)i * 32u);
 #pragma unroll
-        for (int q = 0; q < BA_C; q++) {
-            uint32_t emb = al.x * B0[q];
-            if (NS >= 2) emb += al.y * B1[q];
-            if (NS >= 3) emb += al.z * B2[q];
-            if (NS >= 4) emb += al.w * B3[q];
-            const double e = (q == 0) ? ba_cvt<0>(emb) : (q == 1) ? ba_cvt<1>(emb) : (q == 2) ? ba_cvt<2>(emb)
-                           : (q == 3) ? ba_cvt<3>(emb) : ba_cvt<4>(emb);
-            if (q & 1) s2 = fma(e, ba_lds_f64(rb + ad[q]), s2);
-            else s = fma(e, ba_lds_f64(rb + ad[q]), s);
+        for (int k = 0; k < KMAX; k++) {
+            const double op = ba_lds_f64(rb[k] + (uint32_t)i * BA_ROWB);
+#pragma unroll
+            for (int q = 0; q < BA_GP; q++) {
+                uint32_t e = __dp2a_lo(a.x, Bp[k * BA_GP + q], 0u);
+                if (TYPE == 4) e = __dp2a_hi(a.y, Bp[k * BA_GP + q], e);
+                acc[k * BA_GP + q] = fma(ba_u2d(e), op, acc[k * BA_GP + q]);
+            }
         }
     }
-    return s + s2;
 }
 
-// Dispatch on the warp-uniform depth of the chunk (B_s = 0 implies B_{s+1} = 0).
-__device__ __forceinline__ double ba_fast_chunk(double s, const uint4 *bal, uint32_t rowbase, uint32_t ROWB, int len,
-                                                const uint32_t (&bp)[BA_C], const uint32_t (&ad)[BA_C]) {
-    uint32_t any = 0;
+// The same with the 32-bit alphas of the node records: batches holding an alpha >= 2^16 (n >= 27 only).
+__device__ __forceinline__ void ba_group_loop_wide(double (&acc)[BA_NSLOT], const uint32_t (&Bp)[BA_NSLOT], const uint32_t (&rb)[BA_KG],
+                                                   const BalRec *bal, const NodeRec *rec, int len, int kmax) {
+    for (int i = 0; i < len; i++) {
+        const uint4 a = *(const uint4 *)&rec[bal[i].node].a[0];
 #pragma unroll
-    for (int q = 0; q < BA_C; q++) any |= bp[q];
-    any = __reduce_or_sync(0xffffffffu, any);
-    if (!any) return s;                                     // no pair of this warp in the slot
-    if (any >> 24) return ba_fast_loop<4>(s, bal, rowbase, ROWB, len, bp, ad);
-    if (any >> 16) return ba_fast_loop<3>(s, bal, rowbase, ROWB, len, bp, ad);
-    if (any >> 8) return ba_fast_loop<2>(s, bal, rowbase, ROWB, len, bp, ad);
-    return ba_fast_loop<1>(s, bal, rowbase, ROWB, len, bp, ad);
+        for (int k = 0; k < BA_KG; k++) {
+            if (k >= kmax) break;
+            const double op = ba_lds_f64(rb[k] + (uint32_t)i * BA_ROWB);
+#pragma unroll
+            for (int q = 0; q < BA_GP; q++) {
+                const uint32_t bp = Bp[k * BA_GP + q];
+                const uint32_t e = a.x * (bp & 0xffu) + a.y * ((bp >> 8) & 0xffu) + a.z * ((bp >> 16) & 0xffu) + a.w * (bp >> 24);
+                acc[k * BA_GP + q] = fma(ba_u2d(e), op, acc[k * BA_GP + q]);
+            }
+        }
+    }
+}
+
+// Dispatch on the warp's static (type, levels) and on whether the batch's alphas fit 16 bits.
+__device__ __forceinline__ void ba_group_batch(double (&acc)[BA_NSLOT], const uint32_t (&Bp)[BA_NSLOT], const uint32_t (&rb)[BA_KG],
+                                               const BalRec *bal, const NodeRec *rec, int len, int wmeta, bool big) {
+    const int kmax = wmeta & 15, type = wmeta >> 4;
+    if (kmax == 0) return;
+    if (big) { ba_group_loop_wide(acc, Bp, rb, bal, rec, len, kmax); return; }
+    const uint32_t al16 = ba_smem_addr(bal);
+    if (type == 2) {
+        if (kmax == 4) ba_group_loop<2, 4>(acc, Bp, rb, al16, len);
+        else if (kmax == 3) ba_group_loop<2, 3>(acc, Bp, rb, al16, len);
+        else if (kmax == 2) ba_group_loop<2, 2>(acc, Bp, rb, al16, len);
+        else ba_group_loop<2, 1>(acc, Bp, rb, al16, len);
+    } else {
+        if (kmax == 4) ba_group_loop<4, 4>(acc, Bp, rb, al16, len);
+        else if (kmax == 3) ba_group_loop<4, 3>(acc, Bp, rb, al16, len);
+        else if (kmax == 2) ba_group_loop<4, 2>(acc, Bp, rb, al16, len);
+        else ba_group_loop<4, 1>(acc, Bp, rb, al16, len);
+    }
+}
+
+// Full chain of a pair with all nine B_s (the pair (v, empty) and the riders): alphas as 16-bit halves
+// a01, a23, a45, a67 and alpha_8; B packed B_0..B_3, B_4..B_7, B_8.
+__device__ __forceinline__ uint32_t ba_chain9(uint32_t a01, uint32_t a23, uint32_t a45, uint32_t a67, uint32_t a8,
+                                              uint32_t b0123, uint32_t b4567, uint32_t b8) {
+    uint32_t e = __dp2a_lo(a01, b0123, a8 * b8);
+    e = __dp2a_hi(a23, b0123, e);
+    e = __dp2a_lo(a45, b4567, e);
+    return __dp2a_hi(a67, b4567, e);
+}
+__device__ __forceinline__ uint32_t ba_chain9_wide(const uint32_t *a, uint32_t b0123, uint32_t b4567, uint32_t b8) {
+    return a[0] * (b0123 & 0xffu) + a[1] * ((b0123 >> 8) & 0xffu) + a[2] * ((b0123 >> 16) & 0xffu) + a[3] * (b0123 >> 24) +
+           a[4] * (b4567 & 0xffu) + a[5] * ((b4567 >> 8) & 0xffu) + a[6] * ((b4567 >> 16) & 0xffu) + a[7] * (b4567 >> 24) + a[8] * b8;
 }
 
 // Stable rank of every thread's key among the CTA (keys < NKEY; key < 0 = not ranked): order[pos] = tid with

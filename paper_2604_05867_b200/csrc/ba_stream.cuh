@@ -84,20 +84,26 @@ __global__ void k_fill(size_t N, double *__restrict__ a, double v) {
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (size_t)gridDim.x * blockDim.x) a[i] = v;
 }
 
-// FAST mode epilogue of the input sweep: D = Hc - S and the first-stage reductions, one triple per block.
-__global__ void __launch_bounds__(256) k_fast_D(size_t NX, const double *__restrict__ Hc, const double *__restrict__ S,
-                                                const double *__restrict__ p, double *__restrict__ D,
-                                                double *__restrict__ part) {
+// Epilogue of the input sweep: D = Hc - (S0 + S1) and the first-stage reductions, one triple per block.
+// ENUM mode: S0, S1 are the partial sums of the two lists (ba_enum_in.cuh); FAST mode: S0 is complete, S1 = null.
+// sym (complement symmetry, Theorem 4): only x < NX/2 was enumerated; D(~x) = D(x) and p(~x) = p(x) bit for bit,
+// so the mirrored half enters the sums by doubling.
+__global__ void __launch_bounds__(256) k_in_final(size_t NX, const double *__restrict__ Hc, const double *__restrict__ S0,
+                                                  const double *__restrict__ S1, const double *__restrict__ p,
+                                                  double *__restrict__ D, double *__restrict__ part, int sym) {
     __shared__ double sr[3 * 8];
     double r0 = 0.0, r1 = -INFINITY, r2 = 0.0;
     // fixed assignment: block b handles the contiguous chunk [b*chunk, (b+1)*chunk)
-    const size_t chunk = (NX + gridDim.x - 1) / gridDim.x;
-    const size_t lo = (size_t)blockIdx.x * chunk, hi = (lo + chunk < NX) ? lo + chunk : NX;
+    const size_t NE = sym ? NX / 2 : NX;
+    const size_t chunk = (NE + gridDim.x - 1) / gridDim.x;
+    const size_t lo = (size_t)blockIdx.x * chunk, hi = (lo + chunk < NE) ? lo + chunk : NE;
     for (size_t i = lo + threadIdx.x; i < hi; i += blockDim.x) {
-        const double Dx = Hc[i] - S[i];
+        const double Dx = Hc[i] - (S1 ? S0[i] + S1[i] : S0[i]);
         D[i] = Dx;
         const double px = p[i];
-        r0 += px * Dx; r1 = fmax(r1, Dx); r2 += px * exp2(Dx);
+        double t0 = px * Dx, t2 = px * exp2(Dx);
+        if (sym) { D[NX - 1 - i] = Dx; t0 += t0; t2 += t2; }
+        r0 += t0; r1 = fmax(r1, Dx); r2 += t2;
     }
     for (int o = 16; o > 0; o >>= 1) {
         r0 += __shfl_xor_sync(0xffffffffu, r0, o);
@@ -111,5 +117,15 @@ __global__ void __launch_bounds__(256) k_fast_D(size_t NX, const double *__restr
         double t0 = 0.0, t1 = -INFINITY, t2 = 0.0;
         for (int w = 0; w < (int)(blockDim.x >> 5); w++) { t0 += sr[w * 3]; t1 = fmax(t1, sr[w * 3 + 1]); t2 += sr[w * 3 + 2]; }
         part[(size_t)blockIdx.x * 3] = t0; part[(size_t)blockIdx.x * 3 + 1] = t1; part[(size_t)blockIdx.x * 3 + 2] = t2;
+    }
+}
+
+// Hc = H_0 + H_1 (the two lists of the one-off IN_HC pass), mirrored under complement symmetry.
+__global__ void k_hc_final(size_t NX, const double *__restrict__ H0, const double *__restrict__ H1, double *__restrict__ Hc, int sym) {
+    const size_t NE = sym ? NX / 2 : NX;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < NE; i += (size_t)gridDim.x * blockDim.x) {
+        const double v = H0[i] + H1[i];
+        Hc[i] = v;
+        if (sym) Hc[NX - 1 - i] = v;
     }
 }

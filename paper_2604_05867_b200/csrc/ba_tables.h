@@ -7,32 +7,27 @@
 #include <utility>
 #include <vector>
 
+// One side (input sweep or output sweep) of the pair schedule, see ba_internal.h "GROUPS".
+struct GroupSide {
+    std::vector<uint4> GB;          // [BA_NCLS][2][BA_KG][BA_NT]: B_0 | B_1<<8 | B_2<<16 | B_3<<24 of the group's 4 slots
+    std::vector<uint32_t> GA;       // [2][BA_KG][BA_NT]: byte offset of the group's operand in a staged row
+    std::vector<uint16_t> GO;       // [2][BA_KG][BA_GP][BA_NT]: owner of the slot (in: v, out: code(z)); 0xffff = unused
+    std::vector<uint8_t> GW;        // [2][BA_NT/32]: levels of the warp (0..BA_KG) | loop type << 4 (2: B_2 = B_3 = 0 always, 4)
+    std::vector<uint16_t> csr_off;  // [2][nown + 1]: slots of an owner, per list
+    std::vector<uint16_t> csr_idx;  // [2][BA_KG*BA_GP*BA_NT]: slot index (k*BA_GP + q)*BA_NT + tid
+    int nown = 0;                   // in: 2^m ; out: 2^{m+1} (by code(z))
+    std::vector<uint4> R;           // riders [BA_NCLS][2][nr]: {B0..B3, B4 | owner << 16, row byte offset, 0}, sorted by owner
+    std::vector<uint16_t> r_cnt;    // [BA_NCLS][2]
+    std::vector<uint16_t> r_csr;    // [BA_NCLS][2][nown + 1] rider range of an owner
+    std::vector<uint32_t> R8;       // [BA_NCLS][2][16][nr]: bytes = B_5..B_8 of the rider for sigma bits 4..7
+    int nr = 0;
+    unsigned long long npairs[2] = {0, 0}, nslots[2] = {0, 0}, ngroups[2] = {0, 0};   // statistics
+};
+
 struct TileTables {
     int m = 0, nv = 0;
-    std::vector<uint32_t> Wv;          // v-major prepend links (chain walks): entry vbase[v] + local index
-    std::vector<uint32_t> vbase;       // [nv] entry index of v's list (its null entry)
-    // ---- input sweep: v-major ownership, slot (b, c, tid) <-> v
-    std::vector<uint2> FI;             // [BA_NCLS][2][BA_NC][BA_C][BA_NT] fast pairs
-    std::vector<uint16_t> in_owner;    // [2][BA_NC][BA_NT] v of the slot, 0xffff = unused
-    std::vector<uint16_t> in_csr_off;  // [nv + 1]
-    std::vector<uint16_t> in_csr_idx;  // accumulator slots (b*BA_NC + c)*BA_NT + tid of v's chunks
-    std::vector<uint4> RI;             // [BA_NCLS][2][nri] riders (deep pairs), sorted by v
-    std::vector<uint16_t> ri_cnt;      // [BA_NCLS][2]
-    std::vector<uint16_t> ri_csr;      // [BA_NCLS][2][nv + 1] rider range of v
-    int nri = 0;
-    std::vector<uint2> EPS8;           // [256][nv]: bytes s-1 = B(sigma_s, v), s = 1..8, sigma = the row index
-    std::vector<uint32_t> RI8;         // [BA_NCLS][2][16][nri]: bytes = B_5..B_8 of the rider for sigma bits 4..7
-    // ---- output sweep: z-major ownership per class, slot (cls, b, c, tid) <-> code(z)
-    std::vector<uint2> FO;             // [BA_NCLS][2][BA_NC][BA_C][BA_NT]
-    std::vector<uint16_t> out_owner;   // [BA_NCLS][2][BA_NC][BA_NT] code(z) of the slot, 0xffff = unused
-    std::vector<uint16_t> out_csr_off; // [BA_NCLS][2^{m+1}] by code(z) - 1 (entry 0, the empty z, has no chunks)
-    std::vector<uint16_t> out_csr_idx; // [BA_NCLS][out_ncsr]
-    int out_ncsr = 0;
-    std::vector<uint4> RO;             // [BA_NCLS][2][nro] riders, sorted by code(z)
-    std::vector<uint16_t> ro_cnt;      // [BA_NCLS][2]
-    std::vector<uint16_t> ro_csr;      // [BA_NCLS][2][2^{m+1} + 1] rider range of code(z)
-    int nro = 0;
-    std::vector<uint32_t> RO8;         // [BA_NCLS][2][16][nro]: bytes = B_5..B_8 of the rider for sigma bits 4..7
+    GroupSide in, out;
+    std::vector<uint2> EPS8;        // [256][nv]: bytes s-1 = B(sigma_s, v), s = 1..8, sigma = the row index
     bool ok = false;
 };
 
@@ -42,126 +37,112 @@ static inline uint32_t tt_prepend(uint32_t sig, int s, uint32_t cz) {
     return (1u << (lz + s)) | ((sig & ((1u << s) - 1u)) << lz) | (cz - (1u << lz));
 }
 
-// Logical slot j (slots are dealt heaviest first) -> physical slot (c, tid).  Warp-slots of 32 logical slots go
-// to the warps in snake order, so that the deep chunks of slot column 0 meet the shallow end of column 1 and
-// every warp carries about the same number of IMADs between two barriers.
-static inline void tt_phys(int j, int &c, int &tid) {
-    const int ws = j / 32, nw = BA_NT / 32;
-    c = ws / nw;
-    const int w = (c & 1) ? (nw - 1 - ws % nw) : (ws % nw);
-    tid = w * 32 + j % 32;
-}
+struct TTPair { int v; uint32_t cz; };
 
-// Deal the items of `pool[owner]` to the slots (slot k = (c, tid), k = c*BA_NT + tid, owner slot_owner[k]) and
-// their BA_C pair positions q.  An item is key | depth << 28; key & 15 is the 8-byte bank pair of its operand.
-// The pools arrive sorted by chain depth, deepest first, and only items of the head's depth are candidates, so
-// an owner's deep pairs land in its first slots.  Per (half-warp, q) a bipartite matching lane -> bank pair
-// (augmenting paths, lanes with the fewest options first) picks, where it can, 16 different bank pairs; a local
-// search over swaps then removes most of the remaining conflicts.  emit(k, q, owner, key).
-#define BA_PLACE_WINDOW 12
-template <typename Emit>
-static void tt_place(const std::vector<int> &slot_owner, std::vector<std::vector<uint32_t>> &pool, Emit emit) {
-    const int nslots = (int)slot_owner.size();
-    const uint32_t EMPTY = 0xffffffffu;
-    std::vector<uint32_t> at((size_t)nslots * BA_C, EMPTY);     // at[k*BA_C + q] = item (key | depth << 28)
-    for (int k0 = 0; k0 < nslots; k0 += 16) {
-        for (int q = 0; q < BA_C; q++) {
-            int lanes[16], nl = 0;
-            for (int l = 0; l < 16 && k0 + l < nslots; l++) {
-                const int o = slot_owner[k0 + l];
-                if (o >= 0 && !pool[o].empty()) lanes[nl++] = k0 + l;
-            }
-            if (!nl) continue;
-            int match_res[16];                                  // bank pair -> lane index (into lanes[]) or -1
-            for (int r = 0; r < 16; r++) match_res[r] = -1;
-            uint32_t avail[16];
-            for (int i = 0; i < nl; i++) {
-                uint32_t a = 0;
-                const std::vector<uint32_t> &P = pool[slot_owner[lanes[i]]];
-                for (size_t j = 0; j < P.size() && j < (size_t)BA_PLACE_WINDOW && (P[j] >> 28) == (P[0] >> 28); j++)
-                    a |= 1u << (P[j] & 15u);
-                avail[i] = a;
-            }
-            int order[16];
-            for (int i = 0; i < nl; i++) order[i] = i;
-            std::sort(order, order + nl, [&](int x, int y) { return __builtin_popcount(avail[x]) < __builtin_popcount(avail[y]); });
-            struct Aug {
-                static bool run(int i, uint32_t &seen, const uint32_t *avail, int *match_res) {
-                    for (int r = 0; r < 16; r++) {
-                        if (!((avail[i] >> r) & 1u) || ((seen >> r) & 1u)) continue;
-                        seen |= 1u << r;
-                        if (match_res[r] < 0 || run(match_res[r], seen, avail, match_res)) { match_res[r] = i; return true; }
+// Deal the pairs of one list to (warp, level, lane, slot):
+//   * a GROUP is up to BA_GP pairs that share their gathered operand (`key` = its position in a staged row); the
+//     thread fetches the operand once per node and uses it for the group's pairs;
+//   * groups are of TYPE 2 (no pair of the group ever has B_2 != 0 in a fast slot: one dot-product instruction per
+//     term) or 4; 32 groups of one type, consecutive in operand order, form a LEVEL (one group per lane: their operand
+//     fetch reads neighbouring or equal row positions); a warp carries up to BA_KG levels of ONE type, so that the
+//     node loop is straight-line code chosen per warp;
+//   * warps are filled so that the four schedulers of the SM carry about the same number of instructions.
+template <typename KeyOf, typename OwnerOf, typename BPack, typename DeepOf>
+static bool tt_deal(int m, int b, const std::vector<TTPair> &pairs, KeyOf key_of, OwnerOf owner_of, BPack bpack, DeepOf deep,
+                    GroupSide &S) {
+    struct Grp { int type; uint32_t key; std::vector<int> items; };
+    const int np = (int)pairs.size();
+    std::vector<int> ptype(np, 2);
+    for (int i = 0; i < np; i++)
+        for (int cls = 0; cls < BA_NCLS; cls++)
+            if (!deep(cls, pairs[i]) && (bpack(cls, pairs[i]) >> 16)) ptype[i] = 4;
+    // ---- groups per operand: type-4 pairs first, the type-2 pairs fill up the last type-4 group
+    std::vector<std::vector<int>> by_key(2u << m);
+    for (int i = 0; i < np; i++) by_key[key_of(pairs[i])].push_back(i);
+    std::vector<Grp> groups;
+    for (uint32_t k = 0; k < by_key.size(); k++) {
+        std::vector<int> &L = by_key[k];
+        if (L.empty()) continue;
+        std::stable_sort(L.begin(), L.end(), [&](int x, int y) { return ptype[x] > ptype[y]; });
+        for (size_t i = 0; i < L.size(); i += BA_GP) {
+            Grp g;
+            g.key = k;
+            g.type = ptype[L[i]];
+            for (size_t j = i; j < L.size() && j < i + BA_GP; j++) g.items.push_back(L[j]);
+            groups.push_back(g);
+        }
+    }
+    std::stable_sort(groups.begin(), groups.end(), [](const Grp &x, const Grp &y) { return x.type != y.type ? x.type > y.type : x.key < y.key; });
+    // ---- levels of 32 groups of one type
+    struct Lvl { int type; std::vector<int> g; };
+    std::vector<Lvl> levels;
+    for (size_t i = 0; i < groups.size(); i++) {
+        if (levels.empty() || levels.back().type != groups[i].type || levels.back().g.size() == 32) levels.push_back(Lvl{groups[i].type, {}});
+        levels.back().g.push_back((int)i);
+    }
+    const int NW = BA_NT / 32;
+    int L4 = 0, L2 = 0;
+    for (auto &l : levels) (l.type == 4 ? L4 : L2)++;
+    // ---- warps per type: proportional to the instruction count (5 per term for type 4, 4 for type 2), at least
+    // ceil(levels / BA_KG), all NW warps used
+    int w4 = (L4 + BA_KG - 1) / BA_KG, w2 = (L2 + BA_KG - 1) / BA_KG;
+    if (w4 + w2 > NW) return false;
+    while (w4 + w2 < NW) {
+        const double c4 = w4 ? 5.0 * L4 / w4 : 0.0, c2 = w2 ? 4.0 * L2 / w2 : 0.0;
+        if (c4 >= c2 && L4 > w4) w4++;
+        else if (L2 > w2) w2++;
+        else if (L4 > w4) w4++;
+        else break;
+    }
+    struct Bundle { int type; std::vector<int> lv; double cost; };
+    std::vector<Bundle> bundles;
+    auto split = [&](int type, int nl, int nw, int first) {
+        for (int w = 0; w < nw; w++) {
+            Bundle bd; bd.type = type;
+            const int lo = (int)((long long)nl * w / nw), hi = (int)((long long)nl * (w + 1) / nw);
+            for (int l = lo; l < hi; l++) bd.lv.push_back(first + l);
+            bd.cost = (type == 4 ? 5.0 : 4.0) * (hi - lo);
+            bundles.push_back(bd);
+        }
+    };
+    split(4, L4, w4, 0);
+    split(2, L2, w2, L4);
+    for (auto &bd : bundles) if ((int)bd.lv.size() > BA_KG) return false;
+    // ---- bundles -> warp indices: heaviest first onto the scheduler (warp & 3) with the least load
+    std::stable_sort(bundles.begin(), bundles.end(), [](const Bundle &x, const Bundle &y) { return x.cost > y.cost; });
+    double load[4] = {0, 0, 0, 0};
+    int used[4] = {0, 0, 0, 0};
+    for (auto &bd : bundles) {
+        int best = -1;
+        for (int s = 0; s < 4; s++)
+            if (used[s] < NW / 4 && (best < 0 || load[s] < load[best])) best = s;
+        if (best < 0) return false;
+        const int warp = used[best] * 4 + best;
+        used[best]++; load[best] += bd.cost;
+        S.GW[(size_t)b * NW + warp] = (uint8_t)(bd.lv.size() | (bd.type << 4));
+        for (size_t k = 0; k < bd.lv.size(); k++) {
+            const Lvl &lv = levels[bd.lv[k]];
+            for (size_t l = 0; l < lv.g.size(); l++) {
+                const Grp &g = groups[lv.g[l]];
+                const int tid = warp * 32 + (int)l;
+                S.GA[((size_t)b * BA_KG + k) * BA_NT + tid] = 8u * g.key;
+                for (size_t q = 0; q < g.items.size(); q++) {
+                    const TTPair &pr = pairs[g.items[q]];
+                    S.GO[(((size_t)b * BA_KG + k) * BA_GP + q) * BA_NT + tid] = (uint16_t)owner_of(pr);
+                    for (int cls = 0; cls < BA_NCLS; cls++) {
+                        if (deep(cls, pr)) continue;                   // served by a rider under this class
+                        uint4 &e = S.GB[(((size_t)cls * 2 + b) * BA_KG + k) * BA_NT + tid];
+                        const uint32_t bp = bpack(cls, pr);
+                        (q == 0 ? e.x : q == 1 ? e.y : q == 2 ? e.z : e.w) = bp;
                     }
-                    return false;
                 }
-            };
-            for (int oi = 0; oi < nl; oi++) { uint32_t seen = 0; Aug::run(order[oi], seen, avail, match_res); }
-            int lane_res[16];
-            for (int i = 0; i < nl; i++) lane_res[i] = -1;
-            for (int r = 0; r < 16; r++) if (match_res[r] >= 0) lane_res[match_res[r]] = r;
-            int used[16] = {0};
-            for (int i = 0; i < nl; i++) {
-                std::vector<uint32_t> &P = pool[slot_owner[lanes[i]]];
-                if (P.empty()) continue;                        // a lane sharing its owner's pool took the last item
-                int pick = -1;
-                if (lane_res[i] >= 0)
-                    for (size_t j = 0; j < P.size() && j < (size_t)BA_PLACE_WINDOW && (P[j] >> 28) == (P[0] >> 28); j++)
-                        if ((int)(P[j] & 15u) == lane_res[i]) { pick = (int)j; break; }
-                if (pick < 0) {
-                    pick = 0;
-                    for (size_t j = 1; j < P.size() && j < (size_t)BA_PLACE_WINDOW && (P[j] >> 28) == (P[0] >> 28); j++)
-                        if (used[P[j] & 15u] < used[P[pick] & 15u]) pick = (int)j;
-                }
-                const uint32_t it = P[pick];
-                P.erase(P.begin() + pick);
-                used[it & 15u]++;
-                at[(size_t)lanes[i] * BA_C + q] = it;
+                S.nslots[b] += BA_GP;
             }
         }
     }
-    // ---- local search: swap two items of one owner and one depth between their positions when that lowers
-    // (sum over groups of the worst bank-pair multiplicity, then the sum of squared multiplicities).  A group is
-    // one (half-warp, q) operand load.
-    const int ngrp = ((nslots + 15) / 16) * BA_C;
-    std::vector<uint8_t> cnt((size_t)ngrp * 16, 0);
-    auto grp = [&](int p) { return ((p / BA_C) / 16) * BA_C + p % BA_C; };
-    auto gmax = [&](int g) { int mx = 0; for (int r = 0; r < 16; r++) mx = std::max<int>(mx, cnt[(size_t)g * 16 + r]); return mx; };
-    auto gsq = [&](int g) { int sq = 0; for (int r = 0; r < 16; r++) sq += cnt[(size_t)g * 16 + r] * cnt[(size_t)g * 16 + r]; return sq; };
-    std::vector<std::vector<int>> by_owner(pool.size());
-    std::vector<uint32_t> wdepth((nslots + 31) / 32, 0);          // deepest item of every warp-slot (32 slots)
-    for (int p = 0; p < nslots * BA_C; p++)
-        if (at[p] != EMPTY) {
-            cnt[(size_t)grp(p) * 16 + (at[p] & 15u)]++;
-            by_owner[slot_owner[p / BA_C]].push_back(p);
-            wdepth[p / BA_C / 32] = std::max(wdepth[p / BA_C / 32], at[p] >> 28);
-        }
-    for (int sweep = 0; sweep < 8; sweep++) {
-        int improved = 0;
-        for (int p1 = 0; p1 < nslots * BA_C; p1++) {
-            if (at[p1] == EMPTY) continue;
-            const int g1 = grp(p1);
-            const uint32_t r1 = at[p1] & 15u;
-            if (cnt[(size_t)g1 * 16 + r1] < 2) continue;           // this lane is not part of a conflict
-            const std::vector<int> &cand = by_owner[slot_owner[p1 / BA_C]];
-            for (int p2 : cand) {
-                if (p2 == p1) continue;                            // a swap must not deepen either warp-slot
-                if ((at[p1] >> 28) > wdepth[p2 / BA_C / 32] || (at[p2] >> 28) > wdepth[p1 / BA_C / 32]) continue;
-                const int g2 = grp(p2);
-                const uint32_t r2 = at[p2] & 15u;
-                if (g2 == g1 || r2 == r1) continue;
-                const int b_mx = gmax(g1) + gmax(g2), b_sq = gsq(g1) + gsq(g2);
-                cnt[(size_t)g1 * 16 + r1]--; cnt[(size_t)g1 * 16 + r2]++;
-                cnt[(size_t)g2 * 16 + r2]--; cnt[(size_t)g2 * 16 + r1]++;
-                const int a_mx = gmax(g1) + gmax(g2), a_sq = gsq(g1) + gsq(g2);
-                if (a_mx < b_mx || (a_mx == b_mx && a_sq < b_sq)) { std::swap(at[p1], at[p2]); improved++; break; }
-                cnt[(size_t)g1 * 16 + r1]++; cnt[(size_t)g1 * 16 + r2]--;
-                cnt[(size_t)g2 * 16 + r2]++; cnt[(size_t)g2 * 16 + r1]--;
-            }
-        }
-        if (!improved) break;
-    }
-    for (int p = 0; p < nslots * BA_C; p++)
-        if (at[p] != EMPTY) emit(p / BA_C, p % BA_C, slot_owner[p / BA_C], at[p] & 0x0fffffffu);
+    S.npairs[b] = (unsigned long long)np;
+    S.ngroups[b] = groups.size();
+    return true;
 }
 
 static inline void build_tile_tables(int m, TileTables &T) {
@@ -182,232 +163,113 @@ static inline void build_tile_tables(int m, TileTables &T) {
                 B[(size_t)((1u << lw) | w) * nv + v] = (uint8_t)e[lw];       // <= C(8,4) = 70
             }
     auto Bof = [&](uint32_t cw, int v) -> uint32_t { return (cw < (uint32_t)NZc) ? B[(size_t)cw * nv + v] : 0u; };
-
-    // ---- v-major lists: [0] null  [1] empty string  [2..) the non-empty subsequences of v -----------------
-    std::vector<std::vector<int>> loc(nv);                 // code(z) -> local index, 0 if absent
-    T.vbase.assign(nv, 0);
-    uint32_t total = 0;
-    for (int v = 0; v < nv; v++) {
-        loc[v].assign(NZc, 0);
-        int li = 1;
-        loc[v][1] = li++;
-        for (uint32_t cz = 2; cz < (uint32_t)NZc; cz++)
-            if (Bof(cz, v)) loc[v][cz] = li++;
-        if (li > 256) return;                              // local links are 8 bit
-        T.vbase[v] = total;
-        total += (uint32_t)li;
-    }
-    if ((size_t)total * 4 >= (1u << 20)) return;
-    T.Wv.assign(total, 0u);
-    for (int v = 0; v < nv; v++)
-        for (uint32_t cz = 1; cz < (uint32_t)NZc; cz++) {
-            const int li = loc[v][cz];
-            if (!li) continue;
-            const int lz = 31 - __builtin_clz(cz);
-            uint32_t W = 0;
-            if (lz + 1 <= m)
-                for (uint32_t b = 0; b < 2; b++) {
-                    const uint32_t cbz = tt_prepend(b, 1, cz);
-                    const int lb = loc[v][cbz];
-                    if (lb) W |= ((uint32_t)lb | (Bof(cbz, v) << 8)) << (16 * b);
-                }
-            T.Wv[T.vbase[v] + li] = W;
-        }
-
-    const size_t FSZ = (size_t)BA_NCLS * 2 * BA_NC * BA_C * BA_NT;
-    auto fidx = [](int cls, int b, int c, int q, int tid) -> size_t {
-        return ((((size_t)cls * 2 + b) * BA_NC + c) * BA_C + q) * BA_NT + tid;
-    };
     auto first_bit = [](uint32_t cz) -> int { const int lz = 31 - __builtin_clz(cz); return (int)((cz >> (lz - 1)) & 1u); };
-    auto deep = [&](int cls, uint32_t cz, int v) -> bool {      // chain of (v,z) under class cls reaches s = BA_KB
-        const int lz = 31 - __builtin_clz(cz);
-        return lz + BA_KB <= m && Bof(tt_prepend((uint32_t)cls, BA_KB, cz), v) != 0;
+    auto deep = [&](int cls, const TTPair &p) -> bool {        // chain of (v,z) under class cls reaches s = BA_KB
+        const int lz = 31 - __builtin_clz(p.cz);
+        return lz + BA_KB <= m && Bof(tt_prepend((uint32_t)cls, BA_KB, p.cz), p.v) != 0;
     };
     auto tail_of = [](uint32_t cz) -> uint32_t {               // code(t) for z = b.t
         const int lz = 31 - __builtin_clz(cz);
         return (1u << (lz - 1)) | (cz & ((1u << (lz - 1)) - 1u));
     };
-    auto depth = [&](int cls, uint32_t cz, int v) -> int {     // largest s <= 3 with B_s != 0
-        const int lz = 31 - __builtin_clz(cz);
-        int d = 0;
-        for (int s = 1; s < 4; s++)
-            if (lz + s <= m && Bof(tt_prepend((uint32_t)cls, s, cz), v)) d = s;
-        return d;
-    };
-    auto bpack = [&](int cls, uint32_t cz, int v) -> uint32_t { // B_0..B_3 under class cls
+    auto bpack = [&](int cls, const TTPair &p) -> uint32_t {   // B_0..B_3 under class cls
         uint32_t x = 0;
-        const int lz = 31 - __builtin_clz(cz);
+        const int lz = 31 - __builtin_clz(p.cz);
         for (int s = 0; s < 4; s++)
-            if (lz + s <= m) x |= Bof(tt_prepend((uint32_t)cls, s, cz), v) << (8 * s);
+            if (lz + s <= m) x |= Bof(tt_prepend((uint32_t)cls, s, p.cz), p.v) << (8 * s);
         return x;
     };
-    auto rider = [&](int cls, uint32_t cz, int v, uint32_t off, uint32_t owner) -> uint4 {
-        const uint32_t c4 = tt_prepend((uint32_t)cls, BA_KB, cz);
-        uint4 r;
-        r.x = bpack(cls, cz, v);
-        r.y = Bof(c4, v) | ((uint32_t)loc[v][c4] << 8) | (owner << 16);
-        r.z = off;
-        r.w = T.vbase[v] * 4u;
-        return r;
+
+    const int NW = BA_NT / 32;
+    auto init_side = [&](GroupSide &S, int nown) {
+        S.nown = nown;
+        S.GB.assign((size_t)BA_NCLS * 2 * BA_KG * BA_NT, make_uint4(0u, 0u, 0u, 0u));
+        S.GA.assign((size_t)2 * BA_KG * BA_NT, 0u);
+        S.GO.assign((size_t)2 * BA_KG * BA_GP * BA_NT, 0xffffu);
+        S.GW.assign((size_t)2 * NW, 0);
+        S.csr_off.assign((size_t)2 * (nown + 1), 0);
+        S.csr_idx.assign((size_t)2 * BA_KG * BA_GP * BA_NT, 0);
     };
+    init_side(T.in, nv);
+    init_side(T.out, NZc);
 
-    // ================= input sweep: chunks of v's list b, slots dealt round-robin over v =====================
-    T.FI.assign(FSZ, make_uint2(0u, 0u));
-    T.in_owner.assign((size_t)2 * BA_NC * BA_NT, 0xffffu);
-    std::vector<std::vector<uint16_t>> vslots(nv);
-    std::vector<int> in_slot_owner[2];
-    for (int b = 0; b < 2; b++) {
-        std::vector<int> nch(nv, 0);
-        for (int v = 0; v < nv; v++) {
-            int cnt = 0;
-            for (uint32_t cz = 2; cz < (uint32_t)NZc; cz++) cnt += (Bof(cz, v) && first_bit(cz) == b);
-            nch[v] = (cnt + BA_C - 1) / BA_C;
-        }
-        std::vector<int> &so = in_slot_owner[b];
-        for (int r = 0;; r++) {
-            bool any = false;
-            for (int v = 0; v < nv; v++) if (nch[v] > r) { so.push_back(v); any = true; }
-            if (!any) break;
-        }
-        if (so.size() > (size_t)BA_NC * BA_NT) return;
-        for (size_t k = 0; k < so.size(); k++) {
-            int c, tid;
-            tt_phys((int)k, c, tid);
-            const size_t ai = ((size_t)b * BA_NC + c) * BA_NT + tid;
-            T.in_owner[ai] = (uint16_t)so[k];
-            vslots[so[k]].push_back((uint16_t)ai);
-        }
-    }
-    T.in_csr_off.assign(nv + 1, 0);
-    T.in_csr_idx.clear();
-    for (int v = 0; v < nv; v++) {
-        T.in_csr_off[v] = (uint16_t)T.in_csr_idx.size();
-        for (uint16_t s : vslots[v]) T.in_csr_idx.push_back(s);
-    }
-    T.in_csr_off[nv] = (uint16_t)T.in_csr_idx.size();
-
-    std::vector<std::vector<uint4>> rin((size_t)BA_NCLS * 2);
-    std::vector<std::vector<std::pair<uint32_t, int>>> rin_zv((size_t)BA_NCLS * 2);
-    T.ri_csr.assign((size_t)BA_NCLS * 2 * (nv + 1), 0);
-    for (int cls = 0; cls < BA_NCLS; cls++)
+    for (int side = 0; side < 2; side++) {
+        GroupSide &S = side ? T.out : T.in;
+        // operand position in a staged row.  in: the operand of z = b.t is c(y'.b.t) at position code(t) of the
+        // node's half row; out: the operand of (v, z) is p(u.v) at position v of the node's row.
+        auto key_of = [&](const TTPair &p) -> uint32_t { return side ? (uint32_t)p.v : tail_of(p.cz); };
+        auto owner_of = [&](const TTPair &p) -> uint32_t { return side ? p.cz : (uint32_t)p.v; };
+        std::vector<std::vector<uint4>> riders((size_t)BA_NCLS * 2);
+        std::vector<std::vector<TTPair>> rider_pairs((size_t)BA_NCLS * 2);
+        S.r_csr.assign((size_t)BA_NCLS * 2 * (S.nown + 1), 0);
         for (int b = 0; b < 2; b++) {
-            std::vector<std::vector<uint32_t>> pool(nv);
-            std::vector<uint4> &R = rin[(size_t)cls * 2 + b];
-            for (int v = 0; v < nv; v++) {
-                T.ri_csr[((size_t)cls * 2 + b) * (nv + 1) + v] = (uint16_t)R.size();
-                for (uint32_t cz = 2; cz < (uint32_t)NZc; cz++) {
-                    if (!Bof(cz, v) || first_bit(cz) != b) continue;
-                    // the operand of z = b.t sits at position code(t) of the node's half row
-                    if (deep(cls, cz, v)) {
-                        R.push_back(rider(cls, cz, v, 8u * ba_swz(tail_of(cz)), (uint32_t)v));
-                        rin_zv[(size_t)cls * 2 + b].push_back(std::make_pair(cz, v));
-                    }
-                    else pool[v].push_back(ba_swz(tail_of(cz)) | ((uint32_t)depth(cls, cz, v) << 28));   // key = row position: bank pair = key & 15
-                }
-            }
-            T.ri_csr[((size_t)cls * 2 + b) * (nv + 1) + nv] = (uint16_t)R.size();
+            std::vector<TTPair> pairs;
             for (int v = 0; v < nv; v++)
-                std::stable_sort(pool[v].begin(), pool[v].end(), [](uint32_t x, uint32_t y) { return (x >> 28) > (y >> 28); });
-            tt_place(in_slot_owner[b], pool, [&](int k, int q, int v, uint32_t key) {
-                const uint32_t tc = ba_swz(key);
-                const int lt = 31 - __builtin_clz(tc);
-                const uint32_t cz = (1u << (lt + 1)) | ((uint32_t)b << lt) | (tc - (1u << lt));
-                int c, tid;
-                tt_phys(k, c, tid);
-                T.FI[fidx(cls, b, c, q, tid)] = make_uint2(bpack(cls, cz, v), 8u * key);
-            });
-            for (int v = 0; v < nv; v++) if (!pool[v].empty()) return;
-        }
-
-    // ================= output sweep: per class, chunks of one z sorted by chain depth ========================
-    // The class of an output-sweep item is fixed, so slot ownership (and the CSR of the epilogue) may differ
-    // from class to class: the chunks of a class are sorted by depth and dealt to the slots in that order, so
-    // a warp's 32 x BA_C pairs share one depth and most warps run the 1- or 2-IMAD loop.
-    T.FO.assign(FSZ, make_uint2(0u, 0u));
-    T.out_owner.assign((size_t)BA_NCLS * 2 * BA_NC * BA_NT, 0xffffu);
-    T.out_csr_off.assign((size_t)BA_NCLS * NZc, 0);
-    T.out_ncsr = 2 * BA_NC * BA_NT;
-    T.out_csr_idx.assign((size_t)BA_NCLS * T.out_ncsr, 0);
-    std::vector<std::vector<uint4>> rout((size_t)BA_NCLS * 2);
-    std::vector<std::vector<std::pair<uint32_t, int>>> rout_zv((size_t)BA_NCLS * 2);
-    T.ro_csr.assign((size_t)BA_NCLS * 2 * (NZc + 1), 0);
-    for (int cls = 0; cls < BA_NCLS; cls++) {
-        std::vector<std::vector<uint16_t>> zslots(NZc);
-        for (int b = 0; b < 2; b++) {
-            std::vector<uint4> &R = rout[(size_t)cls * 2 + b];
-            struct Chunk { int cz, depth, ord; std::vector<uint32_t> items; };
-            std::vector<Chunk> chunks;
-            for (uint32_t cz = 0; cz < (uint32_t)NZc; cz++) {
-                T.ro_csr[((size_t)cls * 2 + b) * (NZc + 1) + cz] = (uint16_t)R.size();
-                if (cz < 2 || first_bit(cz) != b) continue;
-                std::vector<uint32_t> pz;
-                for (int v = 0; v < nv; v++) {
-                    if (!Bof(cz, v)) continue;
-                    if (deep(cls, cz, v)) {
-                        R.push_back(rider(cls, cz, v, 8u * ba_swz((uint32_t)v), cz));
-                        rout_zv[(size_t)cls * 2 + b].push_back(std::make_pair(cz, v));
+                for (uint32_t cz = 2; cz < (uint32_t)NZc; cz++)
+                    if (Bof(cz, v) && first_bit(cz) == b) pairs.push_back(TTPair{v, cz});
+            if (!tt_deal(m, b, pairs, key_of, owner_of, bpack, deep, S)) return;
+            // ---- CSR of the epilogue: the slots of every owner, in slot order
+            std::vector<std::vector<uint16_t>> slots(S.nown);
+            for (int k = 0; k < BA_KG; k++)
+                for (int q = 0; q < BA_GP; q++)
+                    for (int tid = 0; tid < BA_NT; tid++) {
+                        const uint16_t ow = S.GO[(((size_t)b * BA_KG + k) * BA_GP + q) * BA_NT + tid];
+                        if (ow != 0xffffu) slots[ow].push_back((uint16_t)((k * BA_GP + q) * BA_NT + tid));
                     }
-                    else pz.push_back(ba_swz((uint32_t)v) | ((uint32_t)depth(cls, cz, v) << 28));   // key = row position: bank pair = key & 15
-                }
-                std::stable_sort(pz.begin(), pz.end(), [](uint32_t x, uint32_t y) { return (x >> 28) > (y >> 28); });
-                for (size_t i = 0; i < pz.size(); i += BA_C) {
-                    Chunk ch;
-                    ch.cz = (int)cz; ch.depth = (int)(pz[i] >> 28); ch.ord = (int)(i / BA_C);
-                    for (size_t j = i; j < pz.size() && j < i + BA_C; j++) ch.items.push_back(pz[j] & 0x0fffffffu);
-                    chunks.push_back(ch);
-                }
+            size_t n = 0;
+            for (int o = 0; o < S.nown; o++) {
+                S.csr_off[(size_t)b * (S.nown + 1) + o] = (uint16_t)n;
+                for (uint16_t sl : slots[o]) S.csr_idx[(size_t)b * BA_KG * BA_GP * BA_NT + n++] = sl;
             }
-            T.ro_csr[((size_t)cls * 2 + b) * (NZc + 1) + NZc] = (uint16_t)R.size();
-            if (chunks.size() > (size_t)BA_NC * BA_NT) return;
-            std::stable_sort(chunks.begin(), chunks.end(), [](const Chunk &x, const Chunk &y) {
-                return x.depth != y.depth ? x.depth > y.depth : x.ord < y.ord;     // neighbours own different z
-            });
-            std::vector<int> so(chunks.size());
-            std::vector<std::vector<uint32_t>> pool(NZc);        // owner = code(z): its items, deepest first
-            for (size_t k = 0; k < chunks.size(); k++) {
-                so[k] = chunks[k].cz;
-                for (uint32_t it : chunks[k].items) pool[chunks[k].cz].push_back(it | ((uint32_t)chunks[k].depth << 28));
-                int c, tid;
-                tt_phys((int)k, c, tid);
-                const size_t ai = ((size_t)b * BA_NC + c) * BA_NT + tid;
-                T.out_owner[(size_t)cls * 2 * BA_NC * BA_NT + ai] = (uint16_t)chunks[k].cz;
-                zslots[chunks[k].cz].push_back((uint16_t)ai);
+            S.csr_off[(size_t)b * (S.nown + 1) + S.nown] = (uint16_t)n;
+            // ---- riders: the pairs that are deep under a class, sorted by owner
+            for (int cls = 0; cls < BA_NCLS; cls++) {
+                std::vector<TTPair> dp;
+                for (const TTPair &p : pairs) if (deep(cls, p)) dp.push_back(p);
+                std::stable_sort(dp.begin(), dp.end(), [&](const TTPair &x, const TTPair &y) { return owner_of(x) < owner_of(y); });
+                std::vector<uint4> &R = riders[(size_t)cls * 2 + b];
+                uint16_t *cs = &S.r_csr[((size_t)cls * 2 + b) * (S.nown + 1)];
+                size_t e = 0;
+                for (int o = 0; o <= S.nown; o++) {
+                    while (e < dp.size() && (int)owner_of(dp[e]) < o) e++;
+                    cs[o] = (uint16_t)e;
+                }
+                for (const TTPair &p : dp) {
+                    uint4 r;
+                    r.x = bpack(cls, p);
+                    r.y = Bof(tt_prepend((uint32_t)cls, BA_KB, p.cz), p.v) | (owner_of(p) << 16);
+                    r.z = 8u * key_of(p);
+                    r.w = 0u;
+                    R.push_back(r);
+                }
+                rider_pairs[(size_t)cls * 2 + b] = dp;
             }
-            for (auto &pl : pool) std::stable_sort(pl.begin(), pl.end(), [](uint32_t x, uint32_t y) { return (x >> 28) > (y >> 28); });
-            tt_place(so, pool, [&](int k, int q, int cz, uint32_t key) {
-                const uint32_t v = ba_swz(key);
-                int c, tid;
-                tt_phys(k, c, tid);
-                T.FO[fidx(cls, b, c, q, tid)] = make_uint2(bpack(cls, (uint32_t)cz, (int)v), 8u * key);
-            });
-            for (auto &pl : pool) if (!pl.empty()) return;
         }
-        size_t n = 0;
-        for (int cz = 1; cz < NZc; cz++) {
-            T.out_csr_off[(size_t)cls * NZc + cz - 1] = (uint16_t)n;
-            for (uint16_t sl : zslots[cz]) T.out_csr_idx[(size_t)cls * T.out_ncsr + n++] = sl;
-        }
-        T.out_csr_off[(size_t)cls * NZc + NZc - 1] = (uint16_t)n;
-    }
-
-    // ---- rider arrays, padded to a common capacity (multiple of 32, at most BA_NT) -------------------------
-    auto pack_riders = [&](std::vector<std::vector<uint4>> &src, std::vector<uint4> &dst, std::vector<uint16_t> &cnt, int &cap) {
+        // ---- rider arrays, padded to a common capacity (multiple of 32)
         size_t mx = 0;
-        for (auto &r : src) mx = std::max(mx, r.size());
-        cap = (int)((mx + 31) / 32 * 32);
-        if (cap == 0) cap = 32;
-        if (cap > BA_NT) return false;
-        dst.assign((size_t)BA_NCLS * 2 * cap, make_uint4(0u, 0u, 0u, 0u));
-        cnt.assign((size_t)BA_NCLS * 2, 0);
-        for (size_t i = 0; i < src.size(); i++) {
-            cnt[i] = (uint16_t)src[i].size();
-            std::copy(src[i].begin(), src[i].end(), dst.begin() + i * cap);
+        for (auto &r : riders) mx = std::max(mx, r.size());
+        S.nr = (int)((mx + 31) / 32 * 32);
+        if (S.nr == 0) S.nr = 32;
+        if (S.nr > BA_NT / 2) return;                          // two replicas of the rider set share the CTA
+        S.R.assign((size_t)BA_NCLS * 2 * S.nr, make_uint4(0u, 0u, 0u, 0u));
+        S.r_cnt.assign((size_t)BA_NCLS * 2, 0);
+        S.R8.assign((size_t)BA_NCLS * 2 * 16 * S.nr, 0u);
+        for (size_t i = 0; i < riders.size(); i++) {
+            S.r_cnt[i] = (uint16_t)riders[i].size();
+            std::copy(riders[i].begin(), riders[i].end(), S.R.begin() + i * S.nr);
+            const int cls = (int)(i / 2);
+            for (uint32_t hi = 0; hi < 16u; hi++)
+                for (size_t e = 0; e < rider_pairs[i].size(); e++) {
+                    const TTPair &p = rider_pairs[i][e];
+                    const int lz = 31 - __builtin_clz(p.cz);
+                    uint32_t x = 0;
+                    for (int sft = 5; sft <= 8; sft++)
+                        if (lz + sft <= m) x |= Bof(tt_prepend((hi << 4) | (uint32_t)cls, sft, p.cz), p.v) << (8 * (sft - 5));
+                    S.R8[(i * 16 + hi) * S.nr + e] = x;
+                }
         }
-        return true;
-    };
-    if (!pack_riders(rin, T.RI, T.ri_cnt, T.nri) || T.nri > BA_NT / 2) return;   // the in sweep runs two replicas
-    if (!pack_riders(rout, T.RO, T.ro_cnt, T.nro)) return;
-    // ---- direct tables for the whole-chain pairs of the input sweep ------------------------------------------
+    }
+    // ---- direct table of the pairs (v, empty): all B(sigma_s, v), s = 1..8 --------------------------------------
     T.EPS8.assign((size_t)256 * nv, make_uint2(0u, 0u));
     for (uint32_t sig = 0; sig < 256u; sig++)
         for (int v = 0; v < nv; v++) {
@@ -416,22 +278,5 @@ static inline void build_tile_tables(int m, TileTables &T) {
                 w[(sft - 1) / 4] |= Bof((1u << sft) | (sig & ((1u << sft) - 1u)), v) << (8 * ((sft - 1) % 4));
             T.EPS8[(size_t)sig * nv + v] = make_uint2(w[0], w[1]);
         }
-    auto tails = [&](const std::vector<std::vector<std::pair<uint32_t, int>>> &zv, int cap, std::vector<uint32_t> &dst) {
-        dst.assign((size_t)BA_NCLS * 2 * 16 * cap, 0u);
-        for (int cls = 0; cls < BA_NCLS; cls++)
-            for (int b = 0; b < 2; b++)
-                for (uint32_t hi = 0; hi < 16u; hi++)
-                    for (size_t e = 0; e < zv[(size_t)cls * 2 + b].size(); e++) {
-                        const uint32_t cz = zv[(size_t)cls * 2 + b][e].first;
-                        const int v = zv[(size_t)cls * 2 + b][e].second;
-                        const int lz = 31 - __builtin_clz(cz);
-                        uint32_t x = 0;
-                        for (int sft = 5; sft <= 8; sft++)
-                            if (lz + sft <= m) x |= Bof(tt_prepend((hi << 4) | (uint32_t)cls, sft, cz), v) << (8 * (sft - 5));
-                        dst[((((size_t)cls * 2 + b) * 16 + hi) * cap) + e] = x;
-                    }
-    };
-    tails(rin_zv, T.nri, T.RI8);
-    tails(rout_zv, T.nro, T.RO8);
     T.ok = true;
 }
