@@ -212,6 +212,7 @@ extern "C" int ba_debug_check_tables(int m, unsigned long long stats[4]) {
                             if (!(e[q] & 0xffu)) { if (e[q]) return BA_EINVAL; continue; }      // unused, or deep under this class
                             if (ow == 0xffffu || k >= (wm & 15)) return BA_EINVAL;              // the warp's loop must reach the slot
                             if ((wm >> 4) == 2 && (e[q] >> 16)) return BA_EINVAL;               // a type-2 loop ignores B_2, B_3
+                            if ((wm >> 4) == 1 && (e[q] >> 8)) return BA_EINVAL;                // a type-1 loop ignores B_1..B_3
                             if (!visit(pos, ow, e[q], 4, nullptr)) return BA_EINVAL;
                             stats[side ? 2 : 0]++;
                         }

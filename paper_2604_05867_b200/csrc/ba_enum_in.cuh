@@ -212,7 +212,12 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 ba_bucket_sort<BA_NCLS>(key, s_ordr + (size_t)rd * BA_NT, s_wcnt, s_seg + rd * (BA_NCLS + 1));
 
                 // ================= eps: the pair (v, empty) of every node of the round =================
-                if (b == 0) {
+#ifndef BA_X_NOEPS
+                if (b == 0)
+#else
+                if (b == 7)
+#endif
+                {
                     auto eps_one = [&](int i) {
                         const NodeRec &rc = s_rec[rd * BA_NT + i];
                         const uint4 r0 = *(const uint4 *)&rc.a[0], r1 = *(const uint4 *)&rc.a[4], r2 = *(const uint4 *)&rc.a[8];
@@ -241,7 +246,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                         for (int i = esub; i < nn; i += epn)
                             if ((int)(s_rec[rd * BA_NT + i].info >> 16) == klen) eps_one(i);
                     } else {
-#pragma unroll 4
+#pragma unroll 8
                         for (int i = esub; i < nn; i += epn) eps_one(i);
                     }
                 }
@@ -363,7 +368,11 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                     }
                 }
                 // ---- riders: deep pairs of this class, one per thread ------------------------------------
-                const int nr = a.g.r_cnt[cls * 2 + b];
+                #ifdef BA_X_NORIDERS
+        const int nr = 0;
+#else
+        const int nr = a.g.r_cnt[cls * 2 + b];
+#endif
                 // two replicas of the rider set (threads 255 - e and 511 - e), each takes every other node
                 const int re = (BA_NT / 2 - 1) - (tid & (BA_NT / 2 - 1)), rh = tid / (BA_NT / 2);
                 if ((BA_NT / 2) - 32 * ((warp & (BA_NT / 64 - 1)) + 1) < nr) {
@@ -374,7 +383,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                         const uint32_t cz = ba_z_of_tail((uint32_t)b, rd.z >> 3);
                         const int jz = ba_len_of_code(cz);
                         const uint32_t *r8 = a.g.R8 + ((size_t)cls * 2 + b) * 16 * a.g.nr + re;
-#pragma unroll 4                                           // four independent L2 reads of the chain tails in flight
+#pragma unroll 8                                           // four independent L2 reads of the chain tails in flight
                         for (int i = rh; i < len; i += 2) {
                             const BalRec bl = bal[i];
                             const uint32_t cy = bl.id;

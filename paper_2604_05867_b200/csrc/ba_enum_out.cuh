@@ -129,7 +129,11 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
         // (v, empty) alone, which item (y', 0) serves
         const int klen = (MODE == OUT_SWEEP) ? a.kc.klen : -1;
         if (klen >= 0 && (klen < t || klen > t + m || (klen == t && b == 1))) { __syncthreads(); continue; }
+#ifndef BA_X_NOEPS
         const bool do_eps = (b == 0) && (klen < 0 || klen == t);
+#else
+        const bool do_eps = false;
+#endif
         const bool do_grp = (klen != t);
         const int cls = (int)(cy & (BA_NCLS - 1));
         const int Lc = t < 8 ? t : 8;
@@ -150,7 +154,11 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
             const uint2 e8 = __ldg(a.EPS8 + (size_t)(cy & 255u) * nv + ev);
             eB0 = 1u | (e8.x << 8); eB1 = (e8.x >> 24) | (e8.y << 8); eB2 = e8.y >> 24;
         }
+        #ifdef BA_X_NORIDERS
+        const int nr = 0;
+#else
         const int nr = a.g.r_cnt[cls * 2 + b];
+#endif
         const int re = BA_NT - 1 - tid;                        // riders sit on the last warps
         uint32_t rB0 = 0, rB1 = 0, rB2 = 0, roff = 0, rown = 0;
         if (re < nr) {
@@ -270,7 +278,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                     for (int i = esub; i < len; i += epn) {
                         uint32_t emb;
                         if (!big) {
-                            const uint4 al = ba_lds_v4(balbase + (uint32_t)i * 32u);
+                            const uint4 al = ba_lds_v4(balbase + (uint32_t)i * BA_BALB);
                             emb = ba_chain9(al.x, al.y, al.z, al.w, bal[i].a8, eB0, eB1, eB2);
                         } else emb = ba_chain9_wide(s_rec[bal[i].node].a, eB0, eB1, eB2);
                         if (MODE == OUT_SWEEP) {
@@ -312,7 +320,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                         for (int i = 0; i < len; i++) {
                             uint32_t emb;
                             if (!big) {
-                                const uint4 al = ba_lds_v4(balbase + (uint32_t)i * 32u);
+                                const uint4 al = ba_lds_v4(balbase + (uint32_t)i * BA_BALB);
                                 emb = ba_chain9(al.x, al.y, al.z, al.w, bal[i].a8, rB0, rB1, rB2);
                             } else emb = ba_chain9_wide(s_rec[bal[i].node].a, rB0, rB1, rB2);
                             if (MODE == OUT_SWEEP) {

@@ -69,13 +69,16 @@ struct NodeRec {                      // 48 bytes, shared memory
     uint32_t pad;
 };
 
-// A node of a staged batch as the hot loops read it: alphas as 16-bit halves (IDP.2A operands), 32 bytes.
+// A node of a staged batch as the hot loops read it: alphas as 16-bit halves (IDP.2A operands), 48 bytes.
 struct BalRec {
     uint32_t a01, a23, a45, a67, a8;  // alpha_0 | alpha_1 << 16, ...; garbage when `big`
     uint32_t big;                     // != 0: an alpha of the node needs more than 16 bits
     uint32_t id;                      // NodeRec::id
     uint32_t node;                    // index of the NodeRec
+    double a0d;                       // (double)alpha_0, exact: the type-1 loop (ba_group_loop<1, .>)
+    double x0;                        // a per-node operand of the sweep (input sweep: c(y'))
 };
+#define BA_BALB 48u
 
 __device__ __forceinline__ BalRec ba_make_bal(const NodeRec &rc, uint32_t node) {
     BalRec bl;
@@ -84,6 +87,7 @@ __device__ __forceinline__ BalRec ba_make_bal(const NodeRec &rc, uint32_t node) 
     bl.a8 = rc.a[8];
     bl.big = (rc.a[0] | rc.a[1] | rc.a[2] | rc.a[3] | rc.a[4] | rc.a[5] | rc.a[6] | rc.a[7]) >> 16;
     bl.id = rc.id; bl.node = node;
+    bl.a0d = (double)rc.a[0]; bl.x0 = 0.0;
     return bl;
 }
 
@@ -154,23 +158,41 @@ __device__ __forceinline__ void ba_mbar_arrive_on_copies(uint32_t addr) {      /
 }
 // A lost arrival must fail loudly, not hang the device: trap after ~20 s of SM clocks (far beyond any batch, also
 // under a profiler's replay or a preempted context, where a poll count would be reached much sooner than a clock).
-__device__ __forceinline__ void ba_mbar_wait(uint32_t addr, uint32_t parity) {
-    uint32_t done = 0;
-    long long t0 = 0;
-    for (uint32_t spin = 0; !done; spin++) {
-        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
-                     : "=r"(done) : "r"(addr), "r"(parity) : "memory");
-        if (!done && (spin & 0xfffu) == 0xfffu) {
-            const long long now = clock64();
-            if (t0 == 0) t0 = now;
-            else if (now - t0 > 40000000000ll) __trap();
-        }
+// try_wait suspends the warp in hardware until the phase completes or a time limit passes; the common case (the
+// phase is already complete, or completes within the first suspensions) costs two instructions.
+__device__ __forceinline__ uint32_t ba_mbar_try(uint32_t addr, uint32_t parity) {
+    uint32_t done;
+    asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                 : "=r"(done) : "r"(addr), "r"(parity) : "memory");
+    return done;
+}
+__device__ __noinline__ void ba_mbar_wait_slow(uint32_t addr, uint32_t parity) {
+    const long long t0 = clock64();
+    for (;;) {
+        for (int i = 0; i < 1024; i++)
+            if (ba_mbar_try(addr, parity)) return;
+        if (clock64() - t0 > 40000000000ll) __trap();
     }
+}
+__device__ __forceinline__ void ba_mbar_wait(uint32_t addr, uint32_t parity) {
+    if (ba_mbar_try(addr, parity)) return;
+    if (ba_mbar_try(addr, parity)) return;
+    ba_mbar_wait_slow(addr, parity);
 }
 
 // exact uint32 -> FP64 on the FP64 pipe (a DADD on the magic number 2^52) instead of the quarter-rate conversion unit
 __device__ __forceinline__ double ba_u2d(uint32_t e) {
     return __hiloint2double(0x43300000, (int)e) - 4503599627370496.0;
+}
+// Pair slots q of a group whose conversion goes to the conversion unit (I2F.F64.U32, 1 instruction on the otherwise
+// idle quarter-rate pipe) instead of the FP64 pipe (MOV + DADD): spreads the per-term conversion over two pipes.
+#ifndef BA_CVT_XU_MASK
+#define BA_CVT_XU_MASK 0x5
+#endif
+template <int Q>
+__device__ __forceinline__ double ba_cvt(uint32_t e) {
+    if ((BA_CVT_XU_MASK >> Q) & 1) return __uint2double_rn(e);
+    return ba_u2d(e);
 }
 
 // The hot loop of both sweeps: the BA_KG x BA_GP pair slots of a thread (Bp = B_0 | B_1<<8 | B_2<<16 | B_3<<24 of the
@@ -180,11 +202,15 @@ __device__ __forceinline__ double ba_u2d(uint32_t e) {
 template <int TYPE, int KMAX>
 __device__ __forceinline__ void ba_group_loop(double (&acc)[BA_NSLOT], const uint32_t (&Bp)[BA_NSLOT], const uint32_t (&rb)[BA_KG],
                                               uint32_t bal, int len) {
-#pragma unroll 2
+#ifndef BA_X_UNR
+#define BA_X_UNR 2
+#endif
+    constexpr int unr = BA_X_UNR;
+#pragma unroll unr
     for (int i = 0; i < len; i++) {
         uint2 a;
-        if (TYPE == 2) { asm volatile("ld.shared.u32 %0, [%1];" : "=r"(a.x) : "r"(bal + (uint32_t)i * 32u)); a.y = 0u; }
-        else a = ba_lds_v2(bal + (uint32_t)i * 32u);
+        if (TYPE == 2) { asm volatile("ld.shared.u32 %0, [%1];" : "=r"(a.x) : "r"(bal + (uint32_t)i * BA_BALB)); a.y = 0u; }
+        else a = ba_lds_v2(bal + (uint32_t)i * BA_BALB);
 #pragma unroll
         for (int k = 0; k < KMAX; k++) {
             const double op = ba_lds_f64(rb[k] + (uint32_t)i * BA_ROWB);
@@ -192,8 +218,30 @@ __device__ __forceinline__ void ba_group_loop(double (&acc)[BA_NSLOT], const uin
             for (int q = 0; q < BA_GP; q++) {
                 uint32_t e = __dp2a_lo(a.x, Bp[k * BA_GP + q], 0u);
                 if (TYPE == 4) e = __dp2a_hi(a.y, Bp[k * BA_GP + q], e);
-                acc[k * BA_GP + q] = fma(ba_u2d(e), op, acc[k * BA_GP + q]);
+                const double ed = (q == 0) ? ba_cvt<0>(e) : (q == 1) ? ba_cvt<1>(e) : (q == 2) ? ba_cvt<2>(e) : ba_cvt<3>(e);
+                acc[k * BA_GP + q] = fma(ed, op, acc[k * BA_GP + q]);
             }
+        }
+    }
+}
+
+// TYPE 1: no slot of the warp ever has B_1 (under any class), so emb = alpha_0 * B_0 is one product of two integer
+// counts (P:181 with a single split point).  The term emb * operand is formed as (alpha_0 * operand) * B_0 with alpha_0
+// and B_0 converted exactly: one DMUL per group and node, one DFMA per term, no integer work in the loop.
+template <int KMAX>
+__device__ __forceinline__ void ba_group_loop1(double (&acc)[BA_NSLOT], const uint32_t (&Bp)[BA_NSLOT], const uint32_t (&rb)[BA_KG],
+                                               uint32_t bal, int len) {
+    double Bd[KMAX * BA_GP];
+#pragma unroll
+    for (int s = 0; s < KMAX * BA_GP; s++) Bd[s] = (double)(Bp[s] & 0xffu);
+#pragma unroll 2
+    for (int i = 0; i < len; i++) {
+        const double a0 = ba_lds_f64(bal + (uint32_t)i * BA_BALB + 32u);
+#pragma unroll
+        for (int k = 0; k < KMAX; k++) {
+            const double t = a0 * ba_lds_f64(rb[k] + (uint32_t)i * BA_ROWB);
+#pragma unroll
+            for (int q = 0; q < BA_GP; q++) acc[k * BA_GP + q] = fma(t, Bd[k * BA_GP + q], acc[k * BA_GP + q]);
         }
     }
 }
@@ -222,9 +270,14 @@ __device__ __forceinline__ void ba_group_batch(double (&acc)[BA_NSLOT], const ui
                                                const BalRec *bal, const NodeRec *rec, int len, int wmeta, bool big) {
     const int kmax = wmeta & 15, type = wmeta >> 4;
     if (kmax == 0) return;
-    if (big) { ba_group_loop_wide(acc, Bp, rb, bal, rec, len, kmax); return; }
+    if (big && type != 1) { ba_group_loop_wide(acc, Bp, rb, bal, rec, len, kmax); return; }
     const uint32_t al16 = ba_smem_addr(bal);
-    if (type == 2) {
+    if (type == 1) {
+        if (kmax == 4) ba_group_loop1<4>(acc, Bp, rb, al16, len);
+        else if (kmax == 3) ba_group_loop1<3>(acc, Bp, rb, al16, len);
+        else if (kmax == 2) ba_group_loop1<2>(acc, Bp, rb, al16, len);
+        else ba_group_loop1<1>(acc, Bp, rb, al16, len);
+    } else if (type == 2) {
         if (kmax == 4) ba_group_loop<2, 4>(acc, Bp, rb, al16, len);
         else if (kmax == 3) ba_group_loop<2, 3>(acc, Bp, rb, al16, len);
         else if (kmax == 2) ba_group_loop<2, 2>(acc, Bp, rb, al16, len);

@@ -12,7 +12,7 @@ struct GroupSide {
     std::vector<uint4> GB;          // [BA_NCLS][2][BA_KG][BA_NT]: B_0 | B_1<<8 | B_2<<16 | B_3<<24 of the group's 4 slots
     std::vector<uint32_t> GA;       // [2][BA_KG][BA_NT]: byte offset of the group's operand in a staged row
     std::vector<uint16_t> GO;       // [2][BA_KG][BA_GP][BA_NT]: owner of the slot (in: v, out: code(z)); 0xffff = unused
-    std::vector<uint8_t> GW;        // [2][BA_NT/32]: levels of the warp (0..BA_KG) | loop type << 4 (2: B_2 = B_3 = 0 always, 4)
+    std::vector<uint8_t> GW;        // [2][BA_NT/32]: levels of the warp (0..BA_KG) | loop type << 4 (1: only B_0 ever; 2: B_2 = B_3 = 0 always; 4)
     std::vector<uint16_t> csr_off;  // [2][nown + 1]: slots of an owner, per list
     std::vector<uint16_t> csr_idx;  // [2][BA_KG*BA_GP*BA_NT]: slot index (k*BA_GP + q)*BA_NT + tid
     int nown = 0;                   // in: 2^m ; out: 2^{m+1} (by code(z))
@@ -52,10 +52,14 @@ static bool tt_deal(int m, int b, const std::vector<TTPair> &pairs, KeyOf key_of
                     GroupSide &S) {
     struct Grp { int type; uint32_t key; std::vector<int> items; };
     const int np = (int)pairs.size();
-    std::vector<int> ptype(np, 2);
+    std::vector<int> ptype(np, 1);
     for (int i = 0; i < np; i++)
-        for (int cls = 0; cls < BA_NCLS; cls++)
-            if (!deep(cls, pairs[i]) && (bpack(cls, pairs[i]) >> 16)) ptype[i] = 4;
+        for (int cls = 0; cls < BA_NCLS; cls++) {
+            if (deep(cls, pairs[i])) continue;
+            const uint32_t bp = bpack(cls, pairs[i]);
+            if ((bp >> 16) && ptype[i] < 4) ptype[i] = 4;
+            else if ((bp >> 8) && ptype[i] < 2) ptype[i] = 2;
+        }
     // ---- groups per operand: type-4 pairs first, the type-2 pairs fill up the last type-4 group
     std::vector<std::vector<int>> by_key(2u << m);
     for (int i = 0; i < np; i++) by_key[key_of(pairs[i])].push_back(i);
@@ -81,32 +85,38 @@ static bool tt_deal(int m, int b, const std::vector<TTPair> &pairs, KeyOf key_of
         levels.back().g.push_back((int)i);
     }
     const int NW = BA_NT / 32;
-    int L4 = 0, L2 = 0;
-    for (auto &l : levels) (l.type == 4 ? L4 : L2)++;
-    // ---- warps per type: proportional to the instruction count (5 per term for type 4, 4 for type 2), at least
-    // ceil(levels / BA_KG), all NW warps used
-    int w4 = (L4 + BA_KG - 1) / BA_KG, w2 = (L2 + BA_KG - 1) / BA_KG;
-    if (w4 + w2 > NW) return false;
-    while (w4 + w2 < NW) {
-        const double c4 = w4 ? 5.0 * L4 / w4 : 0.0, c2 = w2 ? 4.0 * L2 / w2 : 0.0;
-        if (c4 >= c2 && L4 > w4) w4++;
-        else if (L2 > w2) w2++;
-        else if (L4 > w4) w4++;
-        else break;
+    // ---- warps per type: proportional to the instruction count per term (type 4: 2 IDP + MOV + DADD + DFMA = 5,
+    // type 2: 4, type 1: one DFMA and a quarter DMUL), at least ceil(levels / BA_KG), all NW warps used
+    const int types[3] = {4, 2, 1};
+    const double cost_of[3] = {5.0, 4.0, 1.5};
+    int Lt[3] = {0, 0, 0}, wt[3];
+    for (auto &l : levels) Lt[l.type == 4 ? 0 : l.type == 2 ? 1 : 2]++;
+    for (int i = 0; i < 3; i++) wt[i] = (Lt[i] + BA_KG - 1) / BA_KG;
+    if (wt[0] + wt[1] + wt[2] > NW) return false;
+    while (wt[0] + wt[1] + wt[2] < NW) {
+        int best = -1;
+        double bc = -1.0;
+        for (int i = 0; i < 3; i++) {
+            if (Lt[i] <= wt[i]) continue;                      // not more warps than levels
+            const double c = cost_of[i] * Lt[i] / wt[i];
+            if (c > bc) { bc = c; best = i; }
+        }
+        if (best < 0) break;
+        wt[best]++;
     }
     struct Bundle { int type; std::vector<int> lv; double cost; };
     std::vector<Bundle> bundles;
-    auto split = [&](int type, int nl, int nw, int first) {
-        for (int w = 0; w < nw; w++) {
-            Bundle bd; bd.type = type;
-            const int lo = (int)((long long)nl * w / nw), hi = (int)((long long)nl * (w + 1) / nw);
+    int first = 0;
+    for (int i = 0; i < 3; i++) {
+        for (int w = 0; w < wt[i]; w++) {
+            Bundle bd; bd.type = types[i];
+            const int lo = (int)((long long)Lt[i] * w / wt[i]), hi = (int)((long long)Lt[i] * (w + 1) / wt[i]);
             for (int l = lo; l < hi; l++) bd.lv.push_back(first + l);
-            bd.cost = (type == 4 ? 5.0 : 4.0) * (hi - lo);
+            bd.cost = cost_of[i] * (hi - lo);
             bundles.push_back(bd);
         }
-    };
-    split(4, L4, w4, 0);
-    split(2, L2, w2, L4);
+        first += Lt[i];
+    }
     for (auto &bd : bundles) if ((int)bd.lv.size() > BA_KG) return false;
     // ---- bundles -> warp indices: heaviest first onto the scheduler (warp & 3) with the least load
     std::stable_sort(bundles.begin(), bundles.end(), [](const Bundle &x, const Bundle &y) { return x.cost > y.cost; });
