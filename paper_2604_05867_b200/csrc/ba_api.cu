@@ -196,8 +196,8 @@ extern "C" int ba_debug_check_tables(int m, unsigned long long stats[4]) {
                     for (uint32_t hi = 0; hi < 16u; hi++)                                 // rider: B_4 .. B_8
                         for (int s = 4; s <= 8; s++) {
                             const uint32_t want = Bs((hi << 4) | (uint32_t)cls, s, cz, v);
-                            const uint32_t got = (s == 4) ? (uint32_t)nb - 5u : ((tail8[hi] >> (8 * (s - 5))) & 0xffu);
-                            if (want != got) return false;
+                            const uint32_t got = (s == 8) ? 0u : ((tail8[hi] >> (8 * (s - 4))) & 0xffu);
+                            if (want != got || (s == 4 && got != (uint32_t)nb - 5u)) return false;
                         }
                     return true;
                 };

@@ -58,7 +58,7 @@ __host__ __device__ static inline InSmem enum_in_smem(int nr) {
     auto take = [&](size_t bytes) { size_t at = o; o += (bytes + 15) & ~(size_t)15; return at; };
     s.rec = take((size_t)BA_IN_SB * sizeof(NodeRec));
     {                                                      // c(y') of a round (phase A / eps) and the rider sums
-        const size_t ce = (size_t)BA_NT * 8, rs = (size_t)2 * 2 * nr * 8;   // of phase B share one area
+        const size_t ce = (size_t)BA_NT * sizeof(EpsRec), rs = (size_t)2 * 2 * nr * 8;   // of phase B share one area
         s.ceps = take(ce > rs ? ce : rs);
         s.rsum = s.ceps;
     }
@@ -92,7 +92,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
     const InSmem L = enum_in_smem(a.g.nr);
 
     NodeRec *s_rec = (NodeRec *)(smem + L.rec);
-    double *s_ceps = (double *)(smem + L.ceps);
+    EpsRec *s_eps = (EpsRec *)(smem + L.ceps);
     double *s_rows = (double *)(smem + L.rows);
     double *s_acc = s_rows;                                 // epilogue only
     BalRec *s_bal = (BalRec *)(smem + L.bal);
@@ -205,7 +205,14 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                     rc.info = missb | ((uint32_t)(k < 8 ? k : 8) << 8) | ((uint32_t)k << 16);
                     rc.pad = 0u;
                     s_rec[rd * BA_NT + tid] = rc;
-                    if (MODE == IN_SWEEP && b == 0) s_ceps[tid] = a.c[cy];
+                    if (b == 0) {
+                        EpsRec er;
+                        er.a01 = al[0] | (al[1] << 16); er.a23 = al[2] | (al[3] << 16);
+                        er.a45 = al[4] | (al[5] << 16); er.a67 = al[6] | (al[7] << 16);
+                        er.a8 = al[8]; er.cy = cy;
+                        er.c = (MODE == IN_SWEEP) ? a.c[cy] : 0.0;
+                        s_eps[tid] = er;
+                    }
                     if (missb) key = (int)(cy & (BA_NCLS - 1));
                 }
                 // ================= sort: the round's nodes of list b by class (stable) =================
@@ -218,39 +225,49 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 if (b == 7)
 #endif
                 {
-                    auto eps_one = [&](int i) {
-                        const NodeRec &rc = s_rec[rd * BA_NT + i];
-                        const uint4 r0 = *(const uint4 *)&rc.a[0], r1 = *(const uint4 *)&rc.a[4], r2 = *(const uint4 *)&rc.a[8];
-                        const uint32_t cy = r2.y;
-                        const int k = (int)(r2.z >> 16);
-                        const uint2 e8 = __ldg(a.EPS8 + (size_t)(cy & 255u) * nv + ev);   // alpha_s = 0 beyond k
-                        uint32_t emb;
-                        if (!may_big)
-                            emb = ba_chain9(r0.x | (r0.y << 16), r0.z | (r0.w << 16), r1.x | (r1.y << 16), r1.z | (r1.w << 16), r2.x,
-                                            1u | (e8.x << 8), (e8.x >> 24) | (e8.y << 8), e8.y >> 24);
-                        else
-                            emb = ba_chain9_wide(rc.a, 1u | (e8.x << 8), (e8.x >> 24) | (e8.y << 8), e8.y >> 24);
-                        if (MODE == IN_SWEEP) {
-                            acc_eps = fma(ba_u2d(emb), s_ceps[i], acc_eps);
-                        } else if (MODE == IN_HC) {
-                            const double wk = s_w[k];
-                            if (wk != 0.0 && emb > 1u) acc_eps = fma(wk * (double)emb, log2((double)emb) - s_lebar[k], acc_eps);
-                            else if (wk != 0.0) acc_eps = fma(wk, -s_lebar[k], acc_eps);
-                        } else if (MODE == IN_DEBUG) {
-                            if (((u << m) | (uint32_t)ev) == a.dbg_x) a.dbg_out[cy - 1u] = emb;
-                        } else {
-                            cnt_terms += 1ull; cnt_emb += emb;
+                    const uint32_t sv8 = (m == 8) ? (uint32_t)ev : 0xffffffffu;      // B_8 = [sigma_8 = v] (m = 8 only)
+                    if (MODE == IN_SWEEP && !may_big && klen < 0) {
+                        double e0 = 0.0, e1 = 0.0;             // two chains; nodes esub, esub + epn, ...
+#pragma unroll 4
+                        for (int i = esub; i < nn; i += 2 * epn) {
+                            const uint4 p0 = *(const uint4 *)&s_eps[i];
+                            const uint4 q0 = *(const uint4 *)&s_eps[i].a8;
+                            const uint2 e8 = __ldg(a.EPS8 + (size_t)(q0.y & 255u) * nv + ev);   // alpha_s = 0 beyond k
+                            const uint32_t emb = ba_chain9(p0.x, p0.y, p0.z, p0.w, q0.x, e8.x, e8.y, (q0.y & 255u) == sv8);
+                            e0 = fma(ba_u2d(emb), __hiloint2double((int)q0.w, (int)q0.z), e0);
+                            const int i2 = i + epn;
+                            if (i2 < nn) {
+                                const uint4 p1 = *(const uint4 *)&s_eps[i2];
+                                const uint4 q1 = *(const uint4 *)&s_eps[i2].a8;
+                                const uint2 f8 = __ldg(a.EPS8 + (size_t)(q1.y & 255u) * nv + ev);
+                                const uint32_t emb2 = ba_chain9(p1.x, p1.y, p1.z, p1.w, q1.x, f8.x, f8.y, (q1.y & 255u) == sv8);
+                                e1 = fma(ba_u2d(emb2), __hiloint2double((int)q1.w, (int)q1.z), e1);
+                            }
                         }
-                    };
-                    if (klen >= 0) {                           // exact channel: only |y'| = klen has weight
-                        for (int i = esub; i < nn; i += epn)
-                            if ((int)(s_rec[rd * BA_NT + i].info >> 16) == klen) eps_one(i);
+                        acc_eps += e0 + e1;
                     } else {
-#pragma unroll 8
-                        for (int i = esub; i < nn; i += epn) eps_one(i);
+                        for (int i = esub; i < nn; i += epn) {
+                            const NodeRec &rc = s_rec[rd * BA_NT + i];
+                            const uint32_t cy = rc.id;
+                            const int k = (int)(rc.info >> 16);
+                            if (klen >= 0 && k != klen) continue;      // exact channel: only |y'| = klen has weight
+                            const uint2 e8 = __ldg(a.EPS8 + (size_t)(cy & 255u) * nv + ev);
+                            const uint32_t emb = ba_chain9_wide(rc.a, e8.x, e8.y, (cy & 255u) == sv8);
+                            if (MODE == IN_SWEEP) {
+                                acc_eps = fma(ba_u2d(emb), s_eps[i].c, acc_eps);
+                            } else if (MODE == IN_HC) {
+                                const double wk = s_w[k];
+                                if (wk != 0.0 && emb > 1u) acc_eps = fma(wk * (double)emb, log2((double)emb) - s_lebar[k], acc_eps);
+                                else if (wk != 0.0) acc_eps = fma(wk, -s_lebar[k], acc_eps);
+                            } else if (MODE == IN_DEBUG) {
+                                if (((u << m) | (uint32_t)ev) == a.dbg_x) a.dbg_out[cy - 1u] = emb;
+                            } else {
+                                cnt_terms += 1ull; cnt_emb += emb;
+                            }
+                        }
                     }
                 }
-                __syncthreads();                               // s_ceps is rewritten by the next round
+                __syncthreads();                               // s_eps is rewritten by the next round
             }
             // ================= merge the rounds: class bucket = its runs in round order =================
             if (tid < 32) {
@@ -340,7 +357,9 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                     uint32_t rb[BA_KG];
 #pragma unroll
                     for (int k = 0; k < BA_KG; k++) rb[k] = rowbase + gaddr[k];
+#ifndef BA_X_NOLOOP
                     ba_group_batch(acc, Bp, rb, bal, s_rec, len, wmeta, big);
+#endif
                 } else {
                     for (int i = 0; i < len; i++) {
                         const NodeRec &rc = s_rec[bal[i].node];
@@ -379,31 +398,47 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                     double s = 0.0;
                     if (re < nr) {
                         const uint4 rd = __ldg(a.g.R + ((size_t)cls * 2 + b) * a.g.nr + re);
-                        const uint32_t rB1lo = rd.y & 0xffu, ov = rd.y >> 16;
+                        const uint32_t ov = rd.y >> 16;
                         const uint32_t cz = ba_z_of_tail((uint32_t)b, rd.z >> 3);
                         const int jz = ba_len_of_code(cz);
-                        const uint32_t *r8 = a.g.R8 + ((size_t)cls * 2 + b) * 16 * a.g.nr + re;
-#pragma unroll 8                                           // four independent L2 reads of the chain tails in flight
-                        for (int i = rh; i < len; i += 2) {
-                            const BalRec bl = bal[i];
-                            const uint32_t cy = bl.id;
-                            const uint32_t x8 = __ldg(r8 + (size_t)((cy >> 4) & 15u) * a.g.nr);   // alpha_s = 0 beyond k
-                            uint32_t emb;
-                            if (!big) emb = ba_chain9(bl.a01, bl.a23, bl.a45, bl.a67, bl.a8, rd.x, rB1lo | (x8 << 8), x8 >> 24);
-                            else emb = ba_chain9_wide(s_rec[bl.node].a, rd.x, rB1lo | (x8 << 8), x8 >> 24);
-                            if (MODE == IN_SWEEP) {
-                                s = fma(ba_u2d(emb), ba_lds_f64(rowbase + (uint32_t)i * BA_ROWB + rd.z), s);
-                            } else if (MODE == IN_HC) {
-                                const int k = (int)(s_rec[bl.node].info >> 16);
-                                const double wk = s_w[k + jz];
-                                if (wk != 0.0) {
-                                    const double le = (emb > 1u) ? log2((double)emb) : 0.0;
-                                    s = fma(wk * (double)emb, le - s_lebar[k + jz], s);
+                        const uint32_t *r8 = a.g.R8 + ((size_t)cls * 2 + b) * 16 * a.g.nr + re;    // B_4..B_7 by sigma bits 4..7
+                        if (MODE == IN_SWEEP && !big) {
+                            const double *rrow = s_rows + (size_t)(buf * BA_RB_IN) * (BA_ROWB / 8) + (rd.z >> 3);
+                            double r0 = 0.0, r1 = 0.0;         // two chains; this replica's nodes rh, rh + 2, ...
+#pragma unroll 4
+                            for (int i = rh; i < len; i += 4) {
+                                const uint4 al = *(const uint4 *)&bal[i];
+                                const uint32_t x8 = __ldg(r8 + (size_t)((bal[i].id >> 4) & 15u) * a.g.nr);   // alpha_s = 0 beyond k
+                                const uint32_t emb = ba_chain9(al.x, al.y, al.z, al.w, 0u, rd.x, x8, 0u);
+                                r0 = fma(ba_u2d(emb), rrow[(size_t)i * (BA_ROWB / 8)], r0);
+                                if (i + 2 < len) {
+                                    const uint4 al2 = *(const uint4 *)&bal[i + 2];
+                                    const uint32_t y8 = __ldg(r8 + (size_t)((bal[i + 2].id >> 4) & 15u) * a.g.nr);
+                                    const uint32_t emb2 = ba_chain9(al2.x, al2.y, al2.z, al2.w, 0u, rd.x, y8, 0u);
+                                    r1 = fma(ba_u2d(emb2), rrow[(size_t)(i + 2) * (BA_ROWB / 8)], r1);
                                 }
-                            } else if (MODE == IN_DEBUG) {
-                                if (((u << m) | ov) == a.dbg_x) a.dbg_out[((size_t)cy << jz) + (cz - (1u << jz)) - 1u] = emb;
-                            } else {
-                                cnt_terms += 1ull; cnt_emb += emb;
+                            }
+                            s = r0 + r1;
+                        } else {
+                            for (int i = rh; i < len; i += 2) {
+                                const BalRec bl = bal[i];
+                                const uint32_t cy = bl.id;
+                                const uint32_t x8 = __ldg(r8 + (size_t)((cy >> 4) & 15u) * a.g.nr);
+                                const uint32_t emb = ba_chain9_wide(s_rec[bl.node].a, rd.x, x8, 0u);
+                                if (MODE == IN_SWEEP) {
+                                    s = fma(ba_u2d(emb), ba_lds_f64(rowbase + (uint32_t)i * BA_ROWB + rd.z), s);
+                                } else if (MODE == IN_HC) {
+                                    const int k = (int)(s_rec[bl.node].info >> 16);
+                                    const double wk = s_w[k + jz];
+                                    if (wk != 0.0) {
+                                        const double le = (emb > 1u) ? log2((double)emb) : 0.0;
+                                        s = fma(wk * (double)emb, le - s_lebar[k + jz], s);
+                                    }
+                                } else if (MODE == IN_DEBUG) {
+                                    if (((u << m) | ov) == a.dbg_x) a.dbg_out[((size_t)cy << jz) + (cz - (1u << jz)) - 1u] = emb;
+                                } else {
+                                    cnt_terms += 1ull; cnt_emb += emb;
+                                }
                             }
                         }
                     }

@@ -152,7 +152,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
         uint32_t eB0 = 0, eB1 = 0, eB2 = 0;                    // B(sigma_s, ev): B_0 = 1; alpha_s = 0 beyond t
         if (do_eps) {
             const uint2 e8 = __ldg(a.EPS8 + (size_t)(cy & 255u) * nv + ev);
-            eB0 = 1u | (e8.x << 8); eB1 = (e8.x >> 24) | (e8.y << 8); eB2 = e8.y >> 24;
+            eB0 = e8.x; eB1 = e8.y; eB2 = (m == 8 && (cy & 255u) == (uint32_t)ev) ? 1u : 0u;   // B_8 = [sigma_8 = v]
         }
         #ifdef BA_X_NORIDERS
         const int nr = 0;
@@ -164,7 +164,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
         if (re < nr) {
             const uint4 rd = __ldg(a.g.R + ((size_t)cls * 2 + b) * a.g.nr + re);
             const uint32_t x8 = __ldg(a.g.R8 + (((size_t)cls * 2 + b) * 16 + ((cy >> 4) & 15u)) * a.g.nr + re);
-            rB0 = rd.x; rB1 = (rd.y & 0xffu) | (x8 << 8); rB2 = x8 >> 24;     // B_0..3, B_4..7, B_8
+            rB0 = rd.x; rB1 = x8; rB2 = 0u;                     // B_0..3, B_4..7; B_8 = 0 (|z| >= 1)
             roff = rd.z; rown = rd.y >> 16;
         }
 
@@ -275,18 +275,33 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
 
                 // ---- the pair (v, empty) of every node: thread (v, node) ----------------------------------
                 if (do_eps) {
-                    for (int i = esub; i < len; i += epn) {
-                        uint32_t emb;
-                        if (!big) {
-                            const uint4 al = ba_lds_v4(balbase + (uint32_t)i * BA_BALB);
-                            emb = ba_chain9(al.x, al.y, al.z, al.w, bal[i].a8, eB0, eB1, eB2);
-                        } else emb = ba_chain9_wide(s_rec[bal[i].node].a, eB0, eB1, eB2);
-                        if (MODE == OUT_SWEEP) {
-                            acc_eps = fma(ba_u2d(emb), ba_lds_f64(rowbase + (uint32_t)i * BA_ROWB + (uint32_t)ev * 8u), acc_eps);
-                        } else if (MODE == OUT_DEBUG) {
-                            if (a.dbg_cz == 1u) a.dbg_out[((size_t)bal[i].id << m) | (size_t)ev] = emb;
-                        } else {
-                            cnt_terms += 1ull; cnt_emb += emb;
+                    const double *erow = s_rows + (size_t)(buf * BA_RB_OUT) * (BA_ROWB / 8) + ev;
+                    if (MODE == OUT_SWEEP && !big) {
+                        double e0 = 0.0, e1 = 0.0;             // two chains; nodes esub, esub + epn, ...
+#pragma unroll 4
+                        for (int i = esub; i < len; i += 2 * epn) {
+                            const uint4 al = *(const uint4 *)&bal[i];
+                            const uint32_t emb = ba_chain9(al.x, al.y, al.z, al.w, bal[i].a8, eB0, eB1, eB2);
+                            e0 = fma(ba_u2d(emb), erow[(size_t)i * (BA_ROWB / 8)], e0);
+                            const int i2 = i + epn;
+                            if (i2 < len) {
+                                const uint4 al2 = *(const uint4 *)&bal[i2];
+                                const uint32_t emb2 = ba_chain9(al2.x, al2.y, al2.z, al2.w, bal[i2].a8, eB0, eB1, eB2);
+                                e1 = fma(ba_u2d(emb2), erow[(size_t)i2 * (BA_ROWB / 8)], e1);
+                            }
+                        }
+                        acc_eps += e0 + e1;
+                    } else {
+                        for (int i = esub; i < len; i += epn) {
+                            const uint32_t emb = big ? ba_chain9_wide(s_rec[bal[i].node].a, eB0, eB1, eB2)
+                                                     : ba_chain9(bal[i].a01, bal[i].a23, bal[i].a45, bal[i].a67, bal[i].a8, eB0, eB1, eB2);
+                            if (MODE == OUT_SWEEP) {
+                                acc_eps = fma(ba_u2d(emb), erow[(size_t)i * (BA_ROWB / 8)], acc_eps);
+                            } else if (MODE == OUT_DEBUG) {
+                                if (a.dbg_cz == 1u) a.dbg_out[((size_t)bal[i].id << m) | (size_t)ev] = emb;
+                            } else {
+                                cnt_terms += 1ull; cnt_emb += emb;
+                            }
                         }
                     }
                 }
@@ -296,7 +311,9 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                         uint32_t rb[BA_KG];
 #pragma unroll
                         for (int k = 0; k < BA_KG; k++) rb[k] = rowbase + gaddr[k];
-                        ba_group_batch(acc, Bp, rb, bal, s_rec, len, wmeta, big);
+    #ifndef BA_X_NOLOOP
+                    ba_group_batch(acc, Bp, rb, bal, s_rec, len, wmeta, big);
+#endif
                     } else {
                         for (int i = 0; i < len; i++) {
                             const NodeRec &rc = s_rec[bal[i].node];
@@ -316,22 +333,34 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                     }
                     // ---- riders: deep pairs of this class, one per thread, all B_s static -----------------------
                     if (re < nr) {
-                        double s = acc_rid;
-                        for (int i = 0; i < len; i++) {
-                            uint32_t emb;
-                            if (!big) {
-                                const uint4 al = ba_lds_v4(balbase + (uint32_t)i * BA_BALB);
-                                emb = ba_chain9(al.x, al.y, al.z, al.w, bal[i].a8, rB0, rB1, rB2);
-                            } else emb = ba_chain9_wide(s_rec[bal[i].node].a, rB0, rB1, rB2);
-                            if (MODE == OUT_SWEEP) {
-                                s = fma(ba_u2d(emb), ba_lds_f64(rowbase + (uint32_t)i * BA_ROWB + roff), s);
-                            } else if (MODE == OUT_DEBUG) {
-                                if (rown == a.dbg_cz) a.dbg_out[((size_t)bal[i].id << m) | (size_t)(roff >> 3)] = emb;
-                            } else {
-                                cnt_terms += 1ull; cnt_emb += emb;
+                        const double *rrow = s_rows + (size_t)(buf * BA_RB_OUT) * (BA_ROWB / 8) + (roff >> 3);
+                        if (MODE == OUT_SWEEP && !big) {
+                            double r0 = 0.0, r1 = 0.0;
+#pragma unroll 4
+                            for (int i = 0; i < len; i += 2) {
+                                const uint4 al = *(const uint4 *)&bal[i];
+                                const uint32_t emb = ba_chain9(al.x, al.y, al.z, al.w, bal[i].a8, rB0, rB1, rB2);
+                                r0 = fma(ba_u2d(emb), rrow[(size_t)i * (BA_ROWB / 8)], r0);
+                                if (i + 1 < len) {
+                                    const uint4 al2 = *(const uint4 *)&bal[i + 1];
+                                    const uint32_t emb2 = ba_chain9(al2.x, al2.y, al2.z, al2.w, bal[i + 1].a8, rB0, rB1, rB2);
+                                    r1 = fma(ba_u2d(emb2), rrow[(size_t)(i + 1) * (BA_ROWB / 8)], r1);
+                                }
+                            }
+                            acc_rid += r0 + r1;
+                        } else {
+                            for (int i = 0; i < len; i++) {
+                                const uint32_t emb = big ? ba_chain9_wide(s_rec[bal[i].node].a, rB0, rB1, rB2)
+                                                         : ba_chain9(bal[i].a01, bal[i].a23, bal[i].a45, bal[i].a67, bal[i].a8, rB0, rB1, rB2);
+                                if (MODE == OUT_SWEEP) {
+                                    acc_rid = fma(ba_u2d(emb), rrow[(size_t)i * (BA_ROWB / 8)], acc_rid);
+                                } else if (MODE == OUT_DEBUG) {
+                                    if (rown == a.dbg_cz) a.dbg_out[((size_t)bal[i].id << m) | (size_t)(roff >> 3)] = emb;
+                                } else {
+                                    cnt_terms += 1ull; cnt_emb += emb;
+                                }
                             }
                         }
-                        acc_rid = s;
                     }
                 }
                 ba_mbar_arrive(sEmpty + 8u * buf);             // this thread has finished reading the stage

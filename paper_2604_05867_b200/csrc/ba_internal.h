@@ -52,7 +52,7 @@
 #define BA_NCLS 16           // 2^BA_KB classes
 #define BA_ROWB 2048u        // bytes between staged operand rows (2^BA_MLOW doubles)
 #define BA_RB_IN 32          // nodes per batch, input sweep (operand half-rows of 2^m doubles)
-#define BA_SBR 3             // input sweep: phase-A rounds (of BA_NT nodes) per super-batch
+#define BA_SBR 2             // input sweep: phase-A rounds (of BA_NT nodes) per super-batch
 #define BA_RB_OUT 32         // nodes per batch, output sweep (operand rows of 2^m doubles)
 
 struct KConst {                       // passed by value to kernels
@@ -91,6 +91,13 @@ __device__ __forceinline__ BalRec ba_make_bal(const NodeRec &rc, uint32_t node) 
     return bl;
 }
 
+// A node of a phase-A round as the (v, empty) pairs of the input sweep read it, 32 bytes.
+struct EpsRec {
+    uint32_t a01, a23, a45, a67;      // alphas as 16-bit halves (garbage if one needs more: the wide path reads NodeRec)
+    uint32_t a8, cy;                  // alpha_8, code(y')
+    double c;                         // c(y')
+};
+
 // The schedule of one side, device pointers (host side: GroupSide in ba_tables.h)
 struct GroupDev {
     const uint4 *GB;                  // [cls][b][k][tid]
@@ -102,7 +109,7 @@ struct GroupDev {
     const uint4 *R;                   // riders [cls][b][nr]
     const uint16_t *r_cnt;            // [cls][b]
     const uint16_t *r_csr;            // [cls][b][nown + 1]
-    const uint32_t *R8;               // [cls][b][16][nr]
+    const uint32_t *R8;               // [cls][b][16][nr]: B_4..B_7 by the sigma bits 4..7
     int nr, nown;
 };
 

@@ -19,7 +19,7 @@ struct GroupSide {
     std::vector<uint4> R;           // riders [BA_NCLS][2][nr]: {B0..B3, B4 | owner << 16, row byte offset, 0}, sorted by owner
     std::vector<uint16_t> r_cnt;    // [BA_NCLS][2]
     std::vector<uint16_t> r_csr;    // [BA_NCLS][2][nown + 1] rider range of an owner
-    std::vector<uint32_t> R8;       // [BA_NCLS][2][16][nr]: bytes = B_5..B_8 of the rider for sigma bits 4..7
+    std::vector<uint32_t> R8;       // [BA_NCLS][2][16][nr]: bytes = B_4..B_7 of the rider for sigma bits 4..7 (B_8 = 0)
     int nr = 0;
     unsigned long long npairs[2] = {0, 0}, nslots[2] = {0, 0}, ngroups[2] = {0, 0};   // statistics
 };
@@ -27,7 +27,7 @@ struct GroupSide {
 struct TileTables {
     int m = 0, nv = 0;
     GroupSide in, out;
-    std::vector<uint2> EPS8;        // [256][nv]: bytes s-1 = B(sigma_s, v), s = 1..8, sigma = the row index
+    std::vector<uint2> EPS8;        // [256][nv]: byte s = B(sigma_s, v), s = 0..7, sigma = the row index
     bool ok = false;
 };
 
@@ -49,7 +49,7 @@ struct TTPair { int v; uint32_t cz; };
 //   * warps are filled so that the four schedulers of the SM carry about the same number of instructions.
 template <typename KeyOf, typename OwnerOf, typename BPack, typename DeepOf>
 static bool tt_deal(int m, int b, const std::vector<TTPair> &pairs, KeyOf key_of, OwnerOf owner_of, BPack bpack, DeepOf deep,
-                    GroupSide &S) {
+                    const double *warp_extra, GroupSide &S) {
     struct Grp { int type; uint32_t key; std::vector<int> items; };
     const int np = (int)pairs.size();
     std::vector<int> ptype(np, 1);
@@ -120,15 +120,18 @@ static bool tt_deal(int m, int b, const std::vector<TTPair> &pairs, KeyOf key_of
     for (auto &bd : bundles) if ((int)bd.lv.size() > BA_KG) return false;
     // ---- bundles -> warp indices: heaviest first onto the scheduler (warp & 3) with the least load
     std::stable_sort(bundles.begin(), bundles.end(), [](const Bundle &x, const Bundle &y) { return x.cost > y.cost; });
+    // warp_extra[w] = instructions per node the warp spends outside its levels (riders): the heavy bundles go to the
+    // warps without riders, and a scheduler's load counts both
     double load[4] = {0, 0, 0, 0};
-    int used[4] = {0, 0, 0, 0};
+    bool taken[BA_NT / 32] = {false};
     for (auto &bd : bundles) {
-        int best = -1;
-        for (int s = 0; s < 4; s++)
-            if (used[s] < NW / 4 && (best < 0 || load[s] < load[best])) best = s;
-        if (best < 0) return false;
-        const int warp = used[best] * 4 + best;
-        used[best]++; load[best] += bd.cost;
+        int warp = -1;
+        for (int w = 0; w < NW; w++) {
+            if (taken[w]) continue;
+            if (warp < 0 || load[w & 3] + warp_extra[w] < load[warp & 3] + warp_extra[warp] - 1e-9) warp = w;
+        }
+        if (warp < 0) return false;
+        taken[warp] = true; load[warp & 3] += bd.cost + warp_extra[warp];
         S.GW[(size_t)b * NW + warp] = (uint8_t)(bd.lv.size() | (bd.type << 4));
         for (size_t k = 0; k < bd.lv.size(); k++) {
             const Lvl &lv = levels[bd.lv[k]];
@@ -217,7 +220,19 @@ static inline void build_tile_tables(int m, TileTables &T) {
             for (int v = 0; v < nv; v++)
                 for (uint32_t cz = 2; cz < (uint32_t)NZc; cz++)
                     if (Bof(cz, v) && first_bit(cz) == b) pairs.push_back(TTPair{v, cz});
-            if (!tt_deal(m, b, pairs, key_of, owner_of, bpack, deep, S)) return;
+            // riders (the pairs deep under the class) sit on fixed threads: input sweep, two replicas on the last warps
+            // of each half of the CTA, every other node each; output sweep, the last warps
+            size_t ndeep = 0;
+            for (int cls = 0; cls < BA_NCLS; cls++) {
+                size_t c = 0;
+                for (const TTPair &p : pairs) c += deep(cls, p);
+                ndeep = std::max(ndeep, c);
+            }
+            double warp_extra[BA_NT / 32];
+            const int rw = (int)((ndeep + 31) / 32);
+            for (int w = 0; w < NW; w++)
+                warp_extra[w] = side ? (w >= NW - rw ? 14.0 : 0.0) : ((w & (NW / 2 - 1)) >= NW / 2 - rw ? 8.0 : 0.0);
+            if (!tt_deal(m, b, pairs, key_of, owner_of, bpack, deep, warp_extra, S)) return;
             // ---- CSR of the epilogue: the slots of every owner, in slot order
             std::vector<std::vector<uint16_t>> slots(S.nown);
             for (int k = 0; k < BA_KG; k++)
@@ -272,20 +287,21 @@ static inline void build_tile_tables(int m, TileTables &T) {
                 for (size_t e = 0; e < rider_pairs[i].size(); e++) {
                     const TTPair &p = rider_pairs[i][e];
                     const int lz = 31 - __builtin_clz(p.cz);
-                    uint32_t x = 0;
-                    for (int sft = 5; sft <= 8; sft++)
-                        if (lz + sft <= m) x |= Bof(tt_prepend((hi << 4) | (uint32_t)cls, sft, p.cz), p.v) << (8 * (sft - 5));
+                    uint32_t x = 0;                            // B_8 = 0: |z| >= 1
+                    for (int sft = 4; sft <= 7; sft++)
+                        if (lz + sft <= m) x |= Bof(tt_prepend((hi << 4) | (uint32_t)cls, sft, p.cz), p.v) << (8 * (sft - 4));
                     S.R8[(i * 16 + hi) * S.nr + e] = x;
                 }
         }
     }
-    // ---- direct table of the pairs (v, empty): all B(sigma_s, v), s = 1..8 --------------------------------------
+    // ---- direct table of the pairs (v, empty): .x = 1 | B_1 << 8 | B_2 << 16 | B_3 << 24, .y = B_4 | .. | B_7 << 24 with
+    // B_s = B(sigma_s, v) (B_0 = emb(empty, v) = 1; B_8 = [sigma_8 = v] is formed by the kernels) ---------------------
     T.EPS8.assign((size_t)256 * nv, make_uint2(0u, 0u));
     for (uint32_t sig = 0; sig < 256u; sig++)
         for (int v = 0; v < nv; v++) {
-            uint32_t w[2] = {0u, 0u};
-            for (int sft = 1; sft <= 8 && sft <= m; sft++)
-                w[(sft - 1) / 4] |= Bof((1u << sft) | (sig & ((1u << sft) - 1u)), v) << (8 * ((sft - 1) % 4));
+            uint32_t w[2] = {1u, 0u};
+            for (int sft = 1; sft <= 7 && sft <= m; sft++)
+                w[sft / 4] |= Bof((1u << sft) | (sig & ((1u << sft) - 1u)), v) << (8 * (sft % 4));
             T.EPS8[(size_t)sig * nv + v] = make_uint2(w[0], w[1]);
         }
     T.ok = true;
