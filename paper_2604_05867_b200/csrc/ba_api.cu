@@ -30,6 +30,7 @@ struct ba_ctx {
     double *c = nullptr, *Hc = nullptr, *Apart = nullptr, *S = nullptr, *part = nullptr, *scal = nullptr, *hist = nullptr;
     GroupDev gin, gout;              // pair schedules of the two sweeps (device pointers into scratch)
     uint2 *EPS8 = nullptr;
+    uint32_t *EPSH = nullptr;
     unsigned int *counters = nullptr;
     unsigned long long *cnt = nullptr;
     size_t npart_cap = 0;
@@ -68,7 +69,7 @@ static double host_binom(int n, int k) {
 // ------------------------------------------------------------------------------------------------ scratch layout
 struct SideLayout { size_t GB, GA, GO, GW, csr_off, csr_idx, R, r_cnt, r_csr, R8; };
 struct ScratchLayout {
-    size_t c, Hc, Apart, S, part, scal, hist, EPS8, counters, cnt, total;
+    size_t c, Hc, Apart, S, part, scal, hist, EPS8, EPSH, counters, cnt, total;
     SideLayout in, out;
     size_t napart, npart_cap;
 };
@@ -119,6 +120,7 @@ static void scratch_layout(int n, const TileTables &T, ScratchLayout &L) {
     L.scal = o; o += align256(8 * 8);
     L.hist = o; o += align256((size_t)BA_HIST_CAP * 3 * 8);
     L.EPS8 = o; o += align256(T.EPS8.size() * 8);
+    L.EPSH = o; o += align256(T.EPSH.size() * 4);
     side_layout(T.in, L.in, o);
     side_layout(T.out, L.out, o);
     L.counters = o; o += align256(16 * 4);
@@ -321,11 +323,12 @@ static int finish_create(ba_ctx *c) {
     unsigned char *s = c->scratch;
     c->c = (double *)(s + L.c); c->Hc = (double *)(s + L.Hc); c->Apart = (double *)(s + L.Apart); c->S = (double *)(s + L.S);
     c->part = (double *)(s + L.part); c->scal = (double *)(s + L.scal); c->hist = (double *)(s + L.hist);
-    c->EPS8 = (uint2 *)(s + L.EPS8);
+    c->EPS8 = (uint2 *)(s + L.EPS8); c->EPSH = (uint32_t *)(s + L.EPSH);
     c->counters = (unsigned int *)(s + L.counters); c->cnt = (unsigned long long *)(s + L.cnt);
     c->napart = L.napart; c->npart_cap = L.npart_cap;
 
     CK(upload(c->EPS8, T.EPS8, c->st));
+    CK(upload(c->EPSH, T.EPSH, c->st));
     CK(upload_side(s, T.in, L.in, c->gin, c->st));
     CK(upload_side(s, T.out, L.out, c->gout, c->st));
     CK(cudaMemsetAsync(c->c, 0, 8, c->st));                  // c[0] is never written by k_out_final
@@ -450,7 +453,7 @@ extern "C" int ba_set_mode(ba_ctx *c, int mode) {
 // ------------------------------------------------------------------------------------------------ launches
 static InArgs make_in_args(ba_ctx *c) {
     InArgs a;
-    a.kc = c->kc; a.g = c->gin; a.EPS8 = c->EPS8;
+    a.kc = c->kc; a.g = c->gin; a.EPS8 = c->EPS8; a.EPSH = c->EPSH;
     a.c = c->c; a.S = c->S;
     a.counter = c->counters; a.sym = 0; a.dbg_x = 0; a.dbg_out = nullptr; a.cnt = c->cnt;
     return a;

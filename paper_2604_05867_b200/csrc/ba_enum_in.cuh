@@ -35,12 +35,14 @@
 enum { IN_SWEEP = 0, IN_HC = 1, IN_DEBUG = 2, IN_COUNT = 3 };
 
 #define BA_IN_SB (BA_SBR * BA_NT)                           // nodes per super-batch
-#define BA_IN_MAXB (BA_NCLS + BA_IN_SB / BA_RB_IN)
+#define BA_IN_NBKT (2 * BA_NCLS)                            // buckets: class, with / without list b (the latter: b = 0 only)
+#define BA_IN_MAXB (BA_IN_NBKT + BA_IN_SB / BA_RB_IN)
 
 struct InArgs {
     KConst kc;
     GroupDev g;               // schedule of the input sweep (owner = v, operand position = code(z[1:]))
-    const uint2 *EPS8;        // [256][2^m]: B(sigma_s, v), s = 1..8, of the pair (v, empty)
+    const uint2 *EPS8;        // [256][2^m]: B(sigma_s, v), s = 0..7, of the pair (v, empty)
+    const uint32_t *EPSH;     // [cls][16][2^m]: B_4..B_7 of the pair (v, empty) by the sigma bits 4..7: a class's slice
     const double *c;          // IN_SWEEP: c[code(y)], 2^{n+1} entries (entry 0 unused)
     double *S;                // out: [2][2^n] partial sums of the two lists (IN_SWEEP: S_b, IN_HC: H_b)
     unsigned int *counter;    // work counter (zeroed before launch)
@@ -50,26 +52,23 @@ struct InArgs {
     unsigned long long *cnt;  // IN_COUNT: [0] terms, [1] emb sum
 };
 
-struct InSmem { size_t rec, ceps, rows, bal, ordr, seg, order, gstart, wcnt, batch, rsum, sub, kcw, item, total; };
+struct InSmem { size_t rec, slice, rows, bal, ordr, seg, order, gstart, wcnt, batch, rsum, sub, kcw, item, total; };
 
 __host__ __device__ static inline InSmem enum_in_smem(int nr) {
     InSmem s;
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o += (bytes + 15) & ~(size_t)15; return at; };
     s.rec = take((size_t)BA_IN_SB * sizeof(NodeRec));
-    {                                                      // c(y') of a round (phase A / eps) and the rider sums
-        const size_t ce = (size_t)BA_NT * sizeof(EpsRec), rs = (size_t)2 * 2 * nr * 8;   // of phase B share one area
-        s.ceps = take(ce > rs ? ce : rs);
-        s.rsum = s.ceps;
-    }
+    s.rsum = take((size_t)2 * 2 * nr * 8);                 // rider sums of a batch, two replicas, double buffered
+    s.slice = take((size_t)2 * 16 * ((size_t)1 << BA_MLOW) * 4);   // B_4..B_7 of the pairs (v, empty) of a class, double buffered
     size_t rows = (size_t)2 * BA_RB_IN * BA_ROWB, ac = ((size_t)BA_NSLOT + 1) * BA_NT * 8;
     s.rows = take(rows > ac ? rows : ac);                  // the epilogue's accumulator staging aliases the rows
     s.bal = take((size_t)2 * BA_RB_IN * sizeof(BalRec));
     s.ordr = take((size_t)BA_SBR * BA_NT * 2);             // per round: the round's nodes by class
-    s.seg = take((size_t)BA_SBR * (BA_NCLS + 1) * 2);
+    s.seg = take((size_t)BA_SBR * (BA_IN_NBKT + 1) * 2);
     s.order = take((size_t)BA_IN_SB * 2);                  // merged: class-major node ids of the super-batch
-    s.gstart = take((size_t)(BA_NCLS + 1) * 2);
-    s.wcnt = take((size_t)(BA_NT / 32) * BA_NCLS * 2);
+    s.gstart = take((size_t)(BA_IN_NBKT + 1) * 2);
+    s.wcnt = take((size_t)(BA_NT / 32) * BA_IN_NBKT * 2);
     s.batch = take((size_t)BA_IN_MAXB * 4);
     s.sub = take(32 * 4);
     s.kcw = take(2 * (BA_NMAX_I + 1) * 8);
@@ -92,7 +91,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
     const InSmem L = enum_in_smem(a.g.nr);
 
     NodeRec *s_rec = (NodeRec *)(smem + L.rec);
-    EpsRec *s_eps = (EpsRec *)(smem + L.ceps);
+    uint32_t *s_slice = (uint32_t *)(smem + L.slice);
     double *s_rows = (double *)(smem + L.rows);
     double *s_acc = s_rows;                                 // epilogue only
     BalRec *s_bal = (BalRec *)(smem + L.bal);
@@ -203,100 +202,42 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                     for (int s = 0; s < 9; s++) rc.a[s] = al[s];
                     rc.id = cy;
                     rc.info = missb | ((uint32_t)(k < 8 ? k : 8) << 8) | ((uint32_t)k << 16);
-                    rc.pad = 0u;
                     s_rec[rd * BA_NT + tid] = rc;
-                    if (b == 0) {
-                        EpsRec er;
-                        er.a01 = al[0] | (al[1] << 16); er.a23 = al[2] | (al[3] << 16);
-                        er.a45 = al[4] | (al[5] << 16); er.a67 = al[6] | (al[7] << 16);
-                        er.a8 = al[8]; er.cy = cy;
-                        er.c = (MODE == IN_SWEEP) ? a.c[cy] : 0.0;
-                        s_eps[tid] = er;
-                    }
+                    // buckets: class for the nodes that carry list b; for b = 0 the others follow in buckets 16 + class:
+                    // they contribute the pair (v, empty) only (exact channel: only if |y'| = klen)
                     if (missb) key = (int)(cy & (BA_NCLS - 1));
+                    else if (b == 0 && (klen < 0 || k == klen)) key = BA_NCLS + (int)(cy & (BA_NCLS - 1));
                 }
-                // ================= sort: the round's nodes of list b by class (stable) =================
-                ba_bucket_sort<BA_NCLS>(key, s_ordr + (size_t)rd * BA_NT, s_wcnt, s_seg + rd * (BA_NCLS + 1));
-
-                // ================= eps: the pair (v, empty) of every node of the round =================
-#ifndef BA_X_NOEPS
-                if (b == 0)
-#else
-                if (b == 7)
-#endif
-                {
-                    const uint32_t sv8 = (m == 8) ? (uint32_t)ev : 0xffffffffu;      // B_8 = [sigma_8 = v] (m = 8 only)
-                    if (MODE == IN_SWEEP && !may_big && klen < 0) {
-                        double e0 = 0.0, e1 = 0.0;             // two chains; nodes esub, esub + epn, ...
-#pragma unroll 4
-                        for (int i = esub; i < nn; i += 2 * epn) {
-                            const uint4 p0 = *(const uint4 *)&s_eps[i];
-                            const uint4 q0 = *(const uint4 *)&s_eps[i].a8;
-                            const uint2 e8 = __ldg(a.EPS8 + (size_t)(q0.y & 255u) * nv + ev);   // alpha_s = 0 beyond k
-                            const uint32_t emb = ba_chain9(p0.x, p0.y, p0.z, p0.w, q0.x, e8.x, e8.y, (q0.y & 255u) == sv8);
-                            e0 = fma(ba_u2d(emb), __hiloint2double((int)q0.w, (int)q0.z), e0);
-                            const int i2 = i + epn;
-                            if (i2 < nn) {
-                                const uint4 p1 = *(const uint4 *)&s_eps[i2];
-                                const uint4 q1 = *(const uint4 *)&s_eps[i2].a8;
-                                const uint2 f8 = __ldg(a.EPS8 + (size_t)(q1.y & 255u) * nv + ev);
-                                const uint32_t emb2 = ba_chain9(p1.x, p1.y, p1.z, p1.w, q1.x, f8.x, f8.y, (q1.y & 255u) == sv8);
-                                e1 = fma(ba_u2d(emb2), __hiloint2double((int)q1.w, (int)q1.z), e1);
-                            }
-                        }
-                        acc_eps += e0 + e1;
-                    } else {
-                        for (int i = esub; i < nn; i += epn) {
-                            const NodeRec &rc = s_rec[rd * BA_NT + i];
-                            const uint32_t cy = rc.id;
-                            const int k = (int)(rc.info >> 16);
-                            if (klen >= 0 && k != klen) continue;      // exact channel: only |y'| = klen has weight
-                            const uint2 e8 = __ldg(a.EPS8 + (size_t)(cy & 255u) * nv + ev);
-                            const uint32_t emb = ba_chain9_wide(rc.a, e8.x, e8.y, (cy & 255u) == sv8);
-                            if (MODE == IN_SWEEP) {
-                                acc_eps = fma(ba_u2d(emb), s_eps[i].c, acc_eps);
-                            } else if (MODE == IN_HC) {
-                                const double wk = s_w[k];
-                                if (wk != 0.0 && emb > 1u) acc_eps = fma(wk * (double)emb, log2((double)emb) - s_lebar[k], acc_eps);
-                                else if (wk != 0.0) acc_eps = fma(wk, -s_lebar[k], acc_eps);
-                            } else if (MODE == IN_DEBUG) {
-                                if (((u << m) | (uint32_t)ev) == a.dbg_x) a.dbg_out[cy - 1u] = emb;
-                            } else {
-                                cnt_terms += 1ull; cnt_emb += emb;
-                            }
-                        }
-                    }
-                }
-                __syncthreads();                               // s_eps is rewritten by the next round
+                // ================= sort: the round's nodes by bucket (stable) =================
+                ba_bucket_sort<BA_IN_NBKT>(key, s_ordr + (size_t)rd * BA_NT, s_wcnt, s_seg + rd * (BA_IN_NBKT + 1));
             }
-            // ================= merge the rounds: class bucket = its runs in round order =================
+            // ================= merge the rounds: bucket = its runs in round order =================
             if (tid < 32) {
                 int cnt = 0;
-                const int cq = tid & (BA_NCLS - 1);
-                if (tid < BA_NCLS)
-                    for (int rd = 0; rd < nrounds; rd++) {
-                        const uint16_t *sg = s_seg + rd * (BA_NCLS + 1) + cq;
-                        cnt += sg[1] - sg[0];
-                    }
+                for (int rd = 0; rd < nrounds; rd++) {
+                    const uint16_t *sg = s_seg + rd * (BA_IN_NBKT + 1) + tid;
+                    cnt += sg[1] - sg[0];
+                }
                 int incl = cnt;
                 for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += t; }
                 int pos = incl - cnt;
-                if (tid < BA_NCLS) {
-                    s_gstart[tid] = (uint16_t)pos;
-                    if (tid == BA_NCLS - 1) s_gstart[BA_NCLS] = (uint16_t)incl;
-                    for (int rd = 0; rd < nrounds; rd++) {
-                        const uint16_t *sg = s_seg + rd * (BA_NCLS + 1) + cq;
-                        const uint16_t *od = s_ordr + (size_t)rd * BA_NT;
-                        for (int i = sg[0]; i < sg[1]; i++) s_order[pos++] = (uint16_t)(rd * BA_NT + od[i]);
-                    }
+                s_gstart[tid] = (uint16_t)pos;
+                if (tid == 31) s_gstart[32] = (uint16_t)incl;
+                for (int rd = 0; rd < nrounds; rd++) {
+                    const uint16_t *sg = s_seg + rd * (BA_IN_NBKT + 1) + tid;
+                    const uint16_t *od = s_ordr + (size_t)rd * BA_NT;
+                    for (int i = sg[0]; i < sg[1]; i++) s_order[pos++] = (uint16_t)(rd * BA_NT + od[i]);
                 }
                 __syncwarp();
-                if (tid == 0) {                                // batches: <= BA_RB_IN consecutive nodes of one class
+                if (tid == 0) {                                // batches: <= BA_RB_IN consecutive nodes of one bucket, class-major
                     int nb = 0;
-                    for (int kq = 0; kq < BA_NCLS; kq++)
-                        for (int off = s_gstart[kq]; off < s_gstart[kq + 1]; off += BA_RB_IN) {
-                            const int len = (s_gstart[kq + 1] - off < BA_RB_IN) ? (s_gstart[kq + 1] - off) : BA_RB_IN;
-                            s_batch[nb++] = (uint32_t)off | ((uint32_t)len << 16) | ((uint32_t)kq << 24);
+                    for (int cq = 0; cq < BA_NCLS; cq++)
+                        for (int kind = 0; kind < 2; kind++) {
+                            const int kq = kind * BA_NCLS + cq;
+                            for (int off = s_gstart[kq]; off < s_gstart[kq + 1]; off += BA_RB_IN) {
+                                const int len = (s_gstart[kq + 1] - off < BA_RB_IN) ? (s_gstart[kq + 1] - off) : BA_RB_IN;
+                                s_batch[nb++] = (uint32_t)off | ((uint32_t)len << 16) | ((uint32_t)kq << 24);
+                            }
                         }
                     s_item[1] = (uint32_t)nb;
                 }
@@ -305,10 +246,19 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
 
             // ================= phase B: batches of one class =================
             const int nbatch = (int)s_item[1];
+            int st_cls = -1, st_sb = 0, cp_cls = -1, cp_sb = 0;     // slice double buffer: staging side, computing side
             auto stage = [&](int j) {                          // half rows and alphas of batch j
                 const uint32_t bi = s_batch[j];
                 const int start = (int)(bi & 0xffffu), len = (int)((bi >> 16) & 0xffu), buf = j & 1;
-                if (MODE == IN_SWEEP) {
+                const int scls = (int)(bi >> 24) & (BA_NCLS - 1);
+                if (b == 0 && scls != st_cls) {                // a new class: its slice of B_4..B_7 of the pairs (v, empty)
+                    st_cls = scls; st_sb ^= 1;
+                    const uint32_t *src = a.EPSH + (size_t)scls * 16 * nv;
+                    const uint32_t dst = ba_smem_addr(s_slice) + (uint32_t)st_sb * (16u << BA_MLOW) * 4u;
+                    for (int e = tid; e < 16 * nv; e += BA_NT)
+                        asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst + (uint32_t)((e >> m) << BA_MLOW) * 4u + (uint32_t)(e & (nv - 1)) * 4u), "l"(src + e) : "memory");
+                }
+                if (MODE == IN_SWEEP && (bi >> 24) < BA_NCLS) {
                     // 16-byte pieces (positions 2pc, 2pc+1), 2^{m-1} per half row: a thread always copies the same
                     // piece, of every st_step-th row
                     for (int i = st_i0; i < len; i += st_step) {
@@ -323,11 +273,14 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 if (tid < len) {
                     const int node = s_order[start + tid];
                     s_bal[buf * BA_RB_IN + tid] = ba_make_bal(s_rec[node], (uint32_t)node);
+                    if (MODE == IN_SWEEP && b == 0)            // operand of the pair (v, empty): c(y'), lands with the rows
+                        ba_cp_async8(ba_smem_addr(&s_bal[buf * BA_RB_IN + tid].x0), a.c + s_rec[node].id);
                 }
             };
             auto flush = [&](int j) {                          // thread v collects the rider sums of batch j
                 if (MODE != IN_SWEEP && MODE != IN_HC) return;
                 if (tid >= nv) return;
+                if ((s_batch[j] >> 24) >= BA_NCLS) return;     // a batch without list b has no riders
                 const int cls = (int)(s_batch[j] >> 24), buf = j & 1;
                 const uint16_t *cs = a.g.r_csr + (size_t)(cls * 2 + b) * (nv + 1) + tid;
                 const int e0 = cs[0], e1 = cs[1];
@@ -336,12 +289,16 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
             if (nbatch > 0) stage(0);
             for (int j = 0; j < nbatch; j++) {
                 const uint32_t bi = s_batch[j];
-                const int len = (int)((bi >> 16) & 0xffu), cls = (int)(bi >> 24), buf = j & 1;
+                const int len = (int)((bi >> 16) & 0xffu), cls = (int)(bi >> 24) & (BA_NCLS - 1), kind = (int)(bi >> 28), buf = j & 1;
+                if (b == 0 && cls != cp_cls) { cp_cls = cls; cp_sb ^= 1; }
+                uint32_t eB0 = 0u;                             // 1 | B_1..B_3 of the pair (ev, empty): a constant of the class
+                if (b == 0) eB0 = __ldg(a.EPS8 + (size_t)cls * nv + ev).x;
                 // the slots' B_s do not depend on the staged rows: fetch them before waiting
                 uint32_t Bp[BA_NSLOT];
 #pragma unroll
                 for (int k = 0; k < BA_KG; k++) {
-                    const uint4 bb = __ldg(a.g.GB + (((size_t)cls * 2 + b) * BA_KG + k) * BA_NT + tid);
+                    uint4 bb = make_uint4(0u, 0u, 0u, 0u);
+                    if (kind == 0) bb = __ldg(a.g.GB + (((size_t)cls * 2 + b) * BA_KG + k) * BA_NT + tid);
                     Bp[k * BA_GP] = bb.x; Bp[k * BA_GP + 1] = bb.y; Bp[k * BA_GP + 2] = bb.z; Bp[k * BA_GP + 3] = bb.w;
                 }
                 ba_cp_async_wait_all();
@@ -352,6 +309,48 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 const BalRec *bal = s_bal + buf * BA_RB_IN;
                 bool big = false;
                 if (may_big) big = __any_sync(0xffffffffu, lane < len && bal[lane].big != 0u);
+                // ---- the pair (v, empty) of every node of the batch: thread (v, node) -----------------------------
+                if (b == 0 && (kind == 1 || klen < 0)) {
+                    const uint32_t sv8 = (m == 8) ? (uint32_t)ev : 0xffffffffu;      // B_8 = [sigma_8 = v] (m = 8 only)
+                    const uint32_t *sl = s_slice + (size_t)cp_sb * (16u << BA_MLOW) + ev;    // [sigma bits 4..7][v]
+                    if (MODE == IN_SWEEP && !big) {
+                        double e0 = 0.0, e1 = 0.0;             // two chains; nodes esub, esub + epn, ...
+#pragma unroll 4
+                        for (int i = esub; i < len; i += 2 * epn) {
+                            const uint4 al = *(const uint4 *)&bal[i];
+                            const uint32_t cy = bal[i].id;
+                            const uint32_t emb = ba_chain9(al.x, al.y, al.z, al.w, bal[i].a8, eB0, sl[((cy >> 4) & 15u) << BA_MLOW], (cy & 255u) == sv8);
+                            e0 = fma(ba_u2d(emb), bal[i].x0, e0);
+                            const int i2 = i + epn;
+                            if (i2 < len) {
+                                const uint4 al2 = *(const uint4 *)&bal[i2];
+                                const uint32_t cy2 = bal[i2].id;
+                                const uint32_t emb2 = ba_chain9(al2.x, al2.y, al2.z, al2.w, bal[i2].a8, eB0, sl[((cy2 >> 4) & 15u) << BA_MLOW], (cy2 & 255u) == sv8);
+                                e1 = fma(ba_u2d(emb2), bal[i2].x0, e1);
+                            }
+                        }
+                        acc_eps += e0 + e1;
+                    } else {
+                        for (int i = esub; i < len; i += epn) {
+                            const NodeRec &rc = s_rec[bal[i].node];
+                            const uint32_t cy = rc.id;
+                            const int k = (int)(rc.info >> 16);
+                            const uint32_t emb = ba_chain9_wide(rc.a, eB0, sl[((cy >> 4) & 15u) << BA_MLOW], (cy & 255u) == sv8);
+                            if (MODE == IN_SWEEP) {
+                                acc_eps = fma(ba_u2d(emb), bal[i].x0, acc_eps);
+                            } else if (MODE == IN_HC) {
+                                const double wk = s_w[k];
+                                if (wk != 0.0 && emb > 1u) acc_eps = fma(wk * (double)emb, log2((double)emb) - s_lebar[k], acc_eps);
+                                else if (wk != 0.0) acc_eps = fma(wk, -s_lebar[k], acc_eps);
+                            } else if (MODE == IN_DEBUG) {
+                                if (((u << m) | (uint32_t)ev) == a.dbg_x) a.dbg_out[cy - 1u] = emb;
+                            } else {
+                                cnt_terms += 1ull; cnt_emb += emb;
+                            }
+                        }
+                    }
+                }
+                if (kind == 0) {
                 // ---- the thread's pair slots ---------------------------------------------------------------
                 if (MODE == IN_SWEEP) {
                     uint32_t rb[BA_KG];
@@ -444,6 +443,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                     }
                     if ((MODE == IN_SWEEP || MODE == IN_HC) && re < nr) s_rsum[((size_t)buf * 2 + rh) * a.g.nr + re] = s;
                 }
+                }                                              // kind == 0
             }
             if (nbatch > 0) {
                 __syncthreads();                               // rider sums of the last batch are visible

@@ -223,7 +223,6 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                 const uint32_t miss0 = ba_nextpos(u, h, ell, 0u) >= h, miss1 = ba_nextpos(u, h, ell, 1u) >= h;
                 rc.id = u;
                 rc.info = miss0 | (miss1 << 1) | ((uint32_t)Lc << 8) | ((uint32_t)t << 16);
-                rc.pad = 0u;
                 s_rec[tid] = rc;
                 const bool has = do_grp && (b ? miss1 : miss0);
                 key = has ? 0 : (do_eps ? 1 : -1);             // 0: pairs of list b (and eps); 1: the pair (v, empty) only

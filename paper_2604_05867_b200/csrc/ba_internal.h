@@ -62,11 +62,10 @@ struct KConst {                       // passed by value to kernels
     double lebar[BA_NMAX_I + 1];      // log2( C(n,k) / 2^k ): centring constant of the hoisted log
 };
 
-struct NodeRec {                      // 48 bytes, shared memory
+struct NodeRec {                      // 44 bytes, shared memory
     uint32_t a[9];                    // alpha_0..alpha_8 (0 beyond min(k,8))
     uint32_t id;                      // input sweep: code(y') ; output sweep: u
     uint32_t info;                    // mask (bits 0..1) | min(k,8) << 8 | k << 16
-    uint32_t pad;
 };
 
 // A node of a staged batch as the hot loops read it: alphas as 16-bit halves (IDP.2A operands), 48 bytes.
@@ -76,7 +75,7 @@ struct BalRec {
     uint32_t id;                      // NodeRec::id
     uint32_t node;                    // index of the NodeRec
     double a0d;                       // (double)alpha_0, exact: the type-1 loop (ba_group_loop<1, .>)
-    double x0;                        // a per-node operand of the sweep (input sweep: c(y'))
+    double x0;                        // a per-node operand of the sweep (input sweep: c(y'), the operand of the pair (v, empty))
 };
 #define BA_BALB 48u
 
@@ -90,13 +89,6 @@ __device__ __forceinline__ BalRec ba_make_bal(const NodeRec &rc, uint32_t node) 
     bl.a0d = (double)rc.a[0]; bl.x0 = 0.0;
     return bl;
 }
-
-// A node of a phase-A round as the (v, empty) pairs of the input sweep read it, 32 bytes.
-struct EpsRec {
-    uint32_t a01, a23, a45, a67;      // alphas as 16-bit halves (garbage if one needs more: the wide path reads NodeRec)
-    uint32_t a8, cy;                  // alpha_8, code(y')
-    double c;                         // c(y')
-};
 
 // The schedule of one side, device pointers (host side: GroupSide in ba_tables.h)
 struct GroupDev {
@@ -257,7 +249,8 @@ __device__ __forceinline__ void ba_group_loop1(double (&acc)[BA_NSLOT], const ui
 __device__ __forceinline__ void ba_group_loop_wide(double (&acc)[BA_NSLOT], const uint32_t (&Bp)[BA_NSLOT], const uint32_t (&rb)[BA_KG],
                                                    const BalRec *bal, const NodeRec *rec, int len, int kmax) {
     for (int i = 0; i < len; i++) {
-        const uint4 a = *(const uint4 *)&rec[bal[i].node].a[0];
+        const NodeRec &rc = rec[bal[i].node];
+        const uint4 a = make_uint4(rc.a[0], rc.a[1], rc.a[2], rc.a[3]);
 #pragma unroll
         for (int k = 0; k < BA_KG; k++) {
             if (k >= kmax) break;

@@ -28,6 +28,7 @@ struct TileTables {
     int m = 0, nv = 0;
     GroupSide in, out;
     std::vector<uint2> EPS8;        // [256][nv]: byte s = B(sigma_s, v), s = 0..7, sigma = the row index
+    std::vector<uint32_t> EPSH;     // [BA_NCLS][16][nv]: EPS8[(hi << 4) | cls][v].y, the slice of a class (input sweep)
     bool ok = false;
 };
 
@@ -304,5 +305,9 @@ static inline void build_tile_tables(int m, TileTables &T) {
                 w[sft / 4] |= Bof((1u << sft) | (sig & ((1u << sft) - 1u)), v) << (8 * (sft % 4));
             T.EPS8[(size_t)sig * nv + v] = make_uint2(w[0], w[1]);
         }
+    T.EPSH.assign((size_t)BA_NCLS * 16 * nv, 0u);
+    for (uint32_t cls = 0; cls < BA_NCLS; cls++)
+        for (uint32_t hi = 0; hi < 16u; hi++)
+            for (int v = 0; v < nv; v++) T.EPSH[((size_t)cls * 16 + hi) * nv + v] = T.EPS8[(size_t)((hi << 4) | cls) * nv + v].y;
     T.ok = true;
 }
