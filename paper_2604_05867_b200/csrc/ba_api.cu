@@ -95,7 +95,7 @@ static void side_layout(const GroupSide &G, SideLayout &L, size_t &o) {
     L.GB = o; o += align256(G.GB.size() * 16);
     L.GA = o; o += align256(G.GA.size() * 4);
     L.GO = o; o += align256(G.GO.size() * 2);
-    L.GW = o; o += align256(G.GW.size());
+    L.GW = o; o += align256(G.GW.size() * 2);
     L.csr_off = o; o += align256(G.csr_off.size() * 2);
     L.csr_idx = o; o += align256(G.csr_idx.size() * 2);
     L.R = o; o += align256(G.R.size() * 16);
@@ -208,13 +208,13 @@ extern "C" int ba_debug_check_tables(int m, unsigned long long stats[4]) {
                         const uint4 e4 = G.GB[(((size_t)cls * 2 + b) * BA_KG + k) * BA_NT + tid];
                         const uint32_t e[4] = {e4.x, e4.y, e4.z, e4.w};
                         const uint32_t pos = G.GA[((size_t)b * BA_KG + k) * BA_NT + tid] >> 3;
-                        const int wm = G.GW[(size_t)b * (BA_NT / 32) + tid / 32];
+                        const int hm = (G.GW[(size_t)b * (BA_NT / 32) + tid / 32] >> (8 * (k / 2))) & 0xff;    // the half of group k
                         for (int q = 0; q < BA_GP; q++) {
                             const uint32_t ow = G.GO[(((size_t)b * BA_KG + k) * BA_GP + q) * BA_NT + tid];
                             if (!(e[q] & 0xffu)) { if (e[q]) return BA_EINVAL; continue; }      // unused, or deep under this class
-                            if (ow == 0xffffu || k >= (wm & 15)) return BA_EINVAL;              // the warp's loop must reach the slot
-                            if ((wm >> 4) == 2 && (e[q] >> 16)) return BA_EINVAL;               // a type-2 loop ignores B_2, B_3
-                            if ((wm >> 4) == 1 && (e[q] >> 8)) return BA_EINVAL;                // a type-1 loop ignores B_1..B_3
+                            if (ow == 0xffffu || (k & 1) >= (hm & 3)) return BA_EINVAL;         // the half's loop must reach the slot
+                            if ((hm >> 2) == 2 && (e[q] >> 16)) return BA_EINVAL;               // a type-2 loop ignores B_2, B_3
+                            if ((hm >> 2) == 1 && (e[q] >> 8)) return BA_EINVAL;                // a type-1 loop ignores B_1..B_3
                             if (!visit(pos, ow, e[q], 4, nullptr)) return BA_EINVAL;
                             stats[side ? 2 : 0]++;
                         }
@@ -291,7 +291,7 @@ static cudaError_t upload_side(unsigned char *s, const GroupSide &G, const SideL
     if ((e = upload(s + L.r_csr, G.r_csr, st)) != cudaSuccess) return e;
     if ((e = upload(s + L.R8, G.R8, st)) != cudaSuccess) return e;
     D.GB = (const uint4 *)(s + L.GB); D.GA = (const uint32_t *)(s + L.GA); D.GO = (const uint16_t *)(s + L.GO);
-    D.GW = (const uint8_t *)(s + L.GW); D.csr_off = (const uint16_t *)(s + L.csr_off); D.csr_idx = (const uint16_t *)(s + L.csr_idx);
+    D.GW = (const uint16_t *)(s + L.GW); D.csr_off = (const uint16_t *)(s + L.csr_off); D.csr_idx = (const uint16_t *)(s + L.csr_idx);
     D.R = (const uint4 *)(s + L.R); D.r_cnt = (const uint16_t *)(s + L.r_cnt); D.r_csr = (const uint16_t *)(s + L.r_csr);
     D.R8 = (const uint32_t *)(s + L.R8);
     D.nr = G.nr; D.nown = G.nown;

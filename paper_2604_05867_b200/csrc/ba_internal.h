@@ -95,7 +95,7 @@ struct GroupDev {
     const uint4 *GB;                  // [cls][b][k][tid]
     const uint32_t *GA;               // [b][k][tid]
     const uint16_t *GO;               // [b][k][q][tid]
-    const uint8_t *GW;                // [b][warp]
+    const uint16_t *GW;               // [b][warp]: half 0 | half 1 << 8, a half = groups in use | type << 2
     const uint16_t *csr_off;          // [b][nown + 1]
     const uint16_t *csr_idx;          // [b][BA_NSLOT * BA_NT]
     const uint4 *R;                   // riders [cls][b][nr]
@@ -194,66 +194,72 @@ __device__ __forceinline__ double ba_cvt(uint32_t e) {
     return ba_u2d(e);
 }
 
-// The hot loop of both sweeps: the BA_KG x BA_GP pair slots of a thread (Bp = B_0 | B_1<<8 | B_2<<16 | B_3<<24 of the
-// slot, rb[k] = shared-memory address of group k's operand in the first staged row) against the `len` nodes of a batch
-// (bal = shared-memory address of the batch's BalRec array, rows BA_ROWB bytes apart).  TYPE 2: no slot of the warp
-// has B_2 or B_3.
-template <int TYPE, int KMAX>
-__device__ __forceinline__ void ba_group_loop(double (&acc)[BA_NSLOT], const uint32_t (&Bp)[BA_NSLOT], const uint32_t (&rb)[BA_KG],
-                                              uint32_t bal, int len) {
-#ifndef BA_X_UNR
-#define BA_X_UNR 2
+// The hot loop of both sweeps.  A thread's BA_KG groups form two HALVES of two groups; the groups of a half are of one
+// TYPE (chosen per warp by the table builder, so a warp mixes a heavy and a light half and all warps carry about the
+// same number of instructions per node).  A half loops over the `len` nodes of a batch: Bp = B_0 | B_1<<8 | B_2<<16 |
+// B_3<<24 of a slot, rb[k] = shared-memory address of group k's operand in the first staged row, bal = shared-memory
+// address of the batch's BalRec array, rows BA_ROWB bytes apart.  K0 = first group of the half, NL = its groups (1, 2).
+//   TYPE 4  emb = IDP.2A(a01, B) then IDP.2A(a23, B); exact u32 -> f64; DFMA
+//   TYPE 2  no slot of the half ever has B_2 or B_3: one IDP.2A
+//   TYPE 1  no slot of the half ever has B_1 (under any class): emb = alpha_0 * B_0 is one product of two integer
+//           counts (P:181 with a single split point); the term emb * operand is formed as (alpha_0 * operand) * B_0 with
+//           alpha_0 and B_0 converted exactly: one DMUL per group and node, one DFMA per term, no integer work.
+#ifndef BA_UNR1
+#define BA_UNR1 4
 #endif
-    constexpr int unr = BA_X_UNR;
-#pragma unroll unr
-    for (int i = 0; i < len; i++) {
-        uint2 a;
-        if (TYPE == 2) { asm volatile("ld.shared.u32 %0, [%1];" : "=r"(a.x) : "r"(bal + (uint32_t)i * BA_BALB)); a.y = 0u; }
-        else a = ba_lds_v2(bal + (uint32_t)i * BA_BALB);
+#ifndef BA_UNR4
+#define BA_UNR4 4
+#endif
+template <int TYPE, int K0, int NL>
+__device__ __forceinline__ void ba_half_loop(double (&acc)[BA_NSLOT], const uint32_t (&Bp)[BA_NSLOT], const uint32_t (&rb)[BA_KG],
+                                             uint32_t bal, int len) {
+    if (TYPE == 1) {
+        double Bd[NL * BA_GP];
 #pragma unroll
-        for (int k = 0; k < KMAX; k++) {
-            const double op = ba_lds_f64(rb[k] + (uint32_t)i * BA_ROWB);
+        for (int s = 0; s < NL * BA_GP; s++) Bd[s] = (double)(Bp[K0 * BA_GP + s] & 0xffu);
+        constexpr int unr1 = BA_UNR1;
+#pragma unroll unr1
+        for (int i = 0; i < len; i++) {
+            const double a0 = ba_lds_f64(bal + (uint32_t)i * BA_BALB + 32u);
 #pragma unroll
-            for (int q = 0; q < BA_GP; q++) {
-                uint32_t e = __dp2a_lo(a.x, Bp[k * BA_GP + q], 0u);
-                if (TYPE == 4) e = __dp2a_hi(a.y, Bp[k * BA_GP + q], e);
-                const double ed = (q == 0) ? ba_cvt<0>(e) : (q == 1) ? ba_cvt<1>(e) : (q == 2) ? ba_cvt<2>(e) : ba_cvt<3>(e);
-                acc[k * BA_GP + q] = fma(ed, op, acc[k * BA_GP + q]);
+            for (int k = 0; k < NL; k++) {
+                const double t = a0 * ba_lds_f64(rb[K0 + k] + (uint32_t)i * BA_ROWB);
+#pragma unroll
+                for (int q = 0; q < BA_GP; q++) acc[(K0 + k) * BA_GP + q] = fma(t, Bd[k * BA_GP + q], acc[(K0 + k) * BA_GP + q]);
+            }
+        }
+    } else {
+        constexpr int unr4 = BA_UNR4;
+#pragma unroll unr4
+        for (int i = 0; i < len; i++) {
+            uint2 a;
+            if (TYPE == 2) { asm volatile("ld.shared.u32 %0, [%1];" : "=r"(a.x) : "r"(bal + (uint32_t)i * BA_BALB)); a.y = 0u; }
+            else a = ba_lds_v2(bal + (uint32_t)i * BA_BALB);
+#pragma unroll
+            for (int k = 0; k < NL; k++) {
+                const double op = ba_lds_f64(rb[K0 + k] + (uint32_t)i * BA_ROWB);
+#pragma unroll
+                for (int q = 0; q < BA_GP; q++) {
+                    uint32_t e = __dp2a_lo(a.x, Bp[(K0 + k) * BA_GP + q], 0u);
+                    if (TYPE == 4) e = __dp2a_hi(a.y, Bp[(K0 + k) * BA_GP + q], e);
+                    const double ed = (q == 0) ? ba_cvt<0>(e) : (q == 1) ? ba_cvt<1>(e) : (q == 2) ? ba_cvt<2>(e) : ba_cvt<3>(e);
+                    acc[(K0 + k) * BA_GP + q] = fma(ed, op, acc[(K0 + k) * BA_GP + q]);
+                }
             }
         }
     }
 }
 
-// TYPE 1: no slot of the warp ever has B_1 (under any class), so emb = alpha_0 * B_0 is one product of two integer
-// counts (P:181 with a single split point).  The term emb * operand is formed as (alpha_0 * operand) * B_0 with alpha_0
-// and B_0 converted exactly: one DMUL per group and node, one DFMA per term, no integer work in the loop.
-template <int KMAX>
-__device__ __forceinline__ void ba_group_loop1(double (&acc)[BA_NSLOT], const uint32_t (&Bp)[BA_NSLOT], const uint32_t (&rb)[BA_KG],
-                                               uint32_t bal, int len) {
-    double Bd[KMAX * BA_GP];
-#pragma unroll
-    for (int s = 0; s < KMAX * BA_GP; s++) Bd[s] = (double)(Bp[s] & 0xffu);
-#pragma unroll 2
-    for (int i = 0; i < len; i++) {
-        const double a0 = ba_lds_f64(bal + (uint32_t)i * BA_BALB + 32u);
-#pragma unroll
-        for (int k = 0; k < KMAX; k++) {
-            const double t = a0 * ba_lds_f64(rb[k] + (uint32_t)i * BA_ROWB);
-#pragma unroll
-            for (int q = 0; q < BA_GP; q++) acc[k * BA_GP + q] = fma(t, Bd[k * BA_GP + q], acc[k * BA_GP + q]);
-        }
-    }
-}
-
 // The same with the 32-bit alphas of the node records: batches holding an alpha >= 2^16 (n >= 27 only).
+// gmask: bit k = group k is in use.
 __device__ __forceinline__ void ba_group_loop_wide(double (&acc)[BA_NSLOT], const uint32_t (&Bp)[BA_NSLOT], const uint32_t (&rb)[BA_KG],
-                                                   const BalRec *bal, const NodeRec *rec, int len, int kmax) {
+                                                   const BalRec *bal, const NodeRec *rec, int len, int gmask) {
     for (int i = 0; i < len; i++) {
         const NodeRec &rc = rec[bal[i].node];
         const uint4 a = make_uint4(rc.a[0], rc.a[1], rc.a[2], rc.a[3]);
 #pragma unroll
         for (int k = 0; k < BA_KG; k++) {
-            if (k >= kmax) break;
+            if (!((gmask >> k) & 1)) continue;
             const double op = ba_lds_f64(rb[k] + (uint32_t)i * BA_ROWB);
 #pragma unroll
             for (int q = 0; q < BA_GP; q++) {
@@ -265,29 +271,24 @@ __device__ __forceinline__ void ba_group_loop_wide(double (&acc)[BA_NSLOT], cons
     }
 }
 
-// Dispatch on the warp's static (type, levels) and on whether the batch's alphas fit 16 bits.
+template <int K0>
+__device__ __forceinline__ void ba_half_batch(double (&acc)[BA_NSLOT], const uint32_t (&Bp)[BA_NSLOT], const uint32_t (&rb)[BA_KG],
+                                              uint32_t al16, int len, int hm) {
+    const int nl = hm & 3, type = hm >> 2;             // half meta: groups in use (0..2) | type << 2
+    if (nl == 0) return;
+    if (type == 1) { if (nl == 2) ba_half_loop<1, K0, 2>(acc, Bp, rb, al16, len); else ba_half_loop<1, K0, 1>(acc, Bp, rb, al16, len); }
+    else if (type == 2) { if (nl == 2) ba_half_loop<2, K0, 2>(acc, Bp, rb, al16, len); else ba_half_loop<2, K0, 1>(acc, Bp, rb, al16, len); }
+    else { if (nl == 2) ba_half_loop<4, K0, 2>(acc, Bp, rb, al16, len); else ba_half_loop<4, K0, 1>(acc, Bp, rb, al16, len); }
+}
+
+// Dispatch on the warp's static halves (wmeta = half 0 | half 1 << 8) and on whether the batch's alphas fit 16 bits.
 __device__ __forceinline__ void ba_group_batch(double (&acc)[BA_NSLOT], const uint32_t (&Bp)[BA_NSLOT], const uint32_t (&rb)[BA_KG],
                                                const BalRec *bal, const NodeRec *rec, int len, int wmeta, bool big) {
-    const int kmax = wmeta & 15, type = wmeta >> 4;
-    if (kmax == 0) return;
-    if (big && type != 1) { ba_group_loop_wide(acc, Bp, rb, bal, rec, len, kmax); return; }
+    const int h0 = wmeta & 0xff, h1 = (wmeta >> 8) & 0xff;
+    if (big) { ba_group_loop_wide(acc, Bp, rb, bal, rec, len, ((1 << (h0 & 3)) - 1) | (((1 << (h1 & 3)) - 1) << 2)); return; }
     const uint32_t al16 = ba_smem_addr(bal);
-    if (type == 1) {
-        if (kmax == 4) ba_group_loop1<4>(acc, Bp, rb, al16, len);
-        else if (kmax == 3) ba_group_loop1<3>(acc, Bp, rb, al16, len);
-        else if (kmax == 2) ba_group_loop1<2>(acc, Bp, rb, al16, len);
-        else ba_group_loop1<1>(acc, Bp, rb, al16, len);
-    } else if (type == 2) {
-        if (kmax == 4) ba_group_loop<2, 4>(acc, Bp, rb, al16, len);
-        else if (kmax == 3) ba_group_loop<2, 3>(acc, Bp, rb, al16, len);
-        else if (kmax == 2) ba_group_loop<2, 2>(acc, Bp, rb, al16, len);
-        else ba_group_loop<2, 1>(acc, Bp, rb, al16, len);
-    } else {
-        if (kmax == 4) ba_group_loop<4, 4>(acc, Bp, rb, al16, len);
-        else if (kmax == 3) ba_group_loop<4, 3>(acc, Bp, rb, al16, len);
-        else if (kmax == 2) ba_group_loop<4, 2>(acc, Bp, rb, al16, len);
-        else ba_group_loop<4, 1>(acc, Bp, rb, al16, len);
-    }
+    ba_half_batch<0>(acc, Bp, rb, al16, len, h0);
+    ba_half_batch<2>(acc, Bp, rb, al16, len, h1);
 }
 
 // Full chain of a pair with all nine B_s (the pair (v, empty) and the riders): alphas as 16-bit halves

@@ -12,7 +12,7 @@ struct GroupSide {
     std::vector<uint4> GB;          // [BA_NCLS][2][BA_KG][BA_NT]: B_0 | B_1<<8 | B_2<<16 | B_3<<24 of the group's 4 slots
     std::vector<uint32_t> GA;       // [2][BA_KG][BA_NT]: byte offset of the group's operand in a staged row
     std::vector<uint16_t> GO;       // [2][BA_KG][BA_GP][BA_NT]: owner of the slot (in: v, out: code(z)); 0xffff = unused
-    std::vector<uint8_t> GW;        // [2][BA_NT/32]: levels of the warp (0..BA_KG) | loop type << 4 (1: only B_0 ever; 2: B_2 = B_3 = 0 always; 4)
+    std::vector<uint16_t> GW;       // [2][BA_NT/32]: half 0 | half 1 << 8; a half = groups in use (0..2) | loop type << 2 (1: only B_0 ever; 2: B_2 = B_3 = 0 always; 4)
     std::vector<uint16_t> csr_off;  // [2][nown + 1]: slots of an owner, per list
     std::vector<uint16_t> csr_idx;  // [2][BA_KG*BA_GP*BA_NT]: slot index (k*BA_GP + q)*BA_NT + tid
     int nown = 0;                   // in: 2^m ; out: 2^{m+1} (by code(z))
@@ -86,56 +86,50 @@ static bool tt_deal(int m, int b, const std::vector<TTPair> &pairs, KeyOf key_of
         levels.back().g.push_back((int)i);
     }
     const int NW = BA_NT / 32;
-    // ---- warps per type: proportional to the instruction count per term (type 4: 2 IDP + MOV + DADD + DFMA = 5,
-    // type 2: 4, type 1: one DFMA and a quarter DMUL), at least ceil(levels / BA_KG), all NW warps used
-    const int types[3] = {4, 2, 1};
-    const double cost_of[3] = {5.0, 4.0, 1.5};
-    int Lt[3] = {0, 0, 0}, wt[3];
-    for (auto &l : levels) Lt[l.type == 4 ? 0 : l.type == 2 ? 1 : 2]++;
-    for (int i = 0; i < 3; i++) wt[i] = (Lt[i] + BA_KG - 1) / BA_KG;
-    if (wt[0] + wt[1] + wt[2] > NW) return false;
-    while (wt[0] + wt[1] + wt[2] < NW) {
+    // ---- HALVES: up to 2 levels of one type; a warp carries two halves (ba_internal.h "ba_half_loop").  Cost of a level
+    // in instructions per node and lane: type 4: 4 x (2 IDP + MOV + DADD + DFMA), type 2: 4 x 4, type 1: 4 DFMA + DMUL + LDS.
+    struct Half { int type; std::vector<int> lv; double cost; };
+    auto cost_of = [](int type) { return type == 4 ? 20.5 : type == 2 ? 16.5 : 6.5; };
+    std::vector<Half> halves;
+    for (size_t i = 0; i < levels.size();) {
+        Half hf; hf.type = levels[i].type;
+        hf.lv.push_back((int)i);
+        if (i + 1 < levels.size() && levels[i + 1].type == hf.type) hf.lv.push_back((int)i + 1);
+        hf.cost = cost_of(hf.type) * hf.lv.size() + 1.5;
+        i += hf.lv.size();
+        halves.push_back(hf);
+    }
+    if ((int)halves.size() > 2 * NW) return false;
+    // free half slots: split the heaviest two-level halves, so that the warps can be levelled better
+    while ((int)halves.size() < 2 * NW) {
         int best = -1;
-        double bc = -1.0;
-        for (int i = 0; i < 3; i++) {
-            if (Lt[i] <= wt[i]) continue;                      // not more warps than levels
-            const double c = cost_of[i] * Lt[i] / wt[i];
-            if (c > bc) { bc = c; best = i; }
-        }
+        for (size_t i = 0; i < halves.size(); i++)
+            if (halves[i].lv.size() == 2 && (best < 0 || halves[i].cost > halves[best].cost)) best = (int)i;
         if (best < 0) break;
-        wt[best]++;
+        Half nh; nh.type = halves[best].type; nh.lv.push_back(halves[best].lv[1]); nh.cost = cost_of(nh.type) + 1.5;
+        halves[best].lv.pop_back(); halves[best].cost = nh.cost;
+        halves.push_back(nh);
     }
-    struct Bundle { int type; std::vector<int> lv; double cost; };
-    std::vector<Bundle> bundles;
-    int first = 0;
-    for (int i = 0; i < 3; i++) {
-        for (int w = 0; w < wt[i]; w++) {
-            Bundle bd; bd.type = types[i];
-            const int lo = (int)((long long)Lt[i] * w / wt[i]), hi = (int)((long long)Lt[i] * (w + 1) / wt[i]);
-            for (int l = lo; l < hi; l++) bd.lv.push_back(first + l);
-            bd.cost = cost_of[i] * (hi - lo);
-            bundles.push_back(bd);
-        }
-        first += Lt[i];
-    }
-    for (auto &bd : bundles) if ((int)bd.lv.size() > BA_KG) return false;
-    // ---- bundles -> warp indices: heaviest first onto the scheduler (warp & 3) with the least load
-    std::stable_sort(bundles.begin(), bundles.end(), [](const Bundle &x, const Bundle &y) { return x.cost > y.cost; });
-    // warp_extra[w] = instructions per node the warp spends outside its levels (riders): the heavy bundles go to the
-    // warps without riders, and a scheduler's load counts both
-    double load[4] = {0, 0, 0, 0};
-    bool taken[BA_NT / 32] = {false};
-    for (auto &bd : bundles) {
+    // ---- halves -> warps: heaviest first onto the warp with the least load that has a free half; warp_extra[w] =
+    // instructions per node the warp spends outside its levels (riders); ties go to the scheduler (warp & 3) with the
+    // least load
+    std::stable_sort(halves.begin(), halves.end(), [](const Half &x, const Half &y) { return x.cost > y.cost; });
+    double wload[BA_NT / 32], sload[4] = {0, 0, 0, 0};
+    int nh_of[BA_NT / 32];
+    for (int w = 0; w < NW; w++) { wload[w] = warp_extra[w]; nh_of[w] = 0; sload[w & 3] += warp_extra[w]; }
+    for (auto &hf : halves) {
         int warp = -1;
         for (int w = 0; w < NW; w++) {
-            if (taken[w]) continue;
-            if (warp < 0 || load[w & 3] + warp_extra[w] < load[warp & 3] + warp_extra[warp] - 1e-9) warp = w;
+            if (nh_of[w] >= 2) continue;
+            if (warp < 0 || wload[w] < wload[warp] - 1e-9 || (wload[w] < wload[warp] + 1e-9 && sload[w & 3] < sload[warp & 3] - 1e-9)) warp = w;
         }
         if (warp < 0) return false;
-        taken[warp] = true; load[warp & 3] += bd.cost + warp_extra[warp];
-        S.GW[(size_t)b * NW + warp] = (uint8_t)(bd.lv.size() | (bd.type << 4));
-        for (size_t k = 0; k < bd.lv.size(); k++) {
-            const Lvl &lv = levels[bd.lv[k]];
+        const int hslot = nh_of[warp]++;
+        wload[warp] += hf.cost; sload[warp & 3] += hf.cost;
+        S.GW[(size_t)b * NW + warp] |= (uint16_t)(((int)hf.lv.size() | (hf.type << 2)) << (8 * hslot));
+        for (size_t kk = 0; kk < hf.lv.size(); kk++) {
+            const int k = 2 * hslot + (int)kk;
+            const Lvl &lv = levels[hf.lv[kk]];
             for (size_t l = 0; l < lv.g.size(); l++) {
                 const Grp &g = groups[lv.g[l]];
                 const int tid = warp * 32 + (int)l;
