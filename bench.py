@@ -104,24 +104,34 @@ class ClockSampler:
 # ---------------------------------------------------------------------------------------------
 # Roofline of the dominant kernel.  The sweeps are bound by plain ALU issue,
 # not by HBM (compulsory traffic is ~1e-3 of the term work) and not by tensor cores (no contraction).
-#   algorithmic work  : C_MIN lane-instructions per (x,y) term -- integer emb combine (IMAD), int->FP64
+#   algorithmic work  : C_MIN lane-instructions per (x,y) term -- integer emb combine (one IDP.2A / IMAD), int->FP64
 #                       convert, FP64 FMA, fetch of the gathered operand -- times T(n) terms per launch
-#   peak              : 148 SMs x 4 warp schedulers x 32 lanes x SM clock   [lane-instructions / s]
-# The FP64 pipe (64 lanes/clk/SM, 2 FP64-pipe ops per term) gives the same terms/s ceiling.
+#   peak              : MEASURED in this run by libba's microbenchmarks (ba_measure_peaks): per pipe the warp-
+#                       instructions per clock per SM, the clock the kernels saw, the SM count.  Per term the path needs
+#                       at least 2 FP64-pipe instructions (convert + FMA), 1 integer-multiply-pipe instruction, 1 LDS.64
+#                       unless operands are shared, and 4 issue slots; the binding pipe gives the terms/s ceiling, and
+#                       peak = C_MIN x that ceiling.  The nominal formula (4 schedulers x 32 lanes x clock) is kept as a
+#                       cross-check.
 C_MIN = 4
-SMS, SCHED, LANES = 148, 4, 32
+NEED = {"dfma": 2.0, "idp2a": 1.0, "lds64": 1.0, "issue": 4.0}     # pipe instructions per term (c_min per pipe)
 
 
-def alu_peak_tinst(sm_mhz):
-    return SMS * SCHED * LANES * sm_mhz * 1e6 / 1e12
+def measured_alu_peak(pk):
+    """(terms/s ceiling, binding pipe, per-pipe ceilings) from ba_measure_peaks()."""
+    rate = {"dfma": pk["dfma"], "idp2a": pk["idp2a"], "lds64": pk["lds64"], "issue": pk["ffma"]}
+    per_pipe = {k: rate[k] * 32.0 / NEED[k] * pk["sms"] * pk["sm_mhz"] * 1e6 for k in rate}
+    bind = min(per_pipe, key=per_pipe.get)
+    return per_pipe[bind], bind, per_pipe
 
 
-def read_traffic(kernel):
-    """Per-launch DRAM bytes of `kernel` from the committed ncu --set full summary, or None."""
+def read_traffic(kernel, n):
+    """Per-launch DRAM bytes of `kernel` from the committed ncu --set full summary -- only if that capture was taken at
+    this n -- else None."""
     path = os.path.join(ROOT, "profiles", "roofline_traffic.json")
     try:
         with open(path) as f:
-            return json.load(f).get(kernel)
+            d = json.load(f)
+        return d.get(kernel) if int(d.get("n", -1)) == int(n) else None
     except (OSError, ValueError):
         return None
 
@@ -197,6 +207,7 @@ def run_ours(args, rank, world, local_rank):
             dist.barrier()
         torch.cuda.synchronize()
 
+    pk = ba.ba_measure_peaks()               # pipe microbenchmarks on this device, before the timed region
     ctx = ba.ba_create(n, d, device=dev)
     ba.ba_set_mode(ctx, mode)
     if args.exact_k >= 0:
@@ -219,6 +230,7 @@ def run_ours(args, rank, world, local_rank):
     ms_total = ev0.elapsed_time(ev1)
     clocks = sampler.stop() if rank == 0 else None
     tm = ba.ba_last_timing(ctx)
+    setup_ms = ba.ba_setup_ms(ctx)           # the one-off Hc pass (ran inside the warm-up)
     I, U = ba.ba_bounds(ctx)
     hist = ba.ba_get_history(ctx, min(args.steps + args.warmup, 4096))      # {I_t, U_t, log2 Z_t} of every iteration so far
     ms_total = replicas.max_over_ranks(ms_total, world, dev)
@@ -252,22 +264,25 @@ def run_ours(args, rank, world, local_rank):
     # dominant kernel: the slower sweep (per-kernel CUDA events recorded by libba on the launch stream)
     if args.mode == "enum":
         dom_name, dom_ms = ("k_enum_out", tm["out_ms"]) if tm["out_ms"] >= tm["in_ms"] else ("k_enum_in", tm["in_ms"])
-        sm_mhz = float(peaks.get("sm_max_mhz", 1965.0))
-        peak = alu_peak_tinst(sm_mhz)
+        terms_peak, bind, per_pipe = measured_alu_peak(pk)
+        peak = C_MIN * terms_peak / 1e12
         achieved = C_MIN * T / (dom_ms * 1e-3) / 1e12
-        smem_terms = SMS * 128.0 / 8.0 * sm_mhz * 1e6      # 128 B/clk/SM of shared-memory bandwidth, 8 B operand per term
+        oth_ms = min(tm["out_ms"], tm["in_ms"])
         roofline = {"bound": "alu", "kernel": dom_name, "achieved": achieved, "peak": peak, "unit": "Tinstr/s",
-                    "frac": achieved / peak, "traffic": read_traffic(dom_name),
+                    "frac": achieved / peak, "traffic": read_traffic(dom_name, n),
                     "other_kernel": {"name": "k_enum_in" if dom_name == "k_enum_out" else "k_enum_out",
-                                     "kernel_ms": min(tm["out_ms"], tm["in_ms"]),
-                                     "frac": C_MIN * T / (min(tm["out_ms"], tm["in_ms"]) * 1e-3) / 1e12 / peak},
-                    "smem_gather_roof_terms_per_s": smem_terms,
-                    "frac_of_smem_gather_roof": T / (dom_ms * 1e-3) / smem_terms,
-                    "peak_source": f"148 SMs x 4 schedulers x 32 lanes x {sm_mhz:.0f} MHz (DESIGN.md), {peaks_src} max SM clock",
+                                     "kernel_ms": oth_ms, "frac": C_MIN * T / (oth_ms * 1e-3) / 1e12 / peak},
+                    "measured_peaks": {"warp_instr_per_clk_per_sm": {"dfma": pk["dfma"], "idp2a": pk["idp2a"], "lds64": pk["lds64"],
+                                                                     "ffma_issue": pk["ffma"]},
+                                       "sm_mhz": pk["sm_mhz"], "sms": pk["sms"],
+                                       "pipe_instr_per_term": NEED, "binding_pipe": bind,
+                                       "terms_per_s_ceiling_by_pipe": per_pipe},
+                    "nominal_peak_crosscheck": 148 * 4 * 32 * float(peaks.get("sm_max_mhz", 1965.0)) * 1e6 / 1e12,
+                    "peak_source": "measured in this run: ba_measure_peaks (libba microbenchmarks), binding pipe x C_MIN",
                     "algorithmic": f"{C_MIN} lane-instructions per term x T({n})={T} terms per launch",
                     "kernel_ms": dom_ms, "kernel_terms_per_s": T / (dom_ms * 1e-3),
                     "gather_equiv_GBps": 8.0 * T / (dom_ms * 1e-3) / 1e9,
-                    "hbm_peak_GBps": peaks.get("hbm_gbs")}
+                    "hbm_peak_GBps": peaks.get("hbm_gbs"), "hbm_peak_source": peaks_src}
     else:
         # FAST mode: n streaming stages per sweep, each reads <= 3 and writes 1 double per element
         stage_bytes = sum(((4 << s) - 1) * (1 << (n - s - 1)) * 8 * 3 for s in range(n))
@@ -291,9 +306,11 @@ def run_ours(args, rank, world, local_rank):
            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
            "config": {"workload": (f"BDC_d^n BA iteration, n={n}, d={d}, uniform p0 ({config_name(n, d)})" if args.exact_k < 0 else
                                    f"exact channel BDC_{{n,k}} BA iteration, n={n}, k={args.exact_k}, uniform p0 (not a BASELINE.json config; "
-                                   f"the sweeps still enumerate all lengths)"),
+                                   f"the sweeps skip the nodes and prefixes that cannot reach length k)"),
                       "mode": args.mode, "terms_per_iteration": 2 * T,
-                      "term_counting": ("enumerated" if args.mode == "enum" and not args.symmetry else
+                      "term_counting": ("effective (exact channel: nodes / prefixes that cannot reach length k are skipped; value counts 2 T(n))"
+                                        if args.mode == "enum" and args.exact_k >= 0 else
+                                        "enumerated" if args.mode == "enum" and not args.symmetry else
                                         "effective (complement symmetry: half the terms are enumerated, the rest mirrored)" if args.mode == "enum"
                                         else "effective (FAST mode does not enumerate terms)"),
                       "l2_policy": f"inputs_exceed_l2 (p {8 * NX / 1e6:.0f} MB, q and c {16 * NX / 1e6:.0f} MB each, "
@@ -301,6 +318,7 @@ def run_ours(args, rank, world, local_rank):
                                    else "arrays fit L2 at this n (not the headline config)",
                       "parallelism": "single GPU" if world == 1 else f"{world} independent replicas (d sweep), no collective"},
            "kernels_ms": {"out_sweep": tm["out_ms"], "in_sweep": tm["in_ms"], "reduce_update": tm["update_ms"]},
+           "setup_ms": setup_ms,
            "bounds_bits": {"I_lower": I, "maxD_upper": U, "upper_over_n": U / n,
                            "running_min_upper_over_n": float(hist[:, 1].min()) / n,
                            "upper_over_n_by_iteration": [round(float(v) / n, 9) for v in hist[:, 1]][-32:]},

@@ -127,8 +127,21 @@ int ba_get_history(ba_ctx *c, int count, double *out_host);
 
 /* Device-side time of the four phases of the most recent ba_iterate call, averaged per iteration, in
  * milliseconds, measured with CUDA events on the ctx stream: ms[0] output sweep, ms[1] input sweep,
- * ms[2] reductions + update, ms[3] whole iteration.  Synchronises. */
+ * ms[2] reductions + update, ms[3] whole iteration.  Only the LAST 64 iterations of the call are timed (a call of
+ * k > 64 iterations reports the average over its last 64).  BA_ESTATE before the first iteration.  Synchronises. */
 int ba_last_timing(ba_ctx *c, double ms_host[4]);
+
+/* Device-side time, in milliseconds, of the one-off set-up pass that the first ba_iterate (and the first after
+ * ba_set_exact) runs before its iterations: the enumerating pass that builds Hc(x) = sum_y W log2(emb / ebar_k), the
+ * iteration-independent half of the hoisted logarithm.  BA_ESTATE before it ran.  Synchronises. */
+int ba_setup_ms(ba_ctx *c, double *ms_host);
+
+/* Microbenchmarks of the pipes the ENUM sweeps are bound by, on the current device (no ctx needed; default stream;
+ * synchronises the device; a few milliseconds): out[0] FP64 FMA, out[1] IDP.2A (the integer multiply pipe), out[2]
+ * conflict-free LDS.64, out[3] FP32 FMA (= issue rate), each in warp-instructions per clock per SM; out[4] SM clock in
+ * MHz seen by the kernels; out[5] number of SMs.  SURVEY 8(d): the roofline denominators are measured in the same run
+ * as the number they divide.  Host pointer. */
+int ba_measure_peaks(double out_host[6]);
 
 /* Row x of the integer embedding matrix as produced by the input-sweep enumerator:
  * emb_out_host[idx(y)] = emb(y,x) for every y, zero where y is not a subsequence.  2^{n+1}-1 entries. */

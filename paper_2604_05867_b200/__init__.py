@@ -22,7 +22,7 @@ _CODE_NAMES = {0: "BA_OK", -1: "BA_EINVAL", -2: "BA_ENOMEM", -3: "BA_ECUDA", -4:
 
 EXPORTS = ["ba_create", "ba_iterate", "ba_bounds", "ba_get_p", "ba_scratch_bytes", "ba_create_ext",
            "ba_set_mode", "ba_set_exact", "ba_set_symmetry", "ba_set_p", "ba_get_q", "ba_get_D", "ba_stats", "ba_get_history",
-           "ba_last_timing", "ba_debug_emb_row", "ba_debug_emb_col", "ba_terms_per_sweep",
+           "ba_last_timing", "ba_setup_ms", "ba_measure_peaks", "ba_debug_emb_row", "ba_debug_emb_col", "ba_terms_per_sweep",
            "ba_debug_count_terms", "ba_debug_check_tables", "ba_destroy", "ba_last_error"]
 
 
@@ -65,6 +65,8 @@ def load():
     L.ba_stats.argtypes = [vp, dp, ctypes.POINTER(ctypes.c_longlong)]
     L.ba_get_history.argtypes = [vp, ctypes.c_int, dp]
     L.ba_last_timing.argtypes = [vp, dp]
+    L.ba_setup_ms.argtypes = [vp, dp]
+    L.ba_measure_peaks.argtypes = [dp]
     L.ba_debug_emb_row.argtypes = [vp, ctypes.c_uint, up]
     L.ba_debug_emb_col.argtypes = [vp, ctypes.c_uint, up]
     L.ba_terms_per_sweep.argtypes = [ctypes.c_int, ullp]
@@ -188,6 +190,22 @@ def ba_last_timing(ctx):
     ms = np.empty(4, dtype=np.float64)
     _check(ctx, load().ba_last_timing(ctx.handle, _dp(ms)))
     return dict(out_ms=ms[0], in_ms=ms[1], update_ms=ms[2], iter_ms=ms[3])
+
+
+def ba_setup_ms(ctx):
+    """Milliseconds of the one-off Hc pass the first ba_iterate ran."""
+    v = ctypes.c_double()
+    _check(ctx, load().ba_setup_ms(ctx.handle, ctypes.byref(v)))
+    return float(v.value)
+
+
+def ba_measure_peaks():
+    """Pipe microbenchmarks on the current device: warp-instructions per clock per SM, SM MHz, SM count."""
+    out = np.empty(6, dtype=np.float64)
+    rc = load().ba_measure_peaks(_dp(out))
+    if rc:
+        raise BAError(rc, "ba_measure_peaks failed")
+    return dict(dfma=out[0], idp2a=out[1], lds64=out[2], ffma=out[3], sm_mhz=out[4], sms=int(out[5]))
 
 
 def ba_get_p(ctx, out=None):

@@ -6,7 +6,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libba.so")
 SOURCES = ["ba_api.cu"]                       # unity build; the kernels are the .cuh files it includes
-DEPS = ["ba_api.cu", "ba_internal.h", "ba_tables.h", "ba_enum_in.cuh", "ba_enum_out.cuh", "ba_stream.cuh", "ba_fast.cuh",
+DEPS = ["ba_api.cu", "ba_internal.h", "ba_tables.h", "ba_enum_in.cuh", "ba_enum_out.cuh", "ba_stream.cuh", "ba_fast.cuh", "ba_peaks.cuh",
         os.path.join("..", "..", "include", "ba.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

@@ -7,6 +7,7 @@
 #include "ba_enum_out.cuh"
 #include "ba_stream.cuh"
 #include "ba_fast.cuh"
+#include "ba_peaks.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -31,6 +32,7 @@ struct ba_ctx {
     GroupDev gin, gout;              // pair schedules of the two sweeps (device pointers into scratch)
     uint2 *EPS8 = nullptr;
     uint32_t *EPSH = nullptr;
+    double *elog = nullptr;
     unsigned int *counters = nullptr;
     unsigned long long *cnt = nullptr;
     size_t npart_cap = 0;
@@ -39,6 +41,7 @@ struct ba_ctx {
     int num_sms = 0, grid_in = 0, grid_out = 0, block = 0;
     size_t smem_in = 0, smem_out = 0;
     std::vector<cudaEvent_t> ev;     // 4 per timed iteration + 1
+    cudaEvent_t ev_setup[2] = {nullptr, nullptr};      // around the one-off Hc pass
     int ev_iters = 0;
     std::string err;
 };
@@ -69,7 +72,7 @@ static double host_binom(int n, int k) {
 // ------------------------------------------------------------------------------------------------ scratch layout
 struct SideLayout { size_t GB, GA, GO, GW, csr_off, csr_idx, R, r_cnt, r_csr, R8; };
 struct ScratchLayout {
-    size_t c, Hc, Apart, S, part, scal, hist, EPS8, EPSH, counters, cnt, total;
+    size_t c, Hc, Apart, S, part, scal, hist, EPS8, EPSH, elog, counters, cnt, total;
     SideLayout in, out;
     size_t napart, npart_cap;
 };
@@ -121,6 +124,7 @@ static void scratch_layout(int n, const TileTables &T, ScratchLayout &L) {
     L.hist = o; o += align256((size_t)BA_HIST_CAP * 3 * 8);
     L.EPS8 = o; o += align256(T.EPS8.size() * 8);
     L.EPSH = o; o += align256(T.EPSH.size() * 4);
+    L.elog = o; o += align256((size_t)BA_ELOG_N * 8);
     side_layout(T.in, L.in, o);
     side_layout(T.out, L.out, o);
     L.counters = o; o += align256(16 * 4);
@@ -323,12 +327,15 @@ static int finish_create(ba_ctx *c) {
     unsigned char *s = c->scratch;
     c->c = (double *)(s + L.c); c->Hc = (double *)(s + L.Hc); c->Apart = (double *)(s + L.Apart); c->S = (double *)(s + L.S);
     c->part = (double *)(s + L.part); c->scal = (double *)(s + L.scal); c->hist = (double *)(s + L.hist);
-    c->EPS8 = (uint2 *)(s + L.EPS8); c->EPSH = (uint32_t *)(s + L.EPSH);
+    c->EPS8 = (uint2 *)(s + L.EPS8); c->EPSH = (uint32_t *)(s + L.EPSH); c->elog = (double *)(s + L.elog);
     c->counters = (unsigned int *)(s + L.counters); c->cnt = (unsigned long long *)(s + L.cnt);
     c->napart = L.napart; c->npart_cap = L.npart_cap;
 
     CK(upload(c->EPS8, T.EPS8, c->st));
     CK(upload(c->EPSH, T.EPSH, c->st));
+    std::vector<double> elog(BA_ELOG_N, 0.0);
+    for (int e = 2; e < BA_ELOG_N; e++) elog[e] = (double)((long double)e * log2l((long double)e));
+    CK(upload(c->elog, elog, c->st));
     CK(upload_side(s, T.in, L.in, c->gin, c->st));
     CK(upload_side(s, T.out, L.out, c->gout, c->st));
     CK(cudaMemsetAsync(c->c, 0, 8, c->st));                  // c[0] is never written by k_out_final
@@ -403,6 +410,7 @@ extern "C" void ba_destroy(ba_ctx *c) {
     if (!c) return;
     if (c->st || !c->own_stream) cudaStreamSynchronize(c->st);
     for (auto e : c->ev) cudaEventDestroy(e);
+    for (auto e : c->ev_setup) if (e) cudaEventDestroy(e);
     if (c->own_buffers) { cudaFree(c->p); cudaFree(c->q); cudaFree(c->D); cudaFree(c->scratch); }
     if (c->own_stream && c->st) cudaStreamDestroy(c->st);
     delete c;
@@ -454,7 +462,7 @@ extern "C" int ba_set_mode(ba_ctx *c, int mode) {
 static InArgs make_in_args(ba_ctx *c) {
     InArgs a;
     a.kc = c->kc; a.g = c->gin; a.EPS8 = c->EPS8; a.EPSH = c->EPSH;
-    a.c = c->c; a.S = c->S;
+    a.c = c->c; a.elog = c->elog; a.S = c->S;
     a.counter = c->counters; a.sym = 0; a.dbg_x = 0; a.dbg_out = nullptr; a.cnt = c->cnt;
     return a;
 }
@@ -470,13 +478,18 @@ static OutArgs make_out_args(ba_ctx *c) {
 // Hc(x) = sum_y w_k emb(y,x) log2(emb(y,x)/ebar_k): one enumerating pass, independent of the iterate.
 static int ensure_hc(ba_ctx *c) {
     if (c->hc_ready) return BA_OK;
+    for (int i = 0; i < 2; i++) if (!c->ev_setup[i]) CK(cudaEventCreate(&c->ev_setup[i]));
+    CK(cudaEventRecord(c->ev_setup[0], c->st));
     CK(cudaMemsetAsync(c->counters, 0, 16 * 4, c->st));
     InArgs a = make_in_args(c);
     a.sym = c->sym;
     k_enum_in<IN_HC><<<c->grid_in, c->block, c->smem_in, c->st>>>(a);
     CK(cudaGetLastError());
-    k_hc_final<<<c->num_sms * 8, 256, 0, c->st>>>(c->NX, c->S, c->S + c->NX, c->Hc, c->sym);
+    long double K = 0.0L;                                   // sum_k w_k C(n,k) log2(ebar_k)
+    for (int k = 0; k <= c->n; k++) K += (long double)c->kc.w[k] * (long double)host_binom(c->n, k) * (long double)c->kc.lebar[k];
+    k_hc_final<<<c->num_sms * 8, 256, 0, c->st>>>(c->NX, c->S, c->S + c->NX, c->Hc, c->sym, (double)K);
     CK(cudaGetLastError());
+    CK(cudaEventRecord(c->ev_setup[1], c->st));
     c->hc_ready = true;
     return BA_OK;
 }
@@ -728,5 +741,62 @@ extern "C" int ba_debug_count_terms(ba_ctx *c, unsigned long long *in_terms, uns
     if (in_emb_sum) *in_emb_sum = h4[1];
     if (out_terms) *out_terms = h4[2];
     if (out_emb_sum) *out_emb_sum = h4[3];
+    return BA_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ measured peaks
+template <int KIND>
+static cudaError_t run_peak(int sms, int iters, unsigned long long *clk_dev, double *sink_dev, double *per_clk_sm, double *mhz) {
+    k_peak<KIND><<<sms, 512>>>(clk_dev, sink_dev, 16, 12345u);                 // warm-up (instruction cache, clocks)
+    cudaEvent_t e0, e1;
+    cudaError_t e;
+    if ((e = cudaEventCreate(&e0)) != cudaSuccess) return e;
+    if ((e = cudaEventCreate(&e1)) != cudaSuccess) { cudaEventDestroy(e0); return e; }
+    cudaEventRecord(e0);
+    k_peak<KIND><<<sms, 512>>>(clk_dev, sink_dev, iters, 12345u);
+    cudaEventRecord(e1);
+    e = cudaDeviceSynchronize();
+    float ms = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    if (e != cudaSuccess) return e;
+    std::vector<unsigned long long> h(sms);
+    if ((e = cudaMemcpy(h.data(), clk_dev, (size_t)sms * 8, cudaMemcpyDeviceToHost)) != cudaSuccess) return e;
+    double avg = 0;
+    for (auto v : h) avg += (double)v;
+    avg /= sms;
+    *per_clk_sm = (double)iters * 32.0 * 16.0 / avg;                            // 32 instructions per iteration, 16 warps
+    *mhz = avg / (ms * 1e-3) / 1e6;
+    return cudaSuccess;
+}
+
+extern "C" int ba_measure_peaks(double out[6]) {
+    if (!out) return BA_EINVAL;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms < 1)
+        return BA_ECUDA;
+    unsigned long long *clk = nullptr;
+    double *sink = nullptr;
+    if (cudaMalloc(&clk, (size_t)sms * 8) != cudaSuccess) return BA_ENOMEM;
+    if (cudaMalloc(&sink, 8) != cudaSuccess) { cudaFree(clk); return BA_ENOMEM; }
+    double mhz[4] = {0, 0, 0, 0};
+    cudaError_t e = run_peak<PK_DFMA>(sms, 4000, clk, sink, &out[0], &mhz[0]);
+    if (e == cudaSuccess) e = run_peak<PK_IDP>(sms, 4000, clk, sink, &out[1], &mhz[1]);
+    if (e == cudaSuccess) e = run_peak<PK_LDS64>(sms, 4000, clk, sink, &out[2], &mhz[2]);
+    if (e == cudaSuccess) e = run_peak<PK_FFMA>(sms, 8000, clk, sink, &out[3], &mhz[3]);
+    cudaFree(clk); cudaFree(sink);
+    if (e != cudaSuccess) { cudaGetLastError(); return BA_ECUDA; }
+    out[4] = (mhz[0] + mhz[1] + mhz[2] + mhz[3]) / 4.0;
+    out[5] = (double)sms;
+    return BA_OK;
+}
+
+extern "C" int ba_setup_ms(ba_ctx *c, double *ms_host) {
+    if (!c || !ms_host) return c ? fail(c, BA_EINVAL, "ba_setup_ms: null pointer") : BA_EINVAL;
+    if (!c->hc_ready) return fail(c, BA_ESTATE, "ba_setup_ms: no iteration yet");
+    CK(cudaStreamSynchronize(c->st));
+    float f = 0.f;
+    CK(cudaEventElapsedTime(&f, c->ev_setup[0], c->ev_setup[1]));
+    *ms_host = (double)f;
     return BA_OK;
 }

@@ -26,7 +26,8 @@
 // k_in_final (ba_stream.cuh) forms D(x) = Hc(x) - S_0(x) - S_1(x) and the first stage of the reductions of 8(a3).
 // MODE:
 //   IN_SWEEP  S_b(x)
-//   IN_HC     H_b(x) = sum_{y in item} w_k emb log2(emb/ebar_k)   (iteration independent; built once per ctx)
+//   IN_HC     H_b(x) = sum_{y in item} w_k emb log2(emb)   (iteration independent; built once per ctx; k_hc_final
+//             subtracts the constant sum_k w_k C(n,k) log2(ebar_k) that centres it)
 //   IN_DEBUG  emb_out[idx(y)] = emb(y,x) for one x     (ba_debug_emb_row; two CTAs, one per list)
 //   IN_COUNT  number of visited terms and sum of emb   (ba_debug_count_terms)
 #pragma once
@@ -44,6 +45,7 @@ struct InArgs {
     const uint2 *EPS8;        // [256][2^m]: B(sigma_s, v), s = 0..7, of the pair (v, empty)
     const uint32_t *EPSH;     // [cls][16][2^m]: B_4..B_7 of the pair (v, empty) by the sigma bits 4..7: a class's slice
     const double *c;          // IN_SWEEP: c[code(y)], 2^{n+1} entries (entry 0 unused)
+    const double *elog;       // IN_HC: elog[e] = e log2(e), e < BA_ELOG_N
     double *S;                // out: [2][2^n] partial sums of the two lists (IN_SWEEP: S_b, IN_HC: H_b)
     unsigned int *counter;    // work counter (zeroed before launch)
     int sym;                  // 1: p(x) = p(~x) (Theorem 4): only the u with leading bit 0 are enumerated
@@ -75,6 +77,13 @@ __host__ __device__ static inline InSmem enum_in_smem(int nr) {
     s.item = take(16);
     s.total = o;
     return s;
+}
+
+#define BA_ELOG_N 65536
+// e log2(e) of an embedding count: a table for the (overwhelmingly many) small counts, the library log2 otherwise
+__device__ __forceinline__ double ba_elog2e(uint32_t e, const double *tab) {
+    if (e < BA_ELOG_N) return __ldg(tab + e);
+    return (double)e * log2((double)e);
 }
 
 // z = b.t from the list b and code(t)
@@ -340,8 +349,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                                 acc_eps = fma(ba_u2d(emb), bal[i].x0, acc_eps);
                             } else if (MODE == IN_HC) {
                                 const double wk = s_w[k];
-                                if (wk != 0.0 && emb > 1u) acc_eps = fma(wk * (double)emb, log2((double)emb) - s_lebar[k], acc_eps);
-                                else if (wk != 0.0) acc_eps = fma(wk, -s_lebar[k], acc_eps);
+                                if (wk != 0.0 && emb > 1u) acc_eps = fma(wk, ba_elog2e(emb, a.elog), acc_eps);
                             } else if (MODE == IN_DEBUG) {
                                 if (((u << m) | (uint32_t)ev) == a.dbg_x) a.dbg_out[cy - 1u] = emb;
                             } else {
@@ -372,10 +380,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                             const int jz = ba_len_of_code(cz);
                             if (MODE == IN_HC) {
                                 const double wk = s_w[k + jz];
-                                if (wk != 0.0) {
-                                    const double le = (emb > 1u) ? log2((double)emb) : 0.0;
-                                    acc[s] = fma(wk * (double)emb, le - s_lebar[k + jz], acc[s]);
-                                }
+                                if (wk != 0.0 && emb > 1u) acc[s] = fma(wk, ba_elog2e(emb, a.elog), acc[s]);
                             } else if (MODE == IN_DEBUG) {
                                 const uint32_t ov = a.g.GO[(((size_t)b * BA_KG + s / BA_GP) * BA_GP + s % BA_GP) * BA_NT + tid];
                                 if (((u << m) | ov) == a.dbg_x) a.dbg_out[((size_t)rc.id << jz) + (cz - (1u << jz)) - 1u] = emb;
@@ -429,10 +434,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                                 } else if (MODE == IN_HC) {
                                     const int k = (int)(s_rec[bl.node].info >> 16);
                                     const double wk = s_w[k + jz];
-                                    if (wk != 0.0) {
-                                        const double le = (emb > 1u) ? log2((double)emb) : 0.0;
-                                        s = fma(wk * (double)emb, le - s_lebar[k + jz], s);
-                                    }
+                                    if (wk != 0.0 && emb > 1u) s = fma(wk, ba_elog2e(emb, a.elog), s);
                                 } else if (MODE == IN_DEBUG) {
                                     if (((u << m) | ov) == a.dbg_x) a.dbg_out[((size_t)cy << jz) + (cz - (1u << jz)) - 1u] = emb;
                                 } else {
