@@ -56,7 +56,7 @@ enum {
     BA_MODE_FAST = 1  /* position-by-position deletion transform, O(n 2^n)/sweep  */
 };
 
-#define BA_NMAX 30    /* uint32 string codes; run to n = 28 in ENUM mode (profiles/r01c_bench_n28.md) */
+#define BA_NMAX 30    /* uint32 string codes; run to n = 28 in ENUM mode (profiles/) */
 
 /* ---- required by the north star -------------------------------------------------------------- */
 
@@ -89,10 +89,11 @@ int ba_create_ext(int n, double d, void *p_dev, void *q_dev, void *D_dev,
 
 /* Switch the context to the paper's EXACT deletion channel BDC_{n,k}:
  * W(y|x) = emb(y,x) / C(n,k) for |y| = k and 0 for every other length, 0 <= k <= n.  The same kernels run
- * with the weight vector w_j = [j = k] / C(n,k); the sweeps skip the nodes / prefixes that cannot reach length k and
- * otherwise still enumerate every length (the other lengths carry weight 0 and q is 0 there).  ba_bounds then brackets C_{n,k}; Lemma 2
- * combines them into a bound on C_n(d).  Only before the first iteration: BA_ESTATE otherwise; BA_EINVAL for a
- * bad k. */
+ * with the weight vector w_j = [j = k] / C(n,k); the ENUM sweeps skip the nodes / output prefixes that cannot reach
+ * length k (they would only add exact zeros) and enumerate every |z| of the others (the other lengths carry weight 0
+ * and q is 0 there).  ba_bounds then brackets C_{n,k}; Lemma 2 combines them into a bound on
+ * C_n(d) (harness: python -m paper_2604_05867_b200.exact).  Only before the first iteration: BA_ESTATE otherwise;
+ * BA_EINVAL for a bad k. */
 int ba_set_exact(ba_ctx *c, int k);
 
 /* Complement symmetry (the cpl half of Theorem 4): emb(cpl y, cpl x) = emb(y, x), so

@@ -485,8 +485,7 @@ static int ensure_hc(ba_ctx *c) {
     a.sym = c->sym;
     k_enum_in<IN_HC><<<c->grid_in, c->block, c->smem_in, c->st>>>(a);
     CK(cudaGetLastError());
-    long double K = 0.0L;                                   // sum_k w_k C(n,k) log2(ebar_k)
-    for (int k = 0; k <= c->n; k++) K += (long double)c->kc.w[k] * (long double)host_binom(c->n, k) * (long double)c->kc.lebar[k];
+    const long double K = 0.0L;                             // the pass centres term by term
     k_hc_final<<<c->num_sms * 8, 256, 0, c->st>>>(c->NX, c->S, c->S + c->NX, c->Hc, c->sym, (double)K);
     CK(cudaGetLastError());
     CK(cudaEventRecord(c->ev_setup[1], c->st));

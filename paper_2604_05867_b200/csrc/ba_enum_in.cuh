@@ -26,8 +26,8 @@
 // k_in_final (ba_stream.cuh) forms D(x) = Hc(x) - S_0(x) - S_1(x) and the first stage of the reductions of 8(a3).
 // MODE:
 //   IN_SWEEP  S_b(x)
-//   IN_HC     H_b(x) = sum_{y in item} w_k emb log2(emb)   (iteration independent; built once per ctx; k_hc_final
-//             subtracts the constant sum_k w_k C(n,k) log2(ebar_k) that centres it)
+//   IN_HC     H_b(x) = sum_{y in item} w_k (emb log2(emb) - emb log2(ebar_k))   (iteration independent; built once per ctx;
+//             centred term by term: the partial sums stay of the size of D)
 //   IN_DEBUG  emb_out[idx(y)] = emb(y,x) for one x     (ba_debug_emb_row; two CTAs, one per list)
 //   IN_COUNT  number of visited terms and sum of emb   (ba_debug_count_terms)
 #pragma once
@@ -349,7 +349,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                                 acc_eps = fma(ba_u2d(emb), bal[i].x0, acc_eps);
                             } else if (MODE == IN_HC) {
                                 const double wk = s_w[k];
-                                if (wk != 0.0 && emb > 1u) acc_eps = fma(wk, ba_elog2e(emb, a.elog), acc_eps);
+                                if (wk != 0.0) acc_eps = fma(wk, ba_elog2e(emb, a.elog) - (double)emb * s_lebar[k], acc_eps);
                             } else if (MODE == IN_DEBUG) {
                                 if (((u << m) | (uint32_t)ev) == a.dbg_x) a.dbg_out[cy - 1u] = emb;
                             } else {
@@ -380,7 +380,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                             const int jz = ba_len_of_code(cz);
                             if (MODE == IN_HC) {
                                 const double wk = s_w[k + jz];
-                                if (wk != 0.0 && emb > 1u) acc[s] = fma(wk, ba_elog2e(emb, a.elog), acc[s]);
+                                if (wk != 0.0) acc[s] = fma(wk, ba_elog2e(emb, a.elog) - (double)emb * s_lebar[k + jz], acc[s]);
                             } else if (MODE == IN_DEBUG) {
                                 const uint32_t ov = a.g.GO[(((size_t)b * BA_KG + s / BA_GP) * BA_GP + s % BA_GP) * BA_NT + tid];
                                 if (((u << m) | ov) == a.dbg_x) a.dbg_out[((size_t)rc.id << jz) + (cz - (1u << jz)) - 1u] = emb;
@@ -434,7 +434,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                                 } else if (MODE == IN_HC) {
                                     const int k = (int)(s_rec[bl.node].info >> 16);
                                     const double wk = s_w[k + jz];
-                                    if (wk != 0.0 && emb > 1u) s = fma(wk, ba_elog2e(emb, a.elog), s);
+                                    if (wk != 0.0) s = fma(wk, ba_elog2e(emb, a.elog) - (double)emb * s_lebar[k + jz], s);
                                 } else if (MODE == IN_DEBUG) {
                                     if (((u << m) | ov) == a.dbg_x) a.dbg_out[((size_t)cy << jz) + (cz - (1u << jz)) - 1u] = emb;
                                 } else {

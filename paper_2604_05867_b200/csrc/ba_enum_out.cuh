@@ -92,7 +92,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
     const uint32_t sFull = ba_smem_addr(smem + L.mbar), sEmpty = sFull + BA_OUT_NSTG * 8u;
     if (tid == 0) {
         for (int i = 0; i < BA_OUT_NSTG; i++) {
-            ba_mbar_init(sFull + 8u * i, 2u * BA_NT);       // per thread: its copies landed + its plain stores done
+            ba_mbar_init(sFull + 8u * i, 32u);              // the 32 lanes of the staging warp; the rows count in bytes (complete_tx)
             ba_mbar_init(sEmpty + 8u * i, BA_NT);           // per thread: finished reading the stage
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -100,7 +100,6 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
     uint32_t gb = 0;                                        // batches staged so far by this CTA (uniform)
     const int ev = tid & (nv - 1);                          // v of this thread's empty-z pairs
     const int esub = tid >> m, epn = BA_NT >> m;
-    const int st_pc = tid & ((nv >> 1) - 1), st_i0 = (nv > 1) ? (tid >> (m - 1)) : tid, st_step = (nv > 1) ? (BA_NT >> (m - 1)) : BA_NT;   // staging role
     const bool may_big = h > 18;                            // C(h, h/2) >= 2^16 first at h = 19
     __syncthreads();
 
@@ -241,24 +240,21 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
 
             // ================= phase B =================
             const int nbatch = (int)s_item[1];
-            auto stage = [&](int j, uint32_t g) {              // p rows and alphas of batch j = ring batch g
+            auto stage = [&](int j, uint32_t g) {              // p rows and alphas of batch j = ring batch g: warp 0 only
+                if (warp != 0) return;
                 const uint32_t bi = s_batch[j];
                 const int start = (int)(bi & 0xffffu), len = (int)((bi >> 16) & 0xffu), buf = (int)(g % BA_OUT_NSTG);
-                if (MODE == OUT_SWEEP) {
-                    // 16-byte pieces, 2^{m-1} per row: a thread always copies the same piece, of every st_step-th row
-                    for (int i = st_i0; i < len; i += st_step) {
-                        const uint32_t u = s_rec[s_order[start + i]].id;
-                        const uint32_t dst = sRows + (uint32_t)(buf * BA_RB_OUT + i) * BA_ROWB;
-                        if (nv > 1) ba_cp_async16(dst + 16u * (uint32_t)st_pc, a.p + ((u << m) + 2u * (uint32_t)st_pc));   // x fits 32 bits (n <= 30)
-                        else ba_cp_async8(dst, a.p + u);
-                    }
-                }
-                if (tid < len) {
-                    const int node = s_order[start + tid];
-                    s_bal[buf * BA_RB_OUT + tid] = ba_make_bal(s_rec[node], (uint32_t)node);
-                }
-                ba_mbar_arrive_on_copies(sFull + 8u * buf);    // when this thread's rows have landed
-                ba_mbar_arrive(sFull + 8u * buf);              // releases its plain stores above
+                if (lane < len) {                              // lane i: node i of the batch
+                    const int node = s_order[start + lane];
+                    const NodeRec &rc = s_rec[node];
+                    s_bal[buf * BA_RB_OUT + lane] = ba_make_bal(rc, (uint32_t)node);
+                    if (MODE == OUT_SWEEP) {
+                        // the whole row p(u.*) in one bulk copy (x fits 32 bits, n <= 30); its bytes complete the FULL
+                        // barrier of the stage, the arrive releases the BalRec stored above
+                        ba_mbar_arrive_expect_tx(sFull + 8u * buf, (uint32_t)nv * 8u);
+                        ba_bulk_g2s(sRows + (uint32_t)(buf * BA_RB_OUT + lane) * BA_ROWB, a.p + ((size_t)rc.id << m), (uint32_t)nv * 8u, sFull + 8u * buf);
+                    } else ba_mbar_arrive(sFull + 8u * buf);
+                } else ba_mbar_arrive(sFull + 8u * buf);
             };
             for (int j = 0; j < BA_OUT_NSTG - 1 && j < nbatch; j++) stage(j, gb + j);
             for (int j = 0; j < nbatch; j++) {
@@ -365,7 +361,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                 ba_mbar_arrive(sEmpty + 8u * buf);             // this thread has finished reading the stage
                 if (j + BA_OUT_NSTG - 1 < nbatch) {            // refill the stage of ring batch g-1 with batch j+NSTG-1
                     const uint32_t gn = g + BA_OUT_NSTG - 1;
-                    if (j >= 1) ba_mbar_wait(sEmpty + 8u * (gn % BA_OUT_NSTG), ((g - 1) / BA_OUT_NSTG) & 1u);
+                    if (warp == 0 && j >= 1) ba_mbar_wait(sEmpty + 8u * (gn % BA_OUT_NSTG), ((g - 1) / BA_OUT_NSTG) & 1u);
                     stage(j + BA_OUT_NSTG - 1, gn);
                 }
             }

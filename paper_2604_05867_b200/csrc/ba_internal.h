@@ -155,6 +155,17 @@ __device__ __forceinline__ void ba_mbar_arrive(uint32_t addr) {
 __device__ __forceinline__ void ba_mbar_arrive_on_copies(uint32_t addr) {      // arrives when this thread's cp.async landed
     asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(addr) : "memory");
 }
+// TMA-style bulk copy (cp.async.bulk, SASS UBLKCP): `bytes` (a multiple of 16, both addresses 16-byte aligned) from
+// global to shared memory by ONE thread; completion is counted in bytes on the mbarrier (complete_tx), which the same
+// thread armed with arrive.expect_tx.
+__device__ __forceinline__ void ba_mbar_arrive_expect_tx(uint32_t addr, uint32_t bytes) {
+    asm volatile("{ .reg .b64 st; mbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1; }" ::"r"(addr), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void ba_bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t mbar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(mbar) : "memory");
+}
+
 // A lost arrival must fail loudly, not hang the device: trap after ~20 s of SM clocks (far beyond any batch, also
 // under a profiler's replay or a preempted context, where a poll count would be reached much sooner than a clock).
 // try_wait suspends the warp in hardware until the phase completes or a time limit passes; the common case (the

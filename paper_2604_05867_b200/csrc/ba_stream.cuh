@@ -120,8 +120,8 @@ __global__ void __launch_bounds__(256) k_in_final(size_t NX, const double *__res
     }
 }
 
-// Hc = H_0 + H_1 - K (the two lists of the one-off IN_HC pass; K = sum_k w_k C(n,k) log2(ebar_k) turns
-// sum_y W log2(emb) into sum_y W log2(emb / ebar_k), since sum_{|y|=k} emb(y,x) = C(n,k)), mirrored under complement symmetry.
+// Hc = H_0 + H_1 - K (the two lists of the one-off IN_HC pass; K = an optional constant, 0 when the pass centres term by
+// term), mirrored under complement symmetry.
 __global__ void k_hc_final(size_t NX, const double *__restrict__ H0, const double *__restrict__ H1, double *__restrict__ Hc, int sym, double K) {
     const size_t NE = sym ? NX / 2 : NX;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < NE; i += (size_t)gridDim.x * blockDim.x) {

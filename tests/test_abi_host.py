@@ -85,3 +85,12 @@ def test_pair_tables_cover_every_pair_once(m):
     if m == 8:
         assert 0 < st[1] < 0.05 * (st[0] + st[1]) and st[1] == st[3]      # riders: the 3.4 % deep pairs
     assert ba.ba_debug_check_tables(0)[0] == ba.BA_EINVAL and ba.ba_debug_check_tables(9)[0] == ba.BA_EINVAL
+
+
+def test_lemma2_combiner_arithmetic():
+    # Lemma 2: sum_k C(n,k) d^(n-k) (1-d)^k C_{n,k}.  With C_{n,k} = k (the noiseless value, an upper bound
+    # of every C_{n,k}) the sum is the mean of Binomial(n, 1-d): n (1-d), the easy bound C_n(d) <= n (1-d).
+    from paper_2604_05867_b200 import exact
+    for n, d in [(8, 0.5), (12, 0.64), (29, 0.3)]:
+        assert exact.lemma2_bound(n, d, {k: float(k) for k in range(1, n + 1)}) == pytest.approx(n * (1 - d), rel=1e-12)
+    assert exact.lemma2_bound(2, 0.5, {1: 1.0, 2: 2.0}) == pytest.approx(2 * 0.25 * 1.0 + 0.25 * 2.0)   # C_{2,1} = 1, C_{2,2} = 2

@@ -406,3 +406,29 @@ def test_fast_mode_is_refused_while_symmetry_is_on(ba):
         assert ei.value.code == ba.BA_EINVAL
     finally:
         ba.ba_destroy(ctx)
+
+
+# ------------------------------------------------------------------ NEXT-3: the paper's workload (all k, stop rule, Lemma 2)
+
+@pytest.mark.parametrize("mode", [0, 1])
+def test_exact_workflow_all_k_and_lemma2_against_oracle(ba, mode):
+    from paper_2604_05867_b200 import exact
+    n, a = 8, 0.005                                           # the paper's tolerance
+    res = exact.run(n, a=a, ds=(0.3, 0.5, 0.64), mode=mode)
+    assert [r["k"] for r in res["capacities"]] == list(range(1, n + 1)) and all(r["converged"] for r in res["capacities"])
+    up = {}
+    for r in res["capacities"]:                               # every bracket contains the oracle's own converged bracket
+        k = r["k"]
+        ref = orc.ba_run(exact_W(n, k), si.uniform_p0(n), 6000)["hist"]
+        lo_ref, up_ref = ref[-1, 0], ref[:, 1].min()
+        assert r["I_lower"] <= up_ref + 1e-9 and lo_ref <= r["U_upper"] + 1e-9 and r["I_lower"] <= r["U_upper"]
+        assert r["stop_statistic"] < a and r["U_upper"] - r["I_lower"] < 2 * a + 0.05
+        it = r["iterations"]                                  # same iterate as the oracle after the same number of steps
+        assert abs(r["I_lower"] - ref[it - 1, 0]) <= ABS_U
+        up[k] = r["U_upper"]
+    assert res["capacities"][0]["U_upper"] >= 1.0 - 1e-12 and res["capacities"][-1]["I_lower"] == pytest.approx(float(n), abs=1e-12)   # C_{n,1} = 1, C_{n,n} = n (Tables 1-2)
+    for b in res["bounds"]:                                   # Lemma 2 above the direct capacity C_n(d)
+        direct = orc.ba_run(W_of(n, b["d"]), si.uniform_p0(n), 400)["hist"][-1, 0]
+        assert direct <= b["Cn_upper"] + 1e-12
+        assert b["Cn_upper"] == pytest.approx(exact.lemma2_bound(n, b["d"], up), rel=1e-15)
+        assert b["Cd_upper"] == pytest.approx(b["Cn_upper"] / n)
