@@ -28,7 +28,7 @@ struct ba_ctx {
     double *p = nullptr, *q = nullptr, *D = nullptr;
     unsigned char *scratch = nullptr;
     // carved from scratch
-    double *c = nullptr, *Hc = nullptr, *Apart = nullptr, *S = nullptr, *part = nullptr, *scal = nullptr, *hist = nullptr;
+    double *c = nullptr, *crow = nullptr, *Hc = nullptr, *Apart = nullptr, *S = nullptr, *part = nullptr, *scal = nullptr, *hist = nullptr;
     GroupDev gin, gout;              // pair schedules of the two sweeps (device pointers into scratch)
     uint2 *EPS8 = nullptr;
     uint32_t *EPSH = nullptr;
@@ -72,7 +72,7 @@ static double host_binom(int n, int k) {
 // ------------------------------------------------------------------------------------------------ scratch layout
 struct SideLayout { size_t GB, GA, GO, GW, csr_off, csr_idx, R, r_cnt, r_csr, R8; };
 struct ScratchLayout {
-    size_t c, Hc, Apart, S, part, scal, hist, EPS8, EPSH, elog, counters, cnt, total;
+    size_t c, crow, Hc, Apart, S, part, scal, hist, EPS8, EPSH, elog, counters, cnt, total;
     SideLayout in, out;
     size_t napart, npart_cap;
 };
@@ -116,6 +116,7 @@ static void scratch_layout(int n, const TileTables &T, ScratchLayout &L) {
     L.npart_cap = 65536;                                     // >= grid of k_in_final
     size_t o = 0;
     L.c = o; o += align256((NY + 1) * 8);                    // c[code], entry 0 unused
+    L.crow = o; o += align256(((size_t)4 << h) * ((size_t)1 << m) * 8);   // rows (code(y') <= 2^{h+1}-1, b) of 2^m operands
     L.Hc = o; o += align256(NX * 8);
     L.Apart = o; o += align256(L.napart * 8);
     L.S = o; o += align256(2 * NX * 8);                      // partial sums of the two lists (input sweep)
@@ -190,9 +191,10 @@ extern "C" int ba_debug_check_tables(int m, unsigned long long stats[4]) {
                     int v; uint32_t cz;
                     if (side) { v = (int)pos; cz = ow; }
                     else {
-                        if (pos == 0) return false;
-                        const int lt = 31 - __builtin_clz(pos);
-                        v = (int)ow; cz = (1u << (lt + 1)) | ((uint32_t)b << lt) | (pos - (1u << lt));
+                        if (pos < 2 && (int)pos != b) return false;          // z = "b" sits at position b of the half row
+                        const uint32_t tc = (pos < 2) ? 1u : pos;
+                        const int lt = 31 - __builtin_clz(tc);
+                        v = (int)ow; cz = (1u << (lt + 1)) | ((uint32_t)b << lt) | (tc - (1u << lt));
                     }
                     if (v < 0 || v >= nv || cz < 2 || cz >= (uint32_t)NZc) return false;
                     const int lz = 31 - __builtin_clz(cz);
@@ -325,7 +327,7 @@ static int finish_create(ba_ctx *c) {
     ScratchLayout L;
     scratch_layout(c->n, T, L);
     unsigned char *s = c->scratch;
-    c->c = (double *)(s + L.c); c->Hc = (double *)(s + L.Hc); c->Apart = (double *)(s + L.Apart); c->S = (double *)(s + L.S);
+    c->c = (double *)(s + L.c); c->crow = (double *)(s + L.crow); c->Hc = (double *)(s + L.Hc); c->Apart = (double *)(s + L.Apart); c->S = (double *)(s + L.S);
     c->part = (double *)(s + L.part); c->scal = (double *)(s + L.scal); c->hist = (double *)(s + L.hist);
     c->EPS8 = (uint2 *)(s + L.EPS8); c->EPSH = (uint32_t *)(s + L.EPSH); c->elog = (double *)(s + L.elog);
     c->counters = (unsigned int *)(s + L.counters); c->cnt = (unsigned long long *)(s + L.cnt);
@@ -462,7 +464,7 @@ extern "C" int ba_set_mode(ba_ctx *c, int mode) {
 static InArgs make_in_args(ba_ctx *c) {
     InArgs a;
     a.kc = c->kc; a.g = c->gin; a.EPS8 = c->EPS8; a.EPSH = c->EPSH;
-    a.c = c->c; a.elog = c->elog; a.S = c->S;
+    a.c = c->c; a.crow = c->crow; a.elog = c->elog; a.S = c->S;
     a.counter = c->counters; a.sym = 0; a.dbg_x = 0; a.dbg_out = nullptr; a.cnt = c->cnt;
     return a;
 }
@@ -500,7 +502,7 @@ static int launch_out_sweep(ba_ctx *c) {
         a.sym = c->sym;
         k_enum_out<OUT_SWEEP><<<c->grid_out, c->block, c->smem_out, c->st>>>(a);
         CK(cudaGetLastError());
-        k_out_final<<<c->num_sms * 8, 256, 0, c->st>>>(c->kc, c->Apart, nullptr, c->q, c->c, c->sym);
+        k_out_final<<<c->num_sms * 8, 256, 0, c->st>>>(c->kc, c->Apart, nullptr, c->q, c->c, c->crow, c->sym);
         CK(cudaGetLastError());
     } else {
         double *buf0 = c->Apart, *buf1 = c->Apart + (((size_t)2 << c->n) + 64);
@@ -512,7 +514,7 @@ static int launch_out_sweep(ba_ctx *c) {
             in = out;
             out = (out == buf0) ? buf1 : buf0;
         }
-        k_out_final<<<c->num_sms * 8, 256, 0, c->st>>>(c->kc, nullptr, in, c->q, c->c, 0);
+        k_out_final<<<c->num_sms * 8, 256, 0, c->st>>>(c->kc, nullptr, in, c->q, c->c, c->crow, 0);
         CK(cudaGetLastError());
     }
     return BA_OK;

@@ -45,6 +45,7 @@ struct InArgs {
     const uint2 *EPS8;        // [256][2^m]: B(sigma_s, v), s = 0..7, of the pair (v, empty)
     const uint32_t *EPSH;     // [cls][16][2^m]: B_4..B_7 of the pair (v, empty) by the sigma bits 4..7: a class's slice
     const double *c;          // IN_SWEEP: c[code(y)], 2^{n+1} entries (entry 0 unused)
+    const double *crow;       // IN_SWEEP: the same by rows (code(y'), b) of 2^m operands (k_out_final)
     const double *elog;       // IN_HC: elog[e] = e log2(e), e < BA_ELOG_N
     double *S;                // out: [2][2^n] partial sums of the two lists (IN_SWEEP: S_b, IN_HC: H_b)
     unsigned int *counter;    // work counter (zeroed before launch)
@@ -54,7 +55,7 @@ struct InArgs {
     unsigned long long *cnt;  // IN_COUNT: [0] terms, [1] emb sum
 };
 
-struct InSmem { size_t rec, slice, rows, bal, ordr, seg, order, gstart, wcnt, batch, rsum, sub, kcw, item, total; };
+struct InSmem { size_t rec, slice, rows, mbar, bal, ordr, seg, order, gstart, wcnt, batch, rsum, sub, kcw, item, total; };
 
 __host__ __device__ static inline InSmem enum_in_smem(int nr) {
     InSmem s;
@@ -65,6 +66,7 @@ __host__ __device__ static inline InSmem enum_in_smem(int nr) {
     s.slice = take((size_t)2 * 16 * ((size_t)1 << BA_MLOW) * 4);   // B_4..B_7 of the pairs (v, empty) of a class, double buffered
     size_t rows = (size_t)2 * BA_RB_IN * BA_ROWB, ac = ((size_t)BA_NSLOT + 1) * BA_NT * 8;
     s.rows = take(rows > ac ? rows : ac);                  // the epilogue's accumulator staging aliases the rows
+    s.mbar = take(2 * 8);                                  // FULL barrier of the two row buffers
     s.bal = take((size_t)2 * BA_RB_IN * sizeof(BalRec));
     s.ordr = take((size_t)BA_SBR * BA_NT * 2);             // per round: the round's nodes by class
     s.seg = take((size_t)BA_SBR * (BA_IN_NBKT + 1) * 2);
@@ -86,8 +88,10 @@ __device__ __forceinline__ double ba_elog2e(uint32_t e, const double *tab) {
     return (double)e * log2((double)e);
 }
 
-// z = b.t from the list b and code(t)
-__device__ __forceinline__ uint32_t ba_z_of_tail(uint32_t b, uint32_t tc) {
+// z = b.t from the list b and the position of its operand in the staged half row: code(t), except that the
+// one-symbol z = "b" (t empty) sits at position b
+__device__ __forceinline__ uint32_t ba_z_of_tail(uint32_t b, uint32_t pos) {
+    const uint32_t tc = (pos < 2u) ? 1u : pos;
     const int lt = ba_len_of_code(tc);
     return (1u << (lt + 1)) | (b << lt) | (tc - (1u << lt));
 }
@@ -117,14 +121,17 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
     uint32_t *s_item = (uint32_t *)(smem + L.item);        // [0] item, [1] number of batches
 
     for (int i = tid; i <= BA_NMAX_I; i += BA_NT) { s_w[i] = a.kc.w[i]; s_lebar[i] = a.kc.lebar[i]; }
-    for (int i = tid; i < 2 * BA_RB_IN; i += BA_NT) s_rows[(size_t)i * (BA_ROWB / 8)] = 0.0;   // position 0: unused slots
+    const uint32_t sFull = ba_smem_addr(smem + L.mbar);
+    if (tid == 0) {
+        ba_mbar_init(sFull, 32u); ba_mbar_init(sFull + 8u, 32u);        // the 32 lanes of the staging warp; rows count in bytes
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    for (int i = tid; i < 2 * BA_RB_IN * (int)(BA_ROWB / 8); i += BA_NT) s_rows[i] = 0.0;      // unused slots read finite operands
+    uint32_t gb = 0;                                        // batches staged so far by this CTA (uniform): buffer and phase
 
     const uint32_t sRows = ba_smem_addr(s_rows);
     const int ev = tid & (nv - 1);                          // v of this thread's empty-z pairs
     const int esub = tid >> m, epn = BA_NT >> m;            // it serves nodes esub, esub + epn, ...
-    const int st_pc = tid & ((nv >> 1) - 1), st_i0 = (nv > 1) ? (tid >> (m - 1)) : tid, st_step = (nv > 1) ? (BA_NT >> (m - 1)) : BA_NT;   // staging role
-    const int st_lt = st_pc ? ba_len_of_code(2u * (uint32_t)st_pc) : 0;
-    const uint32_t st_tv = st_pc ? (2u * (uint32_t)st_pc - (1u << st_lt)) : 0u, st_dst = 16u * (uint32_t)st_pc;
     const bool may_big = h > 18;                            // C(h, h/2) >= 2^16 first at h = 19
     __syncthreads();
 
@@ -258,7 +265,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
             int st_cls = -1, st_sb = 0, cp_cls = -1, cp_sb = 0;     // slice double buffer: staging side, computing side
             auto stage = [&](int j) {                          // half rows and alphas of batch j
                 const uint32_t bi = s_batch[j];
-                const int start = (int)(bi & 0xffffu), len = (int)((bi >> 16) & 0xffu), buf = j & 1;
+                const int start = (int)(bi & 0xffffu), len = (int)((bi >> 16) & 0xffu), buf = (int)((gb + (uint32_t)j) & 1u);
                 const int scls = (int)(bi >> 24) & (BA_NCLS - 1);
                 if (b == 0 && scls != st_cls) {                // a new class: its slice of B_4..B_7 of the pairs (v, empty)
                     st_cls = scls; st_sb ^= 1;
@@ -267,30 +274,26 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                     for (int e = tid; e < 16 * nv; e += BA_NT)
                         asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst + (uint32_t)((e >> m) << BA_MLOW) * 4u + (uint32_t)(e & (nv - 1)) * 4u), "l"(src + e) : "memory");
                 }
-                if (MODE == IN_SWEEP && (bi >> 24) < BA_NCLS) {
-                    // 16-byte pieces (positions 2pc, 2pc+1), 2^{m-1} per half row: a thread always copies the same
-                    // piece, of every st_step-th row
-                    for (int i = st_i0; i < len; i += st_step) {
-                        const uint32_t cy = s_rec[s_order[start + i]].id;
-                        const uint32_t dst = sRows + (uint32_t)(buf * BA_RB_IN + i) * BA_ROWB;
-                        if (st_pc == 0)                        // position 1: t empty, z = "b"
-                            ba_cp_async8(dst + 8u, a.c + ((cy << 1) + (uint32_t)b));           // codes fit 32 bits (n <= 30)
-                        else
-                            ba_cp_async16(dst + st_dst, a.c + ((cy << (st_lt + 1)) + ((uint32_t)b << st_lt) + st_tv));
-                    }
-                }
-                if (tid < len) {
-                    const int node = s_order[start + tid];
-                    s_bal[buf * BA_RB_IN + tid] = ba_make_bal(s_rec[node], (uint32_t)node);
-                    if (MODE == IN_SWEEP && b == 0)            // operand of the pair (v, empty): c(y'), lands with the rows
-                        ba_cp_async8(ba_smem_addr(&s_bal[buf * BA_RB_IN + tid].x0), a.c + s_rec[node].id);
-                }
+                if (warp != 0) return;                         // rows and node records: the staging warp, lane i = node i
+                if (lane < len) {
+                    const int node = s_order[start + lane];
+                    const NodeRec &rc = s_rec[node];
+                    s_bal[buf * BA_RB_IN + lane] = ba_make_bal(rc, (uint32_t)node);
+                    if (MODE == IN_SWEEP && b == 0)            // operand of the pair (v, empty): c(y'), lands before the CTA barrier
+                        ba_cp_async8(ba_smem_addr(&s_bal[buf * BA_RB_IN + lane].x0), a.c + rc.id);
+                    if (MODE == IN_SWEEP && (bi >> 24) < BA_NCLS) {
+                        // the half row c(y'.b.t), all t, is row (code(y'), b) of crow: one bulk copy
+                        ba_mbar_arrive_expect_tx(sFull + 8u * buf, (uint32_t)nv * 8u);
+                        ba_bulk_g2s(sRows + (uint32_t)(buf * BA_RB_IN + lane) * BA_ROWB, a.crow + (((((size_t)rc.id) << 1) | (size_t)b) << m),
+                                    (uint32_t)nv * 8u, sFull + 8u * buf);
+                    } else ba_mbar_arrive(sFull + 8u * buf);
+                } else ba_mbar_arrive(sFull + 8u * buf);
             };
             auto flush = [&](int j) {                          // thread v collects the rider sums of batch j
                 if (MODE != IN_SWEEP && MODE != IN_HC) return;
                 if (tid >= nv) return;
                 if ((s_batch[j] >> 24) >= BA_NCLS) return;     // a batch without list b has no riders
-                const int cls = (int)(s_batch[j] >> 24), buf = j & 1;
+                const int cls = (int)(s_batch[j] >> 24), buf = (int)((gb + (uint32_t)j) & 1u);
                 const uint16_t *cs = a.g.r_csr + (size_t)(cls * 2 + b) * (nv + 1) + tid;
                 const int e0 = cs[0], e1 = cs[1];
                 for (int e = e0; e < e1; e++) acc_rid += s_rsum[((size_t)buf * 2) * a.g.nr + e] + s_rsum[((size_t)buf * 2 + 1) * a.g.nr + e];
@@ -298,7 +301,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
             if (nbatch > 0) stage(0);
             for (int j = 0; j < nbatch; j++) {
                 const uint32_t bi = s_batch[j];
-                const int len = (int)((bi >> 16) & 0xffu), cls = (int)(bi >> 24) & (BA_NCLS - 1), kind = (int)(bi >> 28), buf = j & 1;
+                const int len = (int)((bi >> 16) & 0xffu), cls = (int)(bi >> 24) & (BA_NCLS - 1), kind = (int)(bi >> 28), buf = (int)((gb + (uint32_t)j) & 1u);
                 if (b == 0 && cls != cp_cls) { cp_cls = cls; cp_sb ^= 1; }
                 uint32_t eB0 = 0u;                             // 1 | B_1..B_3 of the pair (ev, empty): a constant of the class
                 if (b == 0) eB0 = __ldg(a.EPS8 + (size_t)cls * nv + ev).x;
@@ -311,6 +314,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                     Bp[k * BA_GP] = bb.x; Bp[k * BA_GP + 1] = bb.y; Bp[k * BA_GP + 2] = bb.z; Bp[k * BA_GP + 3] = bb.w;
                 }
                 ba_cp_async_wait_all();
+                ba_mbar_wait(sFull + 8u * buf, ((gb + (uint32_t)j) >> 1) & 1u);     // the rows of batch j have landed
                 __syncthreads();                               // batch j staged; batch j-1 fully consumed
                 if (j + 1 < nbatch) stage(j + 1);
                 if (j > 0) flush(j - 1);
@@ -451,6 +455,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 __syncthreads();                               // rider sums of the last batch are visible
                 flush(nbatch - 1);
             }
+            gb += (uint32_t)nbatch;
         }
 
         // ---- epilogue: thread v owns x = u.v ------------------------------------------------------------
@@ -468,8 +473,6 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 for (int q = co[0]; q < co[1]; q++) S += s_acc[ci[q]];
                 a.S[(size_t)b * NX + (((size_t)u << m) | (size_t)tid)] = S;
             }
-            __syncthreads();
-            for (int i = tid; i < 2 * BA_RB_IN; i += BA_NT) s_rows[(size_t)i * (BA_ROWB / 8)] = 0.0;   // restore position 0 of the rows
         }
         if (MODE == IN_DEBUG) break;
         __syncthreads();

@@ -11,14 +11,26 @@
 // C(n,k)/2^k is the mean of emb over a length, which centres both halves.
 // c is stored by CODE (c[code(y)] = c[idx(y)+1], entry 0 unused) so that the 2^j outputs y'.z, |z| = j,
 // of a prefix y' start at the even index code(y') << j: 16-byte aligned pieces for cp.async.
+// crow is the same operand laid out for the input sweep's staging: row (code(y'), b) of 2^m doubles holds c(y'.b.t) at
+// position code(t) (z = "b" alone at position b), for every y' of length <= h -- the half row of node y' and list b is
+// one contiguous, aligned run (one bulk copy); every c(y) is stored once per split y = y'.z, 1 <= |z| <= m.
+__device__ __forceinline__ void ba_store_crow(const KConst &kc, double *__restrict__ crow, uint32_t cy, int k, double v) {
+    const int jhi = (k < kc.m) ? k : kc.m;
+    for (int j = (k - kc.h > 1) ? (k - kc.h) : 1; j <= jhi; j++) {
+        const uint32_t cyp = cy >> j, b = (cy >> (j - 1)) & 1u;
+        const uint32_t pos = (j == 1) ? b : ((1u << (j - 1)) | (cy & ((1u << (j - 1)) - 1u)));
+        crow[((((size_t)cyp << 1) | b) << kc.m) + pos] = v;
+    }
+}
+
 __global__ void k_out_final(KConst kc, const double *__restrict__ Apart, const double *__restrict__ Afull,
-                            double *__restrict__ q, double *__restrict__ c, int sym) {
+                            double *__restrict__ q, double *__restrict__ c, double *__restrict__ crow, int sym) {
     const size_t NY = ((size_t)2 << kc.n) - 1;
     const uint32_t NZ = (2u << kc.m) - 1u;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < NY; i += (size_t)gridDim.x * blockDim.x) {
         const uint32_t cy = (uint32_t)(i + 1);
         const int k = ba_len_of_code(cy);
-        if (kc.w[k] == 0.0) { q[i] = 0.0; c[i + 1] = 0.0; continue; }   // R7: a length without mass (its partials may be unwritten)
+        if (kc.w[k] == 0.0) { q[i] = 0.0; c[i + 1] = 0.0; ba_store_crow(kc, crow, cy, k, 0.0); continue; }   // R7: a length without mass (its partials may be unwritten)
         double A;
         if (Afull) {
             A = Afull[i];
@@ -36,7 +48,9 @@ __global__ void k_out_final(KConst kc, const double *__restrict__ Apart, const d
         }
         const double wk = kc.w[k];
         q[i] = wk * A;
-        c[i + 1] = (wk != 0.0) ? wk * (log2(A) - kc.lebar[k]) : 0.0;
+        const double cv = (wk != 0.0) ? wk * (log2(A) - kc.lebar[k]) : 0.0;
+        c[i + 1] = cv;
+        ba_store_crow(kc, crow, cy, k, cv);
     }
 }
 

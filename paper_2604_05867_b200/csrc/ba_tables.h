@@ -205,7 +205,13 @@ static inline void build_tile_tables(int m, TileTables &T) {
         GroupSide &S = side ? T.out : T.in;
         // operand position in a staged row.  in: the operand of z = b.t is c(y'.b.t) at position code(t) of the
         // node's half row; out: the operand of (v, z) is p(u.v) at position v of the node's row.
-        auto key_of = [&](const TTPair &p) -> uint32_t { return side ? (uint32_t)p.v : tail_of(p.cz); };
+        // (the one-symbol z = "b" sits at position b, not 1: the staged half row starts with the 16-byte pair
+        // c(y'.0), c(y'.1), so that every piece of it is a bulk copy)
+        auto key_of = [&](const TTPair &p) -> uint32_t {
+            if (side) return (uint32_t)p.v;
+            const uint32_t tc = tail_of(p.cz);
+            return tc == 1u ? (uint32_t)(p.cz & 1u) : tc;
+        };
         auto owner_of = [&](const TTPair &p) -> uint32_t { return side ? p.cz : (uint32_t)p.v; };
         std::vector<std::vector<uint4>> riders((size_t)BA_NCLS * 2);
         std::vector<std::vector<TTPair>> rider_pairs((size_t)BA_NCLS * 2);
