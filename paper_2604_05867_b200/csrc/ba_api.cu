@@ -229,7 +229,7 @@ extern "C" int ba_debug_check_tables(int m, unsigned long long stats[4]) {
                 for (int e = 0; e < nr; e++) {
                     const uint4 rd = G.R[((size_t)cls * 2 + b) * G.nr + e];
                     uint32_t tail8[16];
-                    for (uint32_t hi = 0; hi < 16u; hi++) tail8[hi] = G.R8[(((size_t)cls * 2 + b) * 16 + hi) * G.nr + e];
+                    for (uint32_t hi = 0; hi < 16u; hi++) tail8[hi] = G.R8[(((size_t)cls * 2 + b) * 8 + (hi & 7u)) * G.nr + e];   // B_4..B_7 read sigma bits 4..6 only
                     if (!visit(rd.z >> 3, rd.y >> 16, rd.x, 5 + (int)(rd.y & 0xffu), tail8) || (rd.y & 0xffu) == 0) return BA_EINVAL;
                     const uint16_t *cs = &G.r_csr[((size_t)cls * 2 + b) * (G.nown + 1)];
                     const uint32_t ow = rd.y >> 16;

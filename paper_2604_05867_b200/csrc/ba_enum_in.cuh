@@ -43,7 +43,7 @@ struct InArgs {
     KConst kc;
     GroupDev g;               // schedule of the input sweep (owner = v, operand position = code(z[1:]))
     const uint2 *EPS8;        // [256][2^m]: B(sigma_s, v), s = 0..7, of the pair (v, empty)
-    const uint32_t *EPSH;     // [cls][16][2^m]: B_4..B_7 of the pair (v, empty) by the sigma bits 4..7: a class's slice
+    const uint32_t *EPSH;     // [cls][8][2^m]: B_4..B_7 of the pair (v, empty) by the sigma bits 4..6: a class's slice
     const double *c;          // IN_SWEEP: c[code(y)], 2^{n+1} entries (entry 0 unused)
     const double *crow;       // IN_SWEEP: the same by rows (code(y'), b) of 2^m operands (k_out_final)
     const double *elog;       // IN_HC: elog[e] = e log2(e), e < BA_ELOG_N
@@ -55,7 +55,7 @@ struct InArgs {
     unsigned long long *cnt;  // IN_COUNT: [0] terms, [1] emb sum
 };
 
-struct InSmem { size_t rec, slice, rows, mbar, bal, ordr, seg, order, gstart, wcnt, batch, rsum, sub, kcw, item, total; };
+struct InSmem { size_t rec, slice, rslice, rows, mbar, bal, ordr, seg, order, gstart, wcnt, batch, rsum, sub, kcw, item, total; };
 
 __host__ __device__ static inline InSmem enum_in_smem(int nr) {
     InSmem s;
@@ -63,7 +63,8 @@ __host__ __device__ static inline InSmem enum_in_smem(int nr) {
     auto take = [&](size_t bytes) { size_t at = o; o += (bytes + 15) & ~(size_t)15; return at; };
     s.rec = take((size_t)BA_IN_SB * sizeof(NodeRec));
     s.rsum = take((size_t)2 * 2 * nr * 8);                 // rider sums of a batch, two replicas, double buffered
-    s.slice = take((size_t)2 * 16 * ((size_t)1 << BA_MLOW) * 4);   // B_4..B_7 of the pairs (v, empty) of a class, double buffered
+    s.slice = take((size_t)2 * 8 * ((size_t)1 << BA_MLOW) * 4);    // B_4..B_7 of the pairs (v, empty) of a class, double buffered
+    s.rslice = take((size_t)2 * 8 * nr * 4);               // B_4..B_7 of the riders of a class, double buffered
     size_t rows = (size_t)2 * BA_RB_IN * BA_ROWB, ac = ((size_t)BA_NSLOT + 1) * BA_NT * 8;
     s.rows = take(rows > ac ? rows : ac);                  // the epilogue's accumulator staging aliases the rows
     s.mbar = take(2 * 8);                                  // FULL barrier of the two row buffers
@@ -105,6 +106,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
 
     NodeRec *s_rec = (NodeRec *)(smem + L.rec);
     uint32_t *s_slice = (uint32_t *)(smem + L.slice);
+    uint32_t *s_rslice = (uint32_t *)(smem + L.rslice);
     double *s_rows = (double *)(smem + L.rows);
     double *s_acc = s_rows;                                 // epilogue only
     BalRec *s_bal = (BalRec *)(smem + L.bal);
@@ -267,12 +269,20 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 const uint32_t bi = s_batch[j];
                 const int start = (int)(bi & 0xffffu), len = (int)((bi >> 16) & 0xffu), buf = (int)((gb + (uint32_t)j) & 1u);
                 const int scls = (int)(bi >> 24) & (BA_NCLS - 1);
-                if (b == 0 && scls != st_cls) {                // a new class: its slice of B_4..B_7 of the pairs (v, empty)
-                    st_cls = scls; st_sb ^= 1;
-                    const uint32_t *src = a.EPSH + (size_t)scls * 16 * nv;
-                    const uint32_t dst = ba_smem_addr(s_slice) + (uint32_t)st_sb * (16u << BA_MLOW) * 4u;
-                    for (int e = tid; e < 16 * nv; e += BA_NT)
-                        asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst + (uint32_t)((e >> m) << BA_MLOW) * 4u + (uint32_t)(e & (nv - 1)) * 4u), "l"(src + e) : "memory");
+                if (scls != st_cls) {                          // a new class: its slices of B_4..B_7 (by the sigma bits 4..6)
+                    st_cls = scls; st_sb ^= 1;                 // of the riders and, for b = 0, of the pairs (v, empty)
+                    {
+                        const uint32_t *src = a.g.R8 + ((size_t)scls * 2 + b) * 8 * a.g.nr;
+                        const uint32_t dst = ba_smem_addr(s_rslice) + (uint32_t)st_sb * 8u * (uint32_t)a.g.nr * 4u;
+                        for (int e = tid; e < 8 * a.g.nr; e += BA_NT)
+                            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst + (uint32_t)e * 4u), "l"(src + e) : "memory");
+                    }
+                    if (b == 0) {
+                        const uint32_t *src = a.EPSH + (size_t)scls * 8 * nv;
+                        const uint32_t dst = ba_smem_addr(s_slice) + (uint32_t)st_sb * (8u << BA_MLOW) * 4u;
+                        for (int e = tid; e < 8 * nv; e += BA_NT)
+                            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst + (uint32_t)((e >> m) << BA_MLOW) * 4u + (uint32_t)(e & (nv - 1)) * 4u), "l"(src + e) : "memory");
+                    }
                 }
                 if (warp != 0) return;                         // rows and node records: the staging warp, lane i = node i
                 if (lane < len) {
@@ -302,7 +312,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
             for (int j = 0; j < nbatch; j++) {
                 const uint32_t bi = s_batch[j];
                 const int len = (int)((bi >> 16) & 0xffu), cls = (int)(bi >> 24) & (BA_NCLS - 1), kind = (int)(bi >> 28), buf = (int)((gb + (uint32_t)j) & 1u);
-                if (b == 0 && cls != cp_cls) { cp_cls = cls; cp_sb ^= 1; }
+                if (cls != cp_cls) { cp_cls = cls; cp_sb ^= 1; }
                 uint32_t eB0 = 0u;                             // 1 | B_1..B_3 of the pair (ev, empty): a constant of the class
                 if (b == 0) eB0 = __ldg(a.EPS8 + (size_t)cls * nv + ev).x;
                 // the slots' B_s do not depend on the staged rows: fetch them before waiting
@@ -325,20 +335,20 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 // ---- the pair (v, empty) of every node of the batch: thread (v, node) -----------------------------
                 if (b == 0 && (kind == 1 || klen < 0)) {
                     const uint32_t sv8 = (m == 8) ? (uint32_t)ev : 0xffffffffu;      // B_8 = [sigma_8 = v] (m = 8 only)
-                    const uint32_t *sl = s_slice + (size_t)cp_sb * (16u << BA_MLOW) + ev;    // [sigma bits 4..7][v]
+                    const uint32_t *sl = s_slice + (size_t)cp_sb * (8u << BA_MLOW) + ev;     // [sigma bits 4..6][v]
                     if (MODE == IN_SWEEP && !big) {
                         double e0 = 0.0, e1 = 0.0;             // two chains; nodes esub, esub + epn, ...
 #pragma unroll 4
                         for (int i = esub; i < len; i += 2 * epn) {
                             const uint4 al = *(const uint4 *)&bal[i];
                             const uint32_t cy = bal[i].id;
-                            const uint32_t emb = ba_chain9(al.x, al.y, al.z, al.w, bal[i].a8, eB0, sl[((cy >> 4) & 15u) << BA_MLOW], (cy & 255u) == sv8);
+                            const uint32_t emb = ba_chain9(al.x, al.y, al.z, al.w, bal[i].a8, eB0, sl[((cy >> 4) & 7u) << BA_MLOW], (cy & 255u) == sv8);
                             e0 = fma(ba_u2d(emb), bal[i].x0, e0);
                             const int i2 = i + epn;
                             if (i2 < len) {
                                 const uint4 al2 = *(const uint4 *)&bal[i2];
                                 const uint32_t cy2 = bal[i2].id;
-                                const uint32_t emb2 = ba_chain9(al2.x, al2.y, al2.z, al2.w, bal[i2].a8, eB0, sl[((cy2 >> 4) & 15u) << BA_MLOW], (cy2 & 255u) == sv8);
+                                const uint32_t emb2 = ba_chain9(al2.x, al2.y, al2.z, al2.w, bal[i2].a8, eB0, sl[((cy2 >> 4) & 7u) << BA_MLOW], (cy2 & 255u) == sv8);
                                 e1 = fma(ba_u2d(emb2), bal[i2].x0, e1);
                             }
                         }
@@ -348,7 +358,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                             const NodeRec &rc = s_rec[bal[i].node];
                             const uint32_t cy = rc.id;
                             const int k = (int)(rc.info >> 16);
-                            const uint32_t emb = ba_chain9_wide(rc.a, eB0, sl[((cy >> 4) & 15u) << BA_MLOW], (cy & 255u) == sv8);
+                            const uint32_t emb = ba_chain9_wide(rc.a, eB0, sl[((cy >> 4) & 7u) << BA_MLOW], (cy & 255u) == sv8);
                             if (MODE == IN_SWEEP) {
                                 acc_eps = fma(ba_u2d(emb), bal[i].x0, acc_eps);
                             } else if (MODE == IN_HC) {
@@ -409,19 +419,19 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                         const uint32_t ov = rd.y >> 16;
                         const uint32_t cz = ba_z_of_tail((uint32_t)b, rd.z >> 3);
                         const int jz = ba_len_of_code(cz);
-                        const uint32_t *r8 = a.g.R8 + ((size_t)cls * 2 + b) * 16 * a.g.nr + re;    // B_4..B_7 by sigma bits 4..7
+                        const uint32_t *r8 = s_rslice + (size_t)cp_sb * 8 * a.g.nr + re;           // B_4..B_7 by sigma bits 4..6: the class's slice
                         if (MODE == IN_SWEEP && !big) {
                             const double *rrow = s_rows + (size_t)(buf * BA_RB_IN) * (BA_ROWB / 8) + (rd.z >> 3);
                             double r0 = 0.0, r1 = 0.0;         // two chains; this replica's nodes rh, rh + 2, ...
 #pragma unroll 4
                             for (int i = rh; i < len; i += 4) {
                                 const uint4 al = *(const uint4 *)&bal[i];
-                                const uint32_t x8 = __ldg(r8 + (size_t)((bal[i].id >> 4) & 15u) * a.g.nr);   // alpha_s = 0 beyond k
+                                const uint32_t x8 = r8[(size_t)((bal[i].id >> 4) & 7u) * a.g.nr];       // alpha_s = 0 beyond k
                                 const uint32_t emb = ba_chain9(al.x, al.y, al.z, al.w, 0u, rd.x, x8, 0u);
                                 r0 = fma(ba_u2d(emb), rrow[(size_t)i * (BA_ROWB / 8)], r0);
                                 if (i + 2 < len) {
                                     const uint4 al2 = *(const uint4 *)&bal[i + 2];
-                                    const uint32_t y8 = __ldg(r8 + (size_t)((bal[i + 2].id >> 4) & 15u) * a.g.nr);
+                                    const uint32_t y8 = r8[(size_t)((bal[i + 2].id >> 4) & 7u) * a.g.nr];
                                     const uint32_t emb2 = ba_chain9(al2.x, al2.y, al2.z, al2.w, 0u, rd.x, y8, 0u);
                                     r1 = fma(ba_u2d(emb2), rrow[(size_t)(i + 2) * (BA_ROWB / 8)], r1);
                                 }
@@ -431,7 +441,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                             for (int i = rh; i < len; i += 2) {
                                 const BalRec bl = bal[i];
                                 const uint32_t cy = bl.id;
-                                const uint32_t x8 = __ldg(r8 + (size_t)((cy >> 4) & 15u) * a.g.nr);
+                                const uint32_t x8 = r8[(size_t)((cy >> 4) & 7u) * a.g.nr];
                                 const uint32_t emb = ba_chain9_wide(s_rec[bl.node].a, rd.x, x8, 0u);
                                 if (MODE == IN_SWEEP) {
                                     s = fma(ba_u2d(emb), ba_lds_f64(rowbase + (uint32_t)i * BA_ROWB + rd.z), s);

@@ -162,7 +162,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
         uint32_t rB0 = 0, rB1 = 0, rB2 = 0, roff = 0, rown = 0;
         if (re < nr) {
             const uint4 rd = __ldg(a.g.R + ((size_t)cls * 2 + b) * a.g.nr + re);
-            const uint32_t x8 = __ldg(a.g.R8 + (((size_t)cls * 2 + b) * 16 + ((cy >> 4) & 15u)) * a.g.nr + re);
+            const uint32_t x8 = __ldg(a.g.R8 + (((size_t)cls * 2 + b) * 8 + ((cy >> 4) & 7u)) * a.g.nr + re);
             rB0 = rd.x; rB1 = x8; rB2 = 0u;                     // B_0..3, B_4..7; B_8 = 0 (|z| >= 1)
             roff = rd.z; rown = rd.y >> 16;
         }

@@ -101,7 +101,7 @@ struct GroupDev {
     const uint4 *R;                   // riders [cls][b][nr]
     const uint16_t *r_cnt;            // [cls][b]
     const uint16_t *r_csr;            // [cls][b][nown + 1]
-    const uint32_t *R8;               // [cls][b][16][nr]: B_4..B_7 by the sigma bits 4..7
+    const uint32_t *R8;               // [cls][b][8][nr]: B_4..B_7 by the sigma bits 4..6
     int nr, nown;
 };
 

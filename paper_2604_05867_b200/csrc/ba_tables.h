@@ -19,7 +19,7 @@ struct GroupSide {
     std::vector<uint4> R;           // riders [BA_NCLS][2][nr]: {B0..B3, B4 | owner << 16, row byte offset, 0}, sorted by owner
     std::vector<uint16_t> r_cnt;    // [BA_NCLS][2]
     std::vector<uint16_t> r_csr;    // [BA_NCLS][2][nown + 1] rider range of an owner
-    std::vector<uint32_t> R8;       // [BA_NCLS][2][16][nr]: bytes = B_4..B_7 of the rider for sigma bits 4..7 (B_8 = 0)
+    std::vector<uint32_t> R8;       // [BA_NCLS][2][8][nr]: bytes = B_4..B_7 of the rider for sigma bits 4..6 (B_7 reads 7 symbols of sigma; B_8 = 0)
     int nr = 0;
     unsigned long long npairs[2] = {0, 0}, nslots[2] = {0, 0}, ngroups[2] = {0, 0};   // statistics
 };
@@ -28,7 +28,7 @@ struct TileTables {
     int m = 0, nv = 0;
     GroupSide in, out;
     std::vector<uint2> EPS8;        // [256][nv]: byte s = B(sigma_s, v), s = 0..7, sigma = the row index
-    std::vector<uint32_t> EPSH;     // [BA_NCLS][16][nv]: EPS8[(hi << 4) | cls][v].y, the slice of a class (input sweep)
+    std::vector<uint32_t> EPSH;     // [BA_NCLS][8][nv]: EPS8[(hi << 4) | cls][v].y, hi = sigma bits 4..6: the slice of a class (input sweep)
     bool ok = false;
 };
 
@@ -279,19 +279,19 @@ static inline void build_tile_tables(int m, TileTables &T) {
         if (S.nr > BA_NT / 2) return;                          // two replicas of the rider set share the CTA
         S.R.assign((size_t)BA_NCLS * 2 * S.nr, make_uint4(0u, 0u, 0u, 0u));
         S.r_cnt.assign((size_t)BA_NCLS * 2, 0);
-        S.R8.assign((size_t)BA_NCLS * 2 * 16 * S.nr, 0u);
+        S.R8.assign((size_t)BA_NCLS * 2 * 8 * S.nr, 0u);
         for (size_t i = 0; i < riders.size(); i++) {
             S.r_cnt[i] = (uint16_t)riders[i].size();
             std::copy(riders[i].begin(), riders[i].end(), S.R.begin() + i * S.nr);
             const int cls = (int)(i / 2);
-            for (uint32_t hi = 0; hi < 16u; hi++)
+            for (uint32_t hi = 0; hi < 8u; hi++)
                 for (size_t e = 0; e < rider_pairs[i].size(); e++) {
                     const TTPair &p = rider_pairs[i][e];
                     const int lz = 31 - __builtin_clz(p.cz);
                     uint32_t x = 0;                            // B_8 = 0: |z| >= 1
                     for (int sft = 4; sft <= 7; sft++)
                         if (lz + sft <= m) x |= Bof(tt_prepend((hi << 4) | (uint32_t)cls, sft, p.cz), p.v) << (8 * (sft - 4));
-                    S.R8[(i * 16 + hi) * S.nr + e] = x;
+                    S.R8[(i * 8 + hi) * S.nr + e] = x;
                 }
         }
     }
@@ -305,9 +305,9 @@ static inline void build_tile_tables(int m, TileTables &T) {
                 w[sft / 4] |= Bof((1u << sft) | (sig & ((1u << sft) - 1u)), v) << (8 * (sft % 4));
             T.EPS8[(size_t)sig * nv + v] = make_uint2(w[0], w[1]);
         }
-    T.EPSH.assign((size_t)BA_NCLS * 16 * nv, 0u);
+    T.EPSH.assign((size_t)BA_NCLS * 8 * nv, 0u);
     for (uint32_t cls = 0; cls < BA_NCLS; cls++)
-        for (uint32_t hi = 0; hi < 16u; hi++)
-            for (int v = 0; v < nv; v++) T.EPSH[((size_t)cls * 16 + hi) * nv + v] = T.EPS8[(size_t)((hi << 4) | cls) * nv + v].y;
+        for (uint32_t hi = 0; hi < 8u; hi++)
+            for (int v = 0; v < nv; v++) T.EPSH[((size_t)cls * 8 + hi) * nv + v] = T.EPS8[(size_t)((hi << 4) | cls) * nv + v].y;
     T.ok = true;
 }

@@ -307,3 +307,40 @@ def test_T3_T4_one_step_n14_extreme_d(ba, d, seed, mode):
     assert np.max(np.abs(q - ref["q"]) / ref["q"]) <= REL_QD
     assert np.max(np.abs(D - ref["D"]) / np.abs(ref["D"])) <= REL_QD
     assert abs(I - ref["I"]) <= REL_QD * max(1.0, abs(ref["I"])) and abs(U - ref["U"]) <= REL_QD * max(1.0, abs(ref["U"]))
+
+
+# ------------------------------------------------------------------ measurement entry points of the ABI
+
+def test_measured_peaks_and_setup_time(ba):
+    pk = ba.ba_measure_peaks()
+    # B200: FP64 and the integer-multiply pipe issue one warp-instruction every 2 clocks per scheduler (2 per clock per
+    # SM), a conflict-free LDS.64 moves 256 bytes (1 per clock per SM), FP32 FMA fills the issue slots (4 per clock per SM)
+    assert 1.5 <= pk["dfma"] <= 2.1 and 1.8 <= pk["idp2a"] <= 2.1 and 0.8 <= pk["lds64"] <= 1.1 and 3.3 <= pk["ffma"] <= 4.1
+    assert pk["sms"] >= 100 and 1000.0 <= pk["sm_mhz"] <= 2200.0
+    ctx = ba.ba_create(16, 0.7)
+    try:
+        with pytest.raises(ba.BAError) as ei:
+            ba.ba_setup_ms(ctx)                              # the Hc pass has not run yet
+        assert ei.value.code == ba.BA_ESTATE
+        ba.ba_iterate(ctx, 1)
+        assert 0.0 < ba.ba_setup_ms(ctx) < 5000.0
+    finally:
+        ba.ba_destroy(ctx)
+
+
+def test_history_ring_wraps_in_two_pieces(ba):
+    # more iterations than the ring holds (65536): the last `count` entries come back oldest first across the wrap
+    n, d, K = 2, 0.5, 65536 + 300
+    ctx = ba.ba_create(n, d)
+    try:
+        ba.ba_iterate(ctx, K)
+        full = ba.ba_get_history(ctx, 65536)
+        tail = ba.ba_get_history(ctx, 500)
+        I, U = ba.ba_bounds(ctx)
+        with pytest.raises(ba.BAError):
+            ba.ba_get_history(ctx, 65537)
+    finally:
+        ba.ba_destroy(ctx)
+    assert np.array_equal(full[-500:], tail) and tail[-1, 0] == I and tail[-1, 1] == U
+    assert np.all(np.diff(full[:, 0]) >= -1e-15)              # I_t non-decreasing along the whole window (Theorem 1)
+    assert abs(I - 0.8304820237218407) <= 1e-12               # C_2(0.5), closed form
