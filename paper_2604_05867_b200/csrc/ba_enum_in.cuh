@@ -201,10 +201,26 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                         const uint32_t mm = (bb ? ur : ~ur) & ((h >= 32) ? 0xffffffffu : ((1u << h) - 1u));
                         uint32_t run = 0u;
 #pragma unroll
-                        for (int i = 0; i <= BA_HMAX; i++) {       // N[i] = sum_{j<i, u_j=b} E[j]
+                        for (int i = 0; i <= 8; i++) {             // N[i] = sum_{j<i, u_j=b} E[j]
                             const uint32_t old = E[i];
                             E[i] = run;
                             if ((mm >> i) & 1u) run += old;
+                        }
+                        if (h > 8) {                               // mm has no bit at or above h: entries beyond h are never read
+#pragma unroll
+                            for (int i = 9; i <= 16; i++) {
+                                const uint32_t old = E[i];
+                                E[i] = run;
+                                if ((mm >> i) & 1u) run += old;
+                            }
+                        }
+                        if (h > 16) {
+#pragma unroll
+                            for (int i = 17; i <= BA_HMAX; i++) {
+                                const uint32_t old = E[i];
+                                E[i] = run;
+                                if ((mm >> i) & 1u) run += old;
+                            }
                         }
 #pragma unroll
                         for (int s = 8; s >= 1; s--) al[s] = al[s - 1];
@@ -291,7 +307,11 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                     s_bal[buf * BA_RB_IN + lane] = ba_make_bal(rc, (uint32_t)node);
                     if (MODE == IN_SWEEP && b == 0)            // operand of the pair (v, empty): c(y'), lands before the CTA barrier
                         ba_cp_async8(ba_smem_addr(&s_bal[buf * BA_RB_IN + lane].x0), a.c + rc.id);
+#ifdef BA_X_NOSTAGE
+                    if (false) {
+#else
                     if (MODE == IN_SWEEP && (bi >> 24) < BA_NCLS) {
+#endif
                         // the half row c(y'.b.t), all t, is row (code(y'), b) of crow: one bulk copy
                         ba_mbar_arrive_expect_tx(sFull + 8u * buf, (uint32_t)nv * 8u);
                         ba_bulk_g2s(sRows + (uint32_t)(buf * BA_RB_IN + lane) * BA_ROWB, a.crow + (((((size_t)rc.id) << 1) | (size_t)b) << m),
@@ -333,7 +353,12 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 bool big = false;
                 if (may_big) big = __any_sync(0xffffffffu, lane < len && bal[lane].big != 0u);
                 // ---- the pair (v, empty) of every node of the batch: thread (v, node) -----------------------------
-                if (b == 0 && (kind == 1 || klen < 0)) {
+#ifdef BA_X_NOEPS
+                if (b == 7)
+#else
+                if (b == 0 && (kind == 1 || klen < 0))
+#endif
+                {
                     const uint32_t sv8 = (m == 8) ? (uint32_t)ev : 0xffffffffu;      // B_8 = [sigma_8 = v] (m = 8 only)
                     const uint32_t *sl = s_slice + (size_t)cp_sb * (8u << BA_MLOW) + ev;     // [sigma bits 4..6][v]
                     if (MODE == IN_SWEEP && !big) {

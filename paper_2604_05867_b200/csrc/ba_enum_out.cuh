@@ -213,8 +213,18 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                     const uint32_t ub = (u >> (h - 1 - pp)) & 1u;
                     const uint32_t mm = (ub ? yv : ~yv) & tmask;   // bit s: symbol t-s of y' equals u_pp
 #pragma unroll
-                    for (int s = 0; s <= BA_HMAX; s++)
+                    for (int s = 0; s < 8; s++)
                         if ((mm >> s) & 1u) f[s] += f[s + 1];
+                    if (t > 8) {                               // mm has no bit at or above t: the tail of f stays as it is
+#pragma unroll
+                        for (int s = 8; s < 16; s++)
+                            if ((mm >> s) & 1u) f[s] += f[s + 1];
+                    }
+                    if (t > 16) {
+#pragma unroll
+                        for (int s = 16; s <= BA_HMAX; s++)
+                            if ((mm >> s) & 1u) f[s] += f[s + 1];
+                    }
                 }
                 NodeRec rc;
 #pragma unroll
@@ -248,7 +258,11 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                     const int node = s_order[start + lane];
                     const NodeRec &rc = s_rec[node];
                     s_bal[buf * BA_RB_OUT + lane] = ba_make_bal(rc, (uint32_t)node);
+#ifdef BA_X_NOSTAGE
+                    if (false) {
+#else
                     if (MODE == OUT_SWEEP) {
+#endif
                         // the whole row p(u.*) in one bulk copy (x fits 32 bits, n <= 30); its bytes complete the FULL
                         // barrier of the stage, the arrive releases the BalRec stored above
                         ba_mbar_arrive_expect_tx(sFull + 8u * buf, (uint32_t)nv * 8u);

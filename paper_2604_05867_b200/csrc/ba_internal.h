@@ -179,8 +179,9 @@ __device__ __forceinline__ uint32_t ba_mbar_try(uint32_t addr, uint32_t parity) 
 __device__ __noinline__ void ba_mbar_wait_slow(uint32_t addr, uint32_t parity) {
     const long long t0 = clock64();
     for (;;) {
-        for (int i = 0; i < 1024; i++)
+        for (int i = 0; i < 256; i++) {
             if (ba_mbar_try(addr, parity)) return;
+        }
         if (clock64() - t0 > 40000000000ll) __trap();
     }
 }

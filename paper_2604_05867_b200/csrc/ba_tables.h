@@ -39,6 +39,9 @@ static inline uint32_t tt_prepend(uint32_t sig, int s, uint32_t cz) {
 }
 
 struct TTPair { int v; uint32_t cz; };
+#ifndef BA_STAGER_EXTRA
+#define BA_STAGER_EXTRA 12.0
+#endif
 
 // Deal the pairs of one list to (warp, level, lane, slot):
 //   * a GROUP is up to BA_GP pairs that share their gathered operand (`key` = its position in a staged row); the
@@ -233,6 +236,7 @@ static inline void build_tile_tables(int m, TileTables &T) {
             const int rw = (int)((ndeep + 31) / 32);
             for (int w = 0; w < NW; w++)
                 warp_extra[w] = side ? (w >= NW - rw ? 14.0 : 0.0) : ((w & (NW / 2 - 1)) >= NW / 2 - rw ? 8.0 : 0.0);
+            warp_extra[0] += BA_STAGER_EXTRA;                  // warp 0 also stages the batches: it must run ahead, not behind
             if (!tt_deal(m, b, pairs, key_of, owner_of, bpack, deep, warp_extra, S)) return;
             // ---- CSR of the epilogue: the slots of every owner, in slot order
             std::vector<std::vector<uint16_t>> slots(S.nown);
