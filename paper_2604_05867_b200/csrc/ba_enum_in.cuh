@@ -246,34 +246,42 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 ba_bucket_sort<BA_IN_NBKT>(key, s_ordr + (size_t)rd * BA_NT, s_wcnt, s_seg + rd * (BA_IN_NBKT + 1));
             }
             // ================= merge the rounds: bucket = its runs in round order =================
+            uint16_t *s_roff = s_wcnt;                         // [round][bucket]: where the round's run starts inside the bucket
             if (tid < 32) {
                 int cnt = 0;
                 for (int rd = 0; rd < nrounds; rd++) {
                     const uint16_t *sg = s_seg + rd * (BA_IN_NBKT + 1) + tid;
+                    s_roff[rd * BA_IN_NBKT + tid] = (uint16_t)cnt;
                     cnt += sg[1] - sg[0];
                 }
                 int incl = cnt;
                 for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, incl, o); if (lane >= o) incl += t; }
-                int pos = incl - cnt;
-                s_gstart[tid] = (uint16_t)pos;
+                s_gstart[tid] = (uint16_t)(incl - cnt);
                 if (tid == 31) s_gstart[32] = (uint16_t)incl;
-                for (int rd = 0; rd < nrounds; rd++) {
-                    const uint16_t *sg = s_seg + rd * (BA_IN_NBKT + 1) + tid;
-                    const uint16_t *od = s_ordr + (size_t)rd * BA_NT;
-                    for (int i = sg[0]; i < sg[1]; i++) s_order[pos++] = (uint16_t)(rd * BA_NT + od[i]);
+                // batches: <= BA_RB_IN consecutive nodes of one bucket, class-major (list-carrying bucket, then the other);
+                // lane l takes the l-th bucket of that order
+                const int kq = (lane & 1) * BA_NCLS + (lane >> 1);
+                const int ck = __shfl_sync(0xffffffffu, cnt, kq), gk = __shfl_sync(0xffffffffu, incl - cnt, kq);
+                const int nbk = (ck + BA_RB_IN - 1) / BA_RB_IN;
+                int bincl = nbk;
+                for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, bincl, o); if (lane >= o) bincl += t; }
+                int nb = bincl - nbk;
+                for (int off = 0; off < ck; off += BA_RB_IN) {
+                    const int len = (ck - off < BA_RB_IN) ? (ck - off) : BA_RB_IN;
+                    s_batch[nb++] = (uint32_t)(gk + off) | ((uint32_t)len << 16) | ((uint32_t)kq << 24);
                 }
-                __syncwarp();
-                if (tid == 0) {                                // batches: <= BA_RB_IN consecutive nodes of one bucket, class-major
-                    int nb = 0;
-                    for (int cq = 0; cq < BA_NCLS; cq++)
-                        for (int kind = 0; kind < 2; kind++) {
-                            const int kq = kind * BA_NCLS + cq;
-                            for (int off = s_gstart[kq]; off < s_gstart[kq + 1]; off += BA_RB_IN) {
-                                const int len = (s_gstart[kq + 1] - off < BA_RB_IN) ? (s_gstart[kq + 1] - off) : BA_RB_IN;
-                                s_batch[nb++] = (uint32_t)off | ((uint32_t)len << 16) | ((uint32_t)kq << 24);
-                            }
-                        }
-                    s_item[1] = (uint32_t)nb;
+                if (lane == 31) s_item[1] = (uint32_t)bincl;
+            }
+            __syncthreads();
+            for (int rd = 0; rd < nrounds; rd++) {             // every thread moves the entries of the rounds' orders
+                const uint16_t *sg = s_seg + rd * (BA_IN_NBKT + 1);
+                const uint16_t *od = s_ordr + (size_t)rd * BA_NT;
+                for (int idx = tid; idx < (int)sg[BA_IN_NBKT]; idx += BA_NT) {
+                    int kq = 0;                                // the bucket of position idx: largest kq with sg[kq] <= idx
+#pragma unroll
+                    for (int st = BA_IN_NBKT / 2; st > 0; st >>= 1)
+                        if ((int)sg[kq + st] <= idx) kq += st;
+                    s_order[s_gstart[kq] + s_roff[rd * BA_IN_NBKT + kq] + (idx - (int)sg[kq])] = (uint16_t)(rd * BA_NT + od[idx]);
                 }
             }
             __syncthreads();
