@@ -48,7 +48,7 @@ struct OutArgs {
     unsigned long long *cnt;   // OUT_COUNT
 };
 
-struct OutSmem { size_t rec, rows, bal, mbar, order, wcnt, bstart, batch, red, item, total; };
+struct OutSmem { size_t rec, rows, bal, mbar, order, wcnt, bstart, batch, red, binom, item, total; };
 
 __host__ __device__ static inline OutSmem enum_out_smem(int nr) {
     OutSmem s;
@@ -64,6 +64,7 @@ __host__ __device__ static inline OutSmem enum_out_smem(int nr) {
     s.bstart = take(3 * 2);
     s.batch = take((size_t)BA_OUT_MAXB * 4);
     s.red = take(32 * 8);
+    s.binom = take((size_t)(BA_HMAX + 1) * (BA_HMAX + 2) * 4);   // C(a, w), a <= h: per-lane indices (constant memory would serialise)
     s.item = take(16);
     s.total = o;
     return s;
@@ -87,6 +88,9 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
     uint32_t *s_batch = (uint32_t *)(smem + L.batch);
     double *s_red = (double *)(smem + L.red);
     uint32_t *s_item = (uint32_t *)(smem + L.item);        // [0] item, [1] number of batches
+    uint32_t (*s_binom)[BA_HMAX + 2] = (uint32_t (*)[BA_HMAX + 2])(smem + L.binom);
+    for (int i = tid; i < (BA_HMAX + 1) * (BA_HMAX + 2); i += BA_NT)
+        s_binom[i / (BA_HMAX + 2)][i % (BA_HMAX + 2)] = c_binom[i / (BA_HMAX + 2)][i % (BA_HMAX + 2)];
 
     const uint32_t sRows = ba_smem_addr(s_rows), sBal = ba_smem_addr(s_bal);
     const uint32_t sFull = ba_smem_addr(smem + L.mbar), sEmpty = sFull + BA_OUT_NSTG * 8u;
@@ -178,13 +182,13 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
             int key = -1;
             if (base + tid < R) {
                 uint32_t w = 0, rem = base + tid;
-                while (rem >= c_binom[h][w]) { rem -= c_binom[h][w]; w++; }
+                while (rem >= s_binom[h][w]) { rem -= s_binom[h][w]; w++; }
                 // subsetUnrank(h, w, rem): S = the w positions that the leftmost embedding skips (Alg. 5)
                 uint32_t S = 0;
                 {
                     uint32_t ww = w, jj = rem;
                     for (int pp = 0; pp < h && ww > 0; pp++) {
-                        const uint32_t cc = c_binom[h - pp - 1][ww - 1];
+                        const uint32_t cc = s_binom[h - pp - 1][ww - 1];
                         if (jj < cc) { S |= 1u << pp; ww--; } else { jj -= cc; }
                     }
                 }
