@@ -21,11 +21,24 @@ def needs_build():
 
 
 def build(force=False, verbose=False):
+    """Build (if stale) under an exclusive file lock, so that several ranks importing the binding at once (torchrun)
+    do not write libba.so concurrently; the ranks that waited find it fresh."""
+    import fcntl
     if not force and not needs_build():
         return LIB
+    with open(os.path.join(HERE, ".build.lock"), "w") as lk:
+        fcntl.flock(lk, fcntl.LOCK_EX)
+        try:
+            if not force and not needs_build():
+                return LIB
+            return _build(verbose)
+        finally:
+            fcntl.flock(lk, fcntl.LOCK_UN)
+
+
+def _build(verbose):
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    extra = os.environ.get("BA_NVCC_EXTRA", "").split()       # e.g. -DBA_CVT_XU_MASK=0x5 for tuning runs
-    cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + \
+    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + \
           [os.path.join(CSRC, s) for s in SOURCES]
     subprocess.check_call(cmd)
     return LIB

@@ -315,11 +315,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                     s_bal[buf * BA_RB_IN + lane] = ba_make_bal(rc, (uint32_t)node);
                     if (MODE == IN_SWEEP && b == 0)            // operand of the pair (v, empty): c(y'), lands before the CTA barrier
                         ba_cp_async8(ba_smem_addr(&s_bal[buf * BA_RB_IN + lane].x0), a.c + rc.id);
-#ifdef BA_X_NOSTAGE
-                    if (false) {
-#else
                     if (MODE == IN_SWEEP && (bi >> 24) < BA_NCLS) {
-#endif
                         // the half row c(y'.b.t), all t, is row (code(y'), b) of crow: one bulk copy
                         ba_mbar_arrive_expect_tx(sFull + 8u * buf, (uint32_t)nv * 8u);
                         ba_bulk_g2s(sRows + (uint32_t)(buf * BA_RB_IN + lane) * BA_ROWB, a.crow + (((((size_t)rc.id) << 1) | (size_t)b) << m),
@@ -361,12 +357,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 bool big = false;
                 if (may_big) big = __any_sync(0xffffffffu, lane < len && bal[lane].big != 0u);
                 // ---- the pair (v, empty) of every node of the batch: thread (v, node) -----------------------------
-#ifdef BA_X_NOEPS
-                if (b == 7)
-#else
-                if (b == 0 && (kind == 1 || klen < 0))
-#endif
-                {
+                if (b == 0 && (kind == 1 || klen < 0)) {
                     const uint32_t sv8 = (m == 8) ? (uint32_t)ev : 0xffffffffu;      // B_8 = [sigma_8 = v] (m = 8 only)
                     const uint32_t *sl = s_slice + (size_t)cp_sb * (8u << BA_MLOW) + ev;     // [sigma bits 4..6][v]
                     if (MODE == IN_SWEEP && !big) {
@@ -411,9 +402,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                     uint32_t rb[BA_KG];
 #pragma unroll
                     for (int k = 0; k < BA_KG; k++) rb[k] = rowbase + gaddr[k];
-#ifndef BA_X_NOLOOP
                     ba_group_batch(acc, Bp, rb, bal, s_rec, len, wmeta, big);
-#endif
                 } else {
                     for (int i = 0; i < len; i++) {
                         const NodeRec &rc = s_rec[bal[i].node];
@@ -438,11 +427,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                     }
                 }
                 // ---- riders: deep pairs of this class, one per thread ------------------------------------
-                #ifdef BA_X_NORIDERS
-        const int nr = 0;
-#else
-        const int nr = a.g.r_cnt[cls * 2 + b];
-#endif
+                const int nr = a.g.r_cnt[cls * 2 + b];
                 // two replicas of the rider set (threads 255 - e and 511 - e), each takes every other node
                 const int re = (BA_NT / 2 - 1) - (tid & (BA_NT / 2 - 1)), rh = tid / (BA_NT / 2);
                 if ((BA_NT / 2) - 32 * ((warp & (BA_NT / 64 - 1)) + 1) < nr) {

@@ -132,11 +132,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
         // (v, empty) alone, which item (y', 0) serves
         const int klen = (MODE == OUT_SWEEP) ? a.kc.klen : -1;
         if (klen >= 0 && (klen < t || klen > t + m || (klen == t && b == 1))) { __syncthreads(); continue; }
-#ifndef BA_X_NOEPS
         const bool do_eps = (b == 0) && (klen < 0 || klen == t);
-#else
-        const bool do_eps = false;
-#endif
         const bool do_grp = (klen != t);
         const int cls = (int)(cy & (BA_NCLS - 1));
         const int Lc = t < 8 ? t : 8;
@@ -157,11 +153,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
             const uint2 e8 = __ldg(a.EPS8 + (size_t)(cy & 255u) * nv + ev);
             eB0 = e8.x; eB1 = e8.y; eB2 = (m == 8 && (cy & 255u) == (uint32_t)ev) ? 1u : 0u;   // B_8 = [sigma_8 = v]
         }
-        #ifdef BA_X_NORIDERS
-        const int nr = 0;
-#else
         const int nr = a.g.r_cnt[cls * 2 + b];
-#endif
         const int re = BA_NT - 1 - tid;                        // riders sit on the last warps
         uint32_t rB0 = 0, rB1 = 0, rB2 = 0, roff = 0, rown = 0;
         if (re < nr) {
@@ -262,11 +254,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                     const int node = s_order[start + lane];
                     const NodeRec &rc = s_rec[node];
                     s_bal[buf * BA_RB_OUT + lane] = ba_make_bal(rc, (uint32_t)node);
-#ifdef BA_X_NOSTAGE
-                    if (false) {
-#else
                     if (MODE == OUT_SWEEP) {
-#endif
                         // the whole row p(u.*) in one bulk copy (x fits 32 bits, n <= 30); its bytes complete the FULL
                         // barrier of the stage, the arrive releases the BalRec stored above
                         ba_mbar_arrive_expect_tx(sFull + 8u * buf, (uint32_t)nv * 8u);
@@ -324,9 +312,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                         uint32_t rb[BA_KG];
 #pragma unroll
                         for (int k = 0; k < BA_KG; k++) rb[k] = rowbase + gaddr[k];
-    #ifndef BA_X_NOLOOP
-                    ba_group_batch(acc, Bp, rb, bal, s_rec, len, wmeta, big);
-#endif
+                        ba_group_batch(acc, Bp, rb, bal, s_rec, len, wmeta, big);
                     } else {
                         for (int i = 0; i < len; i++) {
                             const NodeRec &rc = s_rec[bal[i].node];

@@ -197,9 +197,7 @@ __device__ __forceinline__ double ba_u2d(uint32_t e) {
 }
 // Pair slots q of a group whose conversion goes to the conversion unit (I2F.F64.U32, 1 instruction on the otherwise
 // idle quarter-rate pipe) instead of the FP64 pipe (MOV + DADD): spreads the per-term conversion over two pipes.
-#ifndef BA_CVT_XU_MASK
 #define BA_CVT_XU_MASK 0x5
-#endif
 template <int Q>
 __device__ __forceinline__ double ba_cvt(uint32_t e) {
     if ((BA_CVT_XU_MASK >> Q) & 1) return __uint2double_rn(e);
@@ -216,12 +214,6 @@ __device__ __forceinline__ double ba_cvt(uint32_t e) {
 //   TYPE 1  no slot of the half ever has B_1 (under any class): emb = alpha_0 * B_0 is one product of two integer
 //           counts (P:181 with a single split point); the term emb * operand is formed as (alpha_0 * operand) * B_0 with
 //           alpha_0 and B_0 converted exactly: one DMUL per group and node, one DFMA per term, no integer work.
-#ifndef BA_UNR1
-#define BA_UNR1 4
-#endif
-#ifndef BA_UNR4
-#define BA_UNR4 4
-#endif
 template <int TYPE, int K0, int NL>
 __device__ __forceinline__ void ba_half_loop(double (&acc)[BA_NSLOT], const uint32_t (&Bp)[BA_NSLOT], const uint32_t (&rb)[BA_KG],
                                              uint32_t bal, int len) {
@@ -229,8 +221,7 @@ __device__ __forceinline__ void ba_half_loop(double (&acc)[BA_NSLOT], const uint
         double Bd[NL * BA_GP];
 #pragma unroll
         for (int s = 0; s < NL * BA_GP; s++) Bd[s] = (double)(Bp[K0 * BA_GP + s] & 0xffu);
-        constexpr int unr1 = BA_UNR1;
-#pragma unroll unr1
+#pragma unroll 4
         for (int i = 0; i < len; i++) {
             const double a0 = ba_lds_f64(bal + (uint32_t)i * BA_BALB + 32u);
 #pragma unroll
@@ -241,8 +232,7 @@ __device__ __forceinline__ void ba_half_loop(double (&acc)[BA_NSLOT], const uint
             }
         }
     } else {
-        constexpr int unr4 = BA_UNR4;
-#pragma unroll unr4
+#pragma unroll 4
         for (int i = 0; i < len; i++) {
             uint2 a;
             if (TYPE == 2) { asm volatile("ld.shared.u32 %0, [%1];" : "=r"(a.x) : "r"(bal + (uint32_t)i * BA_BALB)); a.y = 0u; }
