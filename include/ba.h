@@ -1,7 +1,7 @@
 /*
  * ba.h -- C ABI of libba: Blahut-Arimoto (BA) for the finite-length binary deletion channel
  * BDC_d^n on one NVIDIA B200 (sm_100a).  Hand-written CUDA kernels behind plain pointers;
- * no torch types, no exceptions, no global state, no CPU fallback.
+ * no torch types, no exceptions, no mutable global state (see "Device"), no CPU fallback.
  *
  * Citations: "P:line" = PAPER.md line (arxiv 2604.05867); "NS" = BASELINE.json:north_star;
  * "R#/G#" = readings listed in DESIGN.md.
@@ -22,6 +22,10 @@
  *
  * Which iterate (R6): after a total of K >= 1 iterations, ba_bounds/ba_stats return
  * (I_{K-1}, U_{K-1}, log2 Z_{K-1}), ba_get_q / ba_get_D return q_{K-1}, D_{K-1}, ba_get_p returns p_K.
+ *
+ * Device: a ctx lives on the CUDA device that was current when it was created; the caller keeps that device current
+ * (cudaSetDevice) for every call on the ctx.  The library keeps no global state besides an immutable, lazily built
+ * cache of the static pair tables and the per-kernel shared-memory limit, which is only ever raised.
  *
  * Errors: every function returns BA_OK (0) or a negative code; nothing is printed, thrown or aborted.
  * ba_last_error(ctx) gives a ctx-owned message for the last failure on that ctx (static string if ctx
