@@ -35,6 +35,7 @@
 
 enum { IN_SWEEP = 0, IN_HC = 1, IN_DEBUG = 2, IN_COUNT = 3 };
 
+#define BA_ELOG_S 1024                                     // head of the e log2(e) table kept in shared memory (IN_HC)
 #define BA_IN_SB (BA_SBR * BA_NT)                           // nodes per super-batch
 #define BA_IN_NBKT (2 * BA_NCLS)                            // buckets: class, with / without list b (the latter: b = 0 only)
 #define BA_IN_MAXB (BA_IN_NBKT + BA_IN_SB / BA_RB_IN)
@@ -55,7 +56,7 @@ struct InArgs {
     unsigned long long *cnt;  // IN_COUNT: [0] terms, [1] emb sum
 };
 
-struct InSmem { size_t rec, slice, rslice, rows, mbar, bal, ordr, seg, order, gstart, wcnt, batch, rsum, sub, kcw, item, total; };
+struct InSmem { size_t rec, slice, rslice, elog, rows, mbar, bal, ordr, seg, order, gstart, wcnt, batch, rsum, sub, kcw, item, total; };
 
 __host__ __device__ static inline InSmem enum_in_smem(int nr) {
     InSmem s;
@@ -77,6 +78,7 @@ __host__ __device__ static inline InSmem enum_in_smem(int nr) {
     s.batch = take((size_t)BA_IN_MAXB * 4);
     s.sub = take(32 * 4);
     s.kcw = take(2 * (BA_NMAX_I + 1) * 8);
+    s.elog = take((size_t)BA_ELOG_S * 8);
     s.item = take(16);
     s.total = o;
     return s;
@@ -84,7 +86,8 @@ __host__ __device__ static inline InSmem enum_in_smem(int nr) {
 
 #define BA_ELOG_N 65536
 // e log2(e) of an embedding count: a table for the (overwhelmingly many) small counts, the library log2 otherwise
-__device__ __forceinline__ double ba_elog2e(uint32_t e, const double *tab) {
+__device__ __forceinline__ double ba_elog2e(uint32_t e, const double *tab, const double *stab) {
+    if (e < BA_ELOG_S) return stab[e];
     if (e < BA_ELOG_N) return __ldg(tab + e);
     return (double)e * log2((double)e);
 }
@@ -107,6 +110,9 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
     NodeRec *s_rec = (NodeRec *)(smem + L.rec);
     uint32_t *s_slice = (uint32_t *)(smem + L.slice);
     uint32_t *s_rslice = (uint32_t *)(smem + L.rslice);
+    double *s_elog = (double *)(smem + L.elog);
+    if (MODE == IN_HC)
+        for (int i = tid; i < BA_ELOG_S; i += BA_NT) s_elog[i] = a.elog[i];
     double *s_rows = (double *)(smem + L.rows);
     double *s_acc = s_rows;                                 // epilogue only
     BalRec *s_bal = (BalRec *)(smem + L.bal);
@@ -382,12 +388,13 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                             const NodeRec &rc = s_rec[bal[i].node];
                             const uint32_t cy = rc.id;
                             const int k = (int)(rc.info >> 16);
-                            const uint32_t emb = ba_chain9_wide(rc.a, eB0, sl[((cy >> 4) & 7u) << BA_MLOW], (cy & 255u) == sv8);
+                            const uint32_t emb = big ? ba_chain9_wide(rc.a, eB0, sl[((cy >> 4) & 7u) << BA_MLOW], (cy & 255u) == sv8)
+                                                     : ba_chain9(bal[i].a01, bal[i].a23, bal[i].a45, bal[i].a67, bal[i].a8, eB0, sl[((cy >> 4) & 7u) << BA_MLOW], (cy & 255u) == sv8);
                             if (MODE == IN_SWEEP) {
                                 acc_eps = fma(ba_u2d(emb), bal[i].x0, acc_eps);
                             } else if (MODE == IN_HC) {
                                 const double wk = s_w[k];
-                                if (wk != 0.0) acc_eps = fma(wk, ba_elog2e(emb, a.elog) - (double)emb * s_lebar[k], acc_eps);
+                                if (wk != 0.0) acc_eps = fma(wk, ba_elog2e(emb, a.elog, s_elog) - (double)emb * s_lebar[k], acc_eps);
                             } else if (MODE == IN_DEBUG) {
                                 if (((u << m) | (uint32_t)ev) == a.dbg_x) a.dbg_out[cy - 1u] = emb;
                             } else {
@@ -398,7 +405,29 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 }
                 if (kind == 0) {
                 // ---- the thread's pair slots ---------------------------------------------------------------
-                if (MODE == IN_SWEEP) {
+                if (MODE == IN_HC && !big) {
+                    // the slots of the thread against the nodes of the batch, as in the sweep, with the term
+                    // w_k (emb log2 emb - emb log2 ebar_k) instead of emb * operand (|z| is a constant of the group)
+                    int jz[BA_KG];
+#pragma unroll
+                    for (int g = 0; g < BA_KG; g++) jz[g] = ba_len_of_code(ba_z_of_tail((uint32_t)b, gaddr[g] >> 3));
+#pragma unroll 2
+                    for (int i = 0; i < len; i++) {
+                        const uint2 al = *(const uint2 *)&bal[i];
+                        const int k = ba_len_of_code(bal[i].id);
+#pragma unroll
+                        for (int g = 0; g < BA_KG; g++) {
+                            const double wk = s_w[k + jz[g]], nlb = -s_lebar[k + jz[g]];
+#pragma unroll
+                            for (int q = 0; q < BA_GP; q++) {
+                                uint32_t e = __dp2a_lo(al.x, Bp[g * BA_GP + q], 0u);
+                                e = __dp2a_hi(al.y, Bp[g * BA_GP + q], e);
+                                const double gl = fma((double)e, nlb, ba_elog2e(e, a.elog, s_elog));     // elog(0) = elog(1) = 0
+                                acc[g * BA_GP + q] = fma(wk, gl, acc[g * BA_GP + q]);
+                            }
+                        }
+                    }
+                } else if (MODE == IN_SWEEP) {
                     uint32_t rb[BA_KG];
 #pragma unroll
                     for (int k = 0; k < BA_KG; k++) rb[k] = rowbase + gaddr[k];
@@ -416,7 +445,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                             const int jz = ba_len_of_code(cz);
                             if (MODE == IN_HC) {
                                 const double wk = s_w[k + jz];
-                                if (wk != 0.0) acc[s] = fma(wk, ba_elog2e(emb, a.elog) - (double)emb * s_lebar[k + jz], acc[s]);
+                                if (wk != 0.0) acc[s] = fma(wk, ba_elog2e(emb, a.elog, s_elog) - (double)emb * s_lebar[k + jz], acc[s]);
                             } else if (MODE == IN_DEBUG) {
                                 const uint32_t ov = a.g.GO[(((size_t)b * BA_KG + s / BA_GP) * BA_GP + s % BA_GP) * BA_NT + tid];
                                 if (((u << m) | ov) == a.dbg_x) a.dbg_out[((size_t)rc.id << jz) + (cz - (1u << jz)) - 1u] = emb;
@@ -460,13 +489,13 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                                 const BalRec bl = bal[i];
                                 const uint32_t cy = bl.id;
                                 const uint32_t x8 = r8[(size_t)((cy >> 4) & 7u) * a.g.nr];
-                                const uint32_t emb = ba_chain9_wide(s_rec[bl.node].a, rd.x, x8, 0u);
+                                const uint32_t emb = big ? ba_chain9_wide(s_rec[bl.node].a, rd.x, x8, 0u) : ba_chain9(bl.a01, bl.a23, bl.a45, bl.a67, 0u, rd.x, x8, 0u);
                                 if (MODE == IN_SWEEP) {
                                     s = fma(ba_u2d(emb), ba_lds_f64(rowbase + (uint32_t)i * BA_ROWB + rd.z), s);
                                 } else if (MODE == IN_HC) {
                                     const int k = (int)(s_rec[bl.node].info >> 16);
                                     const double wk = s_w[k + jz];
-                                    if (wk != 0.0) s = fma(wk, ba_elog2e(emb, a.elog) - (double)emb * s_lebar[k + jz], s);
+                                    if (wk != 0.0) s = fma(wk, ba_elog2e(emb, a.elog, s_elog) - (double)emb * s_lebar[k + jz], s);
                                 } else if (MODE == IN_DEBUG) {
                                     if (((u << m) | ov) == a.dbg_x) a.dbg_out[((size_t)cy << jz) + (cz - (1u << jz)) - 1u] = emb;
                                 } else {
