@@ -213,10 +213,11 @@ extern "C" int ba_debug_check_tables(int m, unsigned long long stats[4]) {
                     for (int tid = 0; tid < BA_NT; tid++) {
                         const uint4 e4 = G.GB[(((size_t)cls * 2 + b) * BA_KG + k) * BA_NT + tid];
                         const uint32_t e[4] = {e4.x, e4.y, e4.z, e4.w};
-                        const uint32_t pos = G.GA[((size_t)b * BA_KG + k) * BA_NT + tid] >> 3;
-                        const int hm = (G.GW[(size_t)b * (BA_NT / 32) + tid / 32] >> (8 * (k / 2))) & 0xff;    // the half of group k
+                        const size_t sb = (size_t)((G.nsc > 1) ? cls : 0) * 2 + b;
+                        const uint32_t pos = G.GA[(sb * BA_KG + k) * BA_NT + tid] >> 3;
+                        const int hm = (G.GW[sb * (BA_NT / 32) + tid / 32] >> (8 * (k / 2))) & 0xff;    // the half of group k
                         for (int q = 0; q < BA_GP; q++) {
-                            const uint32_t ow = G.GO[(((size_t)b * BA_KG + k) * BA_GP + q) * BA_NT + tid];
+                            const uint32_t ow = G.GO[((sb * BA_KG + k) * BA_GP + q) * BA_NT + tid];
                             if (!(e[q] & 0xffu)) { if (e[q]) return BA_EINVAL; continue; }      // unused, or deep under this class
                             if (ow == 0xffffu || (k & 1) >= (hm & 3)) return BA_EINVAL;         // the half's loop must reach the slot
                             if ((hm >> 2) == 2 && (e[q] >> 16)) return BA_EINVAL;               // a type-2 loop ignores B_2, B_3
@@ -243,19 +244,19 @@ extern "C" int ba_debug_check_tables(int m, unsigned long long stats[4]) {
                         if ((chk_emb(cz - (1u << lz), lz, (uint32_t)v, m) != 0) != (seen[(size_t)v * NZc + cz] != 0)) return BA_EINVAL;
                     }
             }
-        // the epilogue's CSR lists every used slot exactly once, under its owner
-        for (int b = 0; b < 2; b++) {
+        // the epilogue's CSR lists every used slot exactly once, under its owner (per schedule and list)
+        for (int sb = 0; sb < G.nsc * 2; sb++) {
             std::vector<uint8_t> hit((size_t)BA_NSLOT * BA_NT, 0);
             for (int o = 0; o < G.nown; o++)
-                for (int q = G.csr_off[(size_t)b * (G.nown + 1) + o]; q < G.csr_off[(size_t)b * (G.nown + 1) + o + 1]; q++) {
-                    const uint32_t sl = G.csr_idx[(size_t)b * BA_NSLOT * BA_NT + q];
+                for (int q = G.csr_off[(size_t)sb * (G.nown + 1) + o]; q < G.csr_off[(size_t)sb * (G.nown + 1) + o + 1]; q++) {
+                    const uint32_t sl = G.csr_idx[(size_t)sb * BA_NSLOT * BA_NT + q];
                     const int kq = (int)(sl / BA_NT), tid = (int)(sl % BA_NT);
-                    if (G.GO[(((size_t)b * BA_KG + kq / BA_GP) * BA_GP + kq % BA_GP) * BA_NT + tid] != o || hit[sl]++) return BA_EINVAL;
+                    if (G.GO[(((size_t)sb * BA_KG + kq / BA_GP) * BA_GP + kq % BA_GP) * BA_NT + tid] != o || hit[sl]++) return BA_EINVAL;
                 }
             for (int k = 0; k < BA_KG; k++)
                 for (int q = 0; q < BA_GP; q++)
                     for (int tid = 0; tid < BA_NT; tid++)
-                        if ((G.GO[(((size_t)b * BA_KG + k) * BA_GP + q) * BA_NT + tid] != 0xffffu) != (hit[(size_t)(k * BA_GP + q) * BA_NT + tid] != 0)) return BA_EINVAL;
+                        if ((G.GO[(((size_t)sb * BA_KG + k) * BA_GP + q) * BA_NT + tid] != 0xffffu) != (hit[(size_t)(k * BA_GP + q) * BA_NT + tid] != 0)) return BA_EINVAL;
         }
     }
     return BA_OK;
@@ -300,7 +301,7 @@ static cudaError_t upload_side(unsigned char *s, const GroupSide &G, const SideL
     D.GW = (const uint16_t *)(s + L.GW); D.csr_off = (const uint16_t *)(s + L.csr_off); D.csr_idx = (const uint16_t *)(s + L.csr_idx);
     D.R = (const uint4 *)(s + L.R); D.r_cnt = (const uint16_t *)(s + L.r_cnt); D.r_csr = (const uint16_t *)(s + L.r_csr);
     D.R8 = (const uint32_t *)(s + L.R8);
-    D.nr = G.nr; D.nown = G.nown;
+    D.nr = G.nr; D.nown = G.nown; D.nsc = G.nsc;
     return cudaSuccess;
 }
 

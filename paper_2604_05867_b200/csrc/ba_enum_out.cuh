@@ -140,13 +140,14 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
         for (int w = 0; w <= h - t; w++) R += c_binom[h][w];
 
         // ---- per item: the thread's pair slots, all nine B_s of the eps pair (v = ev) and of its rider ----------
-        const int wmeta = a.g.GW[b * (BA_NT / 32) + warp];
+        const size_t sb = (size_t)((a.g.nsc > 1) ? cls : 0) * 2 + b;      // the schedule of the item's class and list
+        const int wmeta = a.g.GW[sb * (BA_NT / 32) + warp];
         uint32_t Bp[BA_NSLOT], gaddr[BA_KG];
 #pragma unroll
         for (int k = 0; k < BA_KG; k++) {
             const uint4 bb = __ldg(a.g.GB + (((size_t)cls * 2 + b) * BA_KG + k) * BA_NT + tid);
             Bp[k * BA_GP] = bb.x; Bp[k * BA_GP + 1] = bb.y; Bp[k * BA_GP + 2] = bb.z; Bp[k * BA_GP + 3] = bb.w;
-            gaddr[k] = __ldg(a.g.GA + ((size_t)b * BA_KG + k) * BA_NT + tid);
+            gaddr[k] = __ldg(a.g.GA + (sb * BA_KG + k) * BA_NT + tid);
         }
         uint32_t eB0 = 0, eB1 = 0, eB2 = 0;                    // B(sigma_s, ev): B_0 = 1; alpha_s = 0 beyond t
         if (do_eps) {
@@ -322,7 +323,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                                 if (!(bp & 0xffu)) continue;
                                 const uint32_t emb = rc.a[0] * (bp & 0xffu) + rc.a[1] * ((bp >> 8) & 0xffu) + rc.a[2] * ((bp >> 16) & 0xffu) + rc.a[3] * (bp >> 24);
                                 if (MODE == OUT_DEBUG) {
-                                    const uint32_t oz = a.g.GO[(((size_t)b * BA_KG + s / BA_GP) * BA_GP + s % BA_GP) * BA_NT + tid];
+                                    const uint32_t oz = a.g.GO[((sb * BA_KG + s / BA_GP) * BA_GP + s % BA_GP) * BA_NT + tid];
                                     if (oz == a.dbg_cz) a.dbg_out[((size_t)rc.id << m) | (size_t)(gaddr[s / BA_GP] >> 3)] = emb;
                                 } else {
                                     cnt_terms += 1ull; cnt_emb += emb;
@@ -388,7 +389,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                 for (int w = 0; w < BA_NT / 32; w++) s += s_red[w];
                 dst[0] = s;
             }
-            const uint16_t *co = a.g.csr_off + (size_t)b * (a.g.nown + 1), *ci = a.g.csr_idx + (size_t)b * BA_NSLOT * BA_NT;
+            const uint16_t *co = a.g.csr_off + sb * (a.g.nown + 1), *ci = a.g.csr_idx + sb * BA_NSLOT * BA_NT;
             const uint16_t *cs = a.g.r_csr + ((size_t)cls * 2 + b) * (a.g.nown + 1);
             for (uint32_t cz = 2u + tid; cz <= NZ; cz += BA_NT) {      // cz = code(z), z not empty
                 if ((int)((cz >> (ba_len_of_code(cz) - 1)) & 1u) != b) continue;

@@ -16,6 +16,7 @@ struct GroupSide {
     std::vector<uint16_t> csr_off;  // [2][nown + 1]: slots of an owner, per list
     std::vector<uint16_t> csr_idx;  // [2][BA_KG*BA_GP*BA_NT]: slot index (k*BA_GP + q)*BA_NT + tid
     int nown = 0;                   // in: 2^m ; out: 2^{m+1} (by code(z))
+    int nsc = 1;                    // schedules: 1 (input sweep: slot ownership is the same for all classes) or BA_NCLS (output sweep)
     std::vector<uint4> R;           // riders [BA_NCLS][2][nr]: {B0..B3, B4 | owner << 16, row byte offset, 0}, sorted by owner
     std::vector<uint16_t> r_cnt;    // [BA_NCLS][2]
     std::vector<uint16_t> r_csr;    // [BA_NCLS][2][nown + 1] rider range of an owner
@@ -50,13 +51,15 @@ struct TTPair { int v; uint32_t cz; };
 //     node loop is straight-line code chosen per warp;
 //   * warps are filled so that the four schedulers of the SM carry about the same number of instructions.
 template <typename KeyOf, typename OwnerOf, typename BPack, typename DeepOf>
-static bool tt_deal(int m, int b, const std::vector<TTPair> &pairs, KeyOf key_of, OwnerOf owner_of, BPack bpack, DeepOf deep,
-                    const double *warp_extra, GroupSide &S) {
+static bool tt_deal(int m, int b, int sc, int cls_lo, int cls_hi, const std::vector<TTPair> &pairs, KeyOf key_of, OwnerOf owner_of,
+                    BPack bpack, DeepOf deep, const double *warp_extra, GroupSide &S) {
+    // sc = schedule index (input sweep: one schedule for all classes, 0; output sweep: one per class -- an item has
+    // one class, so its slots are typed and filled for that class alone); [cls_lo, cls_hi) = the classes it serves
     struct Grp { int type; uint32_t key; std::vector<int> items; };
     const int np = (int)pairs.size();
     std::vector<int> ptype(np, 1);
     for (int i = 0; i < np; i++)
-        for (int cls = 0; cls < BA_NCLS; cls++) {
+        for (int cls = cls_lo; cls < cls_hi; cls++) {
             if (deep(cls, pairs[i])) continue;
             const uint32_t bp = bpack(cls, pairs[i]);
             if ((bp >> 16) && ptype[i] < 4) ptype[i] = 4;
@@ -127,18 +130,18 @@ static bool tt_deal(int m, int b, const std::vector<TTPair> &pairs, KeyOf key_of
         if (warp < 0) return false;
         const int hslot = nh_of[warp]++;
         wload[warp] += hf.cost; sload[warp & 3] += hf.cost;
-        S.GW[(size_t)b * NW + warp] |= (uint16_t)(((int)hf.lv.size() | (hf.type << 2)) << (8 * hslot));
+        S.GW[((size_t)sc * 2 + b) * NW + warp] |= (uint16_t)(((int)hf.lv.size() | (hf.type << 2)) << (8 * hslot));
         for (size_t kk = 0; kk < hf.lv.size(); kk++) {
             const int k = 2 * hslot + (int)kk;
             const Lvl &lv = levels[hf.lv[kk]];
             for (size_t l = 0; l < lv.g.size(); l++) {
                 const Grp &g = groups[lv.g[l]];
                 const int tid = warp * 32 + (int)l;
-                S.GA[((size_t)b * BA_KG + k) * BA_NT + tid] = 8u * g.key;
+                S.GA[(((size_t)sc * 2 + b) * BA_KG + k) * BA_NT + tid] = 8u * g.key;
                 for (size_t q = 0; q < g.items.size(); q++) {
                     const TTPair &pr = pairs[g.items[q]];
-                    S.GO[(((size_t)b * BA_KG + k) * BA_GP + q) * BA_NT + tid] = (uint16_t)owner_of(pr);
-                    for (int cls = 0; cls < BA_NCLS; cls++) {
+                    S.GO[((((size_t)sc * 2 + b) * BA_KG + k) * BA_GP + q) * BA_NT + tid] = (uint16_t)owner_of(pr);
+                    for (int cls = cls_lo; cls < cls_hi; cls++) {
                         if (deep(cls, pr)) continue;                   // served by a rider under this class
                         uint4 &e = S.GB[(((size_t)cls * 2 + b) * BA_KG + k) * BA_NT + tid];
                         const uint32_t bp = bpack(cls, pr);
@@ -149,8 +152,8 @@ static bool tt_deal(int m, int b, const std::vector<TTPair> &pairs, KeyOf key_of
             }
         }
     }
-    S.npairs[b] = (unsigned long long)np;
-    S.ngroups[b] = groups.size();
+    S.npairs[b] += (unsigned long long)np;
+    S.ngroups[b] += groups.size();
     return true;
 }
 
@@ -190,17 +193,17 @@ static inline void build_tile_tables(int m, TileTables &T) {
     };
 
     const int NW = BA_NT / 32;
-    auto init_side = [&](GroupSide &S, int nown) {
-        S.nown = nown;
+    auto init_side = [&](GroupSide &S, int nown, int nsc) {
+        S.nown = nown; S.nsc = nsc;
         S.GB.assign((size_t)BA_NCLS * 2 * BA_KG * BA_NT, make_uint4(0u, 0u, 0u, 0u));
-        S.GA.assign((size_t)2 * BA_KG * BA_NT, 0u);
-        S.GO.assign((size_t)2 * BA_KG * BA_GP * BA_NT, 0xffffu);
-        S.GW.assign((size_t)2 * NW, 0);
-        S.csr_off.assign((size_t)2 * (nown + 1), 0);
-        S.csr_idx.assign((size_t)2 * BA_KG * BA_GP * BA_NT, 0);
+        S.GA.assign((size_t)nsc * 2 * BA_KG * BA_NT, 0u);
+        S.GO.assign((size_t)nsc * 2 * BA_KG * BA_GP * BA_NT, 0xffffu);
+        S.GW.assign((size_t)nsc * 2 * NW, 0);
+        S.csr_off.assign((size_t)nsc * 2 * (nown + 1), 0);
+        S.csr_idx.assign((size_t)nsc * 2 * BA_KG * BA_GP * BA_NT, 0);
     };
-    init_side(T.in, nv);
-    init_side(T.out, NZc);
+    init_side(T.in, nv, 1);
+    init_side(T.out, NZc, BA_NCLS);
 
     for (int side = 0; side < 2; side++) {
         GroupSide &S = side ? T.out : T.in;
@@ -235,21 +238,28 @@ static inline void build_tile_tables(int m, TileTables &T) {
             for (int w = 0; w < NW; w++)
                 warp_extra[w] = side ? (w >= NW - rw ? 14.0 : 0.0) : ((w & (NW / 2 - 1)) >= NW / 2 - rw ? 8.0 : 0.0);
             warp_extra[0] += BA_STAGER_EXTRA;                  // warp 0 also stages the batches: it must run ahead, not behind
-            if (!tt_deal(m, b, pairs, key_of, owner_of, bpack, deep, warp_extra, S)) return;
-            // ---- CSR of the epilogue: the slots of every owner, in slot order
-            std::vector<std::vector<uint16_t>> slots(S.nown);
-            for (int k = 0; k < BA_KG; k++)
-                for (int q = 0; q < BA_GP; q++)
-                    for (int tid = 0; tid < BA_NT; tid++) {
-                        const uint16_t ow = S.GO[(((size_t)b * BA_KG + k) * BA_GP + q) * BA_NT + tid];
-                        if (ow != 0xffffu) slots[ow].push_back((uint16_t)((k * BA_GP + q) * BA_NT + tid));
-                    }
-            size_t n = 0;
-            for (int o = 0; o < S.nown; o++) {
-                S.csr_off[(size_t)b * (S.nown + 1) + o] = (uint16_t)n;
-                for (uint16_t sl : slots[o]) S.csr_idx[(size_t)b * BA_KG * BA_GP * BA_NT + n++] = sl;
+            for (int sc = 0; sc < S.nsc; sc++) {
+                const int cls_lo = (S.nsc == 1) ? 0 : sc, cls_hi = (S.nsc == 1) ? BA_NCLS : sc + 1;
+                std::vector<TTPair> sp;                        // a per-class schedule leaves the class's deep pairs to the riders
+                for (const TTPair &p : pairs)
+                    if (S.nsc == 1 || !deep(sc, p)) sp.push_back(p);
+                if (!tt_deal(m, b, sc, cls_lo, cls_hi, sp, key_of, owner_of, bpack, deep, warp_extra, S)) return;
+                // ---- CSR of the epilogue: the slots of every owner, in slot order
+                const size_t sb = (size_t)sc * 2 + b;
+                std::vector<std::vector<uint16_t>> slots(S.nown);
+                for (int k = 0; k < BA_KG; k++)
+                    for (int q = 0; q < BA_GP; q++)
+                        for (int tid = 0; tid < BA_NT; tid++) {
+                            const uint16_t ow = S.GO[((sb * BA_KG + k) * BA_GP + q) * BA_NT + tid];
+                            if (ow != 0xffffu) slots[ow].push_back((uint16_t)((k * BA_GP + q) * BA_NT + tid));
+                        }
+                size_t n = 0;
+                for (int o = 0; o < S.nown; o++) {
+                    S.csr_off[sb * (S.nown + 1) + o] = (uint16_t)n;
+                    for (uint16_t sl : slots[o]) S.csr_idx[sb * BA_KG * BA_GP * BA_NT + n++] = sl;
+                }
+                S.csr_off[sb * (S.nown + 1) + S.nown] = (uint16_t)n;
             }
-            S.csr_off[(size_t)b * (S.nown + 1) + S.nown] = (uint16_t)n;
             // ---- riders: the pairs that are deep under a class, sorted by owner
             for (int cls = 0; cls < BA_NCLS; cls++) {
                 std::vector<TTPair> dp;
