@@ -28,7 +28,7 @@ struct ba_ctx {
     double *p = nullptr, *q = nullptr, *D = nullptr;
     unsigned char *scratch = nullptr;
     // carved from scratch
-    double *c = nullptr, *crow = nullptr, *Hc = nullptr, *Apart = nullptr, *S = nullptr, *part = nullptr, *scal = nullptr, *hist = nullptr;
+    double *c = nullptr, *crow = nullptr, *Hc = nullptr, *Apart = nullptr, *S = nullptr, *park = nullptr, *part = nullptr, *scal = nullptr, *hist = nullptr;
     GroupDev gin, gout;              // pair schedules of the two sweeps (device pointers into scratch)
     uint2 *EPS8 = nullptr;
     uint32_t *EPSH = nullptr;
@@ -72,7 +72,7 @@ static double host_binom(int n, int k) {
 // ------------------------------------------------------------------------------------------------ scratch layout
 struct SideLayout { size_t GB, GA, GO, GW, csr_off, csr_idx, R, r_cnt, r_csr, R8; };
 struct ScratchLayout {
-    size_t c, crow, Hc, Apart, S, part, scal, hist, EPS8, EPSH, elog, counters, cnt, total;
+    size_t c, crow, Hc, Apart, S, park, part, scal, hist, EPS8, EPSH, elog, counters, cnt, total;
     SideLayout in, out;
     size_t napart, npart_cap;
 };
@@ -92,6 +92,7 @@ static std::shared_ptr<const TileTables> tile_tables(int m) {
     return cache[m];
 }
 
+#define BA_MAX_GRID_IN 256             // CTAs of the input sweep that have a parking place for their accumulators
 #define BA_FINAL_BLOCKS_PER_SM 8      // grid of k_in_final = SMs x this; one reduction triple per block
 
 static void side_layout(const GroupSide &G, SideLayout &L, size_t &o) {
@@ -120,6 +121,7 @@ static void scratch_layout(int n, const TileTables &T, ScratchLayout &L) {
     L.Hc = o; o += align256(NX * 8);
     L.Apart = o; o += align256(L.napart * 8);
     L.S = o; o += align256(2 * NX * 8);                      // partial sums of the two lists (input sweep)
+    L.park = o; o += align256((size_t)BA_MAX_GRID_IN * 2 * BA_NSLOT * BA_NT * 8);   // parked accumulators, one set per CTA of the input sweep
     L.part = o; o += align256(L.npart_cap * 3 * 8);
     L.scal = o; o += align256(8 * 8);
     L.hist = o; o += align256((size_t)BA_HIST_CAP * 3 * 8);
@@ -213,7 +215,7 @@ extern "C" int ba_debug_check_tables(int m, unsigned long long stats[4]) {
                     for (int tid = 0; tid < BA_NT; tid++) {
                         const uint4 e4 = G.GB[(((size_t)cls * 2 + b) * BA_KG + k) * BA_NT + tid];
                         const uint32_t e[4] = {e4.x, e4.y, e4.z, e4.w};
-                        const size_t sb = (size_t)((G.nsc > 1) ? cls : 0) * 2 + b;
+                        const size_t sb = (size_t)((G.nsc == BA_NCLS) ? cls : (G.nsc == 2) ? (cls & 1) : 0) * 2 + b;
                         const uint32_t pos = G.GA[(sb * BA_KG + k) * BA_NT + tid] >> 3;
                         const int hm = (G.GW[sb * (BA_NT / 32) + tid / 32] >> (8 * (k / 2))) & 0xff;    // the half of group k
                         for (int q = 0; q < BA_GP; q++) {
@@ -328,7 +330,7 @@ static int finish_create(ba_ctx *c) {
     ScratchLayout L;
     scratch_layout(c->n, T, L);
     unsigned char *s = c->scratch;
-    c->c = (double *)(s + L.c); c->crow = (double *)(s + L.crow); c->Hc = (double *)(s + L.Hc); c->Apart = (double *)(s + L.Apart); c->S = (double *)(s + L.S);
+    c->c = (double *)(s + L.c); c->crow = (double *)(s + L.crow); c->Hc = (double *)(s + L.Hc); c->Apart = (double *)(s + L.Apart); c->S = (double *)(s + L.S); c->park = (double *)(s + L.park);
     c->part = (double *)(s + L.part); c->scal = (double *)(s + L.scal); c->hist = (double *)(s + L.hist);
     c->EPS8 = (uint2 *)(s + L.EPS8); c->EPSH = (uint32_t *)(s + L.EPSH); c->elog = (double *)(s + L.elog);
     c->counters = (unsigned int *)(s + L.counters); c->cnt = (unsigned long long *)(s + L.cnt);
@@ -362,6 +364,7 @@ static int finish_create(ba_ctx *c) {
     size_t items_in = (size_t)2 << c->h, items_out = 2 * (((size_t)2 << c->h) - 1);      // (high part, list) pairs
     size_t gi = (size_t)c->num_sms * occ_in, go = (size_t)c->num_sms * occ_out;
     c->grid_in = (int)(items_in < gi ? items_in : gi);
+    if (c->grid_in > BA_MAX_GRID_IN) c->grid_in = BA_MAX_GRID_IN;
     c->grid_out = (int)(items_out < go ? items_out : go);
 
     // p0 uniform
@@ -465,7 +468,7 @@ extern "C" int ba_set_mode(ba_ctx *c, int mode) {
 static InArgs make_in_args(ba_ctx *c) {
     InArgs a;
     a.kc = c->kc; a.g = c->gin; a.EPS8 = c->EPS8; a.EPSH = c->EPSH;
-    a.c = c->c; a.crow = c->crow; a.elog = c->elog; a.S = c->S;
+    a.c = c->c; a.crow = c->crow; a.elog = c->elog; a.S = c->S; a.park = c->park;
     a.counter = c->counters; a.sym = 0; a.dbg_x = 0; a.dbg_out = nullptr; a.cnt = c->cnt;
     return a;
 }

@@ -49,6 +49,7 @@ struct InArgs {
     const double *crow;       // IN_SWEEP: the same by rows (code(y'), b) of 2^m operands (k_out_final)
     const double *elog;       // IN_HC: elog[e] = e log2(e), e < BA_ELOG_N
     double *S;                // out: [2][2^n] partial sums of the two lists (IN_SWEEP: S_b, IN_HC: H_b)
+    double *park;             // [grid][2][BA_NSLOT][BA_NT]: the accumulators of the schedule that is not running
     unsigned int *counter;    // work counter (zeroed before launch)
     int sym;                  // 1: p(x) = p(~x) (Theorem 4): only the u with leading bit 0 are enumerated
     uint32_t dbg_x;           // IN_DEBUG
@@ -63,10 +64,11 @@ __host__ __device__ static inline InSmem enum_in_smem(int nr) {
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o += (bytes + 15) & ~(size_t)15; return at; };
     s.rec = take((size_t)BA_IN_SB * sizeof(NodeRec));
-    s.rsum = take((size_t)2 * 2 * nr * 8);                 // rider sums of a batch, two replicas, double buffered
+    s.rsum = take((size_t)2 * 2 * nr * 8 > (size_t)BA_NT * 8 ? (size_t)2 * 2 * nr * 8 : (size_t)BA_NT * 8);   // rider sums of a batch, two replicas,
+                                                           // double buffered; the epilogue parks acc_eps there
     s.slice = take((size_t)2 * 8 * ((size_t)1 << BA_MLOW) * 4);    // B_4..B_7 of the pairs (v, empty) of a class, double buffered
     s.rslice = take((size_t)2 * 8 * nr * 4);               // B_4..B_7 of the riders of a class, double buffered
-    size_t rows = (size_t)2 * BA_RB_IN * BA_ROWB, ac = ((size_t)BA_NSLOT + 1) * BA_NT * 8;
+    size_t rows = (size_t)2 * BA_RB_IN * BA_ROWB, ac = (size_t)2 * BA_NSLOT * BA_NT * 8;   // both schedules' accumulators
     s.rows = take(rows > ac ? rows : ac);                  // the epilogue's accumulator staging aliases the rows
     s.mbar = take(2 * 8);                                  // FULL barrier of the two row buffers
     s.bal = take((size_t)2 * BA_RB_IN * sizeof(BalRec));
@@ -168,11 +170,13 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
         const uint32_t ur = (h > 0) ? (__brev(u) >> (32 - h)) : 0u;      // bit i = symbol at position i
 
         // ---- per item: the thread's groups (static per list) -----------------------------------------
-        const int wmeta = a.g.GW[b * (BA_NT / 32) + warp];
-        uint32_t gaddr[BA_KG];
-#pragma unroll
-        for (int k = 0; k < BA_KG; k++) gaddr[k] = __ldg(a.g.GA + ((size_t)b * BA_KG + k) * BA_NT + tid);
-
+        // the slots of a thread belong to one of two schedules: sc = last symbol of y' (class bit 0).  The batches
+        // of a super-batch run schedule 0 first, then schedule 1; at the switch the accumulators are parked in global
+        // memory (L2) and the other schedule's are fetched: twice per super-batch.
+        int cur_sc = -1, wmeta = 0;
+        uint32_t parked = 0u;                                  // bit sc: schedule sc has accumulators in its parking place
+        uint32_t gaddr[BA_KG] = {0u, 0u, 0u, 0u};
+        double *park = a.park + (size_t)blockIdx.x * 2 * BA_NSLOT * BA_NT + tid;
         double acc[BA_NSLOT];
 #pragma unroll
         for (int s = 0; s < BA_NSLOT; s++) acc[s] = 0.0;
@@ -266,7 +270,8 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 if (tid == 31) s_gstart[32] = (uint16_t)incl;
                 // batches: <= BA_RB_IN consecutive nodes of one bucket, class-major (list-carrying bucket, then the other);
                 // lane l takes the l-th bucket of that order
-                const int kq = (lane & 1) * BA_NCLS + (lane >> 1);
+                const int cq_l = ((lane >> 1) & 7) * 2 + (lane >> 4);          // class order: bit 0 = 0 first (one schedule switch)
+                const int kq = (lane & 1) * BA_NCLS + cq_l;
                 const int ck = __shfl_sync(0xffffffffu, cnt, kq), gk = __shfl_sync(0xffffffffu, incl - cnt, kq);
                 const int nbk = (ck + BA_RB_IN - 1) / BA_RB_IN;
                 int bincl = nbk;
@@ -404,6 +409,21 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                     }
                 }
                 if (kind == 0) {
+                if ((cls & 1) != cur_sc) {                     // the other schedule: swap the accumulators, reload the slot map
+                    if (MODE == IN_SWEEP || MODE == IN_HC) {
+                        if (cur_sc >= 0) {
+#pragma unroll
+                            for (int s = 0; s < BA_NSLOT; s++) park[((size_t)cur_sc * BA_NSLOT + s) * BA_NT] = acc[s];
+                            parked |= 1u << cur_sc;
+                        }
+#pragma unroll
+                        for (int s = 0; s < BA_NSLOT; s++) acc[s] = ((parked >> (cls & 1)) & 1u) ? park[((size_t)(cls & 1) * BA_NSLOT + s) * BA_NT] : 0.0;
+                    }
+                    cur_sc = cls & 1;
+                    wmeta = a.g.GW[((size_t)cur_sc * 2 + b) * (BA_NT / 32) + warp];
+#pragma unroll
+                    for (int k = 0; k < BA_KG; k++) gaddr[k] = __ldg(a.g.GA + (((size_t)cur_sc * 2 + b) * BA_KG + k) * BA_NT + tid);
+                }
                 // ---- the thread's pair slots ---------------------------------------------------------------
                 if (MODE == IN_HC && !big) {
                     // the slots of the thread against the nodes of the batch, as in the sweep, with the term
@@ -447,7 +467,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                                 const double wk = s_w[k + jz];
                                 if (wk != 0.0) acc[s] = fma(wk, ba_elog2e(emb, a.elog, s_elog) - (double)emb * s_lebar[k + jz], acc[s]);
                             } else if (MODE == IN_DEBUG) {
-                                const uint32_t ov = a.g.GO[(((size_t)b * BA_KG + s / BA_GP) * BA_GP + s % BA_GP) * BA_NT + tid];
+                                const uint32_t ov = a.g.GO[((((size_t)cur_sc * 2 + b) * BA_KG + s / BA_GP) * BA_GP + s % BA_GP) * BA_NT + tid];
                                 if (((u << m) | ov) == a.dbg_x) a.dbg_out[((size_t)rc.id << jz) + (cz - (1u << jz)) - 1u] = emb;
                             } else {
                                 cnt_terms += 1ull; cnt_emb += emb;
@@ -518,16 +538,24 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
         // ---- epilogue: thread v owns x = u.v ------------------------------------------------------------
         __syncthreads();                                       // all rows consumed: the staging area becomes s_acc
         if (MODE == IN_SWEEP || MODE == IN_HC) {
+            // the accumulators of both schedules to shared memory: the running one from registers, the other from its
+            // parking place (zeros if it never ran)
 #pragma unroll
-            for (int s = 0; s < BA_NSLOT; s++) s_acc[(size_t)s * BA_NT + tid] = acc[s];
-            s_acc[(size_t)BA_NSLOT * BA_NT + tid] = acc_eps;
+            for (int sc = 0; sc < 2; sc++)
+#pragma unroll
+                for (int s = 0; s < BA_NSLOT; s++)
+                    s_acc[((size_t)sc * BA_NSLOT + s) * BA_NT + tid] = (sc == cur_sc) ? acc[s] : ((parked >> sc) & 1u) ? park[((size_t)sc * BA_NSLOT + s) * BA_NT] : 0.0;
+            double *s_aeps = s_rsum;                           // the rider sums are all flushed: their area takes acc_eps
+            s_aeps[tid] = acc_eps;
             __syncthreads();
             if (tid < nv) {
                 double S = acc_rid;
                 if (b == 0)
-                    for (int t = ev; t < BA_NT; t += nv) S += s_acc[(size_t)BA_NSLOT * BA_NT + t];
-                const uint16_t *co = a.g.csr_off + (size_t)b * (a.g.nown + 1) + tid, *ci = a.g.csr_idx + (size_t)b * BA_NSLOT * BA_NT;
-                for (int q = co[0]; q < co[1]; q++) S += s_acc[ci[q]];
+                    for (int t = ev; t < BA_NT; t += nv) S += s_aeps[t];
+                for (int sc = 0; sc < 2; sc++) {
+                    const uint16_t *co = a.g.csr_off + ((size_t)sc * 2 + b) * (a.g.nown + 1) + tid, *ci = a.g.csr_idx + ((size_t)sc * 2 + b) * BA_NSLOT * BA_NT;
+                    for (int q = co[0]; q < co[1]; q++) S += s_acc[(size_t)sc * BA_NSLOT * BA_NT + ci[q]];
+                }
                 a.S[(size_t)b * NX + (((size_t)u << m) | (size_t)tid)] = S;
             }
         }

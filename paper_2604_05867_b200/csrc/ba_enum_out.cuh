@@ -140,7 +140,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
         for (int w = 0; w <= h - t; w++) R += c_binom[h][w];
 
         // ---- per item: the thread's pair slots, all nine B_s of the eps pair (v = ev) and of its rider ----------
-        const size_t sb = (size_t)((a.g.nsc > 1) ? cls : 0) * 2 + b;      // the schedule of the item's class and list
+        const size_t sb = (size_t)cls * 2 + b;      // the schedule of the item's class and list
         const int wmeta = a.g.GW[sb * (BA_NT / 32) + warp];
         uint32_t Bp[BA_NSLOT], gaddr[BA_KG];
 #pragma unroll

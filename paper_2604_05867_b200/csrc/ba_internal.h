@@ -103,7 +103,7 @@ struct GroupDev {
     const uint16_t *r_csr;            // [cls][b][nown + 1]
     const uint32_t *R8;               // [cls][b][8][nr]: B_4..B_7 by the sigma bits 4..6
     int nr, nown;
-    int nsc;                          // schedules: 1 (GA, GO, GW, CSR indexed [b]) or BA_NCLS (indexed [cls][b])
+    int nsc;                          // schedules (GA, GO, GW, CSR indexed [sc][b]): 2 (sc = class bit 0) or BA_NCLS (sc = class)
 };
 
 __device__ __forceinline__ int ba_len_of_code(uint32_t code) { return 31 - __clz(code); }

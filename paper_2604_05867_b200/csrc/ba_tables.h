@@ -16,7 +16,7 @@ struct GroupSide {
     std::vector<uint16_t> csr_off;  // [2][nown + 1]: slots of an owner, per list
     std::vector<uint16_t> csr_idx;  // [2][BA_KG*BA_GP*BA_NT]: slot index (k*BA_GP + q)*BA_NT + tid
     int nown = 0;                   // in: 2^m ; out: 2^{m+1} (by code(z))
-    int nsc = 1;                    // schedules: 1 (input sweep: slot ownership is the same for all classes) or BA_NCLS (output sweep)
+    int nsc = 1;                    // schedules: 2 (input sweep: by the last symbol of y') or BA_NCLS (output sweep: by class)
     std::vector<uint4> R;           // riders [BA_NCLS][2][nr]: {B0..B3, B4 | owner << 16, row byte offset, 0}, sorted by owner
     std::vector<uint16_t> r_cnt;    // [BA_NCLS][2]
     std::vector<uint16_t> r_csr;    // [BA_NCLS][2][nown + 1] rider range of an owner
@@ -51,16 +51,18 @@ struct TTPair { int v; uint32_t cz; };
 //     node loop is straight-line code chosen per warp;
 //   * warps are filled so that the four schedulers of the SM carry about the same number of instructions.
 template <typename KeyOf, typename OwnerOf, typename BPack, typename DeepOf>
-static bool tt_deal(int m, int b, int sc, int cls_lo, int cls_hi, const std::vector<TTPair> &pairs, KeyOf key_of, OwnerOf owner_of,
+static bool tt_deal(int m, int b, int sc, uint32_t clsmask, const std::vector<TTPair> &pairs, KeyOf key_of, OwnerOf owner_of,
                     BPack bpack, DeepOf deep, const double *warp_extra, GroupSide &S) {
-    // sc = schedule index (input sweep: one schedule for all classes, 0; output sweep: one per class -- an item has
-    // one class, so its slots are typed and filled for that class alone); [cls_lo, cls_hi) = the classes it serves
+    // sc = schedule index; clsmask = the classes it serves.  Output sweep: one schedule per class (an item has one
+    // class, so its slots are typed and filled for that class alone).  Input sweep: one schedule per LAST SYMBOL of y'
+    // (class bit 0): whether a pair can have B_1 at all depends on that symbol only, and the kernel switches its
+    // accumulators between the two schedules once per super-batch.
     struct Grp { int type; uint32_t key; std::vector<int> items; };
     const int np = (int)pairs.size();
     std::vector<int> ptype(np, 1);
     for (int i = 0; i < np; i++)
-        for (int cls = cls_lo; cls < cls_hi; cls++) {
-            if (deep(cls, pairs[i])) continue;
+        for (int cls = 0; cls < BA_NCLS; cls++) {
+            if (!((clsmask >> cls) & 1u) || deep(cls, pairs[i])) continue;
             const uint32_t bp = bpack(cls, pairs[i]);
             if ((bp >> 16) && ptype[i] < 4) ptype[i] = 4;
             else if ((bp >> 8) && ptype[i] < 2) ptype[i] = 2;
@@ -141,8 +143,8 @@ static bool tt_deal(int m, int b, int sc, int cls_lo, int cls_hi, const std::vec
                 for (size_t q = 0; q < g.items.size(); q++) {
                     const TTPair &pr = pairs[g.items[q]];
                     S.GO[((((size_t)sc * 2 + b) * BA_KG + k) * BA_GP + q) * BA_NT + tid] = (uint16_t)owner_of(pr);
-                    for (int cls = cls_lo; cls < cls_hi; cls++) {
-                        if (deep(cls, pr)) continue;                   // served by a rider under this class
+                    for (int cls = 0; cls < BA_NCLS; cls++) {
+                        if (!((clsmask >> cls) & 1u) || deep(cls, pr)) continue;                   // served by a rider under this class
                         uint4 &e = S.GB[(((size_t)cls * 2 + b) * BA_KG + k) * BA_NT + tid];
                         const uint32_t bp = bpack(cls, pr);
                         (q == 0 ? e.x : q == 1 ? e.y : q == 2 ? e.z : e.w) = bp;
@@ -202,7 +204,7 @@ static inline void build_tile_tables(int m, TileTables &T) {
         S.csr_off.assign((size_t)nsc * 2 * (nown + 1), 0);
         S.csr_idx.assign((size_t)nsc * 2 * BA_KG * BA_GP * BA_NT, 0);
     };
-    init_side(T.in, nv, 1);
+    init_side(T.in, nv, 2);
     init_side(T.out, NZc, BA_NCLS);
 
     for (int side = 0; side < 2; side++) {
@@ -239,11 +241,12 @@ static inline void build_tile_tables(int m, TileTables &T) {
                 warp_extra[w] = side ? (w >= NW - rw ? 14.0 : 0.0) : ((w & (NW / 2 - 1)) >= NW / 2 - rw ? 8.0 : 0.0);
             warp_extra[0] += BA_STAGER_EXTRA;                  // warp 0 also stages the batches: it must run ahead, not behind
             for (int sc = 0; sc < S.nsc; sc++) {
-                const int cls_lo = (S.nsc == 1) ? 0 : sc, cls_hi = (S.nsc == 1) ? BA_NCLS : sc + 1;
+                // input sweep: schedule sc serves the classes with bit 0 = sc; output sweep: class sc
+                const uint32_t clsmask = (S.nsc == BA_NCLS) ? (1u << sc) : (S.nsc == 2) ? (0x5555u << sc) : 0xffffu;
                 std::vector<TTPair> sp;                        // a per-class schedule leaves the class's deep pairs to the riders
                 for (const TTPair &p : pairs)
-                    if (S.nsc == 1 || !deep(sc, p)) sp.push_back(p);
-                if (!tt_deal(m, b, sc, cls_lo, cls_hi, sp, key_of, owner_of, bpack, deep, warp_extra, S)) return;
+                    if (S.nsc != BA_NCLS || !deep(sc, p)) sp.push_back(p);
+                if (!tt_deal(m, b, sc, clsmask, sp, key_of, owner_of, bpack, deep, warp_extra, S)) return;
                 // ---- CSR of the epilogue: the slots of every owner, in slot order
                 const size_t sb = (size_t)sc * 2 + b;
                 std::vector<std::vector<uint16_t>> slots(S.nown);
