@@ -35,7 +35,8 @@
 
 enum { IN_SWEEP = 0, IN_HC = 1, IN_DEBUG = 2, IN_COUNT = 3 };
 
-#define BA_ELOG_S 1024                                     // head of the e log2(e) table kept in shared memory (IN_HC)
+#define BA_ELOG_S 16384                                    // head of the e log2(e) table kept in shared memory (IN_HC): it takes the
+                                                           // place of the operand rows, which that pass does not stage
 #define BA_IN_SB (BA_SBR * BA_NT)                           // nodes per super-batch
 #define BA_IN_NBKT (2 * BA_NCLS)                            // buckets: class, with / without list b (the latter: b = 0 only)
 #define BA_IN_MAXB (BA_IN_NBKT + BA_IN_SB / BA_RB_IN)
@@ -57,7 +58,7 @@ struct InArgs {
     unsigned long long *cnt;  // IN_COUNT: [0] terms, [1] emb sum
 };
 
-struct InSmem { size_t rec, slice, rslice, elog, rows, mbar, bal, ordr, seg, order, gstart, wcnt, batch, rsum, sub, kcw, item, total; };
+struct InSmem { size_t rec, slice, rslice, rows, mbar, bal, ordr, seg, order, gstart, wcnt, batch, rsum, sub, kcw, item, total; };
 
 __host__ __device__ static inline InSmem enum_in_smem(int nr) {
     InSmem s;
@@ -80,7 +81,6 @@ __host__ __device__ static inline InSmem enum_in_smem(int nr) {
     s.batch = take((size_t)BA_IN_MAXB * 4);
     s.sub = take(32 * 4);
     s.kcw = take(2 * (BA_NMAX_I + 1) * 8);
-    s.elog = take((size_t)BA_ELOG_S * 8);
     s.item = take(16);
     s.total = o;
     return s;
@@ -112,11 +112,13 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
     NodeRec *s_rec = (NodeRec *)(smem + L.rec);
     uint32_t *s_slice = (uint32_t *)(smem + L.slice);
     uint32_t *s_rslice = (uint32_t *)(smem + L.rslice);
-    double *s_elog = (double *)(smem + L.elog);
-    if (MODE == IN_HC)
-        for (int i = tid; i < BA_ELOG_S; i += BA_NT) s_elog[i] = a.elog[i];
     double *s_rows = (double *)(smem + L.rows);
     double *s_acc = s_rows;                                 // epilogue only
+    double *s_elog = s_rows;                                // IN_HC: the table's head; the epilogue overwrites it, so it is
+    auto load_elog = [&]() {                                // fetched again (128 KB from L2) after every item
+        static_assert((size_t)BA_ELOG_S * 8 <= (size_t)2 * BA_RB_IN * BA_ROWB, "the table head lives in the row buffers");
+        for (int i = tid; i < BA_ELOG_S / 2; i += BA_NT) ((double2 *)s_elog)[i] = __ldg((const double2 *)a.elog + i);
+    };
     BalRec *s_bal = (BalRec *)(smem + L.bal);
     uint16_t *s_ordr = (uint16_t *)(smem + L.ordr);
     uint16_t *s_seg = (uint16_t *)(smem + L.seg);
@@ -136,7 +138,9 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
         ba_mbar_init(sFull, 32u); ba_mbar_init(sFull + 8u, 32u);        // the 32 lanes of the staging warp; rows count in bytes
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
-    for (int i = tid; i < 2 * BA_RB_IN * (int)(BA_ROWB / 8); i += BA_NT) s_rows[i] = 0.0;      // unused slots read finite operands
+    if (MODE == IN_HC) load_elog();
+    else
+        for (int i = tid; i < 2 * BA_RB_IN * (int)(BA_ROWB / 8); i += BA_NT) s_rows[i] = 0.0;   // unused slots read finite operands
     uint32_t gb = 0;                                        // batches staged so far by this CTA (uniform): buffer and phase
 
     const uint32_t sRows = ba_smem_addr(s_rows);
@@ -561,6 +565,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
         }
         if (MODE == IN_DEBUG) break;
         __syncthreads();
+        if (MODE == IN_HC) load_elog();                        // visible to all after the barriers of the next item's phase A
     }
     if (MODE == IN_COUNT) {
         atomicAdd(&a.cnt[0], cnt_terms);
