@@ -174,6 +174,31 @@ int ba_debug_check_tables(int m, unsigned long long stats[4]);
 void ba_destroy(ba_ctx *c);
 const char *ba_last_error(const ba_ctx *c);
 
+/* ---- no-allocation entry point ------------------------------------------------------------------ */
+
+/* For callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid it): the epilogue of the input sweep without a ctx.  D(x) = Hc(x) - (S0(x) + S1(x)) for the 2^n inputs
+ * (S1_dev may be NULL: D = Hc - S0), and the reductions of the bounds and of the update:
+ *     out3 = { sum_x p(x) D(x),  max_x D(x),  sum_x p(x) 2^D(x) }   (= I_t, U_t, Z_t of ba_bounds / ba_stats).
+ * All pointers are DEVICE pointers to float64, caller-owned: Hc, S0, S1, p of 2^n entries (read), D of 2^n entries
+ * and out3 of 3 entries (written).  The two kernels are queued on `stream` (a cudaStream_t, NULL = the default
+ * stream) of the CURRENT device; the call does not synchronise and copies nothing to the host.
+ *
+ * The first-stage partial sums live in a file-scope device array of the library (BA_NOALLOC_MAXBLK triples = 48 KB,
+ * held by every GPU that loads libba until the process exits) instead of ctx scratch, so the call performs no
+ * cudaMalloc / cudaFree and calls no allocating routine; the first call on a device only looks up the array's device
+ * address.  Limit: n <= BA_NOALLOC_NMAX (one block partial per 2^15 inputs); beyond it BA_EINVAL, nothing is launched,
+ * and ba_noalloc_last_error() says why.  Every call on a device shares the array, which keeps the last call's
+ * contents: a call overwrites every entry it later reads (nothing has to be cleared), and two calls that overlap on
+ * the GPU (different streams, or concurrent graph branches) race on it -- serialise them.  Sums are formed in a
+ * fixed order: results are bit-reproducible for a given n. */
+#define BA_NOALLOC_MAXBLK 2048
+#define BA_NOALLOC_NMAX 26
+int ba_in_final_noalloc(int n, const void *Hc_dev, const void *S0_dev, const void *S1_dev, const void *p_dev,
+                        void *D_dev, void *out3_dev, void *stream);
+/* Message of the calling thread's last failed ba_in_final_noalloc ("" after a success).  Static storage. */
+const char *ba_noalloc_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

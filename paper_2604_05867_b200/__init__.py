@@ -18,12 +18,14 @@ from . import build as _build
 BA_OK, BA_EINVAL, BA_ENOMEM, BA_ECUDA, BA_ESTATE, BA_ENUMERIC = 0, -1, -2, -3, -4, -5
 BA_MODE_ENUM, BA_MODE_FAST = 0, 1
 BA_NMAX = 30
+BA_NOALLOC_NMAX, BA_NOALLOC_MAXBLK = 26, 2048
 _CODE_NAMES = {0: "BA_OK", -1: "BA_EINVAL", -2: "BA_ENOMEM", -3: "BA_ECUDA", -4: "BA_ESTATE", -5: "BA_ENUMERIC"}
 
 EXPORTS = ["ba_create", "ba_iterate", "ba_bounds", "ba_get_p", "ba_scratch_bytes", "ba_create_ext",
            "ba_set_mode", "ba_set_exact", "ba_set_symmetry", "ba_set_p", "ba_get_q", "ba_get_D", "ba_stats", "ba_get_history",
            "ba_last_timing", "ba_setup_ms", "ba_measure_peaks", "ba_debug_emb_row", "ba_debug_emb_col", "ba_terms_per_sweep",
-           "ba_debug_count_terms", "ba_debug_check_tables", "ba_destroy", "ba_last_error"]
+           "ba_debug_count_terms", "ba_debug_check_tables", "ba_destroy", "ba_last_error", "ba_in_final_noalloc",
+           "ba_noalloc_last_error"]
 
 
 class BAError(RuntimeError):
@@ -76,6 +78,9 @@ def load():
     L.ba_destroy.restype = None
     L.ba_last_error.argtypes = [vp]
     L.ba_last_error.restype = ctypes.c_char_p
+    L.ba_in_final_noalloc.argtypes = [ctypes.c_int, vp, vp, vp, vp, vp, vp, vp]
+    L.ba_noalloc_last_error.argtypes = []
+    L.ba_noalloc_last_error.restype = ctypes.c_char_p
     for name in EXPORTS:
         getattr(L, name)
     _lib = L
@@ -206,6 +211,28 @@ def ba_measure_peaks():
     if rc:
         raise BAError(rc, "ba_measure_peaks failed")
     return dict(dfma=out[0], idp2a=out[1], lds64=out[2], ffma=out[3], sm_mhz=out[4], sms=int(out[5]))
+
+
+def ba_in_final_noalloc(n, Hc, S0, S1, p, D, out3, stream=None):
+    """D = Hc - (S0 + S1) and out3 = {sum p D, max D, sum p 2^D} without any device allocation (ba.h): the first-stage
+    partials sit in a static device array of libba.  Hc, S0, S1 (or None), p, D: float64 CUDA tensors of 2^n entries;
+    out3: 3 entries; all on the current device.  Queued on `stream` (a torch.cuda.Stream; default: torch's current
+    stream); does not synchronise."""
+    import torch
+    sized = 1 <= n <= BA_NOALLOC_NMAX                      # otherwise the library rejects the call before touching memory
+    NX = 1 << n if sized else 0
+    for name, t, need in (("Hc", Hc, NX), ("S0", S0, NX), ("S1", S1, NX), ("p", p, NX), ("D", D, NX), ("out3", out3, 3)):
+        if t is None and name == "S1":
+            continue
+        if (t is None or not t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous()
+                or (sized and t.numel() != need)):
+            raise BAError(BA_EINVAL, f"ba_in_final_noalloc: {name} must be a contiguous float64 CUDA tensor of {need} entries")
+    st = stream if stream is not None else torch.cuda.current_stream()
+    L = load()
+    rc = L.ba_in_final_noalloc(n, Hc.data_ptr(), S0.data_ptr(), S1.data_ptr() if S1 is not None else None, p.data_ptr(),
+                               D.data_ptr(), out3.data_ptr(), st.cuda_stream)
+    if rc:
+        raise BAError(rc, L.ba_noalloc_last_error().decode())
 
 
 def ba_get_p(ctx, out=None):

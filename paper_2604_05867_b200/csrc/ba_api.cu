@@ -10,6 +10,7 @@
 #include "ba_peaks.cuh"
 
 #include <cmath>
+#include <cstdarg>
 #include <cstdio>
 #include <cstring>
 #include <memory>
@@ -803,5 +804,110 @@ extern "C" int ba_setup_ms(ba_ctx *c, double *ms_host) {
     float f = 0.f;
     CK(cudaEventElapsedTime(&f, c->ev_setup[0], c->ev_setup[1]));
     *ms_host = (double)f;
+    return BA_OK;
+}
+
+// ------------------------------------------------------------------------------------------------ no-allocation entry point
+// ba_in_final_noalloc (ba.h): the epilogue of the input sweep -- D = Hc - (S0 + S1) and the reductions of 8(a3),
+// for callers that must not allocate (CUDA graph capture, serving loops).  k_in_final keeps its
+// first-stage partials in ctx-owned scratch (`part`, cudaMalloc'ed by ba_create); this variant keeps them in the
+// file-scope device array below: 48 KB that every GPU which loads the library holds until exit.  Its name is a
+// host-side stand-in in host code, so the device address is taken once per device with cudaGetSymbolAddress
+// and handed to the kernels.
+#define BA_NA_CHUNK ((size_t)1 << 15)                          // inputs per block: fixed, so the sums have one order per n
+static __device__ __align__(256) double g_na_part[3 * BA_NOALLOC_MAXBLK];
+
+__global__ void __launch_bounds__(256) k_in_final_na(size_t NX, const double *__restrict__ Hc, const double *__restrict__ S0,
+                                                     const double *__restrict__ S1, const double *__restrict__ p,
+                                                     double *__restrict__ D, double *__restrict__ part) {
+    __shared__ double sr[3 * 8];
+    double r0 = 0.0, r1 = -INFINITY, r2 = 0.0;
+    const size_t lo = (size_t)blockIdx.x * BA_NA_CHUNK, hi = (lo + BA_NA_CHUNK < NX) ? lo + BA_NA_CHUNK : NX;
+    for (size_t i = lo + threadIdx.x; i < hi; i += blockDim.x) {
+        const double Dx = Hc[i] - (S1 ? S0[i] + S1[i] : S0[i]);
+        D[i] = Dx;
+        const double px = p[i];
+        r0 += px * Dx; r1 = fmax(r1, Dx); r2 += px * exp2(Dx);
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        r0 += __shfl_xor_sync(0xffffffffu, r0, o);
+        r1 = fmax(r1, __shfl_xor_sync(0xffffffffu, r1, o));
+        r2 += __shfl_xor_sync(0xffffffffu, r2, o);
+    }
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (lane == 0) { sr[warp * 3] = r0; sr[warp * 3 + 1] = r1; sr[warp * 3 + 2] = r2; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t0 = 0.0, t1 = -INFINITY, t2 = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); w++) { t0 += sr[w * 3]; t1 = fmax(t1, sr[w * 3 + 1]); t2 += sr[w * 3 + 2]; }
+        part[(size_t)blockIdx.x * 3] = t0; part[(size_t)blockIdx.x * 3 + 1] = t1; part[(size_t)blockIdx.x * 3 + 2] = t2;
+    }
+}
+
+// second stage: the npart triples of the scratch, in a fixed order, to out3 = {sum p D, max D, sum p 2^D}
+__global__ void __launch_bounds__(1024) k_finalize_na(const double *__restrict__ part, int npart, double *__restrict__ out3) {
+    __shared__ double s0[1024], s1[1024], s2[1024];
+    const int tid = threadIdx.x;
+    double a0 = 0.0, a1 = -INFINITY, a2 = 0.0;
+    for (int i = tid; i < npart; i += 1024) { a0 += part[3 * i]; a1 = fmax(a1, part[3 * i + 1]); a2 += part[3 * i + 2]; }
+    s0[tid] = a0; s1[tid] = a1; s2[tid] = a2;
+    __syncthreads();
+    for (int o = 512; o > 0; o >>= 1) {
+        if (tid < o) { s0[tid] += s0[tid + o]; s1[tid] = fmax(s1[tid], s1[tid + o]); s2[tid] += s2[tid + o]; }
+        __syncthreads();
+    }
+    if (tid == 0) { out3[0] = s0[0]; out3[1] = s1[0]; out3[2] = s2[0]; }
+}
+
+#define BA_NA_MAXDEV 64
+static std::mutex g_na_mu;
+static double *g_na_ptr[BA_NA_MAXDEV];                         // device address of g_na_part, per device (null = not taken yet)
+static thread_local char g_na_err[256] = "";
+
+static int na_fail(int code, const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_na_err, sizeof g_na_err, fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+extern "C" const char *ba_noalloc_last_error(void) { return g_na_err; }
+
+extern "C" int ba_in_final_noalloc(int n, const void *Hc_dev, const void *S0_dev, const void *S1_dev, const void *p_dev,
+                                   void *D_dev, void *out3_dev, void *stream) {
+    if (n < 1 || n > BA_NOALLOC_NMAX)
+        return na_fail(BA_EINVAL, "ba_in_final_noalloc: n = %d is outside [1, %d]: the static scratch holds %d block partials of %zu inputs each",
+                       n, BA_NOALLOC_NMAX, BA_NOALLOC_MAXBLK, BA_NA_CHUNK);
+    if (!Hc_dev || !S0_dev || !p_dev || !D_dev || !out3_dev) return na_fail(BA_EINVAL, "ba_in_final_noalloc: null pointer");
+    const size_t NX = (size_t)1 << n;
+    const int nblk = (int)((NX + BA_NA_CHUNK - 1) / BA_NA_CHUNK);
+    if (nblk > BA_NOALLOC_MAXBLK) return na_fail(BA_EINVAL, "ba_in_final_noalloc: %d blocks exceed the static scratch (%d)", nblk, BA_NOALLOC_MAXBLK);
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return na_fail(BA_ECUDA, "ba_in_final_noalloc: cudaGetDevice: %s", cudaGetErrorString(e));
+    if (dev < 0 || dev >= BA_NA_MAXDEV) return na_fail(BA_EINVAL, "ba_in_final_noalloc: device ordinal %d not below %d", dev, BA_NA_MAXDEV);
+    double *part = nullptr;
+    {
+        std::lock_guard<std::mutex> lk(g_na_mu);
+        if (!g_na_ptr[dev]) {                                  // once per device, with that device current
+            void *sym = nullptr;
+            e = cudaGetSymbolAddress(&sym, g_na_part);
+            if (e != cudaSuccess || !sym) {
+                cudaGetLastError();
+                return na_fail(BA_ECUDA, "ba_in_final_noalloc: cudaGetSymbolAddress on device %d: %s", dev, cudaGetErrorString(e));
+            }
+            g_na_ptr[dev] = (double *)sym;
+        }
+        part = g_na_ptr[dev];
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    // every triple the second stage reads is written by the first stage of the same call: nothing has to start at zero
+    k_in_final_na<<<nblk, 256, 0, st>>>(NX, (const double *)Hc_dev, (const double *)S0_dev, (const double *)S1_dev,
+                                        (const double *)p_dev, (double *)D_dev, part);
+    k_finalize_na<<<1, 1024, 0, st>>>(part, nblk, (double *)out3_dev);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return na_fail(BA_ECUDA, "ba_in_final_noalloc: launch: %s", cudaGetErrorString(e));
+    g_na_err[0] = 0;
     return BA_OK;
 }
