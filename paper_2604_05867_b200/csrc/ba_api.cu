@@ -32,6 +32,8 @@ struct ba_ctx {
     double *c = nullptr, *crow = nullptr, *Hc = nullptr, *Apart = nullptr, *S = nullptr, *park = nullptr, *part = nullptr, *scal = nullptr, *hist = nullptr;
     GroupDev gin, gout;              // pair schedules of the two sweeps (device pointers into scratch)
     uint2 *EPS8 = nullptr;
+    uint32_t *LTV_off = nullptr, *LTV = nullptr;            // subsequences of every v (input sweep, pairs (v, empty))
+    uint8_t *LT = nullptr;                                  // [2^m][2^{m+1}] emb(w, v) of the low tile (k_low_tile)
     uint32_t *EPSH = nullptr;
     double *elog = nullptr;
     unsigned int *counters = nullptr;
@@ -73,7 +75,7 @@ static double host_binom(int n, int k) {
 // ------------------------------------------------------------------------------------------------ scratch layout
 struct SideLayout { size_t GB, GA, GO, GW, csr_off, csr_idx, R, r_cnt, r_csr, R8; };
 struct ScratchLayout {
-    size_t c, crow, Hc, Apart, S, park, part, scal, hist, EPS8, EPSH, elog, counters, cnt, total;
+    size_t c, crow, Hc, Apart, S, park, part, scal, hist, EPS8, EPSH, LT, LTV_off, LTV, elog, counters, cnt, total;
     SideLayout in, out;
     size_t napart, npart_cap;
 };
@@ -128,6 +130,9 @@ static void scratch_layout(int n, const TileTables &T, ScratchLayout &L) {
     L.hist = o; o += align256((size_t)BA_HIST_CAP * 3 * 8);
     L.EPS8 = o; o += align256(T.EPS8.size() * 8);
     L.EPSH = o; o += align256(T.EPSH.size() * 4);
+    L.LT = o; o += align256(T.LT.size());
+    L.LTV_off = o; o += align256(T.LTV_off.size() * 4);
+    L.LTV = o; o += align256(T.LTV.size() * 4);
     L.elog = o; o += align256((size_t)BA_ELOG_N * 8);
     side_layout(T.in, L.in, o);
     side_layout(T.out, L.out, o);
@@ -333,11 +338,15 @@ static int finish_create(ba_ctx *c) {
     unsigned char *s = c->scratch;
     c->c = (double *)(s + L.c); c->crow = (double *)(s + L.crow); c->Hc = (double *)(s + L.Hc); c->Apart = (double *)(s + L.Apart); c->S = (double *)(s + L.S); c->park = (double *)(s + L.park);
     c->part = (double *)(s + L.part); c->scal = (double *)(s + L.scal); c->hist = (double *)(s + L.hist);
-    c->EPS8 = (uint2 *)(s + L.EPS8); c->EPSH = (uint32_t *)(s + L.EPSH); c->elog = (double *)(s + L.elog);
+    c->EPS8 = (uint2 *)(s + L.EPS8); c->EPSH = (uint32_t *)(s + L.EPSH); c->elog = (double *)(s + L.elog); c->LT = (uint8_t *)(s + L.LT);
+    c->LTV_off = (uint32_t *)(s + L.LTV_off); c->LTV = (uint32_t *)(s + L.LTV);
     c->counters = (unsigned int *)(s + L.counters); c->cnt = (unsigned long long *)(s + L.cnt);
     c->napart = L.napart; c->npart_cap = L.npart_cap;
 
     CK(upload(c->EPS8, T.EPS8, c->st));
+    CK(upload(c->LT, T.LT, c->st));
+    CK(upload(c->LTV_off, T.LTV_off, c->st));
+    CK(upload(c->LTV, T.LTV, c->st));
     CK(upload(c->EPSH, T.EPSH, c->st));
     std::vector<double> elog(BA_ELOG_N, 0.0);
     for (int e = 2; e < BA_ELOG_N; e++) elog[e] = (double)((long double)e * log2l((long double)e));
@@ -468,7 +477,7 @@ extern "C" int ba_set_mode(ba_ctx *c, int mode) {
 // ------------------------------------------------------------------------------------------------ launches
 static InArgs make_in_args(ba_ctx *c) {
     InArgs a;
-    a.kc = c->kc; a.g = c->gin; a.EPS8 = c->EPS8; a.EPSH = c->EPSH;
+    a.kc = c->kc; a.g = c->gin; a.EPS8 = c->EPS8; a.EPSH = c->EPSH; a.LTV_off = c->LTV_off; a.LTV = c->LTV;
     a.c = c->c; a.crow = c->crow; a.elog = c->elog; a.S = c->S; a.park = c->park;
     a.counter = c->counters; a.sym = 0; a.dbg_x = 0; a.dbg_out = nullptr; a.cnt = c->cnt;
     return a;
@@ -477,7 +486,7 @@ static InArgs make_in_args(ba_ctx *c) {
 static OutArgs make_out_args(ba_ctx *c) {
     OutArgs a;
     a.kc = c->kc; a.g = c->gout; a.EPS8 = c->EPS8;
-    a.p = c->p; a.Apart = c->Apart; a.counter = c->counters + 4; a.sym = 0; a.dbg_item = 0; a.dbg_cz = 0; a.dbg_out = nullptr;
+    a.p = c->p; a.M = c->S; a.Apart = c->Apart; a.counter = c->counters + 4; a.sym = 0; a.dbg_item = 0; a.dbg_cz = 0; a.dbg_out = nullptr;
     a.cnt = c->cnt + 2;
     return a;
 }
@@ -505,6 +514,12 @@ static int launch_out_sweep(ba_ctx *c) {
         CK(cudaMemsetAsync(c->counters + 4, 0, 4, c->st));
         OutArgs a = make_out_args(c);
         a.sym = c->sym;
+        // M(u, w) of the low tile, for the pairs (v, empty) of the sweep.  It lives in S: the partial sums of the input
+        // sweep are dead from k_in_final to the next input sweep, and 2^h * 2^{m+1} = 2 * 2^n entries is their size.
+        const size_t NU = (size_t)1 << c->h;
+        const size_t ltb = (NU + BA_LT_UB - 1) / BA_LT_UB;
+        k_low_tile<<<(unsigned)(ltb < (size_t)c->num_sms * 16 ? ltb : (size_t)c->num_sms * 16), 512, 0, c->st>>>(c->m, NU, c->p, c->LT, c->S);
+        CK(cudaGetLastError());
         k_enum_out<OUT_SWEEP><<<c->grid_out, c->block, c->smem_out, c->st>>>(a);
         CK(cudaGetLastError());
         k_out_final<<<c->num_sms * 8, 256, 0, c->st>>>(c->kc, c->Apart, nullptr, c->q, c->c, c->crow, c->sym);

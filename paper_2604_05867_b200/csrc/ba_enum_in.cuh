@@ -40,6 +40,7 @@ enum { IN_SWEEP = 0, IN_HC = 1, IN_DEBUG = 2, IN_COUNT = 3 };
 #define BA_IN_SB (BA_SBR * BA_NT)                           // nodes per super-batch
 #define BA_IN_NBKT (2 * BA_NCLS)                            // buckets: class, with / without list b (the latter: b = 0 only)
 #define BA_IN_MAXB (BA_IN_NBKT + BA_IN_SB / BA_RB_IN)
+#define BA_IN_NG (512 + 5 * BA_NCLS)                        // G sums of an item: by code(w), |w| >= 5; by (class, s), s <= 4
 
 struct InArgs {
     KConst kc;
@@ -48,6 +49,8 @@ struct InArgs {
     const uint32_t *EPSH;     // [cls][8][2^m]: B_4..B_7 of the pair (v, empty) by the sigma bits 4..6: a class's slice
     const double *c;          // IN_SWEEP: c[code(y)], 2^{n+1} entries (entry 0 unused)
     const double *crow;       // IN_SWEEP: the same by rows (code(y'), b) of 2^m operands (k_out_final)
+    const uint32_t *LTV_off;  // [2^m + 1]: the subsequences w of v ...
+    const uint32_t *LTV;      // ... as code(w) << 8 | emb(w, v)   (IN_SWEEP: the pairs (v, empty) in factored form)
     const double *elog;       // IN_HC: elog[e] = e log2(e), e < BA_ELOG_N
     double *S;                // out: [2][2^n] partial sums of the two lists (IN_SWEEP: S_b, IN_HC: H_b)
     double *park;             // [grid][2][BA_NSLOT][BA_NT]: the accumulators of the schedule that is not running
@@ -65,13 +68,13 @@ __host__ __device__ static inline InSmem enum_in_smem(int nr) {
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o += (bytes + 15) & ~(size_t)15; return at; };
     s.rec = take((size_t)BA_IN_SB * sizeof(NodeRec));
-    s.rsum = take((size_t)2 * 2 * nr * 8 > (size_t)BA_NT * 8 ? (size_t)2 * 2 * nr * 8 : (size_t)BA_NT * 8);   // rider sums of a batch, two replicas,
-                                                           // double buffered; the epilogue parks acc_eps there
+    s.rsum = take((size_t)4 * 2 * nr * 8 > (size_t)BA_NT * 8 ? (size_t)4 * 2 * nr * 8 : (size_t)BA_NT * 8);   // rider sums of a batch, two replicas,
+                                                           // four batches deep (collected two batches late); the epilogue parks acc_eps there
     s.slice = take((size_t)2 * 8 * ((size_t)1 << BA_MLOW) * 4);    // B_4..B_7 of the pairs (v, empty) of a class, double buffered
     s.rslice = take((size_t)2 * 8 * nr * 4);               // B_4..B_7 of the riders of a class, double buffered
     size_t rows = (size_t)2 * BA_RB_IN * BA_ROWB, ac = (size_t)2 * BA_NSLOT * BA_NT * 8;   // both schedules' accumulators
     s.rows = take(rows > ac ? rows : ac);                  // the epilogue's accumulator staging aliases the rows
-    s.mbar = take(2 * 8);                                  // FULL barrier of the two row buffers
+    s.mbar = take(4 * 8);                                  // FULL and EMPTY barriers of the two row buffers
     s.bal = take((size_t)2 * BA_RB_IN * sizeof(BalRec));
     s.ordr = take((size_t)BA_SBR * BA_NT * 2);             // per round: the round's nodes by class
     s.seg = take((size_t)BA_SBR * (BA_IN_NBKT + 1) * 2);
@@ -112,6 +115,11 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
     NodeRec *s_rec = (NodeRec *)(smem + L.rec);
     uint32_t *s_slice = (uint32_t *)(smem + L.slice);
     uint32_t *s_rslice = (uint32_t *)(smem + L.rslice);
+    // IN_SWEEP forms the pairs (v, empty) in factored form (see "G sums" below) and stages no slice of them: their area
+    // holds c(y') of the super-batch's nodes and the G sums of the item
+    double *s_c = (double *)s_slice;
+    double *s_G = s_c + BA_IN_SB;
+    static_assert((size_t)(BA_IN_SB + BA_IN_NG) * 8 <= (size_t)2 * 8 * ((size_t)1 << BA_MLOW) * 4, "c(y') and the G sums live in the slice area");
     double *s_rows = (double *)(smem + L.rows);
     double *s_acc = s_rows;                                 // epilogue only
     double *s_elog = s_rows;                                // IN_HC: the table's head; the epilogue overwrites it, so it is
@@ -133,9 +141,10 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
     uint32_t *s_item = (uint32_t *)(smem + L.item);        // [0] item, [1] number of batches
 
     for (int i = tid; i <= BA_NMAX_I; i += BA_NT) { s_w[i] = a.kc.w[i]; s_lebar[i] = a.kc.lebar[i]; }
-    const uint32_t sFull = ba_smem_addr(smem + L.mbar);
+    const uint32_t sFull = ba_smem_addr(smem + L.mbar), sEmpty = sFull + 16u;
     if (tid == 0) {
-        ba_mbar_init(sFull, 32u); ba_mbar_init(sFull + 8u, 32u);        // the 32 lanes of the staging warp; rows count in bytes
+        ba_mbar_init(sFull, 32u); ba_mbar_init(sFull + 8u, 32u);        // the 32 lanes of the staging warp; copies count in bytes
+        ba_mbar_init(sEmpty, BA_NT / 32); ba_mbar_init(sEmpty + 8u, BA_NT / 32);   // one arrival per warp that has left the batch
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     if (MODE == IN_HC) load_elog();
@@ -160,6 +169,13 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
         if (h < 31 && (u >> (h - a.sym)) != 0) break;
         if (MODE == IN_DEBUG && blockIdx.x > 1) break;
         const int klen = (MODE == IN_SWEEP || MODE == IN_HC) ? a.kc.klen : -1;
+        // The pairs (v, empty) (list 0 serves them).  With the concatenation identity at the tile boundary,
+        //     sum_{y' in u} c(y') emb(y', u.v) = sum_w G(w) emb(w, v),   G(w) = sum_{y' ending in w} c(y') alpha_{|w|}(y'),
+        // so IN_SWEEP adds c(y') alpha_s of every node to the nine G sums of its suffixes (eps_fact) and expands them
+        // once per item; the other modes need every emb on its own and enumerate the 2^m terms of a node (eps_enum).
+        const bool eps_fact = MODE == IN_SWEEP && b == 0, eps_enum = MODE != IN_SWEEP && b == 0;
+        if (eps_fact)
+            for (int i = tid; i < BA_IN_NG; i += BA_NT) s_G[i] = 0.0;
 
         // ---- Sub[pos] = number of trie nodes below a node whose leftmost embedding ends at pos -------
         if (tid == 0) {
@@ -251,6 +267,10 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                     rc.id = cy;
                     rc.info = missb | ((uint32_t)(k < 8 ? k : 8) << 8) | ((uint32_t)k << 16);
                     s_rec[rd * BA_NT + tid] = rc;
+                    if (eps_fact) {                                // c(y') of the node (exact channel: only |y'| = klen has weight)
+                        if (klen < 0 || k == klen) ba_cp_async8(ba_smem_addr(&s_c[rd * BA_NT + tid]), a.c + cy);
+                        else s_c[rd * BA_NT + tid] = 0.0;
+                    }
                     // buckets: class for the nodes that carry list b; for b = 0 the others follow in buckets 16 + class:
                     // they contribute the pair (v, empty) only (exact channel: only if |y'| = klen)
                     if (missb) key = (int)(cy & (BA_NCLS - 1));
@@ -277,12 +297,13 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 const int cq_l = ((lane >> 1) & 7) * 2 + (lane >> 4);          // class order: bit 0 = 0 first (one schedule switch)
                 const int kq = (lane & 1) * BA_NCLS + cq_l;
                 const int ck = __shfl_sync(0xffffffffu, cnt, kq), gk = __shfl_sync(0xffffffffu, incl - cnt, kq);
-                const int nbk = (ck + BA_RB_IN - 1) / BA_RB_IN;
+                const int ckb = (MODE == IN_SWEEP && kq >= BA_NCLS) ? 0 : ck;   // IN_SWEEP: no batches without list b
+                const int nbk = (ckb + BA_RB_IN - 1) / BA_RB_IN;
                 int bincl = nbk;
                 for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, bincl, o); if (lane >= o) bincl += t; }
                 int nb = bincl - nbk;
-                for (int off = 0; off < ck; off += BA_RB_IN) {
-                    const int len = (ck - off < BA_RB_IN) ? (ck - off) : BA_RB_IN;
+                for (int off = 0; off < ckb; off += BA_RB_IN) {
+                    const int len = (ckb - off < BA_RB_IN) ? (ckb - off) : BA_RB_IN;
                     s_batch[nb++] = (uint32_t)(gk + off) | ((uint32_t)len << 16) | ((uint32_t)kq << 24);
                 }
                 if (lane == 31) s_item[1] = (uint32_t)bincl;
@@ -299,61 +320,95 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                     s_order[s_gstart[kq] + s_roff[rd * BA_IN_NBKT + kq] + (idx - (int)sg[kq])] = (uint16_t)(rd * BA_NT + od[idx]);
                 }
             }
+            if (eps_fact) ba_cp_async_wait_all();              // this thread's c(y')
             __syncthreads();
+
+            // ================= G sums of the pairs (v, empty) =================
+            // A node y' of length k adds c(y') alpha_s to G(sigma_s) for s = 0 .. min(k, m).  Every sum has one owner
+            // thread, which walks the two buckets of its class in their (stable) order: no atomics, one fixed order.
+            // |w| >= 5: the thread of code(w) takes the nodes of class w mod 16 that end in w.  |w| <= 4: G(w) is the sum
+            // over the classes that end in w of P(class, s) = sum over the class's nodes of length >= s; the 80 P's have
+            // owners of their own (threads 480..511, then 0..47) and are added up in the epilogue.
+            if (eps_fact) {
+                auto scan = [&](int s, int cl, uint32_t wval, int dst) {
+                    const uint32_t mask = (1u << s) - 1u;
+                    double g = 0.0;
+                    for (int part = 0; part < 2; part++) {
+                        const int i0 = s_gstart[part * BA_NCLS + cl], i1 = s_gstart[part * BA_NCLS + cl + 1];
+                        for (int i = i0; i < i1; i++) {
+                            const int node = s_order[i];
+                            const NodeRec &rc = s_rec[node];
+                            if ((int)(rc.info >> 16) >= s && (rc.id & mask) == wval) g = fma((double)rc.a[s], s_c[node], g);
+                        }
+                    }
+                    s_G[dst] += g;
+                };
+                if (tid < 480) {
+                    const uint32_t code = 32u + (uint32_t)tid;
+                    const int s = ba_len_of_code(code);
+                    const uint32_t wval = code - (1u << s);
+                    scan(s, (int)(wval & (BA_NCLS - 1)), wval, (int)code);
+                }
+                if (tid >= 480 || tid < 5 * BA_NCLS - 32) {
+                    const int j = (tid >= 480) ? tid - 480 : 32 + tid, cl = j / 5, s = j % 5;
+                    scan(s, cl, (uint32_t)cl & ((1u << s) - 1u), 512 + j);
+                }
+            }
 
             // ================= phase B: batches of one class =================
             const int nbatch = (int)s_item[1];
             int st_cls = -1, st_sb = 0, cp_cls = -1, cp_sb = 0;     // slice double buffer: staging side, computing side
-            auto stage = [&](int j) {                          // half rows and alphas of batch j
-                const uint32_t bi = s_batch[j];
-                const int start = (int)(bi & 0xffffu), len = (int)((bi >> 16) & 0xffu), buf = (int)((gb + (uint32_t)j) & 1u);
+            // Staging is the work of warp 0 alone; the other warps meet it only through the FULL / EMPTY barriers of the
+            // two buffers, so a warp runs up to one batch ahead of the slowest one and nobody waits at a CTA barrier.
+            auto stage = [&](int j) {                          // half rows, slices and alphas of batch j (warp 0, lane i = node i)
+                const uint32_t bi = s_batch[j], g = gb + (uint32_t)j;
+                const int start = (int)(bi & 0xffffu), len = (int)((bi >> 16) & 0xffu), buf = (int)(g & 1u);
                 const int scls = (int)(bi >> 24) & (BA_NCLS - 1);
-                if (scls != st_cls) {                          // a new class: its slices of B_4..B_7 (by the sigma bits 4..6)
-                    st_cls = scls; st_sb ^= 1;                 // of the riders and, for b = 0, of the pairs (v, empty)
-                    {
-                        const uint32_t *src = a.g.R8 + ((size_t)scls * 2 + b) * 8 * a.g.nr;
-                        const uint32_t dst = ba_smem_addr(s_rslice) + (uint32_t)st_sb * 8u * (uint32_t)a.g.nr * 4u;
-                        for (int e = tid; e < 8 * a.g.nr; e += BA_NT)
-                            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst + (uint32_t)e * 4u), "l"(src + e) : "memory");
-                    }
-                    if (b == 0) {
-                        const uint32_t *src = a.EPSH + (size_t)scls * 8 * nv;
-                        const uint32_t dst = ba_smem_addr(s_slice) + (uint32_t)st_sb * (8u << BA_MLOW) * 4u;
-                        for (int e = tid; e < 8 * nv; e += BA_NT)
-                            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst + (uint32_t)((e >> m) << BA_MLOW) * 4u + (uint32_t)(e & (nv - 1)) * 4u), "l"(src + e) : "memory");
-                    }
+                // every warp has left the batch that used this buffer, its slice buffer and its rider sums before
+                if (g >= 2u) ba_mbar_wait(sEmpty + 8u * buf, ((g >> 1) - 1u) & 1u);
+                const bool newcls = scls != st_cls;            // a new class: its slices of B_4..B_7 (by the sigma bits 4..6)
+                if (newcls) { st_cls = scls; st_sb ^= 1; }     // of the riders and, for b = 0, of the pairs (v, empty)
+                const uint32_t rs_bytes = 32u * (uint32_t)a.g.nr, es_bytes = (eps_enum && m == BA_MLOW) ? (8u << BA_MLOW) * 4u : 0u;
+                const bool row = MODE == IN_SWEEP && lane < len && (bi >> 24) < BA_NCLS;
+                uint32_t tx = row ? (uint32_t)nv * 8u : 0u;
+                if (newcls && lane == 0) tx += rs_bytes + es_bytes;
+                if (newcls && eps_enum && m != BA_MLOW) {      // n < 8: the rows of the slice are shorter than their pitch
+                    const uint32_t *src = a.EPSH + (size_t)scls * 8 * nv;
+                    for (int e = lane; e < 8 * nv; e += 32)
+                        s_slice[(size_t)st_sb * (8u << BA_MLOW) + (size_t)((e >> m) << BA_MLOW) + (size_t)(e & (nv - 1))] = __ldg(src + e);
                 }
-                if (warp != 0) return;                         // rows and node records: the staging warp, lane i = node i
+                const NodeRec *rcp = nullptr;
                 if (lane < len) {
                     const int node = s_order[start + lane];
-                    const NodeRec &rc = s_rec[node];
-                    s_bal[buf * BA_RB_IN + lane] = ba_make_bal(rc, (uint32_t)node);
-                    if (MODE == IN_SWEEP && b == 0)            // operand of the pair (v, empty): c(y'), lands before the CTA barrier
-                        ba_cp_async8(ba_smem_addr(&s_bal[buf * BA_RB_IN + lane].x0), a.c + rc.id);
-                    if (MODE == IN_SWEEP && (bi >> 24) < BA_NCLS) {
-                        // the half row c(y'.b.t), all t, is row (code(y'), b) of crow: one bulk copy
-                        ba_mbar_arrive_expect_tx(sFull + 8u * buf, (uint32_t)nv * 8u);
-                        ba_bulk_g2s(sRows + (uint32_t)(buf * BA_RB_IN + lane) * BA_ROWB, a.crow + (((((size_t)rc.id) << 1) | (size_t)b) << m),
-                                    (uint32_t)nv * 8u, sFull + 8u * buf);
-                    } else ba_mbar_arrive(sFull + 8u * buf);
-                } else ba_mbar_arrive(sFull + 8u * buf);
+                    rcp = &s_rec[node];
+                    s_bal[buf * BA_RB_IN + lane] = ba_make_bal(*rcp, (uint32_t)node);
+                }
+                // the lane's arrival carries the bytes of its bulk copies
+                if (tx) ba_mbar_arrive_expect_tx(sFull + 8u * buf, tx); else ba_mbar_arrive(sFull + 8u * buf);
+                if (newcls && lane == 0) {
+                    if (rs_bytes) ba_bulk_g2s(ba_smem_addr(s_rslice) + (uint32_t)st_sb * rs_bytes, a.g.R8 + ((size_t)scls * 2 + b) * 8 * a.g.nr, rs_bytes, sFull + 8u * buf);
+                    if (es_bytes) ba_bulk_g2s(ba_smem_addr(s_slice) + (uint32_t)st_sb * es_bytes, a.EPSH + (size_t)scls * 8 * nv, es_bytes, sFull + 8u * buf);
+                }
+                if (row)                                       // the half row c(y'.b.t), all t, is row (code(y'), b) of crow: one bulk copy
+                    ba_bulk_g2s(sRows + (uint32_t)(buf * BA_RB_IN + lane) * BA_ROWB, a.crow + (((((size_t)rcp->id) << 1) | (size_t)b) << m),
+                                (uint32_t)nv * 8u, sFull + 8u * buf);
             };
             auto flush = [&](int j) {                          // thread v collects the rider sums of batch j
                 if (MODE != IN_SWEEP && MODE != IN_HC) return;
                 if (tid >= nv) return;
                 if ((s_batch[j] >> 24) >= BA_NCLS) return;     // a batch without list b has no riders
-                const int cls = (int)(s_batch[j] >> 24), buf = (int)((gb + (uint32_t)j) & 1u);
+                const int cls = (int)(s_batch[j] >> 24), rbuf = (int)((gb + (uint32_t)j) & 3u);
                 const uint16_t *cs = a.g.r_csr + (size_t)(cls * 2 + b) * (nv + 1) + tid;
                 const int e0 = cs[0], e1 = cs[1];
-                for (int e = e0; e < e1; e++) acc_rid += s_rsum[((size_t)buf * 2) * a.g.nr + e] + s_rsum[((size_t)buf * 2 + 1) * a.g.nr + e];
+                for (int e = e0; e < e1; e++) acc_rid += s_rsum[((size_t)rbuf * 2) * a.g.nr + e] + s_rsum[((size_t)rbuf * 2 + 1) * a.g.nr + e];
             };
-            if (nbatch > 0) stage(0);
+            if (warp == 0 && nbatch > 0) stage(0);
             for (int j = 0; j < nbatch; j++) {
                 const uint32_t bi = s_batch[j];
                 const int len = (int)((bi >> 16) & 0xffu), cls = (int)(bi >> 24) & (BA_NCLS - 1), kind = (int)(bi >> 28), buf = (int)((gb + (uint32_t)j) & 1u);
                 if (cls != cp_cls) { cp_cls = cls; cp_sb ^= 1; }
                 uint32_t eB0 = 0u;                             // 1 | B_1..B_3 of the pair (ev, empty): a constant of the class
-                if (b == 0) eB0 = __ldg(a.EPS8 + (size_t)cls * nv + ev).x;
+                if (eps_enum) eB0 = __ldg(a.EPS8 + (size_t)cls * nv + ev).x;
                 // the slots' B_s do not depend on the staged rows: fetch them before waiting
                 uint32_t Bp[BA_NSLOT];
 #pragma unroll
@@ -362,46 +417,27 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                     if (kind == 0) bb = __ldg(a.g.GB + (((size_t)cls * 2 + b) * BA_KG + k) * BA_NT + tid);
                     Bp[k * BA_GP] = bb.x; Bp[k * BA_GP + 1] = bb.y; Bp[k * BA_GP + 2] = bb.z; Bp[k * BA_GP + 3] = bb.w;
                 }
-                ba_cp_async_wait_all();
-                ba_mbar_wait(sFull + 8u * buf, ((gb + (uint32_t)j) >> 1) & 1u);     // the rows of batch j have landed
-                __syncthreads();                               // batch j staged; batch j-1 fully consumed
-                if (j + 1 < nbatch) stage(j + 1);
-                if (j > 0) flush(j - 1);
+                ba_mbar_wait(sFull + 8u * buf, ((gb + (uint32_t)j) >> 1) & 1u);     // rows, slices and records of batch j have landed
+                if (warp == 0 && j + 1 < nbatch) stage(j + 1);
+                // the rider sums of batch j-2: batch j was staged after every warp had left j-2, and no warp enters
+                // j+2 (which takes their place) before this warp has left j
+                if (j > 1) flush(j - 2);
                 const uint32_t rowbase = sRows + (uint32_t)(buf * BA_RB_IN) * BA_ROWB;
                 const BalRec *bal = s_bal + buf * BA_RB_IN;
                 bool big = false;
                 if (may_big) big = __any_sync(0xffffffffu, lane < len && bal[lane].big != 0u);
                 // ---- the pair (v, empty) of every node of the batch: thread (v, node) -----------------------------
-                if (b == 0 && (kind == 1 || klen < 0)) {
+                if (eps_enum && (kind == 1 || klen < 0)) {
                     const uint32_t sv8 = (m == 8) ? (uint32_t)ev : 0xffffffffu;      // B_8 = [sigma_8 = v] (m = 8 only)
                     const uint32_t *sl = s_slice + (size_t)cp_sb * (8u << BA_MLOW) + ev;     // [sigma bits 4..6][v]
-                    if (MODE == IN_SWEEP && !big) {
-                        double e0 = 0.0, e1 = 0.0;             // two chains; nodes esub, esub + epn, ...
-#pragma unroll 4
-                        for (int i = esub; i < len; i += 2 * epn) {
-                            const uint4 al = *(const uint4 *)&bal[i];
-                            const uint32_t cy = bal[i].id;
-                            const uint32_t emb = ba_chain9(al.x, al.y, al.z, al.w, bal[i].a8, eB0, sl[((cy >> 4) & 7u) << BA_MLOW], (cy & 255u) == sv8);
-                            e0 = fma(ba_u2d(emb), bal[i].x0, e0);
-                            const int i2 = i + epn;
-                            if (i2 < len) {
-                                const uint4 al2 = *(const uint4 *)&bal[i2];
-                                const uint32_t cy2 = bal[i2].id;
-                                const uint32_t emb2 = ba_chain9(al2.x, al2.y, al2.z, al2.w, bal[i2].a8, eB0, sl[((cy2 >> 4) & 7u) << BA_MLOW], (cy2 & 255u) == sv8);
-                                e1 = fma(ba_u2d(emb2), bal[i2].x0, e1);
-                            }
-                        }
-                        acc_eps += e0 + e1;
-                    } else {
+                    {
                         for (int i = esub; i < len; i += epn) {
                             const NodeRec &rc = s_rec[bal[i].node];
                             const uint32_t cy = rc.id;
                             const int k = (int)(rc.info >> 16);
                             const uint32_t emb = big ? ba_chain9_wide(rc.a, eB0, sl[((cy >> 4) & 7u) << BA_MLOW], (cy & 255u) == sv8)
                                                      : ba_chain9(bal[i].a01, bal[i].a23, bal[i].a45, bal[i].a67, bal[i].a8, eB0, sl[((cy >> 4) & 7u) << BA_MLOW], (cy & 255u) == sv8);
-                            if (MODE == IN_SWEEP) {
-                                acc_eps = fma(ba_u2d(emb), bal[i].x0, acc_eps);
-                            } else if (MODE == IN_HC) {
+                            if (MODE == IN_HC) {
                                 const double wk = s_w[k];
                                 if (wk != 0.0) acc_eps = fma(wk, ba_elog2e(emb, a.elog, s_elog) - (double)emb * s_lebar[k], acc_eps);
                             } else if (MODE == IN_DEBUG) {
@@ -446,7 +482,9 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                             for (int q = 0; q < BA_GP; q++) {
                                 uint32_t e = __dp2a_lo(al.x, Bp[g * BA_GP + q], 0u);
                                 e = __dp2a_hi(al.y, Bp[g * BA_GP + q], e);
-                                const double gl = fma((double)e, nlb, ba_elog2e(e, a.elog, s_elog));     // elog(0) = elog(1) = 0
+                                // exact u32 -> f64, spread over the conversion unit and the FP64 pipe as in the sweep
+                                const double ed = (q == 0) ? ba_cvt<0>(e) : (q == 1) ? ba_cvt<1>(e) : (q == 2) ? ba_cvt<2>(e) : ba_cvt<3>(e);
+                                const double gl = fma(ed, nlb, ba_elog2e(e, a.elog, s_elog));            // elog(0) = elog(1) = 0
                                 acc[g * BA_GP + q] = fma(wk, gl, acc[g * BA_GP + q]);
                             }
                         }
@@ -528,12 +566,15 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                             }
                         }
                     }
-                    if ((MODE == IN_SWEEP || MODE == IN_HC) && re < nr) s_rsum[((size_t)buf * 2 + rh) * a.g.nr + re] = s;
+                    if ((MODE == IN_SWEEP || MODE == IN_HC) && re < nr) s_rsum[((size_t)((gb + (uint32_t)j) & 3u) * 2 + rh) * a.g.nr + re] = s;
                 }
                 }                                              // kind == 0
+                __syncwarp();
+                if (lane == 0) ba_mbar_arrive(sEmpty + 8u * buf);      // this warp has left batch j
             }
             if (nbatch > 0) {
-                __syncthreads();                               // rider sums of the last batch are visible
+                __syncthreads();                               // rider sums of the last two batches are visible
+                if (nbatch > 1) flush(nbatch - 2);
                 flush(nbatch - 1);
             }
             gb += (uint32_t)nbatch;
@@ -551,11 +592,26 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                     s_acc[((size_t)sc * BA_NSLOT + s) * BA_NT + tid] = (sc == cur_sc) ? acc[s] : ((parked >> sc) & 1u) ? park[((size_t)sc * BA_NSLOT + s) * BA_NT] : 0.0;
             double *s_aeps = s_rsum;                           // the rider sums are all flushed: their area takes acc_eps
             s_aeps[tid] = acc_eps;
+            if (eps_fact && tid >= 480 && tid < 511) {         // G(w), |w| <= 4, from the P's of the classes that end in w
+                const uint32_t code = (uint32_t)(tid - 479);
+                const int s = ba_len_of_code(code);
+                double g = 0.0;
+                for (int cl = (int)(code - (1u << s)); cl < BA_NCLS; cl += 1 << s) g += s_G[512 + cl * 5 + s];
+                s_G[code] = g;
+            }
             __syncthreads();
             if (tid < nv) {
                 double S = acc_rid;
-                if (b == 0)
+                if (eps_enum)
                     for (int t = ev; t < BA_NT; t += nv) S += s_aeps[t];
+                if (eps_fact) {                                // sum_w G(w) emb(w, v) over the subsequences w of v
+                    double se = 0.0;
+                    for (uint32_t e = __ldg(a.LTV_off + tid), e1 = __ldg(a.LTV_off + tid + 1); e < e1; e++) {
+                        const uint32_t ent = __ldg(a.LTV + e);
+                        se = fma((double)(ent & 255u), s_G[ent >> 8], se);
+                    }
+                    S += se;
+                }
                 for (int sc = 0; sc < 2; sc++) {
                     const uint16_t *co = a.g.csr_off + ((size_t)sc * 2 + b) * (a.g.nown + 1) + tid, *ci = a.g.csr_idx + ((size_t)sc * 2 + b) * BA_NSLOT * BA_NT;
                     for (int q = co[0]; q < co[1]; q++) S += s_acc[(size_t)sc * BA_NSLOT * BA_NT + ci[q]];

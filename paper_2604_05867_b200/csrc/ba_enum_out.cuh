@@ -39,6 +39,7 @@ struct OutArgs {
     GroupDev g;                // schedule of the output sweep (owner = code(z), operand position = v)
     const uint2 *EPS8;         // [256][2^m]: B(sigma_s, v), s = 1..8, of the pair (v, empty)
     const double *p;           // NX
+    const double *M;           // OUT_SWEEP: [2^h][2^{m+1}] M(u, w) = sum_v p(u.v) emb(w, v) by code(w) (k_low_tile)
     double *Apart;             // (2^{h+1}-1) * (2^{m+1}-1)
     unsigned int *counter;
     int sym;                   // 1: q(y) = q(~y): prefixes y' with leading symbol 1 are skipped (k_out_final mirrors them)
@@ -149,8 +150,13 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
             Bp[k * BA_GP] = bb.x; Bp[k * BA_GP + 1] = bb.y; Bp[k * BA_GP + 2] = bb.z; Bp[k * BA_GP + 3] = bb.w;
             gaddr[k] = __ldg(a.g.GA + (sb * BA_KG + k) * BA_NT + tid);
         }
+        // The pair (v, empty) of a node.  OUT_SWEEP: sum_v p(u.v) emb(y', u.v) = sum_s alpha_s M(u, sigma_s) (P:181 at
+        // the tile boundary; M from k_low_tile), formed in phase A by the thread that unranks the node: no row, no batch.
+        // OUT_DEBUG / OUT_COUNT enumerate its 2^m terms one by one in phase B (eps_enum).
+        const bool eps_enum = do_eps && MODE != OUT_SWEEP;
+        const int Lm = t < m ? t : m;                          // sigma_s, s <= Lm: B(sigma_s, v) = 0 for s > m
         uint32_t eB0 = 0, eB1 = 0, eB2 = 0;                    // B(sigma_s, ev): B_0 = 1; alpha_s = 0 beyond t
-        if (do_eps) {
+        if (eps_enum) {
             const uint2 e8 = __ldg(a.EPS8 + (size_t)(cy & 255u) * nv + ev);
             eB0 = e8.x; eB1 = e8.y; eB2 = (m == 8 && (cy & 255u) == (uint32_t)ev) ? 1u : 0u;   // B_8 = [sigma_8 = v]
         }
@@ -223,6 +229,17 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                             if ((mm >> s) & 1u) f[s] += f[s + 1];
                     }
                 }
+                if (MODE == OUT_SWEEP && do_eps) {
+                    const double *Mu = a.M + ((size_t)u << (m + 1));
+                    double mv[BA_MLOW + 1];
+#pragma unroll
+                    for (int s = 0; s <= BA_MLOW; s++)         // code(sigma_s) = 1 << s | last s symbols of y'
+                        mv[s] = (s <= Lm) ? __ldg(Mu + ((1u << s) | (cy & ((1u << s) - 1u)))) : 0.0;
+                    double e = 0.0;
+#pragma unroll
+                    for (int s = BA_MLOW; s >= 0; s--) e = fma((double)f[s], mv[s], e);    // alpha_s = 0 beyond t
+                    acc_eps += e;
+                }
                 NodeRec rc;
 #pragma unroll
                 for (int s = 0; s < 9; s++) rc.a[s] = f[s];
@@ -231,7 +248,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                 rc.info = miss0 | (miss1 << 1) | ((uint32_t)Lc << 8) | ((uint32_t)t << 16);
                 s_rec[tid] = rc;
                 const bool has = do_grp && (b ? miss1 : miss0);
-                key = has ? 0 : (do_eps ? 1 : -1);             // 0: pairs of list b (and eps); 1: the pair (v, empty) only
+                key = has ? 0 : (eps_enum ? 1 : -1);           // 0: pairs of list b (and eps); 1: the pair (v, empty) only
             }
             ba_bucket_sort<2>(key, s_order, s_wcnt, s_bstart);
             if (tid == 0) {                                    // batches: <= BA_RB_OUT consecutive nodes of one kind
@@ -276,7 +293,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                 if (may_big) big = __any_sync(0xffffffffu, lane < len && bal[lane].big != 0u);
 
                 // ---- the pair (v, empty) of every node: thread (v, node) ----------------------------------
-                if (do_eps) {
+                if (eps_enum) {
                     const double *erow = s_rows + (size_t)(buf * BA_RB_OUT) * (BA_ROWB / 8) + ev;
                     if (MODE == OUT_SWEEP && !big) {
                         double e0 = 0.0, e1 = 0.0;             // two chains; nodes esub, esub + epn, ...

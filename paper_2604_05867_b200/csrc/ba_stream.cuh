@@ -84,6 +84,40 @@ __global__ void __launch_bounds__(1024) k_finalize(const double *__restrict__ pa
     }
 }
 
+// The low tile on its own: M(u, w) = sum_v p(u.v) emb(w, v) for every high part u and every string w of length <= m
+// (by code(w); 2^{m+1} entries per u, entry 0 unused).  With the concatenation identity at the tile boundary,
+//     sum_v p(u.v) emb(y', u.v) = sum_s alpha_s M(u, sigma_s),    alpha_s = emb(y'[0:k-s], u), sigma_s = last s symbols of y',
+// so the output sweep forms the pair (v, empty) of a node from <= m+1 entries of M instead of 2^m terms and a staged row.
+// LT[v][code(w)] = emb(w, v) (bytes).  One block serves four u: every table byte is converted once for four FMAs.
+#define BA_LT_UB 4
+__global__ void __launch_bounds__(512) k_low_tile(int m, size_t NU, const double *__restrict__ p,
+                                                  const uint8_t *__restrict__ LT, double *__restrict__ M) {
+    __shared__ double prow[BA_LT_UB << BA_MLOW];
+    const int nv = 1 << m, W = 2 << m, tid = threadIdx.x;
+    for (size_t u0 = (size_t)blockIdx.x * BA_LT_UB; u0 < NU; u0 += (size_t)gridDim.x * BA_LT_UB) {
+        __syncthreads();
+        for (int i = tid; i < BA_LT_UB * nv; i += blockDim.x) {
+            const size_t uu = u0 + (size_t)(i >> m);
+            prow[i] = (uu < NU) ? p[(uu << m) + (size_t)(i & (nv - 1))] : 0.0;
+        }
+        __syncthreads();
+        if (tid < W) {
+            double acc[BA_LT_UB];
+#pragma unroll
+            for (int j = 0; j < BA_LT_UB; j++) acc[j] = 0.0;
+#pragma unroll 4
+            for (int v = 0; v < nv; v++) {
+                const double bd = ba_u2d((uint32_t)LT[(size_t)v * W + tid]);
+#pragma unroll
+                for (int j = 0; j < BA_LT_UB; j++) acc[j] = fma(bd, prow[j * nv + v], acc[j]);
+            }
+#pragma unroll
+            for (int j = 0; j < BA_LT_UB; j++)
+                if (u0 + j < NU) M[(u0 + j) * (size_t)W + tid] = acc[j];
+        }
+    }
+}
+
 // p(x) <- max( p(x) 2^{D(x)} / Z, 2^-1000 )    (G8)
 __global__ void k_update(size_t NX, double *__restrict__ p, const double *__restrict__ D,
                          const double *__restrict__ scal) {

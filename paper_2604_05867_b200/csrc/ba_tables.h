@@ -30,6 +30,9 @@ struct TileTables {
     GroupSide in, out;
     std::vector<uint2> EPS8;        // [256][nv]: byte s = B(sigma_s, v), s = 0..7, sigma = the row index
     std::vector<uint32_t> EPSH;     // [BA_NCLS][8][nv]: EPS8[(hi << 4) | cls][v].y, hi = sigma bits 4..6: the slice of a class (input sweep)
+    std::vector<uint8_t> LT;        // [nv][2^{m+1}]: emb(w, v) by code(w) (entry 0 unused): the whole low tile (k_low_tile)
+    std::vector<uint32_t> LTV_off;  // [nv + 1]: the subsequences w of v (the empty one included) ...
+    std::vector<uint32_t> LTV;      // ... as code(w) << 8 | emb(w, v), by increasing code (input sweep: pairs (v, empty))
     bool ok = false;
 };
 
@@ -176,6 +179,16 @@ static inline void build_tile_tables(int m, TileTables &T) {
                 }
                 B[(size_t)((1u << lw) | w) * nv + v] = (uint8_t)e[lw];       // <= C(8,4) = 70
             }
+    T.LT.assign((size_t)nv * NZc, 0);
+    for (int v = 0; v < nv; v++)
+        for (int cw = 1; cw < NZc; cw++) T.LT[(size_t)v * NZc + cw] = B[(size_t)cw * nv + v];
+    T.LTV_off.assign((size_t)nv + 1, 0u);
+    T.LTV.clear();
+    for (int v = 0; v < nv; v++) {
+        for (int cw = 1; cw < NZc; cw++)
+            if (B[(size_t)cw * nv + v]) T.LTV.push_back(((uint32_t)cw << 8) | B[(size_t)cw * nv + v]);
+        T.LTV_off[v + 1] = (uint32_t)T.LTV.size();
+    }
     auto Bof = [&](uint32_t cw, int v) -> uint32_t { return (cw < (uint32_t)NZc) ? B[(size_t)cw * nv + v] : 0u; };
     auto first_bit = [](uint32_t cz) -> int { const int lz = 31 - __builtin_clz(cz); return (int)((cz >> (lz - 1)) & 1u); };
     auto deep = [&](int cls, const TTPair &p) -> bool {        // chain of (v,z) under class cls reaches s = BA_KB
