@@ -9,19 +9,19 @@
 //            Sub[pos] in the role of the Count table P:260-274 and NextPos P:256-258 done with clz on bit
 //            masks), and carries the integer embedding-count DP  E[i] = emb(y', u[0:i])  in registers
 //            along the descent; the node record {alpha_0..8, code(y'), mask} goes to shared memory.
-//   eps      (b = 0) the pair (v, empty) of every node of the round: thread (v, node), all nine B(sigma_s, v) from
-//            one 8-byte read of the direct table EPS8[sigma_8][v].
 //   sort     the nodes that carry list b (b cannot follow y' in u) are ranked, stably, by class; the rounds' runs are
 //            merged into one order.
 //   phase B  batches of <= BA_RB_IN nodes of one class.  The operands c(y'.z), z = b.t, of a node
-//            form a HALF ROW of 2^m doubles indexed by code(t) (8 contiguous segments of c), staged with
-//            16-byte cp.async, double buffered.  Every thread owns BA_KG groups of BA_GP pairs (ba_internal.h
-//            "GROUPS"): a group is one z with up to 4 different v, so c(y'.z) is read once per node and group; the
+//            form a HALF ROW of 2^m doubles indexed by code(t): one row of crow, staged by warp 0 with one bulk copy,
+//            double buffered; FULL / EMPTY mbarriers are the only per-batch synchronisation.  Every thread owns BA_KG
+//            groups of BA_GP pairs (ba_internal.h "GROUPS"): a group is one z with up to 4 different v, so c(y'.z) is read once per node and group; the
 //            slots' B_0..B_3 are constants of the batch, and the loop over the nodes of the batch costs, per (x,y) term,
 //                 1-2 IDP.2A (emb) + 1 exact u32->f64 + 1 DFMA
 //            with one FP64 accumulator per slot kept in a register for the whole item.  Deep pairs
 //            ride along, one per thread, their partial sums handed to thread v through shared memory
 //            in a fixed order.
+//   (v, empty) IN_SWEEP sums these pairs in factored form: G sums per suffix of y', expanded once per item (P:181 at
+//            the tile boundary; see "G sums" below and DESIGN.md section 5); the other modes enumerate them.
 //   epilogue thread v adds the accumulators of v's slots in a fixed order: S_b(x) = sum_{y in item} emb(y,x) c(y).
 // k_in_final (ba_stream.cuh) forms D(x) = Hc(x) - S_0(x) - S_1(x) and the first stage of the reductions of 8(a3).
 // MODE:

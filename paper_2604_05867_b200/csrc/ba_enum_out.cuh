@@ -10,15 +10,17 @@
 //            subsetUnrank / RecSuperSeq, Alg. 5-6, with the G3 correction for the unmatched
 //            tail; there are sum_{i<=h-t} C(h,i) of them by Lemma 6) and runs the textbook
 //            integer DP  f[s] = emb(y'[0:t-s], u)  in registers; record {alpha_0..8, u, mask}.
-//   sort     the nodes that carry list b are compacted (stable); for b = 0 the others follow (pair (v, empty) only).
+//            For b = 0 the same thread adds the node's pair (v, empty) in factored form: sum_s alpha_s M(u, sigma_s),
+//            M from k_low_tile (P:181 at the tile boundary).
+//   sort     the nodes that carry list b are compacted (stable); the others are done (OUT_DEBUG / OUT_COUNT, which need
+//            every emb on its own, let them follow in batches of the pair (v, empty) only).
 //   phase B  batches of <= BA_RB_OUT nodes.  For node u the 2^m inputs p(u.*) -- the run of inputs whose low m
 //            bits are free (SURVEY 7.2 "coalescing the gather") -- are one contiguous 2^m-double row, staged with
-//            16-byte cp.async into a 3-stage ring whose FULL / EMPTY mbarriers are the only per-batch
+//            one bulk copy per row by warp 0 into a 3-stage ring whose FULL / EMPTY mbarriers are the only per-batch
 //            synchronisation.  Every thread owns BA_KG groups of BA_GP pairs (ba_internal.h "GROUPS"): a group is one
 //            v with up to 4 different z, so p(u.v) is read once per node and group, and
 //                 1-2 IDP.2A (emb) + 1 exact u32->f64 + 1 DFMA            per (x,y) term.
-//            The pair (v, empty) of every node (b = 0) and the deep pairs (riders) use all nine B_s, read once
-//            per item from direct tables.
+//            The deep pairs (riders) use all nine B_s, read once per item from direct tables.
 //   epilogue the slots of each z are added in a fixed order and written once:
 //            Apart[y'][z] = sum_{u, v} emb(y'.z, u.v) p(u.v) over the nodes where y' is the longest
 //            prefix of y'.z embeddable in u.
@@ -207,6 +209,16 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                     }
                     u = (u << 1) | bit;
                 }
+                // M(u, sigma_s) of the pair (v, empty): loaded now, used after the DP, which covers their latency
+                double mv[BA_MLOW + 1];
+#pragma unroll
+                for (int s = 0; s <= BA_MLOW; s++) mv[s] = 0.0;
+                if (MODE == OUT_SWEEP && do_eps) {
+                    const double *Mu = a.M + ((size_t)u << (m + 1));
+#pragma unroll
+                    for (int s = 0; s <= BA_MLOW; s++)         // code(sigma_s) = 1 << s | last s symbols of y'
+                        if (s <= Lm) mv[s] = __ldg(Mu + ((1u << s) | (cy & ((1u << s) - 1u))));
+                }
                 // f[s] = emb(y'[0:t-s], u): textbook DP over the positions of u, f indexed from the END of y'
                 uint32_t f[BA_HMAX + 2];
 #pragma unroll
@@ -230,11 +242,6 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                     }
                 }
                 if (MODE == OUT_SWEEP && do_eps) {
-                    const double *Mu = a.M + ((size_t)u << (m + 1));
-                    double mv[BA_MLOW + 1];
-#pragma unroll
-                    for (int s = 0; s <= BA_MLOW; s++)         // code(sigma_s) = 1 << s | last s symbols of y'
-                        mv[s] = (s <= Lm) ? __ldg(Mu + ((1u << s) | (cy & ((1u << s) - 1u)))) : 0.0;
                     double e = 0.0;
 #pragma unroll
                     for (int s = BA_MLOW; s >= 0; s--) e = fma((double)f[s], mv[s], e);    // alpha_s = 0 beyond t

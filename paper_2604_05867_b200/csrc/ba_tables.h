@@ -43,7 +43,9 @@ static inline uint32_t tt_prepend(uint32_t sig, int s, uint32_t cz) {
 }
 
 struct TTPair { int v; uint32_t cz; };
+#ifndef BA_STAGER_EXTRA
 #define BA_STAGER_EXTRA 12.0                // instructions per node the stager warp spends on staging (measured best of 0 / 12 / 25)
+#endif
 
 // Deal the pairs of one list to (warp, level, lane, slot):
 //   * a GROUP is up to BA_GP pairs that share their gathered operand (`key` = its position in a staged row); the
