@@ -31,6 +31,7 @@ struct ba_ctx {
     // carved from scratch
     double *c = nullptr, *crow = nullptr, *Hc = nullptr, *Apart = nullptr, *S = nullptr, *park = nullptr, *part = nullptr, *scal = nullptr, *hist = nullptr;
     GroupDev gin, gout;              // pair schedules of the two sweeps (device pointers into scratch)
+    GroupDev ginf;                   // input sweep proper (IN_SWEEP): deep part of the chains in factored form, no riders
     uint2 *EPS8 = nullptr;
     uint32_t *LTV_off = nullptr, *LTV = nullptr;            // subsequences of every v (input sweep, pairs (v, empty))
     uint8_t *LT = nullptr;                                  // [2^m][2^{m+1}] emb(w, v) of the low tile (k_low_tile)
@@ -76,7 +77,7 @@ static double host_binom(int n, int k) {
 struct SideLayout { size_t GB, GA, GO, GW, csr_off, csr_idx, R, r_cnt, r_csr, R8; };
 struct ScratchLayout {
     size_t c, crow, Hc, Apart, S, park, part, scal, hist, EPS8, EPSH, LT, LTV_off, LTV, elog, counters, cnt, total;
-    SideLayout in, out;
+    SideLayout in, out, inf;
     size_t napart, npart_cap;
 };
 
@@ -135,6 +136,7 @@ static void scratch_layout(int n, const TileTables &T, ScratchLayout &L) {
     L.LTV = o; o += align256(T.LTV.size() * 4);
     L.elog = o; o += align256((size_t)BA_ELOG_N * 8);
     side_layout(T.in, L.in, o);
+    side_layout(T.inf, L.inf, o);
     side_layout(T.out, L.out, o);
     L.counters = o; o += align256(16 * 4);
     L.cnt = o; o += align256(8 * 8);
@@ -189,8 +191,10 @@ extern "C" int ba_debug_check_tables(int m, unsigned long long stats[4]) {
         if (lz + s > m) return 0u;
         return chk_emb(((sig & ((1u << s) - 1u)) << lz) | (cz - (1u << lz)), lz + s, (uint32_t)v, m);
     };
-    for (int side = 0; side < 2; side++) {                  // 0: input sweep tables, 1: output sweep tables
-        const GroupSide &G = side ? T.out : T.in;
+    for (int side4 = 0; side4 < 3; side4++) {               // 0: input sweep tables, 1: output sweep tables; 2: the input
+        const int side = side4 & 1;                         // sweep proper (IN_SWEEP), where the deep part of the chains is
+        const bool fact = side4 >= 2;                       // summed in factored form, so there is no rider
+        const GroupSide &G = (side4 == 0) ? T.in : (side4 == 1) ? T.out : T.inf;
         for (int cls = 0; cls < BA_NCLS; cls++)
             for (int b = 0; b < 2; b++) {
                 std::vector<uint8_t> seen((size_t)nv * NZc, 0);
@@ -208,7 +212,7 @@ extern "C" int ba_debug_check_tables(int m, unsigned long long stats[4]) {
                     const int lz = 31 - __builtin_clz(cz);
                     if ((int)((cz >> (lz - 1)) & 1u) != b || seen[(size_t)v * NZc + cz]++) return false;
                     for (int s = 0; s < 4; s++) if (((b0123 >> (8 * s)) & 0xffu) != Bs((uint32_t)cls, s, cz, v)) return false;
-                    if (nb == 4) return Bs((uint32_t)cls, 4, cz, v) == 0;                 // a slot pair must not be deep
+                    if (nb == 4) return fact || Bs((uint32_t)cls, 4, cz, v) == 0;         // a slot pair must not be deep (enumerating tables)
                     for (uint32_t hi = 0; hi < 16u; hi++)                                 // rider: B_4 .. B_8
                         for (int s = 4; s <= 8; s++) {
                             const uint32_t want = Bs((hi << 4) | (uint32_t)cls, s, cz, v);
@@ -231,10 +235,11 @@ extern "C" int ba_debug_check_tables(int m, unsigned long long stats[4]) {
                             if ((hm >> 2) == 2 && (e[q] >> 16)) return BA_EINVAL;               // a type-2 loop ignores B_2, B_3
                             if ((hm >> 2) == 1 && (e[q] >> 8)) return BA_EINVAL;                // a type-1 loop ignores B_1..B_3
                             if (!visit(pos, ow, e[q], 4, nullptr)) return BA_EINVAL;
-                            stats[side ? 2 : 0]++;
+                            if (!fact) stats[side ? 2 : 0]++;
                         }
                     }
                 const int nr = G.r_cnt[cls * 2 + b];
+                if (fact && nr != 0) return BA_EINVAL;
                 for (int e = 0; e < nr; e++) {
                     const uint4 rd = G.R[((size_t)cls * 2 + b) * G.nr + e];
                     uint32_t tail8[16];
@@ -352,6 +357,7 @@ static int finish_create(ba_ctx *c) {
     for (int e = 2; e < BA_ELOG_N; e++) elog[e] = (double)((long double)e * log2l((long double)e));
     CK(upload(c->elog, elog, c->st));
     CK(upload_side(s, T.in, L.in, c->gin, c->st));
+    CK(upload_side(s, T.inf, L.inf, c->ginf, c->st));
     CK(upload_side(s, T.out, L.out, c->gout, c->st));
     CK(cudaMemsetAsync(c->c, 0, 8, c->st));                  // c[0] is never written by k_out_final
     uint32_t hb[BA_NMAX_I + 1][BA_NMAX_I + 1];
@@ -364,7 +370,7 @@ static int finish_create(ba_ctx *c) {
     CK(cudaGetDevice(&dev));
     CK(cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev));
     c->block = BA_NT;
-    c->smem_in = enum_in_smem(c->gin.nr).total;
+    c->smem_in = std::max(enum_in_smem(c->gin.nr, false).total, enum_in_smem(c->ginf.nr, true).total);
     c->smem_out = enum_out_smem(c->gout.nr).total;
     CK(raise_smem_limits(c->smem_in, c->smem_out));
     int occ_in = 1, occ_out = 1;
@@ -498,11 +504,15 @@ static int ensure_hc(ba_ctx *c) {
     CK(cudaEventRecord(c->ev_setup[0], c->st));
     CK(cudaMemsetAsync(c->counters, 0, 16 * 4, c->st));
     InArgs a = make_in_args(c);
-    a.sym = c->sym;
+    // Hc does not depend on the iterate and the channel is invariant under complementing x and y together (Theorem 4,
+    // P:785-791, g = cpl): Hc(~x) = Hc(x) whatever p is.  So the pass always enumerates only the inputs whose leading
+    // symbol is 0 (whenever there is a high part) and k_hc_final mirrors them.
+    const int hsym = (c->h >= 1) ? 1 : 0;
+    a.sym = hsym;
     k_enum_in<IN_HC><<<c->grid_in, c->block, c->smem_in, c->st>>>(a);
     CK(cudaGetLastError());
     const long double K = 0.0L;                             // the pass centres term by term
-    k_hc_final<<<c->num_sms * 8, 256, 0, c->st>>>(c->NX, c->S, c->S + c->NX, c->Hc, c->sym, (double)K);
+    k_hc_final<<<c->num_sms * 8, 256, 0, c->st>>>(c->NX, c->S, c->S + c->NX, c->Hc, hsym, (double)K);
     CK(cudaGetLastError());
     CK(cudaEventRecord(c->ev_setup[1], c->st));
     c->hc_ready = true;
@@ -546,6 +556,7 @@ static int launch_in_sweep(ba_ctx *c, size_t *npart) {
     if (c->mode == BA_MODE_ENUM) {
         CK(cudaMemsetAsync(c->counters, 0, 4, c->st));
         InArgs a = make_in_args(c);
+        a.g = c->ginf;                                      // the sweep's own schedule: no riders, deep part factored
         a.sym = c->sym;
         k_enum_in<IN_SWEEP><<<c->grid_in, c->block, c->smem_in, c->st>>>(a);
         CK(cudaGetLastError());

@@ -61,9 +61,12 @@ struct InArgs {
     unsigned long long *cnt;  // IN_COUNT: [0] terms, [1] emb sum
 };
 
-struct InSmem { size_t rec, slice, rslice, rows, mbar, bal, ordr, seg, order, gstart, wcnt, batch, rsum, sub, kcw, item, total; };
+struct InSmem { size_t rec, slice, rslice, rows, mbar, bal, ordr, seg, order, skey, g2map, gstart, wcnt, batch, rsum, sub, kcw, item, total; };
 
-__host__ __device__ static inline InSmem enum_in_smem(int nr) {
+// sweep = the layout of IN_SWEEP (no riders: nr counts the deep-part targets; sorted keys and split maps instead of the
+// rider slices); otherwise the layout of the modes that enumerate every term (riders, nr = capacity of the rider set)
+__host__ __device__ static inline InSmem enum_in_smem(int nr, bool sweep) {
+    if (sweep) nr = BA_G2_NT;
     InSmem s;
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o += (bytes + 15) & ~(size_t)15; return at; };
@@ -71,7 +74,7 @@ __host__ __device__ static inline InSmem enum_in_smem(int nr) {
     s.rsum = take((size_t)4 * 2 * nr * 8 > (size_t)BA_NT * 8 ? (size_t)4 * 2 * nr * 8 : (size_t)BA_NT * 8);   // rider sums of a batch, two replicas,
                                                            // four batches deep (collected two batches late); the epilogue parks acc_eps there
     s.slice = take((size_t)2 * 8 * ((size_t)1 << BA_MLOW) * 4);    // B_4..B_7 of the pairs (v, empty) of a class, double buffered
-    s.rslice = take((size_t)2 * 8 * nr * 4);               // B_4..B_7 of the riders of a class, double buffered
+    s.rslice = take(sweep ? 0 : (size_t)2 * 8 * nr * 4);   // B_4..B_7 of the riders of a class, double buffered
     size_t rows = (size_t)2 * BA_RB_IN * BA_ROWB, ac = (size_t)2 * BA_NSLOT * BA_NT * 8;   // both schedules' accumulators
     s.rows = take(rows > ac ? rows : ac);                  // the epilogue's accumulator staging aliases the rows
     s.mbar = take(4 * 8);                                  // FULL and EMPTY barriers of the two row buffers
@@ -79,6 +82,8 @@ __host__ __device__ static inline InSmem enum_in_smem(int nr) {
     s.ordr = take((size_t)BA_SBR * BA_NT * 2);             // per round: the round's nodes by class
     s.seg = take((size_t)BA_SBR * (BA_IN_NBKT + 1) * 2);
     s.order = take((size_t)BA_IN_SB * 2);                  // merged: class-major node ids of the super-batch
+    s.skey = take(sweep ? (size_t)BA_IN_SB * 2 : 0);                 // in the same order: last 8 symbols of y' | min(|y'|, 15) << 8 (G sums)
+    s.g2map = take(sweep ? (size_t)2 * 480 * 8 : 0);                 // per list and owner thread of w: (class, target) of the splits of w (deep part)
     s.gstart = take((size_t)(BA_IN_NBKT + 1) * 2);
     s.wcnt = take((size_t)(BA_NT / 32) * BA_IN_NBKT * 2);
     s.batch = take((size_t)BA_IN_MAXB * 4);
@@ -110,7 +115,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
     extern __shared__ __align__(16) unsigned char smem[];
     const int m = a.kc.m, h = a.kc.h, nv = 1 << m;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const InSmem L = enum_in_smem(a.g.nr);
+    const InSmem L = enum_in_smem(a.g.nr, MODE == IN_SWEEP);
 
     NodeRec *s_rec = (NodeRec *)(smem + L.rec);
     uint32_t *s_slice = (uint32_t *)(smem + L.slice);
@@ -131,6 +136,26 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
     uint16_t *s_ordr = (uint16_t *)(smem + L.ordr);
     uint16_t *s_seg = (uint16_t *)(smem + L.seg);
     uint16_t *s_order = (uint16_t *)(smem + L.order);
+    uint16_t *s_skey = (uint16_t *)(smem + L.skey);
+    uint2 *s_g2map = (uint2 *)(smem + L.g2map);
+    if (MODE == IN_SWEEP && tid < 480) {                    // g2map: see "deep part" below; static but for the list
+        const uint32_t code = 32u + (uint32_t)tid;
+        const int Lw = ba_len_of_code(code);
+        const uint32_t wv = code - (1u << Lw);
+        for (int bb = 0; bb < 2; bb++) {
+            uint32_t gm[2] = {0u, 0u};
+            if (Lw <= m && m >= 5)
+                for (int s = 4; s < Lw && s < 8; s++) {
+                    const int zl = Lw - s;
+                    const uint32_t z = wv & ((1u << zl) - 1u), sig = wv >> zl;
+                    if ((int)((z >> (zl - 1)) & 1u) != bb) continue;
+                    const uint32_t tc = (1u << (zl - 1)) | (z & ((1u << (zl - 1)) - 1u)), ext = sig >> 4;
+                    const uint32_t t = (s == 4) ? tc - 1u : (s == 5) ? 15u + ext * 7u + tc - 1u : (s == 6) ? 29u + ext * 3u + tc - 1u : 41u + ext;
+                    gm[(s - 4) >> 1] |= (0x8000u | ((sig & 15u) << 8) | t) << (16 * ((s - 4) & 1));
+                }
+            s_g2map[bb * 480 + tid] = make_uint2(gm[0], gm[1]);
+        }
+    }
     uint16_t *s_gstart = (uint16_t *)(smem + L.gstart);
     uint16_t *s_wcnt = (uint16_t *)(smem + L.wcnt);
     uint32_t *s_batch = (uint32_t *)(smem + L.batch);
@@ -174,8 +199,16 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
         // so IN_SWEEP adds c(y') alpha_s of every node to the nine G sums of its suffixes (eps_fact) and expands them
         // once per item; the other modes need every emb on its own and enumerate the 2^m terms of a node (eps_enum).
         const bool eps_fact = MODE == IN_SWEEP && b == 0, eps_enum = MODE != IN_SWEEP && b == 0;
-        if (eps_fact)
+        if (MODE == IN_SWEEP)
             for (int i = tid; i < BA_IN_NG; i += BA_NT) s_G[i] = 0.0;
+        // The deep part of the chains (s >= 4), IN_SWEEP: the same identity with z kept,
+        //     sum_{y', z} c(y'.z) sum_{s>=4} alpha_s emb(sigma_s.z, v) = sum_w G2(w) emb(w, v),  G2(w) = sum_{sigma_s.z = w} c(y'.z) alpha_s,
+        // so every pair keeps a plain slot with B_0..B_3 (schedule `inf`, no riders) and G2 joins the G sums.  Under one
+        // class and list there are BA_G2_NT = 49 targets (s, bits 4..s-1 of sigma_s, z): 15 + 2*7 + 4*3 + 8*1; a batch's
+        // targets are summed by the last 49 threads of each half of the CTA (every other node each) from the staged
+        // rows, and handed through shared memory to the owner thread of w = sigma_s.z, which collects them two batches
+        // later (as the rider sums of the other modes).  g2map: the (class, target) of the <= 4 splits of this thread's w.
+        double acc_g2 = 0.0;
 
         // ---- Sub[pos] = number of trie nodes below a node whose leftmost embedding ends at pos -------
         if (tid == 0) {
@@ -317,7 +350,12 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
 #pragma unroll
                     for (int st = BA_IN_NBKT / 2; st > 0; st >>= 1)
                         if ((int)sg[kq + st] <= idx) kq += st;
-                    s_order[s_gstart[kq] + s_roff[rd * BA_IN_NBKT + kq] + (idx - (int)sg[kq])] = (uint16_t)(rd * BA_NT + od[idx]);
+                    const int node = rd * BA_NT + od[idx], at = s_gstart[kq] + s_roff[rd * BA_IN_NBKT + kq] + (idx - (int)sg[kq]);
+                    s_order[at] = (uint16_t)node;
+                    if (MODE == IN_SWEEP) {
+                        const uint32_t kk = s_rec[node].info >> 16;
+                        s_skey[at] = (uint16_t)((s_rec[node].id & 0xffu) | ((kk < 15u ? kk : 15u) << 8));
+                    }
                 }
             }
             if (eps_fact) ba_cp_async_wait_all();              // this thread's c(y')
@@ -336,9 +374,11 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                     for (int part = 0; part < 2; part++) {
                         const int i0 = s_gstart[part * BA_NCLS + cl], i1 = s_gstart[part * BA_NCLS + cl + 1];
                         for (int i = i0; i < i1; i++) {
-                            const int node = s_order[i];
-                            const NodeRec &rc = s_rec[node];
-                            if ((int)(rc.info >> 16) >= s && (rc.id & mask) == wval) g = fma((double)rc.a[s], s_c[node], g);
+                            const uint32_t key = s_skey[i];    // one independent load per node; the record only on a match
+                            if ((int)(key >> 8) >= s && (key & mask) == wval) {
+                                const int node = s_order[i];
+                                g = fma((double)s_rec[node].a[s], s_c[node], g);
+                            }
                         }
                     }
                     s_G[dst] += g;
@@ -368,7 +408,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 if (g >= 2u) ba_mbar_wait(sEmpty + 8u * buf, ((g >> 1) - 1u) & 1u);
                 const bool newcls = scls != st_cls;            // a new class: its slices of B_4..B_7 (by the sigma bits 4..6)
                 if (newcls) { st_cls = scls; st_sb ^= 1; }     // of the riders and, for b = 0, of the pairs (v, empty)
-                const uint32_t rs_bytes = 32u * (uint32_t)a.g.nr, es_bytes = (eps_enum && m == BA_MLOW) ? (8u << BA_MLOW) * 4u : 0u;
+                const uint32_t rs_bytes = (MODE == IN_SWEEP) ? 0u : 32u * (uint32_t)a.g.nr, es_bytes = (eps_enum && m == BA_MLOW) ? (8u << BA_MLOW) * 4u : 0u;
                 const bool row = MODE == IN_SWEEP && lane < len && (bi >> 24) < BA_NCLS;
                 uint32_t tx = row ? (uint32_t)nv * 8u : 0u;
                 if (newcls && lane == 0) tx += rs_bytes + es_bytes;
@@ -394,7 +434,20 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                                 (uint32_t)nv * 8u, sFull + 8u * buf);
             };
             auto flush = [&](int j) {                          // thread v collects the rider sums of batch j
-                if (MODE != IN_SWEEP && MODE != IN_HC) return;
+                if (MODE == IN_SWEEP) {                        // the owner of w collects the deep-part sums of its splits
+                    if (tid >= 480) return;
+                    const uint2 gm = s_g2map[b * 480 + tid];
+                    if ((gm.x | gm.y) == 0u) return;
+                    const uint32_t want = 0x80u | (s_batch[j] >> 24);
+                    const double *rs = s_rsum + (size_t)((gb + (uint32_t)j) & 3u) * 2 * BA_G2_NT;
+#pragma unroll
+                    for (int q = 0; q < 4; q++) {
+                        const uint32_t e = (((q >> 1) ? gm.y : gm.x) >> (16 * (q & 1))) & 0xffffu;
+                        if ((e >> 8) == want) acc_g2 += rs[e & 0xffu] + rs[BA_G2_NT + (e & 0xffu)];
+                    }
+                    return;
+                }
+                if (MODE != IN_HC) return;
                 if (tid >= nv) return;
                 if ((s_batch[j] >> 24) >= BA_NCLS) return;     // a batch without list b has no riders
                 const int cls = (int)(s_batch[j] >> 24), rbuf = (int)((gb + (uint32_t)j) & 3u);
@@ -517,8 +570,38 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                         }
                     }
                 }
+                // ---- IN_SWEEP: the deep part of this batch, one target per thread (see acc_g2 above) --------
+                if (MODE == IN_SWEEP && m >= 5) {
+                    const int t2 = (BA_NT / 2 - 1) - (tid & (BA_NT / 2 - 1)), rh2 = tid / (BA_NT / 2);
+                    if (t2 < BA_G2_NT) {
+                        int s;
+                        uint32_t ext, tc;                      // split, bits 4..s-1 of sigma_s, code(t) of z = b.t
+                        if (t2 < 15) { s = 4; ext = 0u; tc = (uint32_t)t2 + 1u; }
+                        else if (t2 < 29) { s = 5; ext = (uint32_t)(t2 - 15) / 7u; tc = (uint32_t)(t2 - 15) % 7u + 1u; }
+                        else if (t2 < 41) { s = 6; ext = (uint32_t)(t2 - 29) / 3u; tc = (uint32_t)(t2 - 29) % 3u + 1u; }
+                        else { s = 7; ext = (uint32_t)(t2 - 41); tc = 1u; }
+                        const uint32_t pos = (tc == 1u) ? (uint32_t)b : tc, emask = (1u << (s - 4)) - 1u;
+                        double g = 0.0;
+                        if (s + 1 + ba_len_of_code(tc) <= m) {     // |sigma_s.z| <= m
+                            const double *rrow = s_rows + (size_t)(buf * BA_RB_IN) * (BA_ROWB / 8) + pos;
+                            for (int i = rh2; i < len; i += 2) {
+                                const uint32_t cyi = bal[i].id;
+                                if (ba_len_of_code(cyi) >= s && ((cyi >> 4) & emask) == ext) {
+                                    uint32_t al;
+                                    if (big) al = s_rec[bal[i].node].a[s];
+                                    else {
+                                        const uint32_t w2 = (s < 6) ? bal[i].a45 : bal[i].a67;
+                                        al = (s & 1) ? (w2 >> 16) : (w2 & 0xffffu);
+                                    }
+                                    g = fma(ba_u2d(al), rrow[(size_t)i * (BA_ROWB / 8)], g);
+                                }
+                            }
+                        }
+                        s_rsum[((size_t)((gb + (uint32_t)j) & 3u) * 2 + rh2) * BA_G2_NT + t2] = g;
+                    }
+                }
                 // ---- riders: deep pairs of this class, one per thread ------------------------------------
-                const int nr = a.g.r_cnt[cls * 2 + b];
+                const int nr = (MODE == IN_SWEEP) ? 0 : a.g.r_cnt[cls * 2 + b];
                 // two replicas of the rider set (threads 255 - e and 511 - e), each takes every other node
                 const int re = (BA_NT / 2 - 1) - (tid & (BA_NT / 2 - 1)), rh = tid / (BA_NT / 2);
                 if ((BA_NT / 2) - 32 * ((warp & (BA_NT / 64 - 1)) + 1) < nr) {
@@ -592,6 +675,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                     s_acc[((size_t)sc * BA_NSLOT + s) * BA_NT + tid] = (sc == cur_sc) ? acc[s] : ((parked >> sc) & 1u) ? park[((size_t)sc * BA_NSLOT + s) * BA_NT] : 0.0;
             double *s_aeps = s_rsum;                           // the rider sums are all flushed: their area takes acc_eps
             s_aeps[tid] = acc_eps;
+            if (MODE == IN_SWEEP && tid < 480) s_G[32 + tid] += acc_g2;    // the owner's deep-part sums join its G(w)
             if (eps_fact && tid >= 480 && tid < 511) {         // G(w), |w| <= 4, from the P's of the classes that end in w
                 const uint32_t code = (uint32_t)(tid - 479);
                 const int s = ba_len_of_code(code);
@@ -604,7 +688,7 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_in(const __grid_constant__ In
                 double S = acc_rid;
                 if (eps_enum)
                     for (int t = ev; t < BA_NT; t += nv) S += s_aeps[t];
-                if (eps_fact) {                                // sum_w G(w) emb(w, v) over the subsequences w of v
+                if (MODE == IN_SWEEP) {                        // sum_w G(w) emb(w, v) over the subsequences w of v
                     double se = 0.0;
                     for (uint32_t e = __ldg(a.LTV_off + tid), e1 = __ldg(a.LTV_off + tid + 1); e < e1; e++) {
                         const uint32_t ent = __ldg(a.LTV + e);

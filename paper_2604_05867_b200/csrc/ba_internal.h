@@ -47,6 +47,7 @@
 #define BA_NT 512            // threads per CTA of the ENUM kernels (one CTA per SM)
 #define BA_KG 4              // groups per thread and list
 #define BA_GP 4              // pair slots per group
+#define BA_G2_NT 49                     // input sweep: (split, suffix bits, z) targets of the deep part under one class and list
 #define BA_NSLOT (BA_KG * BA_GP)
 #define BA_KB 4              // class bits
 #define BA_NCLS 16           // 2^BA_KB classes

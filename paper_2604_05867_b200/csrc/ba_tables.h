@@ -28,6 +28,8 @@ struct GroupSide {
 struct TileTables {
     int m = 0, nv = 0;
     GroupSide in, out;
+    GroupSide inf;                  // input sweep, IN_SWEEP: every pair keeps its slot with B_0..B_3 under every class and there are
+                                    // no riders -- the deep part of the chains (s >= 4) is summed in factored form by the kernel
     std::vector<uint2> EPS8;        // [256][nv]: byte s = B(sigma_s, v), s = 0..7, sigma = the row index
     std::vector<uint32_t> EPSH;     // [BA_NCLS][8][nv]: EPS8[(hi << 4) | cls][v].y, hi = sigma bits 4..6: the slice of a class (input sweep)
     std::vector<uint8_t> LT;        // [nv][2^{m+1}]: emb(w, v) by code(w) (entry 0 unused): the whole low tile (k_low_tile)
@@ -43,6 +45,9 @@ static inline uint32_t tt_prepend(uint32_t sig, int s, uint32_t cz) {
 }
 
 struct TTPair { int v; uint32_t cz; };
+#ifndef BA_G2_EXTRA
+#define BA_G2_EXTRA 3.0                     // instructions per node a warp that sums the deep part spends on it
+#endif
 #ifndef BA_STAGER_EXTRA
 #define BA_STAGER_EXTRA 12.0                // instructions per node the stager warp spends on staging (measured best of 0 / 12 / 25)
 #endif
@@ -221,9 +226,14 @@ static inline void build_tile_tables(int m, TileTables &T) {
     };
     init_side(T.in, nv, 2);
     init_side(T.out, NZc, BA_NCLS);
+    init_side(T.inf, nv, 2);
+    auto deep_real = deep;
 
-    for (int side = 0; side < 2; side++) {
-        GroupSide &S = side ? T.out : T.in;
+    for (int sidx = 0; sidx < 3; sidx++) {
+        const int side = sidx & 1;
+        const bool fact = (sidx == 2);                         // the factored-deep variant of the input side: no pair is left to a rider
+        GroupSide &S = (sidx == 1) ? T.out : (sidx == 2) ? T.inf : T.in;
+        auto deep = [&](int cls, const TTPair &p) -> bool { return fact ? false : deep_real(cls, p); };
         // operand position in a staged row.  in: the operand of z = b.t is c(y'.b.t) at position code(t) of the
         // node's half row; out: the operand of (v, z) is p(u.v) at position v of the node's row.
         // (the one-symbol z = "b" sits at position b, not 1: the staged half row starts with the 16-byte pair
@@ -254,6 +264,8 @@ static inline void build_tile_tables(int m, TileTables &T) {
             const int rw = (int)((ndeep + 31) / 32);
             for (int w = 0; w < NW; w++)
                 warp_extra[w] = side ? (w >= NW - rw ? 14.0 : 0.0) : ((w & (NW / 2 - 1)) >= NW / 2 - rw ? 8.0 : 0.0);
+            if (fact)                                          // in: the warps that sum the deep part (BA_G2_NT targets, two replicas)
+                for (int w = 0; w < NW; w++) warp_extra[w] = (!side && (w & (NW / 2 - 1)) >= NW / 2 - (BA_G2_NT + 31) / 32) ? BA_G2_EXTRA : 0.0;
             warp_extra[0] += BA_STAGER_EXTRA;                  // warp 0 also stages the batches: it must run ahead, not behind
             for (int sc = 0; sc < S.nsc; sc++) {
                 // input sweep: schedule sc serves the classes with bit 0 = sc; output sweep: class sc
