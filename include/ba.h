@@ -56,7 +56,12 @@ enum {
 };
 
 enum {
-    BA_MODE_ENUM = 0, /* contract path (NS): every (x,y) term with emb>0 is enumerated once per sweep */
+    BA_MODE_ENUM = 0, /* contract path (NS): the supersequences of every y / the distinct subsequences of every x are
+                         enumerated once per sweep with their integer embedding counts.  A term (x,y), x = u.v, y = y'.z,
+                         has emb = sum_s alpha_s B(sigma_s.z, v) (P:181 at the boundary of the low 8 positions): the
+                         sweeps form s <= 3 term by term; the pairs with z empty (3.9 % of the terms) and, in the input
+                         sweep, the tail s >= 4 are summed in factored form with the same identity.
+                         The debug entry points below still produce every emb, bit for bit. */
     BA_MODE_FAST = 1  /* position-by-position deletion transform, O(n 2^n)/sweep  */
 };
 
