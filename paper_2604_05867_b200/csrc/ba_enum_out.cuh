@@ -41,7 +41,7 @@ struct OutArgs {
     GroupDev g;                // schedule of the output sweep (owner = code(z), operand position = v)
     const uint2 *EPS8;         // [256][2^m]: B(sigma_s, v), s = 1..8, of the pair (v, empty)
     const double *p;           // NX
-    const double *M;           // OUT_SWEEP: [2^h][2^{m+1}] M(u, w) = sum_v p(u.v) emb(w, v) by code(w) (k_low_tile)
+    const double *M;           // OUT_SWEEP: [2^{m+1}][2^h] M(u, w) = sum_v p(u.v) emb(w, v) at [code(w)][u] (k_low_tile)
     double *Apart;             // (2^{h+1}-1) * (2^{m+1}-1)
     unsigned int *counter;
     int sym;                   // 1: q(y) = q(~y): prefixes y' with leading symbol 1 are skipped (k_out_final mirrors them)
@@ -214,10 +214,12 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
 #pragma unroll
                 for (int s = 0; s <= BA_MLOW; s++) mv[s] = 0.0;
                 if (MODE == OUT_SWEEP && do_eps) {
-                    const double *Mu = a.M + ((size_t)u << (m + 1));
+                    // M is laid out by w, then u: the threads of a warp unrank consecutive supersequences, which differ in
+                    // their late positions, so one load touches a few sectors instead of 32
+                    const double *Mu = a.M + u;
 #pragma unroll
                     for (int s = 0; s <= BA_MLOW; s++)         // code(sigma_s) = 1 << s | last s symbols of y'
-                        if (s <= Lm) mv[s] = __ldg(Mu + ((1u << s) | (cy & ((1u << s) - 1u))));
+                        if (s <= Lm) mv[s] = __ldg(Mu + ((size_t)((1u << s) | (cy & ((1u << s) - 1u))) << h));
                 }
                 // f[s] = emb(y'[0:t-s], u): textbook DP over the positions of u, f indexed from the END of y'
                 uint32_t f[BA_HMAX + 2];

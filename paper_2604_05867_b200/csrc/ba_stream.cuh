@@ -85,7 +85,7 @@ __global__ void __launch_bounds__(1024) k_finalize(const double *__restrict__ pa
 }
 
 // The low tile on its own: M(u, w) = sum_v p(u.v) emb(w, v) for every high part u and every string w of length <= m
-// (by code(w); 2^{m+1} entries per u, entry 0 unused).  With the concatenation identity at the tile boundary,
+// (stored by code(w), then u: M[code(w) * 2^h + u], row 0 unused -- the out sweep gathers a few w for many nearby u).  With the concatenation identity at the tile boundary,
 //     sum_v p(u.v) emb(y', u.v) = sum_s alpha_s M(u, sigma_s),    alpha_s = emb(y'[0:k-s], u), sigma_s = last s symbols of y',
 // so the output sweep forms the pair (v, empty) of a node from <= m+1 entries of M instead of 2^m terms and a staged row.
 // LT[v][code(w)] = emb(w, v) (bytes).  One block serves four u: every table byte is converted once for four FMAs.
@@ -113,7 +113,7 @@ __global__ void __launch_bounds__(512) k_low_tile(int m, size_t NU, const double
             }
 #pragma unroll
             for (int j = 0; j < BA_LT_UB; j++)
-                if (u0 + j < NU) M[(u0 + j) * (size_t)W + tid] = acc[j];
+                if (u0 + j < NU) M[(size_t)tid * NU + (u0 + j)] = acc[j];      // by w, then u: the four u of a block fill one sector
         }
     }
 }
