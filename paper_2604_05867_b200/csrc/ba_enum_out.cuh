@@ -190,24 +190,22 @@ __global__ void __launch_bounds__(BA_NT, 1) k_enum_out(const __grid_constant__ O
                     uint32_t ww = w, jj = rem;
                     for (int pp = 0; pp < h && ww > 0; pp++) {
                         const uint32_t cc = s_binom[h - pp - 1][ww - 1];
-                        if (jj < cc) { S |= 1u << pp; ww--; } else { jj -= cc; }
+                        const bool in = jj < cc;
+                        S |= (in ? 1u : 0u) << pp; ww -= in ? 1u : 0u; jj -= in ? 0u : cc;
                     }
                 }
                 // RecSuperSeq (Alg. 6 with the G3 reading): build u left to right
                 uint32_t u = 0;
                 int r = 0, ell = 0;
+                // (branch-free: the lanes of a warp hold different S, so every branch on S would run both ways)
                 for (int pp = 0; pp < h; pp++) {
-                    uint32_t bit;
-                    if ((S >> pp) & 1u) {
-                        if (t == 0) bit = 1u;
-                        else { const int rr = (r < t) ? r : t - 1; bit = 1u ^ ((yv >> (t - 1 - rr)) & 1u); }
-                    } else if (r < t) {
-                        bit = (yv >> (t - 1 - r)) & 1u; r++;
-                        if (r == t) ell = pp + 1;
-                    } else {
-                        bit = (t == 0) ? 0u : (yv & 1u);
-                    }
-                    u = (u << 1) | bit;
+                    const uint32_t skip = (S >> pp) & 1u;
+                    const int rr = (r < t) ? r : t - 1;            // the symbol of y' in play: the next unmatched one, else the last
+                    const uint32_t yb = (t == 0) ? 0u : ((yv >> (t - 1 - rr)) & 1u);
+                    const uint32_t take = (skip ^ 1u) & (uint32_t)(r < t);
+                    u = (u << 1) | (yb ^ skip);                    // a skipped position avoids that symbol, any other carries it
+                    r += (int)take;
+                    ell = (take && r == t) ? pp + 1 : ell;
                 }
                 // M(u, sigma_s) of the pair (v, empty): loaded now, used after the DP, which covers their latency
                 double mv[BA_MLOW + 1];
